@@ -1,0 +1,425 @@
+// msolve_oracle.cpp -- CPU ORACLE for the multishift Krylov solvers CG-M and BiCGStab-M.
+//
+// TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may build, load or call this file.  It shares no code
+// with the CUDA path (paper_1102_2143_b200/csrc): no common headers, helpers or constants.
+//
+// What it is: a plain, slow, single-threaded, step-by-step restatement of
+//   * eq. (1), PAPER.md:41          (A + sigma_k I) x_k = b            -- the result
+//   * Algorithm 1, PAPER.md:73-142  CG-M, with the garbled lines read as SURVEY.md 8(c) C2
+//                                   (R2-R7)
+//   * BiCGStab-M, named at PAPER.md:31,154 and attributed to [4] PAPER.md:244; the paper never
+//     prints it, so it is derived from the collinear-residual argument (eq. (4))
+//     as SURVEY.md 8(c) C3 / DESIGN.md "BiCGStab-M derivation".
+//   * plain CG and plain BiCGStab (textbook, van der Vorst [13] PAPER.md:253) used ONLY as the
+//     sigma=0 / single-shift pins of the two multishift routines.
+// No blocking, fusion or reordering: every loop below is one line of the algorithm.
+//
+// Precision (R14): vectors are complex<T>, T = float (c64) or double (c128); every
+// dot product accumulates in double, every recurrence scalar (zeta, alpha, beta, rho, chi) is
+// double / complex<double>; a scalar that multiplies a vector is rounded to T once, then the
+// vector arithmetic is done in T.  SpMV accumulates a row in T in stored order.
+//
+// Pins (tests/test_oracle_pins.py, run with -m "not gpu"): dense LU of (A+sigma I) on tiny
+// inputs, A = c*I closed form, diagonal-A finite termination, per-iteration collinearity
+// invariant b-(A+sigma)x_k = zeta_k r (CG-M) / zeta_k rho_k r (BiCGStab-M), sigma=0 reduction to
+// plain CG (bitwise) / plain BiCGStab, independent single-shift solves, FFT closed form on a
+// pure-gauge SU(3) lattice, sine-transform closed form on the paper's 2-D Poisson matrix,
+// monotone conv_iter in sigma, true residual <= tol.  Nothing here is "parity unpinned";
+// the choice of stop/mask rule (R15) is a reading, pinned only as oracle == GPU.
+//
+// Build: g++ -O2 -ffp-contract=off -shared -fPIC (see oracle/__init__.py).
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+typedef std::complex<double> zdouble;
+
+enum { ST_OK = 0, ST_MAXITER = 1, ST_BREAKDOWN = 2, ST_EINVAL = -1 };
+
+template <typename T>
+struct Csr {
+    int64_t n;
+    const int32_t* rowptr;
+    const int32_t* colidx;
+    const std::complex<T>* val;
+};
+
+// y = A x   (Alg. 1 l.18).  Row sum in T, stored order.
+template <typename T>
+void spmv(const Csr<T>& A, const std::complex<T>* x, std::complex<T>* y) {
+    for (int64_t i = 0; i < A.n; ++i) {
+        std::complex<T> acc(0, 0);
+        for (int32_t j = A.rowptr[i]; j < A.rowptr[i + 1]; ++j) acc += A.val[j] * x[A.colidx[j]];
+        y[i] = acc;
+    }
+}
+
+// <u,v> = sum_i conj(u_i) v_i, accumulated in double (r^dagger . r).
+template <typename T>
+zdouble dot(int64_t n, const std::complex<T>* u, const std::complex<T>* v) {
+    zdouble acc(0, 0);
+    for (int64_t i = 0; i < n; ++i) acc += std::conj(zdouble(u[i])) * zdouble(v[i]);
+    return acc;
+}
+
+template <typename T>
+inline std::complex<T> rnd(const zdouble& z) { return std::complex<T>((T)z.real(), (T)z.imag()); }
+
+inline bool finite(double x) { return std::isfinite(x); }
+inline bool finite(const zdouble& z) { return std::isfinite(z.real()) && std::isfinite(z.imag()); }
+
+// ------------------------------------------------------------------------------------------
+// CG-M.  Alg. 1 with the readings of DESIGN.md R2-R7:
+//   beta = -R0/P (sign restored), zeta recurrence with beta_prev and alpha,
+//   beta_k = beta zeta_new/zeta, alpha_k = alpha (zeta_new/zeta)^2, p_k uses zeta_new and new r.
+// Stop / mask rule R15: shift k is frozen at the first n with |zeta_k| ||r|| <= tol ||b||.
+// hist (optional, hist_cap rows of 3+3S doubles): per iteration beta, alpha_next, R1 and per
+// shift zeta_new, beta_k, alpha_k.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+int cgm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, double tol,
+        int max_iter, int stop_rule, std::complex<T>* x, int* iterations, int* conv_iter,
+        double* relres, std::complex<T>* r_out, double* zeta_out, double* hist, int hist_cap) {
+    typedef std::complex<T> C;
+    const int64_t n = A.n;
+    if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
+    std::vector<C> r(b, b + n), p(b, b + n), q(n);           // l.9-10: r <- b, p <- b
+    std::vector<C> pk((size_t)S * n);
+    for (int k = 0; k < S; ++k)
+        for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0, 0); }  // l.11-12
+    double alpha = 0.0, beta_prev = 1.0;                      // l.2, l.4
+    std::vector<double> zeta_prev(S, 1.0), zeta(S, 1.0), zeta_new(S, 1.0), beta_k(S, 0.0), alpha_k(S, 0.0);
+    std::vector<char> active(S, 1);
+    double R1 = dot(n, r.data(), r.data()).real();           // l.13
+    const double bnorm = std::sqrt(R1);
+    int it = 0, status = ST_OK, nactive = S;
+    for (int k = 0; k < S; ++k) { if (conv_iter) conv_iter[k] = -1; }
+    if (bnorm == 0.0) {                                       // b = 0: x_k = 0 is exact
+        for (int k = 0; k < S; ++k) { if (conv_iter) conv_iter[k] = 0; if (relres) relres[k] = 0.0; if (zeta_out) zeta_out[k] = 1.0; }
+        if (r_out) std::memcpy((void*)r_out, (const void*)r.data(), sizeof(C) * n);
+        *iterations = 0;
+        return ST_OK;
+    }
+    while (nactive > 0 && it < max_iter) {                    // l.15
+        const double R0 = R1;                                 // l.16
+        spmv(A, p.data(), q.data());                          // l.18
+        const double P = dot(n, p.data(), q.data()).real();   // l.19  (Hermitian A: Im = 0, R9)
+        if (!(P > 0.0) || !finite(P)) { status = ST_BREAKDOWN; break; }
+        const double beta = -R0 / P;                          // l.20  (R2)
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            const double den = beta * alpha * (zeta_prev[k] - zeta[k])
+                             + zeta_prev[k] * beta_prev * (1.0 - sigma[k] * beta);
+            zeta_new[k] = zeta[k] * zeta_prev[k] * beta_prev / den;     // l.22 (R3)
+            beta_k[k] = beta * zeta_new[k] / zeta[k];                   // l.23 (R4)
+            if (den == 0.0 || !finite(zeta_new[k]) || !finite(beta_k[k])) status = ST_BREAKDOWN;
+        }
+        if (status == ST_BREAKDOWN) break;
+        { const C bt = C((T)beta, 0);
+          for (int64_t i = 0; i < n; ++i) r[i] = r[i] + bt * q[i]; }   // l.21
+        R1 = dot(n, r.data(), r.data()).real();               // l.24
+        const double alpha_next = R1 / R0;                    // l.25
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            const double ratio = zeta_new[k] / zeta[k];
+            alpha_k[k] = alpha_next * ratio * ratio;          // l.26 (R5)
+        }
+        { const C an = C((T)alpha_next, 0);
+          for (int64_t i = 0; i < n; ++i) p[i] = r[i] + an * p[i]; }   // l.27
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            C* xk = x + (size_t)k * n; C* pkk = pk.data() + (size_t)k * n;
+            const C bk = C((T)beta_k[k], 0), zn = C((T)zeta_new[k], 0), ak = C((T)alpha_k[k], 0);
+            for (int64_t i = 0; i < n; ++i) xk[i] = xk[i] - bk * pkk[i];            // l.28
+            for (int64_t i = 0; i < n; ++i) pkk[i] = zn * r[i] + ak * pkk[i];       // l.29 (R6)
+        }
+        if (hist && it < hist_cap) {
+            double* h = hist + (size_t)it * (3 + 3 * S);
+            h[0] = beta; h[1] = alpha_next; h[2] = R1;
+            for (int k = 0; k < S; ++k) { h[3 + k] = zeta_new[k]; h[3 + S + k] = beta_k[k]; h[3 + 2 * S + k] = alpha_k[k]; }
+        }
+        for (int k = 0; k < S; ++k) if (active[k]) { zeta_prev[k] = zeta[k]; zeta[k] = zeta_new[k]; }  // l.30-31
+        beta_prev = beta; alpha = alpha_next; ++it;           // l.17, l.32
+        const double rnorm = std::sqrt(R1);
+        if (stop_rule == 1) {                                 // literal |r| > eps on the base system
+            if (rnorm <= tol * bnorm) { for (int k = 0; k < S; ++k) if (active[k]) { active[k] = 0; if (conv_iter) conv_iter[k] = it; } nactive = 0; }
+        } else {
+            for (int k = 0; k < S; ++k) if (active[k] && std::fabs(zeta[k]) * rnorm <= tol * bnorm) {
+                active[k] = 0; --nactive; if (conv_iter) conv_iter[k] = it;
+                if (relres) relres[k] = std::fabs(zeta[k]) * rnorm / bnorm;
+            }
+        }
+    }
+    const double rnorm = std::sqrt(R1);
+    for (int k = 0; k < S; ++k) {
+        if ((active[k] || stop_rule == 1) && relres) relres[k] = std::fabs(zeta[k]) * rnorm / bnorm;
+        if (zeta_out) zeta_out[k] = zeta[k];
+    }
+    if (r_out) std::memcpy((void*)r_out, (const void*)r.data(), sizeof(C) * n);
+    *iterations = it;
+    if (status == ST_BREAKDOWN) return status;
+    return nactive > 0 ? ST_MAXITER : ST_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// BiCGStab-M.  Shadow vector r0 = b.
+// Shifted residual is zeta_k rho_k r.  zeta_out holds (Re, Im) of zeta_k*rho_k per shift.
+// hist rows: 8+6S doubles: beta(2) chi(2) alpha_new(2) |r|^2 delta-unused, then zeta_new,
+// beta_k, chi_k (complex each).
+// ------------------------------------------------------------------------------------------
+template <typename T>
+int bicgstabm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, double tol,
+              int max_iter, int stop_rule, std::complex<T>* x, int* iterations, int* conv_iter,
+              double* relres, std::complex<T>* r_out, double* zeta_out, double* hist, int hist_cap) {
+    typedef std::complex<T> C;
+    const int64_t n = A.n;
+    if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
+    std::vector<C> r(b, b + n), p(b, b + n), r0(b, b + n), q(n), s(n), t(n), rnew(n);
+    std::vector<C> pk((size_t)S * n);
+    for (int k = 0; k < S; ++k)
+        for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0, 0); }
+    zdouble alpha(0, 0), beta_prev(1, 0);
+    std::vector<zdouble> zeta_prev(S, 1.0), zeta(S, 1.0), zeta_new(S, 1.0), rho(S, 1.0), rho_new(S, 1.0),
+        beta_k(S), alpha_k(S), chi_k(S);
+    std::vector<char> active(S, 1);
+    zdouble delta = dot(n, r0.data(), r.data());
+    double rr = delta.real();
+    const double bnorm = std::sqrt(rr);
+    int it = 0, status = ST_OK, nactive = S;
+    for (int k = 0; k < S; ++k) { if (conv_iter) conv_iter[k] = -1; }
+    if (bnorm == 0.0) {
+        for (int k = 0; k < S; ++k) { if (conv_iter) conv_iter[k] = 0; if (relres) relres[k] = 0.0; if (zeta_out) { zeta_out[2 * k] = 1.0; zeta_out[2 * k + 1] = 0.0; } }
+        if (r_out) std::memcpy((void*)r_out, (const void*)r.data(), sizeof(C) * n);
+        *iterations = 0;
+        return ST_OK;
+    }
+    while (nactive > 0 && it < max_iter) {
+        spmv(A, p.data(), q.data());                                       // q = A p
+        const zdouble r0q = dot(n, r0.data(), q.data());
+        if (r0q == zdouble(0, 0) || delta == zdouble(0, 0) || !finite(r0q)) { status = ST_BREAKDOWN; break; }
+        const zdouble beta = -delta / r0q;                                  // beta = -delta/<r0,q>
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            const zdouble den = beta * alpha * (zeta_prev[k] - zeta[k])
+                              + zeta_prev[k] * beta_prev * (1.0 - sigma[k] * beta);
+            zeta_new[k] = zeta[k] * zeta_prev[k] * beta_prev / den;
+            beta_k[k] = beta * zeta_new[k] / zeta[k];
+            if (den == zdouble(0, 0) || !finite(zeta_new[k]) || !finite(beta_k[k])) status = ST_BREAKDOWN;
+        }
+        if (status == ST_BREAKDOWN) break;
+        { const C bt = rnd<T>(beta);
+          for (int64_t i = 0; i < n; ++i) s[i] = r[i] + bt * q[i]; }       // s = r + beta q
+        spmv(A, s.data(), t.data());                                       // t = A s
+        const zdouble ts = dot(n, t.data(), s.data());
+        const double tt = dot(n, t.data(), t.data()).real();
+        if (!(tt > 0.0) || !finite(tt) || !finite(ts)) { status = ST_BREAKDOWN; break; }
+        const zdouble chi = ts / tt;                                        // chi = <t,s>/<t,t>
+        if (chi == zdouble(0, 0)) { status = ST_BREAKDOWN; break; }
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            const zdouble one_cs = 1.0 + chi * sigma[k];
+            if (one_cs == zdouble(0, 0)) { status = ST_BREAKDOWN; break; }
+            chi_k[k] = chi / one_cs;                                        // chi_k = chi/(1+chi sigma)
+            rho_new[k] = rho[k] / one_cs;                                   // rho'_k = rho_k/(1+chi sigma)
+        }
+        if (status == ST_BREAKDOWN) break;
+        { const C ch = rnd<T>(chi);
+          for (int64_t i = 0; i < n; ++i) rnew[i] = s[i] - ch * t[i]; }    // r' = s - chi t
+        const zdouble delta_new = dot(n, r0.data(), rnew.data());           // delta' = <r0,r'>
+        const zdouble alpha_new = -beta * delta_new / (delta * chi);        // alpha' = -beta delta'/(delta chi)
+        if (!finite(alpha_new)) { status = ST_BREAKDOWN; break; }
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            const zdouble ratio = zeta_new[k] / zeta[k];
+            alpha_k[k] = alpha_new * ratio * ratio;
+        }
+        for (int k = 0; k < S; ++k) if (active[k]) {
+            C* xk = x + (size_t)k * n; C* pkk = pk.data() + (size_t)k * n;
+            const C bk = rnd<T>(beta_k[k]);
+            const C cs = rnd<T>(chi_k[k] * rho[k] * zeta_new[k]);           // coefficient of s in x_k
+            const C zr = rnd<T>(zeta_new[k] * rho_new[k]);                  // coefficient of r' in p_k
+            const C ak = rnd<T>(alpha_k[k]);
+            const C cb = rnd<T>(chi_k[k] / beta_k[k]);
+            const C zs = rnd<T>(zeta_new[k] * rho[k]);                      // s^sigma = zs * s
+            const C zo = rnd<T>(zeta[k] * rho[k]);                          // r^sigma = zo * r
+            for (int64_t i = 0; i < n; ++i) xk[i] = (xk[i] - bk * pkk[i]) + cs * s[i];
+            for (int64_t i = 0; i < n; ++i)
+                pkk[i] = zr * rnew[i] + ak * (pkk[i] - cb * (zs * s[i] - zo * r[i]));
+        }
+        { const C an = rnd<T>(alpha_new), ch = rnd<T>(chi);
+          for (int64_t i = 0; i < n; ++i) p[i] = rnew[i] + an * (p[i] - ch * q[i]); }  // p = r' + alpha'(p - chi q)
+        for (int64_t i = 0; i < n; ++i) r[i] = rnew[i];
+        rr = dot(n, r.data(), r.data()).real();
+        if (hist && it < hist_cap) {
+            double* h = hist + (size_t)it * (8 + 6 * S);
+            h[0] = beta.real(); h[1] = beta.imag(); h[2] = chi.real(); h[3] = chi.imag();
+            h[4] = alpha_new.real(); h[5] = alpha_new.imag(); h[6] = rr; h[7] = 0.0;
+            for (int k = 0; k < S; ++k) {
+                h[8 + 2 * k] = zeta_new[k].real(); h[8 + 2 * k + 1] = zeta_new[k].imag();
+                h[8 + 2 * S + 2 * k] = beta_k[k].real(); h[8 + 2 * S + 2 * k + 1] = beta_k[k].imag();
+                h[8 + 4 * S + 2 * k] = chi_k[k].real(); h[8 + 4 * S + 2 * k + 1] = chi_k[k].imag();
+            }
+        }
+        for (int k = 0; k < S; ++k) if (active[k]) { zeta_prev[k] = zeta[k]; zeta[k] = zeta_new[k]; rho[k] = rho_new[k]; }
+        delta = delta_new; alpha = alpha_new; beta_prev = beta; ++it;
+        const double rnorm = std::sqrt(rr);
+        if (!finite(rr)) { status = ST_BREAKDOWN; break; }
+        if (stop_rule == 1) {
+            if (rnorm <= tol * bnorm) { for (int k = 0; k < S; ++k) if (active[k]) { active[k] = 0; if (conv_iter) conv_iter[k] = it; } nactive = 0; }
+        } else {
+            for (int k = 0; k < S; ++k) if (active[k] && std::abs(zeta[k] * rho[k]) * rnorm <= tol * bnorm) {
+                active[k] = 0; --nactive; if (conv_iter) conv_iter[k] = it;
+                if (relres) relres[k] = std::abs(zeta[k] * rho[k]) * rnorm / bnorm;
+            }
+        }
+    }
+    const double rnorm = std::sqrt(rr);
+    for (int k = 0; k < S; ++k) {
+        if ((active[k] || stop_rule == 1) && relres) relres[k] = std::abs(zeta[k] * rho[k]) * rnorm / bnorm;
+        if (zeta_out) { const zdouble z = zeta[k] * rho[k]; zeta_out[2 * k] = z.real(); zeta_out[2 * k + 1] = z.imag(); }
+    }
+    if (r_out) std::memcpy((void*)r_out, (const void*)r.data(), sizeof(C) * n);
+    *iterations = it;
+    if (status == ST_BREAKDOWN) return status;
+    return nactive > 0 ? ST_MAXITER : ST_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// Plain CG on (A + sigma I), textbook form ([13]).  Pin only.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+int cg(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol, int max_iter,
+       std::complex<T>* x, int* iterations, double* relres) {
+    typedef std::complex<T> C;
+    const int64_t n = A.n;
+    std::vector<C> r(b, b + n), p(b, b + n), q(n);
+    for (int64_t i = 0; i < n; ++i) x[i] = C(0, 0);
+    double rr = dot(n, r.data(), r.data()).real();
+    const double bnorm = std::sqrt(rr);
+    int it = 0, status = ST_MAXITER;
+    if (bnorm == 0.0) { *iterations = 0; if (relres) *relres = 0.0; return ST_OK; }
+    while (it < max_iter) {
+        spmv(A, p.data(), q.data());
+        if (sigma != 0.0) { const C sg((T)sigma, 0); for (int64_t i = 0; i < n; ++i) q[i] = q[i] + sg * p[i]; }
+        const double pq = dot(n, p.data(), q.data()).real();
+        if (!(pq > 0.0)) { status = ST_BREAKDOWN; break; }
+        const double a = rr / pq;
+        const C ac((T)a, 0);
+        for (int64_t i = 0; i < n; ++i) x[i] = x[i] + ac * p[i];
+        for (int64_t i = 0; i < n; ++i) r[i] = r[i] - ac * q[i];
+        const double rr_new = dot(n, r.data(), r.data()).real();
+        const double bt = rr_new / rr;
+        const C bc((T)bt, 0);
+        for (int64_t i = 0; i < n; ++i) p[i] = r[i] + bc * p[i];
+        rr = rr_new; ++it;
+        if (std::sqrt(rr) <= tol * bnorm) { status = ST_OK; break; }
+    }
+    *iterations = it;
+    if (relres) *relres = std::sqrt(rr) / bnorm;
+    return status;
+}
+
+// ------------------------------------------------------------------------------------------
+// Plain BiCGStab on (A + sigma I), van der Vorst's form, shadow vector b.  Pin only.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+int bicgstab(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol, int max_iter,
+             std::complex<T>* x, int* iterations, double* relres) {
+    typedef std::complex<T> C;
+    const int64_t n = A.n;
+    std::vector<C> r(b, b + n), p(b, b + n), rhat(b, b + n), v(n), s(n), t(n);
+    for (int64_t i = 0; i < n; ++i) x[i] = C(0, 0);
+    zdouble rho = dot(n, rhat.data(), r.data());
+    double rr = rho.real();
+    const double bnorm = std::sqrt(rr);
+    int it = 0, status = ST_MAXITER;
+    if (bnorm == 0.0) { *iterations = 0; if (relres) *relres = 0.0; return ST_OK; }
+    const C sg((T)sigma, 0);
+    while (it < max_iter) {
+        spmv(A, p.data(), v.data());
+        if (sigma != 0.0) for (int64_t i = 0; i < n; ++i) v[i] = v[i] + sg * p[i];
+        const zdouble rv = dot(n, rhat.data(), v.data());
+        if (rv == zdouble(0, 0) || rho == zdouble(0, 0)) { status = ST_BREAKDOWN; break; }
+        const zdouble a = rho / rv;
+        const C ac = rnd<T>(a);
+        for (int64_t i = 0; i < n; ++i) s[i] = r[i] - ac * v[i];
+        spmv(A, s.data(), t.data());
+        if (sigma != 0.0) for (int64_t i = 0; i < n; ++i) t[i] = t[i] + sg * s[i];
+        const zdouble ts = dot(n, t.data(), s.data());
+        const double tt = dot(n, t.data(), t.data()).real();
+        if (!(tt > 0.0)) { status = ST_BREAKDOWN; break; }
+        const zdouble w = ts / tt;
+        const C wc = rnd<T>(w);
+        for (int64_t i = 0; i < n; ++i) x[i] = (x[i] + ac * p[i]) + wc * s[i];
+        for (int64_t i = 0; i < n; ++i) r[i] = s[i] - wc * t[i];
+        const zdouble rho_new = dot(n, rhat.data(), r.data());
+        const zdouble bt = (rho_new / rho) * (a / w);
+        const C bc = rnd<T>(bt);
+        for (int64_t i = 0; i < n; ++i) p[i] = r[i] + bc * (p[i] - wc * v[i]);
+        rho = rho_new; ++it;
+        rr = dot(n, r.data(), r.data()).real();
+        if (std::sqrt(rr) <= tol * bnorm) { status = ST_OK; break; }
+    }
+    *iterations = it;
+    if (relres) *relres = std::sqrt(rr) / bnorm;
+    return status;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------
+// C entry points (host pointers only).  dtype: 0 = complex64, 1 = complex128.
+// ------------------------------------------------------------------------------------------
+#define DISPATCH(call_f, call_d) (dtype == 0 ? (call_f) : dtype == 1 ? (call_d) : (int)ST_EINVAL)
+
+template <typename T>
+static Csr<T> mk(int64_t n, const int32_t* rp, const int32_t* ci, const void* v) {
+    Csr<T> A; A.n = n; A.rowptr = rp; A.colidx = ci; A.val = (const std::complex<T>*)v; return A;
+}
+
+extern "C" {
+
+int oracle_spmv_csr(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx,
+                    const void* val, const void* x, void* y) {
+    if (dtype == 0) { spmv(mk<float>(n, rowptr, colidx, val), (const std::complex<float>*)x, (std::complex<float>*)y); return 0; }
+    if (dtype == 1) { spmv(mk<double>(n, rowptr, colidx, val), (const std::complex<double>*)x, (std::complex<double>*)y); return 0; }
+    return ST_EINVAL;
+}
+
+int oracle_cgm(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
+               const void* b, const double* shifts, int nshifts, double tol, int max_iter, int stop_rule,
+               void* x, int* iterations, int* conv_iter, double* relres,
+               void* r_out, double* zeta_out, double* hist, int hist_cap) {
+    return DISPATCH(
+        cgm(mk<float>(n, rowptr, colidx, val), (const std::complex<float>*)b, shifts, nshifts, tol, max_iter, stop_rule,
+            (std::complex<float>*)x, iterations, conv_iter, relres, (std::complex<float>*)r_out, zeta_out, hist, hist_cap),
+        cgm(mk<double>(n, rowptr, colidx, val), (const std::complex<double>*)b, shifts, nshifts, tol, max_iter, stop_rule,
+            (std::complex<double>*)x, iterations, conv_iter, relres, (std::complex<double>*)r_out, zeta_out, hist, hist_cap));
+}
+
+int oracle_bicgstabm(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
+                     const void* b, const double* shifts, int nshifts, double tol, int max_iter, int stop_rule,
+                     void* x, int* iterations, int* conv_iter, double* relres,
+                     void* r_out, double* zeta_out, double* hist, int hist_cap) {
+    return DISPATCH(
+        bicgstabm(mk<float>(n, rowptr, colidx, val), (const std::complex<float>*)b, shifts, nshifts, tol, max_iter, stop_rule,
+                  (std::complex<float>*)x, iterations, conv_iter, relres, (std::complex<float>*)r_out, zeta_out, hist, hist_cap),
+        bicgstabm(mk<double>(n, rowptr, colidx, val), (const std::complex<double>*)b, shifts, nshifts, tol, max_iter, stop_rule,
+                  (std::complex<double>*)x, iterations, conv_iter, relres, (std::complex<double>*)r_out, zeta_out, hist, hist_cap));
+}
+
+int oracle_cg(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
+              double sigma, const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
+    return DISPATCH(
+        cg(mk<float>(n, rowptr, colidx, val), sigma, (const std::complex<float>*)b, tol, max_iter, (std::complex<float>*)x, iterations, relres),
+        cg(mk<double>(n, rowptr, colidx, val), sigma, (const std::complex<double>*)b, tol, max_iter, (std::complex<double>*)x, iterations, relres));
+}
+
+int oracle_bicgstab(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
+                    double sigma, const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
+    return DISPATCH(
+        bicgstab(mk<float>(n, rowptr, colidx, val), sigma, (const std::complex<float>*)b, tol, max_iter, (std::complex<float>*)x, iterations, relres),
+        bicgstab(mk<double>(n, rowptr, colidx, val), sigma, (const std::complex<double>*)b, tol, max_iter, (std::complex<double>*)x, iterations, relres));
+}
+
+}  // extern "C"
