@@ -1,0 +1,152 @@
+/* msolve.h -- C ABI of the B200-native multishift Krylov solvers CG-M and BiCGStab-M.
+ *
+ * The library solves the family of shifted systems of eq. (1), PAPER.md:41,
+ *
+ *        (A + sigma_k I) x_k = b ,   k = 0 .. nshifts-1 ,
+ *
+ * for all shifts from ONE Krylov sequence (eq. (4)): CG-M is Algorithm 1
+ * for Hermitian positive-definite A, BiCGStab-M is its
+ * non-Hermitian analogue.  The argument lists follow the paper's statement of the problem and
+ * the call of Fig. 1: a sparse A, a right-hand side b of length n, an array
+ * of shifts, a relative tolerance and an iteration limit (the paper's
+ * `default_monitor(b, 2000, 1e-5)`) and ONE output array of n*nshifts holding one
+ * solution per shift.  The initial guess is zero by construction of the method
+ * (PAPER.md:97, 232).
+ *
+ * Everything on the iteration path runs in hand-written sm_100a kernels; the whole iteration
+ * is captured in a CUDA graph and loops on the device without host synchronisation
+ * (the paper's "entire solution on the GPU").
+ *
+ * Conventions
+ *  - Plain C, no exceptions.  Every int-returning call returns an MSOLVE_* status code;
+ *    msolve_last_error() gives the text of the last failure of the calling thread.
+ *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  Device buffers are owned
+ *    by the caller (e.g. torch tensors); the library never frees them.
+ *  - Complex numbers are interleaved (re, im) pairs of float (MSOLVE_C64) or double
+ *    (MSOLVE_C128).  Indices are int32.  All device arrays must be 16-byte aligned.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *  - A handle may be used by one solve at a time (it owns the device-side solver state and the
+ *    cached CUDA graphs); different handles are independent.
+ */
+#ifndef MSOLVE_H
+#define MSOLVE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct msolve_matrix msolve_matrix; /* opaque */
+
+enum { MSOLVE_C64 = 0, MSOLVE_C128 = 1 };
+
+enum { MSOLVE_ALG_CGM = 0, MSOLVE_ALG_BICGSTABM = 1 };
+
+/* Status codes.  > 0: x is valid but the solve did not end with every shift converged. */
+enum {
+    MSOLVE_OK = 0,         /* every shift reached |zeta_k| ||r|| <= tol ||b||                      */
+    MSOLVE_MAXITER = 1,    /* iteration limit reached first                                        */
+    MSOLVE_BREAKDOWN = 2,  /* <p,Ap> <= 0, <r0,Ap> = 0, <t,t> = 0, zero zeta denominator, NaN/Inf */
+    MSOLVE_EINVAL = -1,    /* bad argument (nothing was launched)                                  */
+    MSOLVE_ECUDA = -2,     /* a CUDA call failed; see msolve_last_error()                          */
+    MSOLVE_ENOMEM = -3     /* workspace too small / allocation failed                              */
+};
+
+/* create-time flags: SpMV kernel choice for CSR (Alg. 1 l.18). */
+enum {
+    MSOLVE_SPMV_AUTO = 0,    /* vector kernel for short regular rows, merge-path otherwise */
+    MSOLVE_SPMV_VECTOR = 1,  /* sub-warp-per-row vector-CSR                                 */
+    MSOLVE_SPMV_MERGE = 2    /* merge-path CSR (load-balanced over rows + non-zeros)        */
+};
+
+#define MSOLVE_MAX_SHIFTS 128
+
+/* msolve_config keys */
+enum {
+    MSOLVE_CFG_LOOP_MODE = 0 /* 0 = device WHILE graph node (default), 1 = chunked relaunch of an
+                                unrolled iteration graph with a device `done` flag */
+};
+
+/* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay
+ * valid and unchanged until msolve_destroy.  Column indices must lie in [0, n).  May allocate
+ * library-owned auxiliary device data (merge-path partition table, solver state).
+ * Errors: EINVAL (null pointer, n < 0, nnz < 0, bad dtype/flags, nnz >= 2^31), ECUDA, ENOMEM. */
+int msolve_create_csr(msolve_matrix **A, int64_t n, int64_t nnz,
+                      const int32_t *d_rowptr /* n+1 */, const int32_t *d_colidx /* nnz */,
+                      const void *d_val /* nnz complex */, int dtype, int flags, void *stream);
+
+/* Build a handle for a 3x3-block BSR matrix (3*nbrows x 3*nbrows), the SU(3) layout:
+ * block k is 9 complex numbers, row-major 3x3, at d_blocks + 9*k.  Same borrowing rules. */
+int msolve_create_bsr3(msolve_matrix **A, int64_t nbrows, int64_t nblocks,
+                       const int32_t *d_browptr /* nbrows+1 */, const int32_t *d_bcolidx /* nblocks */,
+                       const void *d_blocks /* nblocks*9 complex */, int dtype, int flags, void *stream);
+
+/* Bytes of caller-provided device workspace a solve with `nshifts` shifts needs
+ * (r, p, Ap [, s, t] and one search direction p_k per shift, Alg. 1 l.10-11).  0 on bad input. */
+size_t msolve_workspace_bytes(const msolve_matrix *A, int nshifts, int algorithm);
+
+/* CG-M, Algorithm 1 as read in DESIGN.md ("Readings of the paper").
+ *   d_b          in   n complex, device.  Not modified.
+ *   h_shifts     in   nshifts real shifts sigma_k (host), any order, 1 <= nshifts <= MSOLVE_MAX_SHIFTS.
+ *   tol          in   relative tolerance: shift k stops (and x_k is frozen) at the first iteration
+ *                     with |zeta_k| ||r|| <= tol ||b||; the solve ends when all shifts stopped.
+ *   max_iter     in   limit on loop bodies (one SpMV each for CG-M, two for BiCGStab-M).
+ *   d_x          out  nshifts*n complex, device, shift-major: x_k[i] at d_x[k*n + i].  Fully
+ *                     overwritten (zero initial guess is part of the method).
+ *   d_workspace       device scratch of >= msolve_workspace_bytes(), 256-byte aligned.
+ *   h_iterations out  loop bodies executed (may be NULL).
+ *   h_conv_iter  out  nshifts ints: iteration at which shift k converged, -1 if it did not (or NULL).
+ *   h_relres     out  nshifts doubles: recurrence residual |zeta_k| ||r|| / ||b|| when shift k
+ *                     stopped / at exit (or NULL).
+ * Host outputs are written after ONE stream synchronisation at the end of the solve; there is no
+ * host synchronisation per iteration.  Returns OK / MAXITER / BREAKDOWN or a negative error. */
+int msolve_cgm(const msolve_matrix *A, const void *d_b, const double *h_shifts, int nshifts,
+               double tol, int max_iter, void *d_x, void *d_workspace, size_t workspace_bytes,
+               int *h_iterations, int *h_conv_iter, double *h_relres, void *stream);
+
+/* BiCGStab-M (derivation in DESIGN.md), shadow vector r0 = b.  Same arguments.
+ * Stop test per shift: |zeta_k rho_k| ||r|| <= tol ||b||, evaluated at the end of a full iteration. */
+int msolve_bicgstabm(const msolve_matrix *A, const void *d_b, const double *h_shifts, int nshifts,
+                     double tol, int max_iter, void *d_x, void *d_workspace, size_t workspace_bytes,
+                     int *h_iterations, int *h_conv_iter, double *h_relres, void *stream);
+
+/* The call of Fig. 1 with HOST vectors: copies h_b to the device, solves,
+ * copies all nshifts*n solutions back to h_x (both inside the call, on `stream`).  The library
+ * allocates and frees the device vectors and workspace itself.  algorithm = MSOLVE_ALG_*. */
+int msolve_solve_host(const msolve_matrix *A, int algorithm, const void *h_b, const double *h_shifts,
+                      int nshifts, double tol, int max_iter, void *h_x,
+                      int *h_iterations, int *h_conv_iter, double *h_relres, void *stream);
+
+/* One SpMV y = A x with the fused reduction of the CG-M step (Alg. 1 l.18-19):
+ * h_dot[0..1] receives <x, A x> = sum_i conj(x_i) y_i (may be NULL).  d_x, d_y: n complex, device.
+ * Exposed for parity tests of the SpMV kernels and for per-kernel timing. */
+int msolve_spmv(const msolve_matrix *A, const void *d_x, void *d_y, double *h_dot, void *stream);
+
+/* Per-kernel timing of `iters` steady-state iterations (no convergence test, all shifts active),
+ * each kernel bracketed by CUDA events on `stream`.  h_ms[j] receives the mean duration in ms of
+ * kernel j, h_launches[j] its launches per iteration; names via msolve_kernel_name(algorithm, j).
+ * Returns the number of kernels (<= 8) or a negative error.  d_x / workspace as for the solvers. */
+int msolve_profile_iteration(const msolve_matrix *A, int algorithm, const void *d_b,
+                             const double *h_shifts, int nshifts, int iters, void *d_x,
+                             void *d_workspace, size_t workspace_bytes,
+                             float *h_ms /* 8 */, int *h_launches /* 8 */, void *stream);
+const char *msolve_kernel_name(int algorithm, int j);
+
+/* Kernel launches issued (graph kernel nodes executed) by the last solve on this handle. */
+int64_t msolve_last_launch_count(const msolve_matrix *A);
+
+/* Process-wide options (MSOLVE_CFG_*).  Returns MSOLVE_OK or MSOLVE_EINVAL. */
+int msolve_config(int key, int value);
+
+/* Free the handle and everything the library allocated for it (never the caller's arrays). */
+void msolve_destroy(msolve_matrix *A);
+
+/* Text of the last error on this thread ("" if none).  Never NULL. */
+const char *msolve_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MSOLVE_H */

@@ -1,0 +1,273 @@
+"""Thin Python binding of the C ABI in include/msolve.h (argument marshalling only).
+
+Same names as the C entry points.  PyTorch is used for device memory and streams; every step
+of the solver path runs inside libmsolve.so's CUDA kernels.  There is NO fallback: if the
+library is missing or fails to load, every call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmsolve.so")
+
+MSOLVE_C64, MSOLVE_C128 = 0, 1
+MSOLVE_ALG_CGM, MSOLVE_ALG_BICGSTABM = 0, 1
+MSOLVE_OK, MSOLVE_MAXITER, MSOLVE_BREAKDOWN = 0, 1, 2
+MSOLVE_EINVAL, MSOLVE_ECUDA, MSOLVE_ENOMEM = -1, -2, -3
+MSOLVE_SPMV_AUTO, MSOLVE_SPMV_VECTOR, MSOLVE_SPMV_MERGE = 0, 1, 2
+MSOLVE_MAX_SHIFTS = 128
+MSOLVE_CFG_LOOP_MODE = 0
+
+EXPORTS = (
+    "msolve_create_csr", "msolve_create_bsr3", "msolve_workspace_bytes", "msolve_cgm",
+    "msolve_bicgstabm", "msolve_solve_host", "msolve_spmv", "msolve_profile_iteration",
+    "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_destroy",
+    "msolve_last_error",
+)
+
+_lib = None
+
+
+class MsolveError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__("msolve error %d: %s" % (code, text))
+        self.code = code
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libmsolve.so and declare the prototypes.  Raises if it is not there."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("libmsolve.so is not built (run `python -m paper_1102_2143_b200.build` "
+                           "or __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64, dbl, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_size_t
+    lib.msolve_create_csr.argtypes = [ctypes.POINTER(vp), i64, i64, vp, vp, vp, i32, i32, vp]
+    lib.msolve_create_bsr3.argtypes = [ctypes.POINTER(vp), i64, i64, vp, vp, vp, i32, i32, vp]
+    lib.msolve_workspace_bytes.argtypes = [vp, i32, i32]
+    lib.msolve_workspace_bytes.restype = sz
+    solver_args = [vp, vp, vp, i32, dbl, i32, vp, vp, sz, vp, vp, vp, vp]
+    lib.msolve_cgm.argtypes = solver_args
+    lib.msolve_bicgstabm.argtypes = solver_args
+    lib.msolve_solve_host.argtypes = [vp, i32, vp, vp, i32, dbl, i32, vp, vp, vp, vp, vp]
+    lib.msolve_spmv.argtypes = [vp, vp, vp, vp, vp]
+    lib.msolve_profile_iteration.argtypes = [vp, i32, vp, vp, i32, i32, vp, vp, sz, vp, vp, vp]
+    lib.msolve_kernel_name.argtypes = [i32, i32]
+    lib.msolve_kernel_name.restype = ctypes.c_char_p
+    lib.msolve_last_launch_count.argtypes = [vp]
+    lib.msolve_last_launch_count.restype = i64
+    lib.msolve_config.argtypes = [i32, i32]
+    lib.msolve_destroy.argtypes = [vp]
+    lib.msolve_destroy.restype = None
+    lib.msolve_last_error.restype = ctypes.c_char_p
+    for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_cgm", "msolve_bicgstabm",
+                 "msolve_solve_host", "msolve_spmv", "msolve_profile_iteration", "msolve_config"):
+        getattr(lib, name).restype = i32
+    _lib = lib
+    return lib
+
+
+def msolve_last_error() -> str:
+    return load_library().msolve_last_error().decode()
+
+
+def _check(rc: int) -> int:
+    if rc < 0:
+        raise MsolveError(rc, msolve_last_error())
+    return rc
+
+
+def _dtype_code(t: torch.Tensor) -> int:
+    if t.dtype == torch.complex64:
+        return MSOLVE_C64
+    if t.dtype == torch.complex128:
+        return MSOLVE_C128
+    raise TypeError("expected complex64 / complex128, got %s" % t.dtype)
+
+
+def _dev(t: torch.Tensor, dtype=None) -> torch.Tensor:
+    if not t.is_cuda:
+        raise ValueError("expected a CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError("expected %s, got %s" % (dtype, t.dtype))
+    return t.contiguous()
+
+
+def _stream(stream) -> int:
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+class Matrix:
+    """Owner of an `msolve_matrix*`; keeps the borrowed device arrays alive."""
+
+    def __init__(self, handle: int, dtype: torch.dtype, n: int, keep):
+        self.handle = ctypes.c_void_p(handle)
+        self.dtype = dtype
+        self.n = n
+        self._keep = keep
+
+    def destroy(self):
+        if self.handle:
+            load_library().msolve_destroy(self.handle)
+            self.handle = None
+            self._keep = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def msolve_create_csr(rowptr: torch.Tensor, colidx: torch.Tensor, val: torch.Tensor,
+                      flags: int = MSOLVE_SPMV_AUTO, stream=None) -> Matrix:
+    lib = load_library()
+    rowptr, colidx, val = _dev(rowptr, torch.int32), _dev(colidx, torch.int32), _dev(val)
+    h = ctypes.c_void_p()
+    n = rowptr.numel() - 1
+    _check(lib.msolve_create_csr(ctypes.byref(h), n, colidx.numel(), rowptr.data_ptr(), colidx.data_ptr(),
+                                 val.data_ptr(), _dtype_code(val), flags, _stream(stream)))
+    return Matrix(h.value, val.dtype, n, (rowptr, colidx, val))
+
+
+def msolve_create_bsr3(browptr: torch.Tensor, bcolidx: torch.Tensor, blocks: torch.Tensor,
+                       flags: int = 0, stream=None) -> Matrix:
+    lib = load_library()
+    browptr, bcolidx, blocks = _dev(browptr, torch.int32), _dev(bcolidx, torch.int32), _dev(blocks)
+    if blocks.numel() != 9 * bcolidx.numel():
+        raise ValueError("blocks must hold 9 complex numbers per block")
+    h = ctypes.c_void_p()
+    nbrows = browptr.numel() - 1
+    _check(lib.msolve_create_bsr3(ctypes.byref(h), nbrows, bcolidx.numel(), browptr.data_ptr(), bcolidx.data_ptr(),
+                                  blocks.data_ptr(), _dtype_code(blocks), flags, _stream(stream)))
+    return Matrix(h.value, blocks.dtype, 3 * nbrows, (browptr, bcolidx, blocks))
+
+
+def msolve_destroy(A: Matrix) -> None:
+    A.destroy()
+
+
+def msolve_workspace_bytes(A: Matrix, nshifts: int, algorithm: int) -> int:
+    return int(load_library().msolve_workspace_bytes(A.handle, nshifts, algorithm))
+
+
+def msolve_config(key: int, value: int) -> None:
+    _check(load_library().msolve_config(key, value))
+
+
+def msolve_last_launch_count(A: Matrix) -> int:
+    return int(load_library().msolve_last_launch_count(A.handle))
+
+
+@dataclass
+class SolveResult:
+    status: int
+    iterations: int
+    x: torch.Tensor            # [S, n] on the device (host tensor for msolve_solve_host)
+    conv_iter: np.ndarray      # int32 [S]
+    relres: np.ndarray         # float64 [S]
+
+
+def _solve(fn_name: str, algorithm: int, A: Matrix, b: torch.Tensor, shifts: Sequence[float], tol: float,
+           max_iter: int, x: Optional[torch.Tensor], workspace: Optional[torch.Tensor], stream) -> SolveResult:
+    lib = load_library()
+    b = _dev(b, A.dtype)
+    if b.numel() != A.n:
+        raise ValueError("b has %d elements, matrix has %d rows" % (b.numel(), A.n))
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    s = sh.size
+    if x is None:
+        x = torch.empty((s, A.n), dtype=A.dtype, device=b.device)
+    x = _dev(x, A.dtype)
+    if x.numel() != s * A.n:
+        raise ValueError("x must hold nshifts*n elements")
+    need = msolve_workspace_bytes(A, s, algorithm)
+    if need == 0:
+        raise MsolveError(MSOLVE_EINVAL, "nshifts must be in [1, %d]" % MSOLVE_MAX_SHIFTS)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=b.device)
+    it = ctypes.c_int(0)
+    conv = np.full(s, -1, dtype=np.int32)
+    rel = np.zeros(s, dtype=np.float64)
+    rc = getattr(lib, fn_name)(A.handle, b.data_ptr(), sh.ctypes.data, s, float(tol), int(max_iter), x.data_ptr(),
+                               workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                               ctypes.addressof(it), conv.ctypes.data, rel.ctypes.data, _stream(stream))
+    _check(rc)
+    return SolveResult(rc, it.value, x.view(s, A.n), conv, rel)
+
+
+def msolve_cgm(A: Matrix, b: torch.Tensor, shifts, tol: float, max_iter: int, x: Optional[torch.Tensor] = None,
+               workspace: Optional[torch.Tensor] = None, stream=None) -> SolveResult:
+    """CG-M (Alg. 1): solve (A + shifts[k] I) x[k] = b for every k."""
+    return _solve("msolve_cgm", MSOLVE_ALG_CGM, A, b, shifts, tol, max_iter, x, workspace, stream)
+
+
+def msolve_bicgstabm(A: Matrix, b: torch.Tensor, shifts, tol: float, max_iter: int, x: Optional[torch.Tensor] = None,
+                     workspace: Optional[torch.Tensor] = None, stream=None) -> SolveResult:
+    """BiCGStab-M."""
+    return _solve("msolve_bicgstabm", MSOLVE_ALG_BICGSTABM, A, b, shifts, tol, max_iter, x, workspace, stream)
+
+
+def msolve_solve_host(A: Matrix, algorithm: int, b: torch.Tensor, shifts, tol: float, max_iter: int,
+                      x: Optional[torch.Tensor] = None, stream=None) -> SolveResult:
+    """Fig. 1's call shape with HOST vectors: b and x are CPU tensors
+    (pinned for full copy speed); H2D of b and D2H of all solutions happen inside the call."""
+    lib = load_library()
+    if b.is_cuda or b.dtype != A.dtype:
+        raise ValueError("b must be a CPU tensor of the matrix dtype")
+    b = b.contiguous()
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    s = sh.size
+    if x is None:
+        x = torch.empty((s, A.n), dtype=A.dtype, pin_memory=True)
+    if x.is_cuda or x.dtype != A.dtype or x.numel() != s * A.n or not x.is_contiguous():
+        raise ValueError("x must be a contiguous CPU tensor of nshifts*n elements")
+    it = ctypes.c_int(0)
+    conv = np.full(s, -1, dtype=np.int32)
+    rel = np.zeros(s, dtype=np.float64)
+    rc = lib.msolve_solve_host(A.handle, algorithm, b.data_ptr(), sh.ctypes.data, s, float(tol), int(max_iter),
+                               x.data_ptr(), ctypes.addressof(it), conv.ctypes.data, rel.ctypes.data, _stream(stream))
+    _check(rc)
+    return SolveResult(rc, it.value, x.view(s, A.n), conv, rel)
+
+
+def msolve_spmv(A: Matrix, x: torch.Tensor, y: Optional[torch.Tensor] = None, stream=None):
+    """y = A x and <x, A x> (Alg. 1 l.18-19).  Returns (y, complex dot)."""
+    lib = load_library()
+    x = _dev(x, A.dtype)
+    if y is None:
+        y = torch.empty_like(x)
+    dot = np.zeros(2, dtype=np.float64)
+    _check(lib.msolve_spmv(A.handle, x.data_ptr(), y.data_ptr(), dot.ctypes.data, _stream(stream)))
+    return y, complex(dot[0], dot[1])
+
+
+def msolve_profile_iteration(A: Matrix, algorithm: int, b: torch.Tensor, shifts, iters: int,
+                             x: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None, stream=None):
+    """Mean per-kernel milliseconds of `iters` steady-state iterations -> {kernel name: ms}."""
+    lib = load_library()
+    b = _dev(b, A.dtype)
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    s = sh.size
+    if x is None:
+        x = torch.empty((s, A.n), dtype=A.dtype, device=b.device)
+    need = msolve_workspace_bytes(A, s, algorithm)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=b.device)
+    ms = np.zeros(8, dtype=np.float32)
+    nl = np.zeros(8, dtype=np.int32)
+    nk = _check(lib.msolve_profile_iteration(A.handle, algorithm, b.data_ptr(), sh.ctypes.data, s, int(iters),
+                                             x.data_ptr(), workspace.data_ptr(), workspace.numel(),
+                                             ms.ctypes.data, nl.ctypes.data, _stream(stream)))
+    return {lib.msolve_kernel_name(algorithm, j).decode(): float(ms[j]) for j in range(nk)}

@@ -1,0 +1,184 @@
+// common.cuh -- shared device helpers for the msolve kernels (sm_100a).
+// Complex arithmetic on interleaved (re,im) pairs, streaming load/store wrappers, deterministic
+// block reductions and the device-resident solver state (the zeta /
+// alpha / beta recurrences never leave the GPU).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/msolve.h"
+
+namespace msolve {
+
+constexpr int kMaxShifts = MSOLVE_MAX_SHIFTS;
+constexpr int kMaxPartials = 4096;  // upper bound on any reducing kernel's grid size
+constexpr int kAccMax = 5;          // doubles reduced per CTA (BiCGStab-M SpMV#2 needs 5)
+constexpr int kThreads = 256;
+
+// ----------------------------------------------------------------------------- complex types
+template <typename T> struct Cx;
+template <> struct Cx<float> { typedef float2 type; };
+template <> struct Cx<double> { typedef double2 type; };
+
+template <typename C> __device__ __forceinline__ C cmake(double re, double im);
+template <> __device__ __forceinline__ float2 cmake<float2>(double re, double im) { return make_float2((float)re, (float)im); }
+template <> __device__ __forceinline__ double2 cmake<double2>(double re, double im) { return make_double2(re, im); }
+
+template <typename C> __device__ __forceinline__ C cadd(C a, C b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
+template <typename C> __device__ __forceinline__ C csub(C a, C b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
+template <typename C> __device__ __forceinline__ C cmul(C a, C b) { C r; r.x = a.x * b.x - a.y * b.y; r.y = a.x * b.y + a.y * b.x; return r; }
+// acc + a*b
+template <typename C> __device__ __forceinline__ C cfma(C a, C b, C acc) {
+    acc.x += a.x * b.x; acc.x -= a.y * b.y;
+    acc.y += a.x * b.y; acc.y += a.y * b.x;
+    return acc;
+}
+// a + s*b with real s
+template <typename C, typename S> __device__ __forceinline__ C caxpy_r(C a, S s, C b) { C r; r.x = a.x + s * b.x; r.y = a.y + s * b.y; return r; }
+
+// ----------------------------------------------------------------------------- memory access
+// Streaming (touched once per iteration, far larger than L2): evict-first loads / stores.
+template <typename V> __device__ __forceinline__ V ld_stream(const V* p) { return __ldcs(p); }
+template <typename V> __device__ __forceinline__ void st_stream(V* p, V v) { __stcs(p, v); }
+// Read-only data reused by neighbouring rows / the next kernel: default caching, nc path.
+template <typename V> __device__ __forceinline__ V ld_ro(const V* p) { return __ldg(p); }
+
+// ----------------------------------------------------------------------------- reductions
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Fixed-order CTA reduction of NACC doubles per thread; result valid in thread 0.
+template <int NACC>
+__device__ __forceinline__ void block_sum(double (&acc)[NACC], double* smem /* NACC * 32 */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = warp_sum(acc[a]);
+    if (lane == 0) {
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) smem[a * 32 + warp] = acc[a];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) {
+            double v = lane < nwarp ? smem[a * 32 + lane] : 0.0;
+            acc[a] = warp_sum(v);
+        }
+    }
+}
+
+// ----------------------------------------------------------------------------- solver state
+struct zd { double re, im; };  // complex double scalar on the device
+
+__device__ __forceinline__ zd zmul(zd a, zd b) { return {a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re}; }
+__device__ __forceinline__ zd zadd(zd a, zd b) { return {a.re + b.re, a.im + b.im}; }
+__device__ __forceinline__ zd zsub(zd a, zd b) { return {a.re - b.re, a.im - b.im}; }
+__device__ __forceinline__ zd zneg(zd a) { return {-a.re, -a.im}; }
+__device__ __forceinline__ zd zscale(zd a, double s) { return {a.re * s, a.im * s}; }
+__device__ __forceinline__ zd zdiv(zd a, zd b) {  // Smith's algorithm
+    if (fabs(b.re) >= fabs(b.im)) {
+        const double r = b.im / b.re, d = b.re + b.im * r;
+        return {(a.re + a.im * r) / d, (a.im - a.re * r) / d};
+    }
+    const double r = b.re / b.im, d = b.re * r + b.im;
+    return {(a.re * r + a.im) / d, (a.im * r - a.re) / d};
+}
+__device__ __forceinline__ double zabs(zd a) { return hypot(a.re, a.im); }
+__device__ __forceinline__ bool zfinite(zd a) { return isfinite(a.re) && isfinite(a.im); }
+__device__ __forceinline__ bool zzero(zd a) { return a.re == 0.0 && a.im == 0.0; }
+
+// Everything the iteration kernels need, resident in device memory for the whole solve.
+// Pointers are read from here (not baked into kernel arguments) so one captured CUDA graph per
+// handle serves every call.  Layout: [header: written by the host before a solve]
+// [result: read back by the host after it] [device-only scratch].
+struct SolveHeader {
+    // vectors (complex<T>, T from the handle's dtype)
+    const void* b;   // rhs; also the BiCGStab-M shadow vector r0
+    void* x;         // [S][n] shift-major, caller's output
+    void* r;         // base residual
+    void* p;         // base search direction
+    void* q;         // A p
+    void* s;         // BiCGStab-M: s = r + beta q
+    void* t;         // BiCGStab-M: t = A s
+    void* pk;        // [S][pk_stride] per-shift search directions
+    // generic SpMV roles (msolve_spmv)
+    const void* sp_x; void* sp_y; const void* sp_u;
+    long long n;
+    long long pk_stride;
+    double tol;
+    int S;
+    int max_iter;
+    int force_all;   // profiling: never converge, never stop before max_iter
+    int pad0;
+    double sigma[kMaxShifts];
+};
+
+struct SolveResult {
+    int n_iter;
+    int done;
+    int status;
+    int nactive;
+    int zero_rhs;
+    int pad1;
+    int conv_iter[kMaxShifts];
+    double relres[kMaxShifts];
+};
+
+struct SolveState {
+    SolveHeader h;
+    SolveResult res;
+    // base scalars (CG-M uses .re only)
+    zd alpha, beta, beta_prev, delta, chi, alpha_new, delta_new;
+    double R0, R1, bnorm;
+    // per shift
+    zd zeta_prev[kMaxShifts], zeta[kMaxShifts], zeta_new[kMaxShifts];
+    zd rho[kMaxShifts], rho_new[kMaxShifts];
+    zd beta_k[kMaxShifts], alpha_k[kMaxShifts], chi_k[kMaxShifts];
+    int active[kMaxShifts];      // compact list of active shift indices, length res.nactive
+    // per-ACTIVE-shift coefficients consumed by the fused update kernels (index = position in
+    // `active`): CG-M uses 3 reals (zeta, alpha_k, beta_k); BiCGStab-M 7 complex.
+    double coef[kMaxShifts * 14];
+    // per-CTA partial sums of the fused reductions, [kAccMax][kMaxPartials]
+    double partial[kAccMax * kMaxPartials];
+    int partial_count;           // how many CTAs wrote partials in the last reducing kernel
+};
+
+// Fixed-order reduction of the per-CTA partials by ONE CTA (deterministic for a fixed grid).
+template <int NACC>
+__device__ __forceinline__ void reduce_partials(const SolveState* st, double (&out)[NACC], double* smem) {
+    const int count = st->partial_count;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    for (int i = threadIdx.x; i < count; i += blockDim.x) {
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) acc[a] += st->partial[a * kMaxPartials + i];
+    }
+    block_sum<NACC>(acc, smem);
+    __shared__ double bc[kAccMax];
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) bc[a] = acc[a];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) out[a] = bc[a];
+}
+
+// Matrix description passed by value to the SpMV kernels.
+struct MatDev {
+    const int32_t* rowptr;   // CSR: n+1 ; BSR3: nbrows+1
+    const int32_t* colidx;   // CSR: nnz ; BSR3: nblocks (block column)
+    const void* val;         // CSR: nnz complex ; BSR3: nblocks*9 complex
+    long long n;             // scalar rows
+    long long nbrows;        // BSR3 block rows (0 for CSR)
+    long long nnz;           // CSR nnz / BSR3 blocks
+    const int32_t* aux;      // merge-path partition table / BSR tile table
+    int aux_count;
+};
+
+}  // namespace msolve

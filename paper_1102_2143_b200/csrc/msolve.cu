@@ -1,0 +1,494 @@
+// msolve.cu -- C ABI (include/msolve.h) and host-side driver of the multishift solvers.
+//
+// The host does three things per solve: copy a ~1.6 KB header (pointers, n, shifts, tol) into the
+// handle's device-resident SolveState, launch two init kernels and ONE CUDA graph whose WHILE
+// node iterates the captured kernel sequence on the device until the device-side stop test
+// clears the condition ("entire solution on the GPU"),
+// then read back a ~1.6 KB result block after a single stream synchronisation.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+#include "kernels.cuh"
+#include "spmv.cuh"
+
+using namespace msolve;
+
+// ------------------------------------------------------------------------------------- errors
+static thread_local char g_err[512] = "";
+static int g_loop_mode = 0;
+
+static int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(MSOLVE_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+    } while (0)
+
+// ------------------------------------------------------------------------------------- handle
+enum { FMT_CSR = 0, FMT_BSR3 = 1 };
+enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3 };
+constexpr int kChunk = 8;  // iteration bodies per graph launch in chunked mode
+
+struct LoopGraph {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    int mode = -1;
+};
+
+struct msolve_matrix {
+    int format = FMT_CSR;
+    int dtype = MSOLVE_C128;
+    int kernel = KERNEL_VECTOR;
+    int lanes = 8;
+    MatDev dev{};
+    int device = 0;
+    int num_sms = 148;
+    SolveState* d_state = nullptr;      // library-owned
+    SolveState* h_stage = nullptr;      // pinned staging for header / result
+    void* d_aux = nullptr;              // library-owned auxiliary matrix data
+    cudaStream_t capture_stream = nullptr;
+    LoopGraph graphs[2];
+    int64_t last_launches = 0;
+};
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+static size_t elem_bytes(int dtype) { return dtype == MSOLVE_C64 ? 8 : 16; }
+
+// ------------------------------------------------------------------------------------- launch
+template <typename K>
+static int blocks_per_sm(K kernel) {
+    int nb = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, kThreads, 0) != cudaSuccess || nb < 1) nb = 1;
+    return nb;
+}
+
+// persistent grid: enough CTAs for `work_items` at `items_per_cta`, capped at full occupancy
+template <typename K>
+static int grid_for(const msolve_matrix* A, K kernel, long long work_items, long long items_per_cta) {
+    long long full = (long long)A->num_sms * blocks_per_sm(kernel);
+    long long need = (work_items + items_per_cta - 1) / items_per_cta;
+    long long g = std::max(1ll, std::min(full, need));
+    return (int)std::min<long long>(g, kMaxPartials);
+}
+
+template <typename T, int ROLE>
+static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
+    if (A->format == FMT_BSR3) {
+        auto k = k_spmv_bsr3_rows<T, ROLE>;
+        k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
+        return;
+    }
+#define VEC_CASE(L)                                                                                     \
+    case L: {                                                                                           \
+        auto k = k_spmv_csr_vector<T, L, ROLE>;                                                         \
+        k<<<grid_for(A, k, A->dev.n, kThreads / L), kThreads, 0, s>>>(A->dev, A->d_state);              \
+        break;                                                                                          \
+    }
+    switch (A->lanes) {
+        VEC_CASE(2) VEC_CASE(4) VEC_CASE(8) VEC_CASE(16) VEC_CASE(32)
+        default: break;
+    }
+#undef VEC_CASE
+}
+
+template <int ROLE>
+static void launch_spmv(const msolve_matrix* A, cudaStream_t s) {
+    if (A->dtype == MSOLVE_C64) launch_spmv_t<float, ROLE>(A, s);
+    else launch_spmv_t<double, ROLE>(A, s);
+}
+
+// element-wise kernels: VEC complex per 16-byte access when the length allows it
+static int vec_width(const msolve_matrix* A) { return (A->dtype == MSOLVE_C64 && (A->dev.n % 2 == 0)) ? 2 : 1; }
+
+#define DISPATCH_VEC(A, KERNEL, ...)                                                       \
+    do {                                                                                   \
+        if ((A)->dtype == MSOLVE_C128) { KERNEL(double, 1, __VA_ARGS__); }                 \
+        else if (vec_width(A) == 2) { KERNEL(float, 2, __VA_ARGS__); }                     \
+        else { KERNEL(float, 1, __VA_ARGS__); }                                            \
+    } while (0)
+
+constexpr int kUnrollCgm = 4;
+constexpr int kUnrollBi = 2;
+
+#define L_INIT(T, V, A, s) { auto k = k_init_vectors<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
+#define L_PUPD(T, V, A, s) { auto k = k_cgm_pupdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
+#define L_CUPD(T, V, A, s) { auto k = k_cgm_update<T, V, kUnrollCgm>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
+#define L_SUPD(T, V, A, s) { auto k = k_bi_supdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
+#define L_BUPD(T, V, A, s) { auto k = k_bi_update<T, V, kUnrollBi>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
+
+static const char* kCgmNames[] = {"cgm_pupdate", "spmv_dot", "cgm_scal1", "cgm_update", "cgm_scal2"};
+static const char* kBiNames[] = {"spmv1_dot", "bi_scal1", "bi_supdate", "spmv2_dots", "bi_scal2", "bi_update", "bi_scal3"};
+static int kernels_per_iter(int alg) { return alg == MSOLVE_ALG_CGM ? 5 : 7; }
+
+// One kernel of the iteration body.  Used for graph capture, and one-by-one for profiling.
+static void launch_body_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s,
+                               cudaGraphConditionalHandle cond, int use_cond) {
+    SolveState* st = A->d_state;
+    if (alg == MSOLVE_ALG_CGM) {
+        switch (j) {
+            case 0: DISPATCH_VEC(A, L_PUPD, A, s); break;
+            case 1: launch_spmv<ROLE_CG>(A, s); break;
+            case 2: k_cgm_scal1<<<1, kThreads, 0, s>>>(st); break;
+            case 3: DISPATCH_VEC(A, L_CUPD, A, s); break;
+            case 4: k_cgm_scal2<<<1, kThreads, 0, s>>>(st, cond, use_cond); break;
+        }
+    } else {
+        switch (j) {
+            case 0: launch_spmv<ROLE_B1>(A, s); break;
+            case 1: k_bi_scal1<<<1, kThreads, 0, s>>>(st); break;
+            case 2: DISPATCH_VEC(A, L_SUPD, A, s); break;
+            case 3: launch_spmv<ROLE_B2>(A, s); break;
+            case 4: k_bi_scal2<<<1, kThreads, 0, s>>>(st); break;
+            case 5: DISPATCH_VEC(A, L_BUPD, A, s); break;
+            case 6: k_bi_scal3<<<1, kThreads, 0, s>>>(st, cond, use_cond); break;
+        }
+    }
+}
+
+static void launch_init(const msolve_matrix* A, cudaStream_t s) {
+    DISPATCH_VEC(A, L_INIT, A, s);
+    k_init_state<<<1, kThreads, 0, s>>>(A->d_state);
+}
+
+// ------------------------------------------------------------------------------------- graph
+static int build_graph(msolve_matrix* A, int alg, int mode) {
+    LoopGraph& g = A->graphs[alg];
+    if (g.exec && g.mode == mode) return MSOLVE_OK;
+    if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
+    if (g.graph) { cudaGraphDestroy(g.graph); g.graph = nullptr; }
+    const int nk = kernels_per_iter(alg);
+    if (mode == 0) {
+        CU(cudaGraphCreate(&g.graph, 0));
+        cudaGraphConditionalHandle cond;
+        CU(cudaGraphConditionalHandleCreate(&cond, g.graph, 1, cudaGraphCondAssignDefault));
+        cudaGraphNodeParams np = {};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = cond;
+        np.conditional.type = cudaGraphCondTypeWhile;
+        np.conditional.size = 1;
+        cudaGraphNode_t node;
+        CU(cudaGraphAddNode(&node, g.graph, nullptr, 0, &np));
+        cudaGraph_t body = np.conditional.phGraph_out[0];
+        CU(cudaStreamBeginCaptureToGraph(A->capture_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+        for (int j = 0; j < nk; ++j) launch_body_kernel(A, alg, j, A->capture_stream, cond, 1);
+        cudaError_t le = cudaGetLastError();
+        cudaGraph_t dummy = nullptr;
+        CU(cudaStreamEndCapture(A->capture_stream, &dummy));
+        if (le != cudaSuccess) return fail(MSOLVE_ECUDA, "kernel launch during capture failed: %s", cudaGetErrorString(le));
+    } else {
+        CU(cudaStreamBeginCapture(A->capture_stream, cudaStreamCaptureModeThreadLocal));
+        for (int c = 0; c < kChunk; ++c)
+            for (int j = 0; j < nk; ++j) launch_body_kernel(A, alg, j, A->capture_stream, 0, 0);
+        cudaError_t le = cudaGetLastError();
+        CU(cudaStreamEndCapture(A->capture_stream, &g.graph));
+        if (le != cudaSuccess) return fail(MSOLVE_ECUDA, "kernel launch during capture failed: %s", cudaGetErrorString(le));
+    }
+    CU(cudaGraphInstantiate(&g.exec, g.graph, 0));
+    g.mode = mode;
+    return MSOLVE_OK;
+}
+
+// ------------------------------------------------------------------------------------- create
+static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t stream) {
+    (void)stream;
+    CU(cudaGetDevice(&A->device));
+    CU(cudaDeviceGetAttribute(&A->num_sms, cudaDevAttrMultiProcessorCount, A->device));
+    CU(cudaMalloc((void**)&A->d_state, sizeof(SolveState)));
+    CU(cudaMemset(A->d_state, 0, sizeof(SolveState)));
+    CU(cudaMallocHost((void**)&A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult)));
+    CU(cudaStreamCreateWithFlags(&A->capture_stream, cudaStreamNonBlocking));
+    *out = A;
+    return MSOLVE_OK;
+}
+
+static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
+
+extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
+                                 const int32_t* d_colidx, const void* d_val, int dtype, int flags, void* stream) {
+    if (!out) return fail(MSOLVE_EINVAL, "msolve_create_csr: A is NULL");
+    *out = nullptr;
+    if (n < 0 || nnz < 0 || nnz >= (1ll << 31) || n >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad n/nnz");
+    if (!d_rowptr || (nnz > 0 && (!d_colidx || !d_val))) return fail(MSOLVE_EINVAL, "msolve_create_csr: NULL array");
+    if (dtype != MSOLVE_C64 && dtype != MSOLVE_C128) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad dtype");
+    if (flags < MSOLVE_SPMV_AUTO || flags > MSOLVE_SPMV_MERGE) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad flags");
+    if (!aligned16(d_val) || ((uintptr_t)d_colidx & 3u) || ((uintptr_t)d_rowptr & 3u)) return fail(MSOLVE_EINVAL, "msolve_create_csr: misaligned array");
+    msolve_matrix* A = new (std::nothrow) msolve_matrix();
+    if (!A) return fail(MSOLVE_ENOMEM, "out of host memory");
+    A->format = FMT_CSR;
+    A->dtype = dtype;
+    A->dev.rowptr = d_rowptr; A->dev.colidx = d_colidx; A->dev.val = d_val;
+    A->dev.n = n; A->dev.nbrows = 0; A->dev.nnz = nnz; A->dev.aux = nullptr; A->dev.aux_count = 0;
+    A->kernel = KERNEL_VECTOR;
+    const double mean = n > 0 ? (double)nnz / (double)n : 0.0;
+    A->lanes = mean > 48 ? 32 : mean > 20 ? 8 : mean > 6 ? 4 : 2;
+    int rc = create_common(out, A, (cudaStream_t)stream);
+    if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
+    return rc;
+}
+
+extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t nblocks, const int32_t* d_browptr,
+                                  const int32_t* d_bcolidx, const void* d_blocks, int dtype, int flags, void* stream) {
+    if (!out) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: A is NULL");
+    *out = nullptr;
+    if (nbrows < 0 || nblocks < 0 || nblocks >= (1ll << 31) / 9 || 3 * nbrows >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad sizes");
+    if (!d_browptr || (nblocks > 0 && (!d_bcolidx || !d_blocks))) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: NULL array");
+    if (dtype != MSOLVE_C64 && dtype != MSOLVE_C128) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad dtype");
+    if (flags != 0) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad flags");
+    if (!aligned16(d_blocks)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: misaligned array");
+    msolve_matrix* A = new (std::nothrow) msolve_matrix();
+    if (!A) return fail(MSOLVE_ENOMEM, "out of host memory");
+    A->format = FMT_BSR3;
+    A->dtype = dtype;
+    A->dev.rowptr = d_browptr; A->dev.colidx = d_bcolidx; A->dev.val = d_blocks;
+    A->dev.n = 3 * nbrows; A->dev.nbrows = nbrows; A->dev.nnz = nblocks; A->dev.aux = nullptr; A->dev.aux_count = 0;
+    A->kernel = KERNEL_BSR_ROWS;
+    int rc = create_common(out, A, (cudaStream_t)stream);
+    if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
+    return rc;
+}
+
+extern "C" void msolve_destroy(msolve_matrix* A) {
+    if (!A) return;
+    for (int i = 0; i < 2; ++i) {
+        if (A->graphs[i].exec) cudaGraphExecDestroy(A->graphs[i].exec);
+        if (A->graphs[i].graph) cudaGraphDestroy(A->graphs[i].graph);
+    }
+    if (A->capture_stream) cudaStreamDestroy(A->capture_stream);
+    if (A->d_state) cudaFree(A->d_state);
+    if (A->h_stage) cudaFreeHost(A->h_stage);
+    if (A->d_aux) cudaFree(A->d_aux);
+    delete A;
+}
+
+extern "C" const char* msolve_last_error(void) { return g_err; }
+
+extern "C" int msolve_config(int key, int value) {
+    if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { g_loop_mode = value; return MSOLVE_OK; }
+    return fail(MSOLVE_EINVAL, "msolve_config: bad key/value");
+}
+
+extern "C" int64_t msolve_last_launch_count(const msolve_matrix* A) { return A ? A->last_launches : 0; }
+
+extern "C" const char* msolve_kernel_name(int alg, int j) {
+    if (alg == MSOLVE_ALG_CGM && j >= 0 && j < 5) return kCgmNames[j];
+    if (alg == MSOLVE_ALG_BICGSTABM && j >= 0 && j < 7) return kBiNames[j];
+    return "";
+}
+
+// ------------------------------------------------------------------------------------- workspace
+static long long pk_stride_elems(const msolve_matrix* A) { return (long long)align_up((size_t)A->dev.n, 16); }
+static int base_vectors(int alg) { return alg == MSOLVE_ALG_CGM ? 3 : 5; }  // r p q [s t]
+
+extern "C" size_t msolve_workspace_bytes(const msolve_matrix* A, int nshifts, int algorithm) {
+    if (!A || nshifts < 1 || nshifts > kMaxShifts || (algorithm != MSOLVE_ALG_CGM && algorithm != MSOLVE_ALG_BICGSTABM)) return 0;
+    const size_t vb = align_up((size_t)pk_stride_elems(A) * elem_bytes(A->dtype), 256);
+    return vb * (size_t)(base_vectors(algorithm) + nshifts) + 256;
+}
+
+static int fill_header(const msolve_matrix* A, int alg, const void* d_b, const double* h_shifts, int S, double tol,
+                       int max_iter, void* d_x, void* ws, size_t ws_bytes, int force_all, SolveHeader* h) {
+    if (!A) return fail(MSOLVE_EINVAL, "solve: A is NULL");
+    if (S < 1 || S > kMaxShifts) return fail(MSOLVE_EINVAL, "solve: nshifts must be in [1, %d]", kMaxShifts);
+    if (!d_b || !d_x || !h_shifts || !ws) return fail(MSOLVE_EINVAL, "solve: NULL argument");
+    if (!(tol >= 0.0) || max_iter < 0) return fail(MSOLVE_EINVAL, "solve: bad tol / max_iter");
+    if (!aligned16(d_b) || !aligned16(d_x)) return fail(MSOLVE_EINVAL, "solve: d_b / d_x must be 16-byte aligned");
+    const size_t need = msolve_workspace_bytes(A, S, alg);
+    if (ws_bytes < need) return fail(MSOLVE_ENOMEM, "solve: workspace too small (%zu < %zu)", ws_bytes, need);
+    const size_t vb = align_up((size_t)pk_stride_elems(A) * elem_bytes(A->dtype), 256);
+    char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
+    memset(h, 0, sizeof(*h));
+    h->b = d_b; h->x = d_x;
+    h->r = base; h->p = base + vb; h->q = base + 2 * vb;
+    char* next = base + 3 * vb;
+    if (alg == MSOLVE_ALG_BICGSTABM) { h->s = next; h->t = next + vb; next += 2 * vb; }
+    h->pk = next;
+    h->n = A->dev.n;
+    h->pk_stride = pk_stride_elems(A);
+    h->tol = tol; h->S = S; h->max_iter = max_iter; h->force_all = force_all;
+    for (int k = 0; k < S; ++k) h->sigma[k] = h_shifts[k];
+    return MSOLVE_OK;
+}
+
+static void fill_result_init(SolveResult* r, int S) {
+    memset(r, 0, sizeof(*r));
+    r->nactive = S;
+    for (int k = 0; k < kMaxShifts; ++k) { r->conv_iter[k] = -1; r->relres[k] = 1.0; }
+}
+
+// ------------------------------------------------------------------------------------- solve
+static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const double* h_shifts, int S, double tol,
+                      int max_iter, void* d_x, void* ws, size_t ws_bytes, int* h_iterations, int* h_conv_iter,
+                      double* h_relres, void* stream_) {
+    msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
+    cudaStream_t stream = (cudaStream_t)stream_;
+    SolveHeader* hh = &A->h_stage->h;
+    SolveResult* hr = &A->h_stage->res;
+    int rc = fill_header(A, alg, d_b, h_shifts, S, tol, max_iter, d_x, ws, ws_bytes, 0, hh);
+    if (rc != MSOLVE_OK) return rc;
+    fill_result_init(hr, S);
+    const size_t xbytes = (size_t)S * (size_t)A->dev.n * elem_bytes(A->dtype);
+    if (A->dev.n == 0 || max_iter == 0) {  // nothing to iterate: x = 0
+        CU(cudaMemsetAsync(d_x, 0, xbytes, stream));
+        CU(cudaStreamSynchronize(stream));
+        if (h_iterations) *h_iterations = 0;
+        for (int k = 0; k < S; ++k) { if (h_conv_iter) h_conv_iter[k] = A->dev.n == 0 ? 0 : -1; if (h_relres) h_relres[k] = A->dev.n == 0 ? 0.0 : 1.0; }
+        A->last_launches = 0;
+        return A->dev.n == 0 ? MSOLVE_OK : MSOLVE_MAXITER;
+    }
+    const int mode = g_loop_mode;
+    rc = build_graph(A, alg, mode);
+    if (rc != MSOLVE_OK) return rc;
+    CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
+    launch_init(A, stream);
+    CU(cudaGetLastError());
+    int64_t launches = 2;
+    const int nk = kernels_per_iter(alg);
+    if (mode == 0) {
+        CU(cudaGraphLaunch(A->graphs[alg].exec, stream));
+        CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
+        CU(cudaStreamSynchronize(stream));
+        launches += (int64_t)nk * std::max(1, hr->n_iter + (hr->status == MSOLVE_BREAKDOWN ? 1 : 0));
+    } else {
+        for (;;) {
+            CU(cudaGraphLaunch(A->graphs[alg].exec, stream));
+            launches += (int64_t)nk * kChunk;
+            CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
+            CU(cudaStreamSynchronize(stream));
+            if (hr->done) break;
+        }
+    }
+    if (hr->zero_rhs) {
+        CU(cudaMemsetAsync(d_x, 0, xbytes, stream));
+        CU(cudaStreamSynchronize(stream));
+    }
+    A->last_launches = launches;
+    if (h_iterations) *h_iterations = hr->n_iter;
+    for (int k = 0; k < S; ++k) {
+        if (h_conv_iter) h_conv_iter[k] = hr->conv_iter[k];
+        if (h_relres) h_relres[k] = hr->relres[k];
+    }
+    return hr->status;
+}
+
+extern "C" int msolve_cgm(const msolve_matrix* A, const void* d_b, const double* h_shifts, int nshifts, double tol,
+                          int max_iter, void* d_x, void* d_workspace, size_t workspace_bytes, int* h_iterations,
+                          int* h_conv_iter, double* h_relres, void* stream) {
+    return run_solver(MSOLVE_ALG_CGM, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_workspace, workspace_bytes,
+                      h_iterations, h_conv_iter, h_relres, stream);
+}
+
+extern "C" int msolve_bicgstabm(const msolve_matrix* A, const void* d_b, const double* h_shifts, int nshifts, double tol,
+                                int max_iter, void* d_x, void* d_workspace, size_t workspace_bytes, int* h_iterations,
+                                int* h_conv_iter, double* h_relres, void* stream) {
+    return run_solver(MSOLVE_ALG_BICGSTABM, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_workspace, workspace_bytes,
+                      h_iterations, h_conv_iter, h_relres, stream);
+}
+
+extern "C" int msolve_solve_host(const msolve_matrix* A, int algorithm, const void* h_b, const double* h_shifts,
+                                 int nshifts, double tol, int max_iter, void* h_x, int* h_iterations,
+                                 int* h_conv_iter, double* h_relres, void* stream_) {
+    if (!A || !h_b || !h_x) return fail(MSOLVE_EINVAL, "msolve_solve_host: NULL argument");
+    if (algorithm != MSOLVE_ALG_CGM && algorithm != MSOLVE_ALG_BICGSTABM) return fail(MSOLVE_EINVAL, "msolve_solve_host: bad algorithm");
+    const size_t wsb = msolve_workspace_bytes(A, nshifts, algorithm);
+    if (!wsb) return fail(MSOLVE_EINVAL, "msolve_solve_host: bad nshifts");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t eb = elem_bytes(A->dtype);
+    const size_t bbytes = (size_t)A->dev.n * eb, xbytes = bbytes * (size_t)nshifts;
+    char* d_all = nullptr;
+    const size_t boff = 0, xoff = align_up(bbytes, 256), woff = xoff + align_up(xbytes, 256);
+    if (cudaMalloc((void**)&d_all, woff + wsb + 256) != cudaSuccess) return fail(MSOLVE_ENOMEM, "msolve_solve_host: cudaMalloc of %zu bytes failed", woff + wsb);
+    int rc;
+    cudaError_t e = cudaMemcpyAsync(d_all + boff, h_b, bbytes, cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) { cudaFree(d_all); return fail(MSOLVE_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e)); }
+    rc = run_solver(algorithm, A, d_all + boff, h_shifts, nshifts, tol, max_iter, d_all + xoff, d_all + woff, wsb + 256,
+                    h_iterations, h_conv_iter, h_relres, stream_);
+    if (rc >= 0) {
+        e = cudaMemcpyAsync(h_x, d_all + xoff, xbytes, cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) rc = fail(MSOLVE_ECUDA, "D2H copy failed: %s", cudaGetErrorString(e));
+    }
+    cudaFree(d_all);
+    return rc;
+}
+
+// ------------------------------------------------------------------------------------- spmv / profile
+extern "C" int msolve_spmv(const msolve_matrix* Ac, const void* d_x, void* d_y, double* h_dot, void* stream_) {
+    msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
+    if (!A || !d_x || !d_y) return fail(MSOLVE_EINVAL, "msolve_spmv: NULL argument");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    SolveHeader* hh = &A->h_stage->h;
+    memset(hh, 0, sizeof(*hh));
+    hh->sp_x = d_x; hh->sp_y = d_y; hh->sp_u = d_x; hh->n = A->dev.n; hh->S = 1;
+    fill_result_init(&A->h_stage->res, 1);
+    CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
+    if (A->dev.n > 0) launch_spmv<ROLE_GEN>(A, stream);
+    CU(cudaGetLastError());
+    if (h_dot) {
+        h_dot[0] = h_dot[1] = 0.0;
+        if (A->dev.n > 0) {
+            int count = 0;
+            CU(cudaMemcpyAsync(&count, &A->d_state->partial_count, sizeof(int), cudaMemcpyDeviceToHost, stream));
+            CU(cudaStreamSynchronize(stream));
+            double* tmp = new double[2 * kMaxPartials];
+            cudaError_t e = cudaMemcpy(tmp, A->d_state->partial, sizeof(double) * 2 * kMaxPartials, cudaMemcpyDeviceToHost);
+            if (e == cudaSuccess)
+                for (int i = 0; i < count; ++i) { h_dot[0] += tmp[i]; h_dot[1] += tmp[kMaxPartials + i]; }
+            delete[] tmp;
+            if (e != cudaSuccess) return fail(MSOLVE_ECUDA, "msolve_spmv: D2H failed: %s", cudaGetErrorString(e));
+        }
+    } else {
+        CU(cudaStreamSynchronize(stream));
+    }
+    return MSOLVE_OK;
+}
+
+extern "C" int msolve_profile_iteration(const msolve_matrix* Ac, int alg, const void* d_b, const double* h_shifts,
+                                        int S, int iters, void* d_x, void* ws, size_t ws_bytes, float* h_ms,
+                                        int* h_launches, void* stream_) {
+    msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
+    if (alg != MSOLVE_ALG_CGM && alg != MSOLVE_ALG_BICGSTABM) return fail(MSOLVE_EINVAL, "profile: bad algorithm");
+    if (iters < 1 || !h_ms) return fail(MSOLVE_EINVAL, "profile: bad iters / h_ms");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    int rc = fill_header(A, alg, d_b, h_shifts, S, 0.0, iters + 1, d_x, ws, ws_bytes, 1, &A->h_stage->h);
+    if (rc != MSOLVE_OK) return rc;
+    fill_result_init(&A->h_stage->res, S);
+    CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
+    launch_init(A, stream);
+    const int nk = kernels_per_iter(alg);
+    cudaEvent_t ev[9];
+    for (int j = 0; j <= nk; ++j) CU(cudaEventCreate(&ev[j]));
+    double sum[8] = {0};
+    // one untimed warm-up iteration (also leaves n_iter > 0 so the steady-state paths are timed)
+    for (int it = 0; it <= iters; ++it) {
+        for (int j = 0; j < nk; ++j) {
+            CU(cudaEventRecord(ev[j], stream));
+            launch_body_kernel(A, alg, j, stream, 0, 0);
+        }
+        CU(cudaEventRecord(ev[nk], stream));
+        CU(cudaStreamSynchronize(stream));
+        CU(cudaGetLastError());
+        if (it == 0) continue;
+        for (int j = 0; j < nk; ++j) {
+            float ms = 0.f;
+            CU(cudaEventElapsedTime(&ms, ev[j], ev[j + 1]));
+            sum[j] += ms;
+        }
+    }
+    for (int j = 0; j <= nk; ++j) cudaEventDestroy(ev[j]);
+    for (int j = 0; j < 8; ++j) { h_ms[j] = j < nk ? (float)(sum[j] / iters) : 0.f; if (h_launches) h_launches[j] = j < nk ? 1 : 0; }
+    return nk;
+}

@@ -1,0 +1,221 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Bars are BASELINE.json's: per-shift relative L2 difference <= 1e-9
+(complex128) / 1e-4 (complex64), true residual <= 10 tol, iteration counts within +-2.
+Run with `pytest -m gpu` on the B200 box."""
+import numpy as np
+import pytest
+import scipy.sparse as sp
+import torch
+
+import oracle
+from paper_1102_2143_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+REL = {np.complex128: 1e-9, np.complex64: 1e-4}
+TORCH = {np.complex128: torch.complex128, np.complex64: torch.complex64}
+
+
+@pytest.fixture(scope="module")
+def ms():
+    from paper_1102_2143_b200 import binding, build
+    build.build()
+    binding.load_library()
+    return binding
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_matrix(ms, w, dtype, fmt, flags=0):
+    if fmt == "bsr3":
+        return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
+    return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), flags)
+
+
+def gpu_solve(ms, w, dtype, fmt, tol=None, max_iter=None, shifts=None, flags=0):
+    A = make_matrix(ms, w, dtype, fmt, flags)
+    fn = ms.msolve_cgm if w.algorithm == "cgm" else ms.msolve_bicgstabm
+    res = fn(A, dev(w.b.astype(dtype)), w.shifts if shifts is None else shifts,
+             w.tol if tol is None else tol, w.max_iter if max_iter is None else max_iter)
+    torch.cuda.synchronize()
+    out = (res.status, res.iterations, res.x.cpu().numpy(), res.conv_iter.copy(), res.relres.copy())
+    launches = ms.msolve_last_launch_count(A)
+    ms.msolve_destroy(A)
+    return out + (launches,)
+
+
+def oracle_solve(w, dtype, tol=None, max_iter=None, shifts=None):
+    fn = oracle.cgm if w.algorithm == "cgm" else oracle.bicgstabm
+    return fn(w.rowptr, w.colidx, w.val.astype(dtype), w.b.astype(dtype), w.shifts if shifts is None else shifts,
+              w.tol if tol is None else tol, w.max_iter if max_iter is None else max_iter)
+
+
+def check_parity(w, dtype, g, o, tol):
+    status, it, x, conv, rel, _ = g
+    assert status == o.status == oracle.OK
+    assert abs(it - o.iterations) <= 2
+    assert np.all(np.abs(conv - o.conv_iter) <= 2)
+    A = sp.csr_matrix((w.val, w.colidx, w.rowptr), shape=(w.n, w.n))
+    for k, s in enumerate(w.shifts):
+        d = np.linalg.norm(x[k].astype(np.complex128) - o.x[k].astype(np.complex128)) / np.linalg.norm(o.x[k])
+        assert d <= REL[dtype], (k, d)
+        xk = x[k].astype(np.complex128)
+        true = np.linalg.norm(w.b - (A @ xk + s * xk)) / np.linalg.norm(w.b)
+        assert true <= 10.0 * tol, (k, true)
+        assert rel[k] <= tol * (1 + 1e-12)
+
+
+# ------------------------------------------------------------------------------- SpMV
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c5", "csr")])
+def test_spmv_matches_oracle(ms, dtype, which, fmt):
+    w = {"c1": lambda: W.config1(), "c2": lambda: W.config2(extents=(4, 4, 6, 5)),
+         "c5": lambda: W.config5(n=5003)}[which]()
+    rng = np.random.default_rng(3)
+    x = (rng.standard_normal(w.n) + 1j * rng.standard_normal(w.n)).astype(dtype)
+    A = make_matrix(ms, w, dtype, fmt)
+    y, dot = ms.msolve_spmv(A, dev(x))
+    y = y.cpu().numpy()
+    ref = oracle.spmv(w.rowptr, w.colidx, w.val.astype(dtype), x)
+    eps = 1e-13 if dtype == np.complex128 else 1e-5
+    assert np.linalg.norm(y - ref) / np.linalg.norm(ref) < eps
+    ref_dot = np.vdot(x.astype(np.complex128), ref.astype(np.complex128))
+    assert abs(dot - ref_dot) / abs(ref_dot) < eps
+    ms.msolve_destroy(A)
+
+
+# ------------------------------------------------------------------------------- CG-M
+def test_config1_cgm_c128(ms):
+    w = W.config1()
+    g = gpu_solve(ms, w, np.complex128, "csr")
+    o = oracle_solve(w, np.complex128)
+    check_parity(w, np.complex128, g, o, w.tol)
+    assert g[5] == 2 + 5 * g[1]          # init + 5 kernels per iteration, no host round trips
+
+
+@pytest.mark.parametrize("fmt", ["csr", "bsr3"])
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+def test_config2_cgm(ms, fmt, dtype, tol):
+    w = W.config2()
+    g = gpu_solve(ms, w, dtype, fmt, tol=tol)
+    o = oracle_solve(w, dtype, tol=tol)
+    check_parity(w, dtype, g, o, tol)
+
+
+@pytest.mark.parametrize("fmt", ["csr", "bsr3"])
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+def test_config4_scaled_cgm(ms, fmt, dtype, tol):
+    w = W.config4(extents=(8, 8, 8, 16), tol=tol)
+    g = gpu_solve(ms, w, dtype, fmt)
+    o = oracle_solve(w, dtype)
+    check_parity(w, dtype, g, o, tol)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+def test_config5_scaled_cgm(ms, dtype, tol):
+    w = W.config5(n=(1 << 15) + 37, tol=tol)       # ragged size
+    g = gpu_solve(ms, w, dtype, "csr")
+    o = oracle_solve(w, dtype)
+    check_parity(w, dtype, g, o, tol)
+    assert np.all(np.diff(g[3]) <= 0)              # larger shifts never converge later
+
+
+# ------------------------------------------------------------------------------- BiCGStab-M
+@pytest.mark.parametrize("fmt", ["csr", "bsr3"])
+def test_config3_bicgstabm_c128(ms, fmt):
+    w = W.config3()                                 # full size: 16^4, N = 196608
+    g = gpu_solve(ms, w, np.complex128, fmt)
+    o = oracle_solve(w, np.complex128)
+    check_parity(w, np.complex128, g, o, w.tol)
+    assert g[5] == 2 + 7 * g[1]
+
+
+def test_config3_scaled_bicgstabm_c64(ms):
+    w = W.config3(extents=(8, 8, 8, 8))
+    g = gpu_solve(ms, w, np.complex64, "bsr3", tol=1e-5)
+    o = oracle_solve(w, np.complex64, tol=1e-5)
+    check_parity(w, np.complex64, g, o, 1e-5)
+
+
+# ------------------------------------------------------------------------------- edge cases
+def test_zero_rhs_and_zero_iterations(ms):
+    w = W.config1()
+    A = make_matrix(ms, w, np.complex128, "csr")
+    x = torch.full((4, w.n), 7.0, dtype=torch.complex128, device="cuda")
+    res = ms.msolve_cgm(A, torch.zeros(w.n, dtype=torch.complex128, device="cuda"), w.shifts, 1e-10, 100, x=x)
+    assert res.status == ms.MSOLVE_OK and res.iterations == 0 and not res.x.abs().max().item()
+    assert np.all(res.conv_iter == 0)
+    x.fill_(7.0)
+    res = ms.msolve_cgm(A, dev(w.b), w.shifts, 1e-10, 0, x=x)
+    assert res.status == ms.MSOLVE_MAXITER and res.iterations == 0 and not res.x.abs().max().item()
+    ms.msolve_destroy(A)
+
+
+@pytest.mark.parametrize("alg", ["cgm", "bicgstabm"])
+def test_maxiter_matches_oracle_iterate(ms, alg):
+    # stopped early, the GPU iterate equals the oracle's iterate at the same n
+    w = W.config2(extents=(4, 4, 4, 4)) if alg == "cgm" else W.config3(extents=(4, 4, 4, 4))
+    for nit in (1, 2, 5):
+        g = gpu_solve(ms, w, np.complex128, "csr", tol=0.0, max_iter=nit)
+        o = oracle_solve(w, np.complex128, tol=0.0, max_iter=nit)
+        assert g[0] == o.status == oracle.MAXITER and g[1] == o.iterations == nit
+        for k in range(w.shifts.size):
+            assert np.linalg.norm(g[2][k] - o.x[k]) / np.linalg.norm(o.x[k]) < 1e-12
+        assert np.allclose(g[4], o.relres, rtol=1e-10)
+
+
+def test_odd_length_c64_and_duplicate_shifts(ms):
+    w = W.config5(n=2051, tol=1e-5)                # odd n: 8-byte access path for complex64
+    shifts = np.array([0.5, 0.5, 0.001, 3.0])      # unsorted, duplicated
+    g = gpu_solve(ms, w, np.complex64, "csr", shifts=shifts)
+    o = oracle_solve(w, np.complex64, shifts=shifts)
+    w.shifts = shifts
+    check_parity(w, np.complex64, g, o, 1e-5)
+    assert np.array_equal(g[2][0], g[2][1])
+
+
+def test_max_shifts_and_too_many(ms):
+    w = W.config1()
+    shifts = np.linspace(0.0, 2.0, ms.MSOLVE_MAX_SHIFTS)
+    g = gpu_solve(ms, w, np.complex128, "csr", shifts=shifts)
+    o = oracle_solve(w, np.complex128, shifts=shifts)
+    w.shifts = shifts
+    check_parity(w, np.complex128, g, o, w.tol)
+    A = make_matrix(ms, w, np.complex128, "csr")
+    with pytest.raises(ms.MsolveError):
+        ms.msolve_cgm(A, dev(w.b), np.zeros(ms.MSOLVE_MAX_SHIFTS + 1), 1e-10, 10)
+    ms.msolve_destroy(A)
+
+
+def test_breakdown_reported(ms):
+    n = 64
+    rowptr = np.arange(n + 1, dtype=np.int32)
+    colidx = np.arange(n, dtype=np.int32)
+    A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(-np.ones(n, dtype=np.complex128)))
+    res = ms.msolve_cgm(A, dev(W.unit_rhs(1, n)), [0.0], 1e-10, 10)
+    assert res.status == ms.MSOLVE_BREAKDOWN
+    ms.msolve_destroy(A)
+
+
+def test_chunked_loop_mode_same_result(ms):
+    w = W.config2(extents=(4, 4, 4, 4))
+    a = gpu_solve(ms, w, np.complex128, "bsr3")
+    ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 1)
+    try:
+        b = gpu_solve(ms, w, np.complex128, "bsr3")
+    finally:
+        ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 0)
+    assert a[1] == b[1] and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3])
+
+
+def test_handle_reuse_and_solve_host(ms):
+    w = W.config2(extents=(4, 4, 4, 4))
+    A = make_matrix(ms, w, np.complex128, "bsr3")
+    r1 = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, 500)
+    r2 = ms.msolve_cgm(A, dev(w.b), w.shifts[:3], w.tol, 500)        # other S, same cached graph
+    assert torch.equal(r1.x[:3], r2.x) and np.array_equal(r1.conv_iter[:3], r2.conv_iter)
+    rh = ms.msolve_solve_host(A, ms.MSOLVE_ALG_CGM, torch.from_numpy(w.b), w.shifts, w.tol, 500)
+    assert not rh.x.is_cuda and torch.equal(rh.x, r1.x.cpu()) and rh.iterations == r1.iterations
+    ms.msolve_destroy(A)
