@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the multishift solver hot path (contract: see DESIGN.md).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload NAME]
+
+A "step" is one complete CG-M solve (every iteration runs rows A1-A7 of SURVEY.md 8(a)) of the
+workload BASELINE.json's target is quoted on: the 32^3x64 SU(3) lattice (configs[3]), complex128,
+3x3-block BSR, 16 shifts, tol 1e-10.  `value` = solver iterations/s with inputs resident in HBM;
+`ms_per_step` = time to solution; `e2e` = the same through msolve_solve_host with HOST b and x
+(H2D/D2H inside the timed region); `roofline` = the dominant kernel (fused multishift update)
+against the measured HBM copy bandwidth; `cpu_baseline` = the CPU oracle on this box's cores.
+N > 1: independent replicas (one problem per GPU, different right-hand sides), no collective on
+the data path ("replicas only"); value = all ranks' iterations / max-over-ranks time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1102_2143_b200 import workloads as W  # noqa: E402
+
+METRIC = "multishift_solver_iterations_per_s"
+UNIT = "iterations/s"
+
+
+# ----------------------------------------------------------------------------------- workloads
+def make_workload(name: str, rank: int, want_csr: bool):
+    """Returns (workload, dtype, format).  Right-hand side differs per rank (replicas)."""
+    if name == "config4_c128_bsr3":
+        w, dt, fmt = W.config4(want_csr=want_csr), np.complex128, "bsr3"
+    elif name == "config4_c64_bsr3":
+        w, dt, fmt = W.config4(want_csr=want_csr, tol=1e-5), np.complex64, "bsr3"
+    elif name == "config4_c128_csr":
+        w, dt, fmt = W.config4(want_csr=True), np.complex128, "csr"
+    elif name == "config4_small_c128_bsr3":          # quick functional check of the bench itself
+        w, dt, fmt = W.config4(extents=(8, 8, 8, 16), want_csr=want_csr), np.complex128, "bsr3"
+    elif name == "config2_c128_bsr3":
+        w, dt, fmt = W.config2(), np.complex128, "bsr3"
+    elif name == "config3_c128_bsr3":
+        w, dt, fmt = W.config3(), np.complex128, "bsr3"
+    elif name == "config5_c128_csr":
+        w, dt, fmt = W.config5(), np.complex128, "csr"
+    elif name == "config5_c64_csr":
+        w, dt, fmt = W.config5(tol=1e-5), np.complex64, "csr"
+    elif name == "config5_small_c128_csr":
+        w, dt, fmt = W.config5(n=1 << 16), np.complex128, "csr"
+    else:
+        raise SystemExit("unknown workload %s" % name)
+    if rank:
+        w.b = W.unit_rhs(W.DEFAULT_SEED + rank, w.n)
+    return w, dt, fmt
+
+
+def algorithmic_bytes(w, dtype, fmt, s_active):
+    """bytes the method must move per kernel launch (x gathered once)."""
+    e = 16 if dtype == np.complex128 else 8
+    n = w.n
+    if fmt == "bsr3":
+        nb = w.bcolidx.size
+        spmv = nb * (9 * e + 4) + (n // 3 + 1) * 4 + 2 * n * e
+    else:
+        spmv = w.nnz * (e + 4) + (n + 1) * 4 + 2 * n * e
+    if w.algorithm == "cgm":
+        return {"cgm_pupdate": 3 * n * e, "spmv_dot": spmv, "cgm_update": (3 + 4 * s_active) * n * e,
+                "cgm_scal1": 0, "cgm_scal2": 0}
+    return {"spmv1_dot": spmv + n * e, "spmv2_dots": spmv + 2 * n * e, "bi_supdate": 3 * n * e,
+            "bi_update": (7 + 4 * s_active) * n * e, "bi_scal1": 0, "bi_scal2": 0, "bi_scal3": 0}
+
+
+# ----------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peak_gbs():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic_bytes(kernel_regex: str):
+    """dram read+write bytes per launch of the dominant kernel from the committed ncu summary, or None."""
+    p = os.path.join(ROOT, "profiles", "r01_ncu_dram_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    try:
+        for ln in open(p):
+            f = ln.strip().split(",")
+            if len(f) >= 2 and f[0] == kernel_regex:
+                return float(f[1])
+    except Exception:
+        return None
+    return None
+
+
+# ----------------------------------------------------------------------------------- oracle legs
+def oracle_sample(w, dtype, iters):
+    """The CPU oracle, as it stands, on the first `iters` iterations of the same workload."""
+    import oracle
+    oracle.build()
+    fn = oracle.cgm if w.algorithm == "cgm" else oracle.bicgstabm
+    t0 = time.perf_counter()
+    res = fn(w.rowptr, w.colidx, w.val.astype(dtype, copy=False), w.b.astype(dtype), w.shifts, 0.0, iters)
+    dt = time.perf_counter() - t0
+    return res.iterations / dt, dt, res.iterations
+
+
+def run_reference(args, rank):
+    """--impl reference: the oracle on the host cores; each step = a bounded sample (2 iterations)."""
+    if rank != 0:
+        return
+    w, dtype, fmt = make_workload(args.workload, 0, want_csr=True)
+    per_step = 2
+    for _ in range(args.warmup):
+        oracle_sample(w, dtype, per_step)
+    t_tot, it_tot = 0.0, 0
+    for _ in range(args.steps):
+        _, dt, it = oracle_sample(w, dtype, per_step)
+        t_tot += dt
+        it_tot += it
+    value = it_tot / t_tot
+    sample = "first %d iterations of %s per step (tol=0), all %d shifts active" % (per_step, w.name, w.shifts.size)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "c128" if dtype == np.complex128 else "c64", "data": "synthetic",
+            "config": {"workload": args.workload, "n": w.n, "nnz": int(w.nnz), "shifts": int(w.shifts.size),
+                       "format": "csr", "algorithm": w.algorithm},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config4_c128_bsr3")
+    ap.add_argument("--profile-iters", type=int, default=20)
+    ap.add_argument("--cpu-iters", type=int, default=6, help="oracle iterations timed for cpu_baseline (0 = skip)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--loop-mode", default="while", choices=["while", "chunk"],
+                    help="while: device WHILE graph node (default). chunk: unrolled graph relaunched by the host; "
+                         "same kernels, used for ncu (kernel nodes of conditional graphs cannot be profiled)")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3                                      # timing rule: W >= 3
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1102_2143_b200 import binding as ms, build as _build
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    _build.build()
+    ms.load_library()
+    ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 0 if args.loop_mode == "while" else 1)
+
+    need_csr = args.workload.endswith("_csr") or (rank == 0 and world == 1 and args.cpu_iters > 0)
+    w, dtype, fmt = make_workload(args.workload, rank, want_csr=need_csr)
+    tdt = torch.complex128 if dtype == np.complex128 else torch.complex64
+    alg = ms.MSOLVE_ALG_CGM if w.algorithm == "cgm" else ms.MSOLVE_ALG_BICGSTABM
+    solve = ms.msolve_cgm if w.algorithm == "cgm" else ms.msolve_bicgstabm
+
+    def dev(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+    t_create = time.perf_counter()
+    if fmt == "bsr3":
+        A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype, copy=False)))
+    else:
+        A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype, copy=False)))
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t_create
+    S = int(w.shifts.size)
+    b_host = torch.from_numpy(w.b.astype(dtype)).pin_memory()
+    b_dev = b_host.cuda()
+    x_dev = torch.empty((S, w.n), dtype=tdt, device="cuda")
+    ws = torch.empty(ms.msolve_workspace_bytes(A, S, alg), dtype=torch.uint8, device="cuda")
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-resident timing: K complete solves
+    for _ in range(args.warmup):
+        res = solve(A, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev, workspace=ws)
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    iters, launches = 0, 0
+    ev0.record()
+    for _ in range(args.steps):
+        res = solve(A, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev, workspace=ws)
+        iters += res.iterations
+        launches += ms.msolve_last_launch_count(A)
+    ev1.record()
+    barrier()
+    clocks = sampler.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    status, conv_iter = res.status, res.conv_iter.tolist()
+
+    # ---- end to end: host b in, host x out, every step
+    e2e = None
+    if not args.no_e2e:
+        x_host = torch.empty((S, w.n), dtype=tdt, pin_memory=True)
+        for _ in range(2):
+            ms.msolve_solve_host(A, alg, b_host, w.shifts, w.tol, w.max_iter, x=x_host)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        it_e2e = 0
+        e0.record()
+        for _ in range(args.steps):
+            it_e2e += ms.msolve_solve_host(A, alg, b_host, w.shifts, w.tol, w.max_iter, x=x_host).iterations
+        e1.record()
+        barrier()
+        ms_e2e = e0.elapsed_time(e1)
+        e2e = (it_e2e, ms_e2e, b_host.numel() * b_host.element_size() + 8 * S,
+               x_host.numel() * x_host.element_size())
+        del x_host
+
+    # ---- per-kernel steady state (all shifts active), CUDA events around every kernel launch
+    prof = ms.msolve_profile_iteration(A, alg, b_dev, w.shifts, args.profile_iters, x=x_dev, workspace=ws)
+    torch.cuda.synchronize()
+
+    # ---- reduce over ranks
+    t = torch.tensor([ms_total, e2e[1] if e2e else 0.0], dtype=torch.float64, device="cuda")
+    c = torch.tensor([iters, launches, e2e[0] if e2e else 0], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    ms_total, ms_e2e = t.tolist()
+    iters_all, launches_all, it_e2e_all = c.tolist()
+
+    if rank == 0:
+        peak, peak_src = measured_peak_gbs()
+        ab = algorithmic_bytes(w, dtype, fmt, S)
+        kernels = {}
+        for name, kms in prof.items():
+            gbs = ab.get(name, 0) / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
+            kernels[name] = {"ms": round(kms, 5), "alg_GB": round(ab.get(name, 0) / 1e9, 4),
+                             "GBps": round(gbs, 1), "frac_measured_peak": round(gbs / peak, 4),
+                             "frac_8TBps": round(gbs / 8000.0, 4)}
+        dom = "cgm_update" if w.algorithm == "cgm" else "bi_update"
+        traffic = ncu_traffic_bytes(dom)
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["GBps"], "peak": peak,
+                    "unit": "GB/s", "frac": round(kernels[dom]["GBps"] / peak, 4), "peak_source": peak_src,
+                    "traffic": traffic, "algorithmic_bytes_per_launch": ab[dom]}
+        iter_ms = sum(v["ms"] for v in kernels.values())
+        cpu = None
+        if args.cpu_iters > 0 and world == 1:
+            v, dt, it = oracle_sample(w, dtype, args.cpu_iters)
+            cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": "first %d iterations of %s (tol=0, all %d shifts active), %.1f s, single thread, %d host cores present"
+                             % (it, w.name, S, dt, os.cpu_count())}
+        line = {
+            "metric": METRIC, "value": iters_all / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "c128" if dtype == np.complex128 else "c64", "data": "synthetic",
+            "config": {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt,
+                       "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.nnz), "shifts": S, "tol": w.tol,
+                       "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode,
+                       "l2": "inputs larger than L2 (matrix + %d vectors >> 126 MB), no flush" % (3 + 2 * S)},
+            "time_to_solution_ms": ms_total / args.steps, "iterations_per_solve": iters_all / args.steps / world,
+            "status": status, "conv_iter": conv_iter, "create_ms": 1e3 * t_create,
+            "steady_state_ms_per_iteration": round(iter_ms, 4),
+            "steady_state_iterations_per_s": round(1e3 / iter_ms, 2) if iter_ms > 0 else None,
+            "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu,
+            "e2e": None if e2e is None else {"value": it_e2e_all / (ms_e2e * 1e-3), "unit": UNIT,
+                                             "h2d_bytes_per_step": e2e[2], "d2h_bytes_per_step": e2e[3],
+                                             "ms_per_step": ms_e2e / args.steps},
+            "gpu_launches": int(launches_all), "clocks": clocks,
+        }
+        print(json.dumps(line))
+    ms.msolve_destroy(A)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -78,7 +78,9 @@ int msolve_create_csr(msolve_matrix **A, int64_t n, int64_t nnz,
                       const void *d_val /* nnz complex */, int dtype, int flags, void *stream);
 
 /* Build a handle for a 3x3-block BSR matrix (3*nbrows x 3*nbrows), the SU(3) layout:
- * block k is 9 complex numbers, row-major 3x3, at d_blocks + 9*k.  Same borrowing rules. */
+ * block k is 9 complex numbers, row-major 3x3, at d_blocks + 9*k.  Same borrowing rules.
+ * flags: MSOLVE_SPMV_AUTO = TMA-staged tile kernel when the rows allow it (reads d_browptr once
+ * at create time to build its tile table), MSOLVE_SPMV_VECTOR = simple thread-per-row kernel. */
 int msolve_create_bsr3(msolve_matrix **A, int64_t nbrows, int64_t nblocks,
                        const int32_t *d_browptr /* nbrows+1 */, const int32_t *d_bcolidx /* nblocks */,
                        const void *d_blocks /* nblocks*9 complex */, int dtype, int flags, void *stream);

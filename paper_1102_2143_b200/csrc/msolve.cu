@@ -12,6 +12,7 @@
 #include <cstdio>
 #include <cstring>
 #include <new>
+#include <vector>
 
 #include "common.cuh"
 #include "kernels.cuh"
@@ -40,7 +41,7 @@ static int fail(int code, const char* fmt, ...) {
 
 // ------------------------------------------------------------------------------------- handle
 enum { FMT_CSR = 0, FMT_BSR3 = 1 };
-enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3 };
+enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3, KERNEL_BSR_TMA = 4 };
 constexpr int kChunk = 8;  // iteration bodies per graph launch in chunked mode
 
 struct LoopGraph {
@@ -85,8 +86,28 @@ static int grid_for(const msolve_matrix* A, K kernel, long long work_items, long
     return (int)std::min<long long>(g, kMaxPartials);
 }
 
+// TMA-staged BSR3 kernel configuration: block rows per tile, lanes per scalar row, pipeline depth
+template <typename T> struct BsrTile;
+#ifndef MSOLVE_BSR_TB
+#define MSOLVE_BSR_TB 16
+#define MSOLVE_BSR_STAGES 4
+#define MSOLVE_BSR_CPS 2
+#endif
+template <> struct BsrTile<double> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
+template <> struct BsrTile<float>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
+
 template <typename T, int ROLE>
 static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
+    if (A->format == FMT_BSR3 && A->kernel == KERNEL_BSR_TMA) {
+        typedef BsrTile<T> B;
+        auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, B::CPS, ROLE>;
+        const int smem = BsrTmaCfg<T, B::TB>::smem_bytes(B::STAGES);
+        static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
+        if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+        const int grid = std::max(1, std::min(A->num_sms * B::CPS, A->dev.aux_count));
+        k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+        return;
+    }
     if (A->format == FMT_BSR3) {
         auto k = k_spmv_bsr3_rows<T, ROLE>;
         k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
@@ -215,6 +236,36 @@ static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t str
     return MSOLVE_OK;
 }
 
+// Tile table of the TMA-staged BSR3 kernel: consecutive block rows, at most TB rows and 9*TB
+// blocks per tile, every tile starting at a block index that is a multiple of 4 (16-byte aligned
+// bulk copies for both dtypes).  Falls back to the row kernel when no such partition exists.
+static int build_bsr_tiles(msolve_matrix* A) {
+    const int TB = A->dtype == MSOLVE_C64 ? BsrTile<float>::TB : BsrTile<double>::TB;
+    const int maxb = 9 * TB;
+    const long long nbr = A->dev.nbrows;
+    std::vector<int32_t> rp((size_t)nbr + 1);
+    CU(cudaMemcpy(rp.data(), A->dev.rowptr, sizeof(int32_t) * (size_t)(nbr + 1), cudaMemcpyDeviceToHost));
+    if (rp[0] != 0) return MSOLVE_OK;  // unusual base: keep the row kernel
+    std::vector<int4> tiles;
+    long long r = 0;
+    while (r < nbr) {
+        long long end = r, best = -1;
+        while (end < nbr && end - r < TB && rp[end + 1] - rp[r] <= maxb) {
+            ++end;
+            if (rp[end] % 4 == 0 || end == nbr) best = end;
+        }
+        if (best <= r) return MSOLVE_OK;  // a row is too dense or alignment impossible: row kernel
+        tiles.push_back(make_int4((int)r, (int)best, rp[r], rp[best]));
+        r = best;
+    }
+    CU(cudaMalloc(&A->d_aux, sizeof(int4) * tiles.size()));
+    CU(cudaMemcpy(A->d_aux, tiles.data(), sizeof(int4) * tiles.size(), cudaMemcpyHostToDevice));
+    A->dev.aux = (const int32_t*)A->d_aux;
+    A->dev.aux_count = (int)tiles.size();
+    A->kernel = KERNEL_BSR_TMA;
+    return MSOLVE_OK;
+}
+
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
 extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
@@ -247,7 +298,7 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     if (nbrows < 0 || nblocks < 0 || nblocks >= (1ll << 31) / 9 || 3 * nbrows >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad sizes");
     if (!d_browptr || (nblocks > 0 && (!d_bcolidx || !d_blocks))) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: NULL array");
     if (dtype != MSOLVE_C64 && dtype != MSOLVE_C128) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad dtype");
-    if (flags != 0) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad flags");
+    if (flags != MSOLVE_SPMV_AUTO && flags != MSOLVE_SPMV_VECTOR) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad flags");
     if (!aligned16(d_blocks)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: misaligned array");
     msolve_matrix* A = new (std::nothrow) msolve_matrix();
     if (!A) return fail(MSOLVE_ENOMEM, "out of host memory");
@@ -257,6 +308,7 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     A->dev.n = 3 * nbrows; A->dev.nbrows = nbrows; A->dev.nnz = nblocks; A->dev.aux = nullptr; A->dev.aux_count = 0;
     A->kernel = KERNEL_BSR_ROWS;
     int rc = create_common(out, A, (cudaStream_t)stream);
+    if (rc == MSOLVE_OK && flags == MSOLVE_SPMV_AUTO && nbrows > 0) rc = build_bsr_tiles(A);
     if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
     return rc;
 }

@@ -150,3 +150,171 @@ __global__ void __launch_bounds__(kThreads) k_spmv_bsr3_rows(MatDev A, SolveStat
 }
 
 }  // namespace msolve
+
+namespace msolve {
+
+// ------------------------------------------------------------------------------------------
+// PTX wrappers: mbarrier + 1-D bulk async copy (TMA engine, SASS UBLKCP) + L2 cache policies.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
+}
+// global -> shared bulk copy; bytes % 16 == 0, both addresses 16-byte aligned; completes on `bar`
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t policy) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
+}
+__device__ __forceinline__ double2 ld_hint(const double2* p, uint64_t policy) {
+    double2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(policy)); return r;
+}
+__device__ __forceinline__ float2 ld_hint(const float2* p, uint64_t policy) {
+    float2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(policy)); return r;
+}
+
+// ------------------------------------------------------------------------------------------
+// BSR3, TMA-staged (the SU(3) lattice kernel).  Persistent CTAs, CPS of them per SM.  A producer
+// thread streams tiles of TB block rows -- the tile's 3x3 blocks and its block-column indices
+// are one contiguous byte range each -- into a STAGES-deep shared-memory ring with 1-D bulk
+// async copies (evict-first in L2: the matrix is read once per SpMV), signalled by mbarriers.
+// Phase 1: one consumer thread per 3x3 BLOCK gathers its x 3-vector ONCE (evict-last in L2:
+// every x element is used by its 2d+1 neighbour rows), multiplies the block out of shared
+// memory and leaves a 3-vector partial in shared memory; all gathers of a tile are in flight
+// at once.  Phase 2 (after one named barrier): one thread per scalar row sums its row's
+// partials, writes y and feeds the fused dot products.
+// Tile table (A.aux, built at create time): int4 {row_begin, row_end, block_begin, block_end},
+// block_begin % 4 == 0 so that every bulk copy is 16-byte aligned for both dtypes.
+// ------------------------------------------------------------------------------------------
+template <typename T, int TB> struct BsrTmaCfg {
+    static constexpr int kMaxBlocks = 9 * TB;
+    static constexpr int kConsumers = (kMaxBlocks + 31) / 32 * 32;
+    static constexpr int kThreadsTotal = kConsumers + 32;
+    static constexpr int kValBytes = kMaxBlocks * 9 * 2 * (int)sizeof(T);
+    static constexpr int kIdxBytes = kMaxBlocks * 4;
+    static constexpr int kStageBytes = kValBytes + kIdxBytes;
+    static constexpr int kPartBytes = kMaxBlocks * 3 * 2 * (int)sizeof(T);   // one partial buffer
+    static constexpr int smem_bytes(int stages) { return stages * kStageBytes + 2 * kPartBytes + 2 * stages * 8; }
+};
+
+template <typename T, int TB, int STAGES, int CPS, int ROLE>
+__global__ void __launch_bounds__(BsrTmaCfg<T, TB>::kThreadsTotal, CPS) k_spmv_bsr3_tma(MatDev A, SolveState* st) {
+    typedef typename Cx<T>::type C;
+    typedef BsrTmaCfg<T, TB> Cfg;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    constexpr int NCT = Cfg::kConsumers;
+    constexpr int NCW = NCT / 32;
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    C* part = (C*)(smem + STAGES * Cfg::kStageBytes);
+    uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::kStageBytes + 2 * Cfg::kPartBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, NCW); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    const int4* __restrict__ tiles = (const int4*)A.aux;
+    const int ntiles = A.aux_count;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    int stage = 0;
+    uint32_t phase = 0;
+    if (threadIdx.x >= NCT) {
+        // ---------------- producer: one elected lane of the last warp
+        if (threadIdx.x == NCT) {
+            const uint64_t pol = policy_evict_first();
+            const C* __restrict__ val = (const C*)A.val;
+            int t = blockIdx.x;
+            int4 e = t < ntiles ? tiles[t] : make_int4(0, 0, 0, 0);
+            while (t < ntiles) {
+                const int tn = t + gridDim.x;
+                const int4 en = tn < ntiles ? tiles[tn] : make_int4(0, 0, 0, 0);
+                mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                unsigned char* sb = smem + stage * Cfg::kStageBytes;
+                const uint32_t nb = (uint32_t)(e.w - e.z);
+                const uint32_t vbytes = nb * 9u * (uint32_t)sizeof(C), ibytes = nb * 4u;
+                const uint32_t vb16 = vbytes & ~15u, ib16 = ibytes & ~15u;
+                const unsigned char* vsrc = (const unsigned char*)(val + (long long)e.z * 9);
+                const unsigned char* isrc = (const unsigned char*)(A.colidx + e.z);
+                // ragged tail of the very last tile: < 16 bytes each, copied through the generic proxy
+                for (uint32_t o = vb16; o < vbytes; o += 4) *(uint32_t*)(sb + o) = *(const uint32_t*)(vsrc + o);
+                for (uint32_t o = ib16; o < ibytes; o += 4) *(uint32_t*)(sb + Cfg::kValBytes + o) = *(const uint32_t*)(isrc + o);
+                mbar_expect_tx(full0 + 8 * stage, vb16 + ib16);
+                if (vb16) bulk_g2s(smem_u32(sb), vsrc, vb16, full0 + 8 * stage, pol);
+                if (ib16) bulk_g2s(smem_u32(sb + Cfg::kValBytes), isrc, ib16, full0 + 8 * stage, pol);
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+                t = tn; e = en;
+            }
+        }
+    } else {
+        // ---------------- consumers
+        const uint64_t polx = policy_evict_last();
+        const int tid = threadIdx.x;
+        const int lbr = tid / 3, rr = tid - 3 * lbr;     // phase-2 role: scalar row (lbr, rr)
+        const int32_t* __restrict__ browptr = A.rowptr;
+        int pbuf = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            const int4 e = tiles[t];
+            const int nb = e.w - e.z;
+            const bool rvalid = lbr < e.y - e.x;
+            int jb = 0, je = 0;
+            if (rvalid) { jb = browptr[e.x + lbr] - e.z; je = browptr[e.x + lbr + 1] - e.z; }
+            mbar_wait(full0 + 8 * stage, phase);
+            C* pb = part + pbuf * (Cfg::kMaxBlocks * 3);
+            if (tid < nb) {                                   // phase 1: block `tid` of the tile
+                const C* blk = (const C*)(smem + stage * Cfg::kStageBytes) + tid * 9;
+                const int32_t c = ((const int32_t*)(smem + stage * Cfg::kStageBytes + Cfg::kValBytes))[tid];
+                const C* xv = x + 3ll * c;
+                const C x0 = ld_hint(xv, polx), x1 = ld_hint(xv + 1, polx), x2 = ld_hint(xv + 2, polx);
+                C a[9];
+#pragma unroll
+                for (int k = 0; k < 9; ++k) a[k] = blk[k];
+#pragma unroll
+                for (int r3 = 0; r3 < 3; ++r3) {
+                    C v = cmul(a[3 * r3], x0);
+                    v = cfma(a[3 * r3 + 1], x1, v);
+                    v = cfma(a[3 * r3 + 2], x2, v);
+                    pb[tid * 3 + r3] = v;
+                }
+            }
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);     // this warp no longer reads the stage
+            asm volatile("bar.sync 1, %0;" ::"n"(NCT) : "memory");     // partials visible to all consumers
+            if (rvalid) {                                     // phase 2: scalar row (lbr, rr)
+                C sum = cmake<C>(0.0, 0.0);
+                for (int j = jb; j < je; ++j) sum = cadd(sum, pb[j * 3 + rr]);
+                const long long row = 3ll * (e.x + lbr) + rr;
+                y[row] = sum;
+                role_epilogue<C, ROLE>(acc, row, sum, x, u);
+            }
+            pbuf ^= 1;
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+    }
+    write_partials<NACC>(st, acc);
+}
+
+}  // namespace msolve

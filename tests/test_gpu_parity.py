@@ -29,6 +29,8 @@ def dev(a):
 
 
 def make_matrix(ms, w, dtype, fmt, flags=0):
+    if fmt == "bsr3rows":   # the simple one-thread-per-row BSR3 kernel instead of the TMA-staged one
+        return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
     if fmt == "bsr3":
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
     return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), flags)
@@ -69,9 +71,11 @@ def check_parity(w, dtype, g, o, tol):
 
 # ------------------------------------------------------------------------------- SpMV
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
-@pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c5", "csr")])
+@pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c2", "bsr3rows"),
+                                       ("c2big", "bsr3"), ("c5", "csr")])
 def test_spmv_matches_oracle(ms, dtype, which, fmt):
     w = {"c1": lambda: W.config1(), "c2": lambda: W.config2(extents=(4, 4, 6, 5)),
+         "c2big": lambda: W.config2(extents=(12, 10, 9, 11)),   # 11880 sites: many tiles per CTA, ragged tail
          "c5": lambda: W.config5(n=5003)}[which]()
     rng = np.random.default_rng(3)
     x = (rng.standard_normal(w.n) + 1j * rng.standard_normal(w.n)).astype(dtype)
@@ -95,7 +99,7 @@ def test_config1_cgm_c128(ms):
     assert g[5] == 2 + 5 * g[1]          # init + 5 kernels per iteration, no host round trips
 
 
-@pytest.mark.parametrize("fmt", ["csr", "bsr3"])
+@pytest.mark.parametrize("fmt", ["csr", "bsr3", "bsr3rows"])
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 def test_config2_cgm(ms, fmt, dtype, tol):
     w = W.config2()
