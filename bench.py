@@ -146,6 +146,24 @@ def ncu_traffic_bytes(kernel_regex: str):
     return None
 
 
+# ----------------------------------------------------------------------------------- ranks
+def aggregate_over_ranks(times_ms, counts, device, world):
+    """Whole-job numbers from per-rank ones: elapsed times -> MAX over ranks, counts -> SUM.
+    (device = "cuda" under NCCL, "cpu" under gloo in the CPU test.)"""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    c = torch.tensor(list(counts), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(c, op=dist.ReduceOp.SUM)
+    return t.tolist(), c.tolist()
+
+
+def throughput(total_iterations, max_ms):
+    return total_iterations / (max_ms * 1e-3)
+
+
 # ----------------------------------------------------------------------------------- oracle legs
 def oracle_sample(w, dtype, iters):
     """The CPU oracle, as it stands, on the first `iters` iterations of the same workload."""
@@ -292,13 +310,8 @@ def main():
     torch.cuda.synchronize()
 
     # ---- reduce over ranks
-    t = torch.tensor([ms_total, e2e[1] if e2e else 0.0], dtype=torch.float64, device="cuda")
-    c = torch.tensor([iters, launches, e2e[0] if e2e else 0], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(c, op=dist.ReduceOp.SUM)
-    ms_total, ms_e2e = t.tolist()
-    iters_all, launches_all, it_e2e_all = c.tolist()
+    (ms_total, ms_e2e), (iters_all, launches_all, it_e2e_all) = aggregate_over_ranks(
+        [ms_total, e2e[1] if e2e else 0.0], [iters, launches, e2e[0] if e2e else 0], "cuda", world)
 
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
@@ -322,7 +335,7 @@ def main():
                    "sample": "first %d iterations of %s (tol=0, all %d shifts active), %.1f s, single thread, %d host cores present"
                              % (it, w.name, S, dt, os.cpu_count())}
         line = {
-            "metric": METRIC, "value": iters_all / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
+            "metric": METRIC, "value": throughput(iters_all, ms_total), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "c128" if dtype == np.complex128 else "c64", "data": "synthetic",
@@ -335,7 +348,7 @@ def main():
             "steady_state_ms_per_iteration": round(iter_ms, 4),
             "steady_state_iterations_per_s": round(1e3 / iter_ms, 2) if iter_ms > 0 else None,
             "kernels": kernels, "roofline": roofline, "cpu_baseline": cpu,
-            "e2e": None if e2e is None else {"value": it_e2e_all / (ms_e2e * 1e-3), "unit": UNIT,
+            "e2e": None if e2e is None else {"value": throughput(it_e2e_all, ms_e2e), "unit": UNIT,
                                              "h2d_bytes_per_step": e2e[2], "d2h_bytes_per_step": e2e[3],
                                              "ms_per_step": ms_e2e / args.steps},
             "gpu_launches": int(launches_all), "clocks": clocks,

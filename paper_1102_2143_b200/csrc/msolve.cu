@@ -88,13 +88,19 @@ static int grid_for(const msolve_matrix* A, K kernel, long long work_items, long
 
 // TMA-staged BSR3 kernel configuration: block rows per tile, lanes per scalar row, pipeline depth
 template <typename T> struct BsrTile;
+// Tuned on B200 (profiles/r01_spmv_bsr3_tile_sweep.md): many small CTAs per SM (independent
+// tiles in flight hide the x-gather latency), a 2-deep ring is enough for the bulk copies, and a
+// small shared-memory footprint leaves L1 for the gathers.
 #ifndef MSOLVE_BSR_TB
-#define MSOLVE_BSR_TB 16
-#define MSOLVE_BSR_STAGES 4
-#define MSOLVE_BSR_CPS 2
+#define MSOLVE_BSR_TB 12
+#define MSOLVE_BSR_STAGES 2
+#define MSOLVE_BSR_CPS 5
+#endif
+#ifndef MSOLVE_BSR_CPS_F
+#define MSOLVE_BSR_CPS_F 4
 #endif
 template <> struct BsrTile<double> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
-template <> struct BsrTile<float>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
+template <> struct BsrTile<float>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS_F; };
 
 template <typename T, int ROLE>
 static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {

@@ -185,10 +185,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
 }
+#ifndef MSOLVE_X_HINT
+#define MSOLVE_X_HINT 0
+#endif
 __device__ __forceinline__ double2 ld_hint(const double2* p, uint64_t policy) {
+    if (!MSOLVE_X_HINT) return __ldg(p);
     double2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(policy)); return r;
 }
 __device__ __forceinline__ float2 ld_hint(const float2* p, uint64_t policy) {
+    if (!MSOLVE_X_HINT) return __ldg(p);
     float2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(policy)); return r;
 }
 
@@ -197,8 +202,9 @@ __device__ __forceinline__ float2 ld_hint(const float2* p, uint64_t policy) {
 // thread streams tiles of TB block rows -- the tile's 3x3 blocks and its block-column indices
 // are one contiguous byte range each -- into a STAGES-deep shared-memory ring with 1-D bulk
 // async copies (evict-first in L2: the matrix is read once per SpMV), signalled by mbarriers.
-// Phase 1: one consumer thread per 3x3 BLOCK gathers its x 3-vector ONCE (evict-last in L2:
-// every x element is used by its 2d+1 neighbour rows), multiplies the block out of shared
+// Phase 1: one consumer thread per 3x3 BLOCK gathers its x 3-vector ONCE (through L1/L2: every
+// x element is used by its 2d+1 neighbour rows; a software pipeline issues the gathers of the
+// next tile before the current one is multiplied), multiplies the block out of shared
 // memory and leaves a 3-vector partial in shared memory; all gathers of a tile are in flight
 // at once.  Phase 2 (after one named barrier): one thread per scalar row sums its row's
 // partials, writes y and feeds the fused dot products.
@@ -270,25 +276,50 @@ __global__ void __launch_bounds__(BsrTmaCfg<T, TB>::kThreadsTotal, CPS) k_spmv_b
             }
         }
     } else {
-        // ---------------- consumers
+        // ---------------- consumers.  Software-pipelined: the x gathers of tile t+1 are issued
+        // (into registers) before tile t is multiplied, so their L2 latency overlaps the math,
+        // the named barrier and phase 2 of tile t.  Tile-table entries are fetched two ahead.
         const uint64_t polx = policy_evict_last();
         const int tid = threadIdx.x;
         const int lbr = tid / 3, rr = tid - 3 * lbr;     // phase-2 role: scalar row (lbr, rr)
         const int32_t* __restrict__ browptr = A.rowptr;
+        const int G = gridDim.x;
         int pbuf = 0;
-        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-            const int4 e = tiles[t];
+        int t = blockIdx.x;
+        const int4 zero4 = make_int4(0, 0, 0, 0);
+        int4 e = t < ntiles ? tiles[t] : zero4;
+        int4 en = t + G < ntiles ? tiles[t + G] : zero4;
+        C xn0 = cmake<C>(0.0, 0.0), xn1 = xn0, xn2 = xn0;
+        if (t < ntiles) {
+            mbar_wait(full0, 0u);
+            if (tid < e.w - e.z) {
+                const int32_t c = ((const int32_t*)(smem + Cfg::kValBytes))[tid];
+                const C* xv = x + 3ll * c;
+                xn0 = ld_hint(xv, polx); xn1 = ld_hint(xv + 1, polx); xn2 = ld_hint(xv + 2, polx);
+            }
+        }
+        while (t < ntiles) {
+            const int tn = t + G;
+            const int4 enn = tn + G < ntiles ? tiles[tn + G] : zero4;
             const int nb = e.w - e.z;
             const bool rvalid = lbr < e.y - e.x;
             int jb = 0, je = 0;
             if (rvalid) { jb = browptr[e.x + lbr] - e.z; je = browptr[e.x + lbr + 1] - e.z; }
-            mbar_wait(full0 + 8 * stage, phase);
+            const C x0 = xn0, x1 = xn1, x2 = xn2;
+            int nstage = stage + 1;
+            uint32_t nphase = phase;
+            if (nstage == STAGES) { nstage = 0; nphase ^= 1u; }
+            if (tn < ntiles) {                                // gathers of the NEXT tile
+                mbar_wait(full0 + 8 * nstage, nphase);
+                if (tid < en.w - en.z) {
+                    const int32_t c = ((const int32_t*)(smem + nstage * Cfg::kStageBytes + Cfg::kValBytes))[tid];
+                    const C* xv = x + 3ll * c;
+                    xn0 = ld_hint(xv, polx); xn1 = ld_hint(xv + 1, polx); xn2 = ld_hint(xv + 2, polx);
+                }
+            }
             C* pb = part + pbuf * (Cfg::kMaxBlocks * 3);
             if (tid < nb) {                                   // phase 1: block `tid` of the tile
                 const C* blk = (const C*)(smem + stage * Cfg::kStageBytes) + tid * 9;
-                const int32_t c = ((const int32_t*)(smem + stage * Cfg::kStageBytes + Cfg::kValBytes))[tid];
-                const C* xv = x + 3ll * c;
-                const C x0 = ld_hint(xv, polx), x1 = ld_hint(xv + 1, polx), x2 = ld_hint(xv + 2, polx);
                 C a[9];
 #pragma unroll
                 for (int k = 0; k < 9; ++k) a[k] = blk[k];
@@ -311,7 +342,8 @@ __global__ void __launch_bounds__(BsrTmaCfg<T, TB>::kThreadsTotal, CPS) k_spmv_b
                 role_epilogue<C, ROLE>(acc, row, sum, x, u);
             }
             pbuf ^= 1;
-            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            stage = nstage; phase = nphase;
+            t = tn; e = en; en = enn;
         }
     }
     write_partials<NACC>(st, acc);
