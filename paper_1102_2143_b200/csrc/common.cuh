@@ -178,6 +178,7 @@ struct MatDev {
     long long nbrows;        // BSR3 block rows (0 for CSR)
     long long nnz;           // CSR nnz / BSR3 blocks
     const int32_t* aux;      // merge-path partition table / BSR tile table
+    void* carry;             // merge-path: per-tile head / tail partial sums, 2 * aux_count complex
     int aux_count;
 };
 

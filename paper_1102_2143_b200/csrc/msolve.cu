@@ -17,6 +17,7 @@
 #include "common.cuh"
 #include "kernels.cuh"
 #include "spmv.cuh"
+#include "spmv_merge.cuh"
 
 using namespace msolve;
 
@@ -61,6 +62,7 @@ struct msolve_matrix {
     SolveState* d_state = nullptr;      // library-owned
     SolveState* h_stage = nullptr;      // pinned staging for header / result
     void* d_aux = nullptr;              // library-owned auxiliary matrix data
+    void* d_carry = nullptr;            // merge-path carries (library-owned)
     cudaStream_t capture_stream = nullptr;
     LoopGraph graphs[2];
     int64_t last_launches = 0;
@@ -102,8 +104,39 @@ template <typename T> struct BsrTile;
 template <> struct BsrTile<double> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
 template <> struct BsrTile<float>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS_F; };
 
+// Merge-path CSR kernel configuration: tile capacity (non-zeros), ring depth, CTAs per SM.
+#ifndef MSOLVE_MERGE_CAP
+#define MSOLVE_MERGE_CAP 1024
+#define MSOLVE_MERGE_CAP_F 2048
+#define MSOLVE_MERGE_STAGES 2
+#define MSOLVE_MERGE_CPS 4
+#define MSOLVE_MERGE_CPS_F 3
+#endif
+template <typename T> struct MergeTile;
+template <> struct MergeTile<double> { static constexpr int CAP = MSOLVE_MERGE_CAP, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS; };
+template <> struct MergeTile<float>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
+
+static int merge_grid(const msolve_matrix* A) {
+    const int cps = A->dtype == MSOLVE_C64 ? MergeTile<float>::CPS : MergeTile<double>::CPS;
+    return std::max(1, std::min(A->num_sms * cps, A->dev.aux_count));
+}
+static int merge_fixup_grid(const msolve_matrix* A) {
+    return std::max(1, std::min(A->num_sms, (A->dev.aux_count + kThreads - 1) / kThreads));
+}
+
 template <typename T, int ROLE>
 static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
+    if (A->format == FMT_CSR && A->kernel == KERNEL_MERGE) {
+        typedef MergeTile<T> M;
+        auto k = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE>;
+        const int smem = MergeCfg<T, M::CAP>::smem_bytes(M::STAGES);
+        static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
+        if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+        const int grid = merge_grid(A);
+        k<<<grid, MergeCfg<T, M::CAP>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+        k_spmv_csr_merge_fixup<T, ROLE><<<merge_fixup_grid(A), kThreads, 0, s>>>(A->dev, A->d_state, grid);
+        return;
+    }
     if (A->format == FMT_BSR3 && A->kernel == KERNEL_BSR_TMA) {
         typedef BsrTile<T> B;
         auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, B::CPS, ROLE>;
@@ -160,6 +193,11 @@ constexpr int kUnrollBi = 2;
 static const char* kCgmNames[] = {"cgm_pupdate", "spmv_dot", "cgm_scal1", "cgm_update", "cgm_scal2"};
 static const char* kBiNames[] = {"spmv1_dot", "bi_scal1", "bi_supdate", "spmv2_dots", "bi_scal2", "bi_update", "bi_scal3"};
 static int kernels_per_iter(int alg) { return alg == MSOLVE_ALG_CGM ? 5 : 7; }
+// kernel launches per iteration body: the merge-path SpMV is two launches (tiles + carry fix-up)
+static int launches_per_iter(const msolve_matrix* A, int alg) {
+    const int spmvs = alg == MSOLVE_ALG_CGM ? 1 : 2;
+    return kernels_per_iter(alg) + (A->kernel == KERNEL_MERGE ? spmvs : 0);
+}
 
 // One kernel of the iteration body.  Used for graph capture, and one-by-one for profiling.
 static void launch_body_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s,
@@ -274,6 +312,66 @@ static int build_bsr_tiles(msolve_matrix* A) {
 
 static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
+// Merge-path partition (spmv_merge.cuh): the n + nnz merge items (row ends, non-zeros) are cut
+// every kDiag items.  Split point on diagonal d: i = number of row ends consumed, found by binary
+// search for the first i with rowptr[i+1] > d-i-1; k = d - i.  k is then moved up to the next
+// multiple of 4 (16-byte aligned bulk copies for values and indices) and i to the first row not
+// yet finished at that k.  Tile t = {i0, i1, k0, k1}: rows i0..i1-1 end inside the tile, row i1
+// (if < n) may continue.  Also decides AUTO: merge-path when the row lengths are irregular.
+static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int32_t>& rp) {
+    const long long n = A->dev.n, nnz = A->dev.nnz;
+    if (n == 0) return MSOLVE_OK;
+    if (rp[0] != 0 || rp[(size_t)n] != nnz) return force ? fail(MSOLVE_EINVAL, "msolve_create_csr: rowptr[0] != 0 or rowptr[n] != nnz") : MSOLVE_OK;
+    long long maxlen = 0;
+    for (long long i = 0; i < n; ++i) {
+        if (rp[i + 1] < rp[i]) return force ? fail(MSOLVE_EINVAL, "msolve_create_csr: rowptr is not non-decreasing") : MSOLVE_OK;
+        maxlen = std::max<long long>(maxlen, rp[i + 1] - rp[i]);
+    }
+    if (!force) {
+        const double mean = (double)nnz / (double)n;
+        if ((double)maxlen <= 2.0 * mean + 4.0) return MSOLVE_OK;   // regular rows: vector kernel
+    }
+    const int D = A->dtype == MSOLVE_C64 ? MergeCfg<float, MergeTile<float>::CAP>::kDiag
+                                         : MergeCfg<double, MergeTile<double>::CAP>::kDiag;
+    const long long items = n + nnz;
+    const long long ntiles = (items + D - 1) / D;
+    if (ntiles >= (1ll << 31) - 1) return force ? fail(MSOLVE_EINVAL, "msolve_create_csr: too many tiles") : MSOLVE_OK;
+    std::vector<int4> tiles((size_t)ntiles);
+    long long pi = 0, pk = 0;
+    for (long long t = 1; t <= ntiles; ++t) {
+        long long i, k;
+        if (t == ntiles) { i = n; k = nnz; }
+        else {
+            const long long d = t * D;
+            long long lo = std::max(0ll, d - nnz), hi = std::min(d, n);
+            while (lo < hi) {
+                const long long mid = (lo + hi) >> 1;
+                if ((long long)rp[mid + 1] <= d - mid - 1) lo = mid + 1; else hi = mid;
+            }
+            i = lo; k = d - lo;
+            const long long k4 = std::min(nnz, (k + 3) & ~3ll);
+            if (k4 > k) {
+                i = std::lower_bound(rp.begin() + i + 1, rp.begin() + n + 1, (int32_t)k4) - (rp.begin() + 1);
+                k = k4;
+            }
+            if (i > n) i = n;
+            if (i < pi || k < pk) { i = pi; k = pk; }
+        }
+        tiles[(size_t)t - 1] = make_int4((int)pi, (int)i, (int)pk, (int)k);
+        pi = i; pk = k;
+    }
+    const size_t cb = 2 * (size_t)ntiles * elem_bytes(A->dtype);
+    CU(cudaMalloc(&A->d_aux, sizeof(int4) * tiles.size()));
+    CU(cudaMemcpy(A->d_aux, tiles.data(), sizeof(int4) * tiles.size(), cudaMemcpyHostToDevice));
+    CU(cudaMalloc(&A->d_carry, cb));
+    CU(cudaMemset(A->d_carry, 0, cb));
+    A->dev.aux = (const int32_t*)A->d_aux;
+    A->dev.aux_count = (int)ntiles;
+    A->dev.carry = A->d_carry;
+    A->kernel = KERNEL_MERGE;
+    return MSOLVE_OK;
+}
+
 extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, const int32_t* d_rowptr,
                                  const int32_t* d_colidx, const void* d_val, int dtype, int flags, void* stream) {
     if (!out) return fail(MSOLVE_EINVAL, "msolve_create_csr: A is NULL");
@@ -288,11 +386,22 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
     A->format = FMT_CSR;
     A->dtype = dtype;
     A->dev.rowptr = d_rowptr; A->dev.colidx = d_colidx; A->dev.val = d_val;
-    A->dev.n = n; A->dev.nbrows = 0; A->dev.nnz = nnz; A->dev.aux = nullptr; A->dev.aux_count = 0;
+    A->dev.n = n; A->dev.nbrows = 0; A->dev.nnz = nnz; A->dev.aux = nullptr; A->dev.aux_count = 0; A->dev.carry = nullptr;
     A->kernel = KERNEL_VECTOR;
     const double mean = n > 0 ? (double)nnz / (double)n : 0.0;
     A->lanes = mean > 48 ? 32 : mean > 20 ? 8 : mean > 6 ? 4 : 2;
     int rc = create_common(out, A, (cudaStream_t)stream);
+    if (rc == MSOLVE_OK && flags != MSOLVE_SPMV_VECTOR && n > 0) {
+        const bool force = flags == MSOLVE_SPMV_MERGE;
+        if (!aligned16(d_rowptr) || !aligned16(d_colidx)) {
+            if (force) rc = fail(MSOLVE_EINVAL, "msolve_create_csr: merge-path needs 16-byte aligned rowptr / colidx");
+        } else {
+            std::vector<int32_t> rp((size_t)n + 1);
+            cudaError_t e = cudaMemcpy(rp.data(), d_rowptr, sizeof(int32_t) * (size_t)(n + 1), cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) rc = fail(MSOLVE_ECUDA, "msolve_create_csr: reading rowptr failed: %s", cudaGetErrorString(e));
+            else rc = build_merge_tiles(A, force, rp);
+        }
+    }
     if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
     return rc;
 }
@@ -311,7 +420,7 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     A->format = FMT_BSR3;
     A->dtype = dtype;
     A->dev.rowptr = d_browptr; A->dev.colidx = d_bcolidx; A->dev.val = d_blocks;
-    A->dev.n = 3 * nbrows; A->dev.nbrows = nbrows; A->dev.nnz = nblocks; A->dev.aux = nullptr; A->dev.aux_count = 0;
+    A->dev.n = 3 * nbrows; A->dev.nbrows = nbrows; A->dev.nnz = nblocks; A->dev.aux = nullptr; A->dev.aux_count = 0; A->dev.carry = nullptr;
     A->kernel = KERNEL_BSR_ROWS;
     int rc = create_common(out, A, (cudaStream_t)stream);
     if (rc == MSOLVE_OK && flags == MSOLVE_SPMV_AUTO && nbrows > 0) rc = build_bsr_tiles(A);
@@ -329,6 +438,7 @@ extern "C" void msolve_destroy(msolve_matrix* A) {
     if (A->d_state) cudaFree(A->d_state);
     if (A->h_stage) cudaFreeHost(A->h_stage);
     if (A->d_aux) cudaFree(A->d_aux);
+    if (A->d_carry) cudaFree(A->d_carry);
     delete A;
 }
 
@@ -419,11 +529,11 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
         CU(cudaGraphLaunch(A->graphs[alg].exec, stream));
         CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
         CU(cudaStreamSynchronize(stream));
-        launches += (int64_t)nk * std::max(1, hr->n_iter + (hr->status == MSOLVE_BREAKDOWN ? 1 : 0));
+        launches += (int64_t)launches_per_iter(A, alg) * std::max(1, hr->n_iter + (hr->status == MSOLVE_BREAKDOWN ? 1 : 0));
     } else {
         for (;;) {
             CU(cudaGraphLaunch(A->graphs[alg].exec, stream));
-            launches += (int64_t)nk * kChunk;
+            launches += (int64_t)launches_per_iter(A, alg) * kChunk;
             CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
             CU(cudaStreamSynchronize(stream));
             if (hr->done) break;
@@ -548,5 +658,8 @@ extern "C" int msolve_profile_iteration(const msolve_matrix* Ac, int alg, const 
     }
     for (int j = 0; j <= nk; ++j) cudaEventDestroy(ev[j]);
     for (int j = 0; j < 8; ++j) { h_ms[j] = j < nk ? (float)(sum[j] / iters) : 0.f; if (h_launches) h_launches[j] = j < nk ? 1 : 0; }
+    if (h_launches && A->kernel == KERNEL_MERGE) {   // merge-path SpMV slots are two launches each
+        if (alg == MSOLVE_ALG_CGM) h_launches[1] = 2; else { h_launches[0] = 2; h_launches[3] = 2; }
+    }
     return nk;
 }

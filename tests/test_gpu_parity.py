@@ -33,6 +33,10 @@ def make_matrix(ms, w, dtype, fmt, flags=0):
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
     if fmt == "bsr3":
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
+    if fmt == "csrmerge":   # merge-path CSR forced (AUTO picks it only for irregular rows)
+        return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), ms.MSOLVE_SPMV_MERGE)
+    if fmt == "csrvector":
+        return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
     return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), flags)
 
 
@@ -72,11 +76,12 @@ def check_parity(w, dtype, g, o, tol):
 # ------------------------------------------------------------------------------- SpMV
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 @pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c2", "bsr3rows"),
-                                       ("c2big", "bsr3"), ("c5", "csr")])
+                                       ("c2big", "bsr3"), ("c5", "csr"), ("c5", "csrvector"), ("c5", "csrmerge"),
+                                       ("c1", "csrmerge"), ("c2big", "csrmerge"), ("c5big", "csrmerge")])
 def test_spmv_matches_oracle(ms, dtype, which, fmt):
     w = {"c1": lambda: W.config1(), "c2": lambda: W.config2(extents=(4, 4, 6, 5)),
          "c2big": lambda: W.config2(extents=(12, 10, 9, 11)),   # 11880 sites: many tiles per CTA, ragged tail
-         "c5": lambda: W.config5(n=5003)}[which]()
+         "c5": lambda: W.config5(n=5003), "c5big": lambda: W.config5(n=200003)}[which]()
     rng = np.random.default_rng(3)
     x = (rng.standard_normal(w.n) + 1j * rng.standard_normal(w.n)).astype(dtype)
     A = make_matrix(ms, w, dtype, fmt)
@@ -87,6 +92,66 @@ def test_spmv_matches_oracle(ms, dtype, which, fmt):
     assert np.linalg.norm(y - ref) / np.linalg.norm(ref) < eps
     ref_dot = np.vdot(x.astype(np.complex128), ref.astype(np.complex128))
     assert abs(dot - ref_dot) / abs(ref_dot) < eps
+    ms.msolve_destroy(A)
+
+
+def _random_csr(rng, lengths, n):
+    rowptr = np.zeros(n + 1, dtype=np.int32)
+    rowptr[1:] = np.cumsum(lengths)
+    nnz = int(rowptr[-1])
+    colidx = rng.integers(0, n, nnz).astype(np.int32)
+    val = (rng.standard_normal(nnz) + 1j * rng.standard_normal(nnz))
+    return rowptr, colidx, val
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("shape", ["empty_rows", "one_long_row", "long_rows_mixed", "all_empty", "single_row", "tiny"])
+def test_merge_path_degenerate_rows(ms, dtype, shape):
+    # merge-path tiles cut rows anywhere: empty rows (also in floods at a tile boundary), rows
+    # spanning many tiles, matrices smaller than one tile.  Not a solver workload: SpMV only.
+    rng = np.random.default_rng(11)
+    if shape == "empty_rows":
+        n = 30011
+        lengths = rng.integers(0, 40, n) * (rng.random(n) < 0.3)
+        lengths[5000:12000] = 0                                   # a flood of empty rows
+    elif shape == "one_long_row":
+        n = 4099
+        lengths = np.full(n, 3)
+        lengths[1234] = 50001                                     # spans ~25-50 tiles
+    elif shape == "long_rows_mixed":
+        n = 2500
+        lengths = rng.integers(1, 12, n)
+        lengths[rng.integers(0, n, 12)] = rng.integers(1500, 9000, 12)
+        lengths[-1] = 4097                                        # long last row
+        lengths[0] = 3000                                         # long first row
+    elif shape == "all_empty":
+        n = 5000
+        lengths = np.zeros(n, dtype=np.int64)
+    elif shape == "single_row":
+        n = 1
+        lengths = np.array([1])
+    else:
+        n = 7
+        lengths = np.array([0, 2, 0, 0, 5, 1, 0])
+    rowptr, colidx, val = _random_csr(rng, lengths, n)
+    if colidx.size == 0:                                          # keep the arrays non-NULL
+        colidx_d, val_d = torch.zeros(4, dtype=torch.int32, device="cuda"), torch.zeros(4, dtype=TORCH[dtype], device="cuda")
+        A = ms.msolve_create_csr(dev(rowptr), colidx_d[:0], val_d[:0], ms.MSOLVE_SPMV_MERGE)
+    else:
+        A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val.astype(dtype)), ms.MSOLVE_SPMV_MERGE)
+    x = (rng.standard_normal(n) + 1j * rng.standard_normal(n)).astype(dtype)
+    y, dot = ms.msolve_spmv(A, dev(x), torch.full((n,), 7.0, dtype=TORCH[dtype], device="cuda"))
+    y = y.cpu().numpy()
+    ref = oracle.spmv(rowptr, colidx, val.astype(dtype), x)
+    eps = 1e-13 if dtype == np.complex128 else 2e-5
+    scale = max(np.linalg.norm(ref), 1e-300)
+    assert np.linalg.norm(y - ref) <= eps * scale
+    assert np.array_equal(y[lengths == 0], np.zeros(int((lengths == 0).sum()), dtype=dtype))   # every row written
+    ref_dot = np.vdot(x.astype(np.complex128), ref.astype(np.complex128))
+    assert abs(dot - ref_dot) <= eps * max(abs(ref_dot), np.linalg.norm(x) * scale)
+    # bit-reproducible: a second launch gives the same bytes
+    y2, dot2 = ms.msolve_spmv(A, dev(x))
+    assert np.array_equal(y2.cpu().numpy(), y) and dot2 == dot
     ms.msolve_destroy(A)
 
 
@@ -117,13 +182,25 @@ def test_config4_scaled_cgm(ms, fmt, dtype, tol):
     check_parity(w, dtype, g, o, tol)
 
 
+@pytest.mark.parametrize("fmt", ["csr", "csrvector", "csrmerge"])
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
-def test_config5_scaled_cgm(ms, dtype, tol):
-    w = W.config5(n=(1 << 15) + 37, tol=tol)       # ragged size
-    g = gpu_solve(ms, w, dtype, "csr")
+def test_config5_scaled_cgm(ms, fmt, dtype, tol):
+    w = W.config5(n=(1 << 15) + 37, tol=tol)       # ragged size; "csr" = AUTO picks merge-path here
+    g = gpu_solve(ms, w, dtype, fmt)
     o = oracle_solve(w, dtype)
     check_parity(w, dtype, g, o, tol)
     assert np.all(np.diff(g[3]) <= 0)              # larger shifts never converge later
+    per_iter = 5 if fmt == "csrvector" else 6      # merge-path SpMV = tile kernel + carry fix-up
+    assert g[5] == 2 + per_iter * g[1]
+
+
+def test_bicgstabm_merge_path(ms):
+    # both SpMV roles of BiCGStab-M (incl. the quadratic <t,t> on rows cut by tile boundaries)
+    w = W.config3(extents=(6, 6, 6, 6))
+    g = gpu_solve(ms, w, np.complex128, "csrmerge")
+    o = oracle_solve(w, np.complex128)
+    check_parity(w, np.complex128, g, o, w.tol)
+    assert g[5] == 2 + 9 * g[1]
 
 
 # ------------------------------------------------------------------------------- BiCGStab-M
