@@ -22,7 +22,7 @@ _LIB = os.path.join(_HERE, "libmsolve_oracle.so")
 _lib = None
 
 OK, MAXITER, BREAKDOWN = 0, 1, 2
-C64, C128 = 0, 1
+C64, C128, F32, F64 = 0, 1, 2, 3
 
 
 def build(force: bool = False) -> str:
@@ -49,7 +49,11 @@ def _dt(val: np.ndarray) -> int:
         return C64
     if val.dtype == np.complex128:
         return C128
-    raise TypeError("oracle wants complex64 or complex128, got %s" % val.dtype)
+    if val.dtype == np.float32:      # real: the paper's own Table 1 runs
+        return F32
+    if val.dtype == np.float64:
+        return F64
+    raise TypeError("oracle wants complex64/128 or float32/64, got %s" % val.dtype)
 
 
 def _p(a: Optional[np.ndarray]):

@@ -15,7 +15,8 @@
 //     sigma=0 / single-shift pins of the two multishift routines.
 // No blocking, fusion or reordering: every loop below is one line of the algorithm.
 //
-// Precision (R14): vectors are complex<T>, T = float (c64) or double (c128); every
+// Precision (R14): vectors are complex<T> or, for the paper's own real-valued workload
+// (Table 1), plain T; T = float or double; every
 // dot product accumulates in double, every recurrence scalar (zeta, alpha, beta, rho, chi) is
 // double / complex<double>; a scalar that multiplies a vector is rounded to T once, then the
 // vector arithmetic is done in T.  SpMV accumulates a row in T in stored order.
@@ -42,34 +43,47 @@ typedef std::complex<double> zdouble;
 
 enum { ST_OK = 0, ST_MAXITER = 1, ST_BREAKDOWN = 2, ST_EINVAL = -1 };
 
-template <typename T>
+// Element type C of matrices and vectors: std::complex<T> (the BASELINE configs) or plain T (the
+// paper's own real-valued runs, Table 1); T = float or double.
+template <typename C> struct RealOf { typedef C type; };
+template <typename T> struct RealOf<std::complex<T> > { typedef T type; };
+
+template <typename C>
 struct Csr {
     int64_t n;
     const int32_t* rowptr;
     const int32_t* colidx;
-    const std::complex<T>* val;
+    const C* val;
 };
 
 // y = A x   (Alg. 1 l.18).  Row sum in T, stored order.
-template <typename T>
-void spmv(const Csr<T>& A, const std::complex<T>* x, std::complex<T>* y) {
+template <typename C>
+void spmv(const Csr<C>& A, const C* x, C* y) {
     for (int64_t i = 0; i < A.n; ++i) {
-        std::complex<T> acc(0, 0);
+        C acc(0);
         for (int32_t j = A.rowptr[i]; j < A.rowptr[i + 1]; ++j) acc += A.val[j] * x[A.colidx[j]];
         y[i] = acc;
     }
 }
 
 // <u,v> = sum_i conj(u_i) v_i, accumulated in double (r^dagger . r).
-template <typename T>
-zdouble dot(int64_t n, const std::complex<T>* u, const std::complex<T>* v) {
+template <typename C>
+zdouble dot(int64_t n, const C* u, const C* v) {
     zdouble acc(0, 0);
     for (int64_t i = 0; i < n; ++i) acc += std::conj(zdouble(u[i])) * zdouble(v[i]);
     return acc;
 }
 
-template <typename T>
-inline std::complex<T> rnd(const zdouble& z) { return std::complex<T>((T)z.real(), (T)z.imag()); }
+// A recurrence scalar rounded ONCE to the vectors' element type (R14).  Real data: every dot
+// product is real, so every scalar has an exactly zero imaginary part and the real part is it.
+template <typename C> struct Rnd;
+template <typename T> struct Rnd<std::complex<T> > {
+    static std::complex<T> of(const zdouble& z) { return std::complex<T>((T)z.real(), (T)z.imag()); }
+};
+template <> struct Rnd<float> { static float of(const zdouble& z) { return (float)z.real(); } };
+template <> struct Rnd<double> { static double of(const zdouble& z) { return z.real(); } };
+template <typename C> inline C rnd(const zdouble& z) { return Rnd<C>::of(z); }
+template <typename C> inline C rnd(double v) { return Rnd<C>::of(zdouble(v, 0)); }
 
 inline bool finite(double x) { return std::isfinite(x); }
 inline bool finite(const zdouble& z) { return std::isfinite(z.real()) && std::isfinite(z.imag()); }
@@ -82,17 +96,16 @@ inline bool finite(const zdouble& z) { return std::isfinite(z.real()) && std::is
 // hist (optional, hist_cap rows of 3+3S doubles): per iteration beta, alpha_next, R1 and per
 // shift zeta_new, beta_k, alpha_k.
 // ------------------------------------------------------------------------------------------
-template <typename T>
-int cgm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, double tol,
-        int max_iter, int stop_rule, std::complex<T>* x, int* iterations, int* conv_iter,
-        double* relres, std::complex<T>* r_out, double* zeta_out, double* hist, int hist_cap) {
-    typedef std::complex<T> C;
+template <typename C>
+int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
+        int max_iter, int stop_rule, C* x, int* iterations, int* conv_iter,
+        double* relres, C* r_out, double* zeta_out, double* hist, int hist_cap) {
     const int64_t n = A.n;
     if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
     std::vector<C> r(b, b + n), p(b, b + n), q(n);           // l.9-10: r <- b, p <- b
     std::vector<C> pk((size_t)S * n);
     for (int k = 0; k < S; ++k)
-        for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0, 0); }  // l.11-12
+        for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0); }  // l.11-12
     double alpha = 0.0, beta_prev = 1.0;                      // l.2, l.4
     std::vector<double> zeta_prev(S, 1.0), zeta(S, 1.0), zeta_new(S, 1.0), beta_k(S, 0.0), alpha_k(S, 0.0);
     std::vector<char> active(S, 1);
@@ -120,7 +133,7 @@ int cgm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, d
             if (den == 0.0 || !finite(zeta_new[k]) || !finite(beta_k[k])) status = ST_BREAKDOWN;
         }
         if (status == ST_BREAKDOWN) break;
-        { const C bt = C((T)beta, 0);
+        { const C bt = rnd<C>(beta);
           for (int64_t i = 0; i < n; ++i) r[i] = r[i] + bt * q[i]; }   // l.21
         R1 = dot(n, r.data(), r.data()).real();               // l.24
         const double alpha_next = R1 / R0;                    // l.25
@@ -128,11 +141,11 @@ int cgm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, d
             const double ratio = zeta_new[k] / zeta[k];
             alpha_k[k] = alpha_next * ratio * ratio;          // l.26 (R5)
         }
-        { const C an = C((T)alpha_next, 0);
+        { const C an = rnd<C>(alpha_next);
           for (int64_t i = 0; i < n; ++i) p[i] = r[i] + an * p[i]; }   // l.27
         for (int k = 0; k < S; ++k) if (active[k]) {
             C* xk = x + (size_t)k * n; C* pkk = pk.data() + (size_t)k * n;
-            const C bk = C((T)beta_k[k], 0), zn = C((T)zeta_new[k], 0), ak = C((T)alpha_k[k], 0);
+            const C bk = rnd<C>(beta_k[k]), zn = rnd<C>(zeta_new[k]), ak = rnd<C>(alpha_k[k]);
             for (int64_t i = 0; i < n; ++i) xk[i] = xk[i] - bk * pkk[i];            // l.28
             for (int64_t i = 0; i < n; ++i) pkk[i] = zn * r[i] + ak * pkk[i];       // l.29 (R6)
         }
@@ -170,17 +183,16 @@ int cgm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, d
 // hist rows: 8+6S doubles: beta(2) chi(2) alpha_new(2) |r|^2 delta-unused, then zeta_new,
 // beta_k, chi_k (complex each).
 // ------------------------------------------------------------------------------------------
-template <typename T>
-int bicgstabm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, int S, double tol,
-              int max_iter, int stop_rule, std::complex<T>* x, int* iterations, int* conv_iter,
-              double* relres, std::complex<T>* r_out, double* zeta_out, double* hist, int hist_cap) {
-    typedef std::complex<T> C;
+template <typename C>
+int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
+              int max_iter, int stop_rule, C* x, int* iterations, int* conv_iter,
+              double* relres, C* r_out, double* zeta_out, double* hist, int hist_cap) {
     const int64_t n = A.n;
     if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
     std::vector<C> r(b, b + n), p(b, b + n), r0(b, b + n), q(n), s(n), t(n), rnew(n);
     std::vector<C> pk((size_t)S * n);
     for (int k = 0; k < S; ++k)
-        for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0, 0); }
+        for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0); }
     zdouble alpha(0, 0), beta_prev(1, 0);
     std::vector<zdouble> zeta_prev(S, 1.0), zeta(S, 1.0), zeta_new(S, 1.0), rho(S, 1.0), rho_new(S, 1.0),
         beta_k(S), alpha_k(S), chi_k(S);
@@ -209,7 +221,7 @@ int bicgstabm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, in
             if (den == zdouble(0, 0) || !finite(zeta_new[k]) || !finite(beta_k[k])) status = ST_BREAKDOWN;
         }
         if (status == ST_BREAKDOWN) break;
-        { const C bt = rnd<T>(beta);
+        { const C bt = rnd<C>(beta);
           for (int64_t i = 0; i < n; ++i) s[i] = r[i] + bt * q[i]; }       // s = r + beta q
         spmv(A, s.data(), t.data());                                       // t = A s
         const zdouble ts = dot(n, t.data(), s.data());
@@ -224,7 +236,7 @@ int bicgstabm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, in
             rho_new[k] = rho[k] / one_cs;                                   // rho'_k = rho_k/(1+chi sigma)
         }
         if (status == ST_BREAKDOWN) break;
-        { const C ch = rnd<T>(chi);
+        { const C ch = rnd<C>(chi);
           for (int64_t i = 0; i < n; ++i) rnew[i] = s[i] - ch * t[i]; }    // r' = s - chi t
         const zdouble delta_new = dot(n, r0.data(), rnew.data());           // delta' = <r0,r'>
         const zdouble alpha_new = -beta * delta_new / (delta * chi);        // alpha' = -beta delta'/(delta chi)
@@ -235,18 +247,18 @@ int bicgstabm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, in
         }
         for (int k = 0; k < S; ++k) if (active[k]) {
             C* xk = x + (size_t)k * n; C* pkk = pk.data() + (size_t)k * n;
-            const C bk = rnd<T>(beta_k[k]);
-            const C cs = rnd<T>(chi_k[k] * rho[k] * zeta_new[k]);           // coefficient of s in x_k
-            const C zr = rnd<T>(zeta_new[k] * rho_new[k]);                  // coefficient of r' in p_k
-            const C ak = rnd<T>(alpha_k[k]);
-            const C cb = rnd<T>(chi_k[k] / beta_k[k]);
-            const C zs = rnd<T>(zeta_new[k] * rho[k]);                      // s^sigma = zs * s
-            const C zo = rnd<T>(zeta[k] * rho[k]);                          // r^sigma = zo * r
+            const C bk = rnd<C>(beta_k[k]);
+            const C cs = rnd<C>(chi_k[k] * rho[k] * zeta_new[k]);           // coefficient of s in x_k
+            const C zr = rnd<C>(zeta_new[k] * rho_new[k]);                  // coefficient of r' in p_k
+            const C ak = rnd<C>(alpha_k[k]);
+            const C cb = rnd<C>(chi_k[k] / beta_k[k]);
+            const C zs = rnd<C>(zeta_new[k] * rho[k]);                      // s^sigma = zs * s
+            const C zo = rnd<C>(zeta[k] * rho[k]);                          // r^sigma = zo * r
             for (int64_t i = 0; i < n; ++i) xk[i] = (xk[i] - bk * pkk[i]) + cs * s[i];
             for (int64_t i = 0; i < n; ++i)
                 pkk[i] = zr * rnew[i] + ak * (pkk[i] - cb * (zs * s[i] - zo * r[i]));
         }
-        { const C an = rnd<T>(alpha_new), ch = rnd<T>(chi);
+        { const C an = rnd<C>(alpha_new), ch = rnd<C>(chi);
           for (int64_t i = 0; i < n; ++i) p[i] = rnew[i] + an * (p[i] - ch * q[i]); }  // p = r' + alpha'(p - chi q)
         for (int64_t i = 0; i < n; ++i) r[i] = rnew[i];
         rr = dot(n, r.data(), r.data()).real();
@@ -287,29 +299,28 @@ int bicgstabm(const Csr<T>& A, const std::complex<T>* b, const double* sigma, in
 // ------------------------------------------------------------------------------------------
 // Plain CG on (A + sigma I), textbook form ([13]).  Pin only.
 // ------------------------------------------------------------------------------------------
-template <typename T>
-int cg(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol, int max_iter,
-       std::complex<T>* x, int* iterations, double* relres) {
-    typedef std::complex<T> C;
+template <typename C>
+int cg(const Csr<C>& A, double sigma, const C* b, double tol, int max_iter,
+       C* x, int* iterations, double* relres) {
     const int64_t n = A.n;
     std::vector<C> r(b, b + n), p(b, b + n), q(n);
-    for (int64_t i = 0; i < n; ++i) x[i] = C(0, 0);
+    for (int64_t i = 0; i < n; ++i) x[i] = C(0);
     double rr = dot(n, r.data(), r.data()).real();
     const double bnorm = std::sqrt(rr);
     int it = 0, status = ST_MAXITER;
     if (bnorm == 0.0) { *iterations = 0; if (relres) *relres = 0.0; return ST_OK; }
     while (it < max_iter) {
         spmv(A, p.data(), q.data());
-        if (sigma != 0.0) { const C sg((T)sigma, 0); for (int64_t i = 0; i < n; ++i) q[i] = q[i] + sg * p[i]; }
+        if (sigma != 0.0) { const C sg = rnd<C>(sigma); for (int64_t i = 0; i < n; ++i) q[i] = q[i] + sg * p[i]; }
         const double pq = dot(n, p.data(), q.data()).real();
         if (!(pq > 0.0)) { status = ST_BREAKDOWN; break; }
         const double a = rr / pq;
-        const C ac((T)a, 0);
+        const C ac = rnd<C>(a);
         for (int64_t i = 0; i < n; ++i) x[i] = x[i] + ac * p[i];
         for (int64_t i = 0; i < n; ++i) r[i] = r[i] - ac * q[i];
         const double rr_new = dot(n, r.data(), r.data()).real();
         const double bt = rr_new / rr;
-        const C bc((T)bt, 0);
+        const C bc = rnd<C>(bt);
         for (int64_t i = 0; i < n; ++i) p[i] = r[i] + bc * p[i];
         rr = rr_new; ++it;
         if (std::sqrt(rr) <= tol * bnorm) { status = ST_OK; break; }
@@ -322,26 +333,25 @@ int cg(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol, int 
 // ------------------------------------------------------------------------------------------
 // Plain BiCGStab on (A + sigma I), van der Vorst's form, shadow vector b.  Pin only.
 // ------------------------------------------------------------------------------------------
-template <typename T>
-int bicgstab(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol, int max_iter,
-             std::complex<T>* x, int* iterations, double* relres) {
-    typedef std::complex<T> C;
+template <typename C>
+int bicgstab(const Csr<C>& A, double sigma, const C* b, double tol, int max_iter,
+             C* x, int* iterations, double* relres) {
     const int64_t n = A.n;
     std::vector<C> r(b, b + n), p(b, b + n), rhat(b, b + n), v(n), s(n), t(n);
-    for (int64_t i = 0; i < n; ++i) x[i] = C(0, 0);
+    for (int64_t i = 0; i < n; ++i) x[i] = C(0);
     zdouble rho = dot(n, rhat.data(), r.data());
     double rr = rho.real();
     const double bnorm = std::sqrt(rr);
     int it = 0, status = ST_MAXITER;
     if (bnorm == 0.0) { *iterations = 0; if (relres) *relres = 0.0; return ST_OK; }
-    const C sg((T)sigma, 0);
+    const C sg = rnd<C>(sigma);
     while (it < max_iter) {
         spmv(A, p.data(), v.data());
         if (sigma != 0.0) for (int64_t i = 0; i < n; ++i) v[i] = v[i] + sg * p[i];
         const zdouble rv = dot(n, rhat.data(), v.data());
         if (rv == zdouble(0, 0) || rho == zdouble(0, 0)) { status = ST_BREAKDOWN; break; }
         const zdouble a = rho / rv;
-        const C ac = rnd<T>(a);
+        const C ac = rnd<C>(a);
         for (int64_t i = 0; i < n; ++i) s[i] = r[i] - ac * v[i];
         spmv(A, s.data(), t.data());
         if (sigma != 0.0) for (int64_t i = 0; i < n; ++i) t[i] = t[i] + sg * s[i];
@@ -349,12 +359,12 @@ int bicgstab(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol
         const double tt = dot(n, t.data(), t.data()).real();
         if (!(tt > 0.0)) { status = ST_BREAKDOWN; break; }
         const zdouble w = ts / tt;
-        const C wc = rnd<T>(w);
+        const C wc = rnd<C>(w);
         for (int64_t i = 0; i < n; ++i) x[i] = (x[i] + ac * p[i]) + wc * s[i];
         for (int64_t i = 0; i < n; ++i) r[i] = s[i] - wc * t[i];
         const zdouble rho_new = dot(n, rhat.data(), r.data());
         const zdouble bt = (rho_new / rho) * (a / w);
-        const C bc = rnd<T>(bt);
+        const C bc = rnd<C>(bt);
         for (int64_t i = 0; i < n; ++i) p[i] = r[i] + bc * (p[i] - wc * v[i]);
         rho = rho_new; ++it;
         rr = dot(n, r.data(), r.data()).real();
@@ -368,58 +378,86 @@ int bicgstab(const Csr<T>& A, double sigma, const std::complex<T>* b, double tol
 }  // namespace
 
 // ------------------------------------------------------------------------------------------
-// C entry points (host pointers only).  dtype: 0 = complex64, 1 = complex128.
+// C entry points (host pointers only).
+// dtype: 0 = complex64, 1 = complex128, 2 = float32, 3 = float64 (real: the paper's Table 1 runs).
 // ------------------------------------------------------------------------------------------
-#define DISPATCH(call_f, call_d) (dtype == 0 ? (call_f) : dtype == 1 ? (call_d) : (int)ST_EINVAL)
+typedef std::complex<float> cfloat;
 
-template <typename T>
-static Csr<T> mk(int64_t n, const int32_t* rp, const int32_t* ci, const void* v) {
-    Csr<T> A; A.n = n; A.rowptr = rp; A.colidx = ci; A.val = (const std::complex<T>*)v; return A;
+template <typename C>
+static Csr<C> mk(int64_t n, const int32_t* rp, const int32_t* ci, const void* v) {
+    Csr<C> A; A.n = n; A.rowptr = rp; A.colidx = ci; A.val = (const C*)v; return A;
+}
+
+#define DISPATCH(F, ...)                                  \
+    switch (dtype) {                                      \
+        case 0: return F<cfloat>(__VA_ARGS__);            \
+        case 1: return F<zdouble>(__VA_ARGS__);           \
+        case 2: return F<float>(__VA_ARGS__);             \
+        case 3: return F<double>(__VA_ARGS__);            \
+        default: return (int)ST_EINVAL;                   \
+    }
+
+template <typename C>
+static int spmv_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, const void* x, void* y) {
+    spmv(mk<C>(n, rowptr, colidx, val), (const C*)x, (C*)y);
+    return 0;
+}
+template <typename C>
+static int cgm_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, const void* b,
+                     const double* shifts, int nshifts, double tol, int max_iter, int stop_rule, void* x,
+                     int* iterations, int* conv_iter, double* relres, void* r_out, double* zeta_out, double* hist, int hist_cap) {
+    return cgm(mk<C>(n, rowptr, colidx, val), (const C*)b, shifts, nshifts, tol, max_iter, stop_rule, (C*)x,
+               iterations, conv_iter, relres, (C*)r_out, zeta_out, hist, hist_cap);
+}
+template <typename C>
+static int bicgstabm_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, const void* b,
+                           const double* shifts, int nshifts, double tol, int max_iter, int stop_rule, void* x,
+                           int* iterations, int* conv_iter, double* relres, void* r_out, double* zeta_out, double* hist, int hist_cap) {
+    return bicgstabm(mk<C>(n, rowptr, colidx, val), (const C*)b, shifts, nshifts, tol, max_iter, stop_rule, (C*)x,
+                     iterations, conv_iter, relres, (C*)r_out, zeta_out, hist, hist_cap);
+}
+template <typename C>
+static int cg_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, double sigma,
+                    const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
+    return cg(mk<C>(n, rowptr, colidx, val), sigma, (const C*)b, tol, max_iter, (C*)x, iterations, relres);
+}
+template <typename C>
+static int bicgstab_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, double sigma,
+                          const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
+    return bicgstab(mk<C>(n, rowptr, colidx, val), sigma, (const C*)b, tol, max_iter, (C*)x, iterations, relres);
 }
 
 extern "C" {
 
 int oracle_spmv_csr(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx,
                     const void* val, const void* x, void* y) {
-    if (dtype == 0) { spmv(mk<float>(n, rowptr, colidx, val), (const std::complex<float>*)x, (std::complex<float>*)y); return 0; }
-    if (dtype == 1) { spmv(mk<double>(n, rowptr, colidx, val), (const std::complex<double>*)x, (std::complex<double>*)y); return 0; }
-    return ST_EINVAL;
+    DISPATCH(spmv_entry, n, rowptr, colidx, val, x, y)
 }
 
 int oracle_cgm(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
                const void* b, const double* shifts, int nshifts, double tol, int max_iter, int stop_rule,
                void* x, int* iterations, int* conv_iter, double* relres,
                void* r_out, double* zeta_out, double* hist, int hist_cap) {
-    return DISPATCH(
-        cgm(mk<float>(n, rowptr, colidx, val), (const std::complex<float>*)b, shifts, nshifts, tol, max_iter, stop_rule,
-            (std::complex<float>*)x, iterations, conv_iter, relres, (std::complex<float>*)r_out, zeta_out, hist, hist_cap),
-        cgm(mk<double>(n, rowptr, colidx, val), (const std::complex<double>*)b, shifts, nshifts, tol, max_iter, stop_rule,
-            (std::complex<double>*)x, iterations, conv_iter, relres, (std::complex<double>*)r_out, zeta_out, hist, hist_cap));
+    DISPATCH(cgm_entry, n, rowptr, colidx, val, b, shifts, nshifts, tol, max_iter, stop_rule, x, iterations,
+             conv_iter, relres, r_out, zeta_out, hist, hist_cap)
 }
 
 int oracle_bicgstabm(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
                      const void* b, const double* shifts, int nshifts, double tol, int max_iter, int stop_rule,
                      void* x, int* iterations, int* conv_iter, double* relres,
                      void* r_out, double* zeta_out, double* hist, int hist_cap) {
-    return DISPATCH(
-        bicgstabm(mk<float>(n, rowptr, colidx, val), (const std::complex<float>*)b, shifts, nshifts, tol, max_iter, stop_rule,
-                  (std::complex<float>*)x, iterations, conv_iter, relres, (std::complex<float>*)r_out, zeta_out, hist, hist_cap),
-        bicgstabm(mk<double>(n, rowptr, colidx, val), (const std::complex<double>*)b, shifts, nshifts, tol, max_iter, stop_rule,
-                  (std::complex<double>*)x, iterations, conv_iter, relres, (std::complex<double>*)r_out, zeta_out, hist, hist_cap));
+    DISPATCH(bicgstabm_entry, n, rowptr, colidx, val, b, shifts, nshifts, tol, max_iter, stop_rule, x, iterations,
+             conv_iter, relres, r_out, zeta_out, hist, hist_cap)
 }
 
 int oracle_cg(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
               double sigma, const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
-    return DISPATCH(
-        cg(mk<float>(n, rowptr, colidx, val), sigma, (const std::complex<float>*)b, tol, max_iter, (std::complex<float>*)x, iterations, relres),
-        cg(mk<double>(n, rowptr, colidx, val), sigma, (const std::complex<double>*)b, tol, max_iter, (std::complex<double>*)x, iterations, relres));
+    DISPATCH(cg_entry, n, rowptr, colidx, val, sigma, b, tol, max_iter, x, iterations, relres)
 }
 
 int oracle_bicgstab(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
                     double sigma, const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
-    return DISPATCH(
-        bicgstab(mk<float>(n, rowptr, colidx, val), sigma, (const std::complex<float>*)b, tol, max_iter, (std::complex<float>*)x, iterations, relres),
-        bicgstab(mk<double>(n, rowptr, colidx, val), sigma, (const std::complex<double>*)b, tol, max_iter, (std::complex<double>*)x, iterations, relres));
+    DISPATCH(bicgstab_entry, n, rowptr, colidx, val, sigma, b, tol, max_iter, x, iterations, relres)
 }
 
 }  // extern "C"

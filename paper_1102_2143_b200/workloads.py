@@ -49,6 +49,12 @@ def unit_rhs(seed: int, n: int) -> np.ndarray:
     return b / np.sqrt(np.sum(b.real ** 2 + b.imag ** 2))
 
 
+def real_unit_rhs(seed: int, n: int) -> np.ndarray:
+    """b: real Gaussian, ||b|| = 1 (the paper's own runs are real-valued)."""
+    b = _substream(seed, "b").standard_normal(n)
+    return b / np.sqrt(np.sum(b * b))
+
+
 def log_shifts(lo: float, hi: float, count: int) -> np.ndarray:
     """`count` points log-spaced from lo to hi, endpoints included."""
     return np.logspace(np.log10(lo), np.log10(hi), count).astype(np.float64)
@@ -194,18 +200,22 @@ def u1_operator_csr(seed: int, extents: Sequence[int], diag: float):
     return rowptr, cols.reshape(-1).astype(np.int32), vals.reshape(-1)
 
 
-def poisson5pt_csr(nx: int, ny: int):
-    """The paper's own test matrix: 2-D 5-point Laplacian, Dirichlet."""
+def poisson5pt_csr(nx: int, ny: int, dtype=np.complex128, drift: float = 0.0):
+    """The paper's own test matrix: 2-D 5-point Laplacian, Dirichlet.
+
+    drift != 0 adds a centred first-derivative term in x (east -1+drift, west -1-drift): a real
+    NON-symmetric convection-diffusion matrix, the real-valued input of the BiCGStab-M tests.
+    """
     idx = np.arange(nx * ny, dtype=np.int64).reshape(ny, nx)
     rows, cols, vals = [idx.ravel()], [idx.ravel()], [np.full(nx * ny, 4.0)]
-    for sl_a, sl_b in (((slice(None), slice(0, nx - 1)), (slice(None), slice(1, nx))),
-                       ((slice(0, ny - 1), slice(None)), (slice(1, ny), slice(None)))):
+    for (sl_a, sl_b), d in ((((slice(None), slice(0, nx - 1)), (slice(None), slice(1, nx))), drift),
+                            (((slice(0, ny - 1), slice(None)), (slice(1, ny), slice(None))), 0.0)):
         a, b = idx[sl_a].ravel(), idx[sl_b].ravel()
         rows += [a, b]
         cols += [b, a]
-        vals += [np.full(a.size, -1.0), np.full(a.size, -1.0)]
+        vals += [np.full(a.size, -1.0 + d), np.full(a.size, -1.0 - d)]
     return coo_to_csr(nx * ny, np.concatenate(rows), np.concatenate(cols),
-                      np.concatenate(vals).astype(np.complex128))
+                      np.concatenate(vals).astype(dtype))
 
 
 def coo_to_csr(n: int, rows: np.ndarray, cols: np.ndarray, vals: np.ndarray):
@@ -369,9 +379,14 @@ def config5(seed: int = DEFAULT_SEED, n: int = 1 << 22, tol: float = 1e-10) -> W
 
 
 def poisson_workload(nx: int, ny: int, nshifts: int = 15, tol: float = 1e-5,
-                     seed: int = DEFAULT_SEED) -> Workload:
-    """The paper's Table-1 workload shape: 2-D Poisson, 15 shifts."""
-    rowptr, colidx, val = poisson5pt_csr(nx, ny)
+                     seed: int = DEFAULT_SEED, real: bool = False, drift: float = 0.0) -> Workload:
+    """The paper's Table-1 workload shape: 2-D Poisson, 15 shifts (the paper does
+    not state their values: log-spaced 1e-3..1 here).  real=True: float64 matrix and right-hand
+    side, as the paper ran it; otherwise the same numbers stored as complex.  drift != 0: the
+    non-symmetric variant for BiCGStab-M."""
+    rowptr, colidx, val = poisson5pt_csr(nx, ny, np.float64 if real else np.complex128, drift)
     n = nx * ny
-    return Workload("poisson5pt_%dx%d" % (nx, ny), "cgm", n, log_shifts(1e-3, 1.0, nshifts), tol,
-                    20000, unit_rhs(seed, n), rowptr, colidx, val, meta={"nx": nx, "ny": ny})
+    b = real_unit_rhs(seed, n) if real else unit_rhs(seed, n)
+    return Workload("poisson5pt_%dx%d%s" % (nx, ny, "_drift" if drift else ""),
+                    "bicgstabm" if drift else "cgm", n, log_shifts(1e-3, 1.0, nshifts), tol,
+                    20000, b, rowptr, colidx, val, meta={"nx": nx, "ny": ny, "drift": drift})

@@ -313,3 +313,46 @@ def test_c64_oracle_tracks_c128(cfg2_small, cfg3_small):
         assert abs(lo.iterations - hi.iterations) <= 1
         for k in range(w.shifts.size):
             assert np.linalg.norm(lo.x[k] - hi.x[k]) / np.linalg.norm(hi.x[k]) < 2e-5
+
+
+# ------------------------------------------------------------------ real dtypes (the paper's own runs)
+def test_real_cgm_poisson_sine_transform():
+    # the paper's runs are REAL fp32/fp64 on the 2-D Poisson matrix.
+    nx, ny = 19, 23
+    w = W.poisson_workload(nx, ny, nshifts=4, tol=1e-13, real=True)
+    assert w.val.dtype == np.float64 and w.b.dtype == np.float64
+    res = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, w.shifts, 1e-13, 5000)
+    assert res.status == oracle.OK and res.x.dtype == np.float64
+    lam = (4.0 - 2.0 * np.cos(np.pi * np.arange(1, nx + 1) / (nx + 1))[None, :]
+           - 2.0 * np.cos(np.pi * np.arange(1, ny + 1) / (ny + 1))[:, None])
+    f = scipy.fft.dstn(w.b.reshape(ny, nx), type=1, norm="ortho")
+    for k, s in enumerate(w.shifts):
+        xe = scipy.fft.idstn(f / (lam + s), type=1, norm="ortho").ravel()
+        assert np.linalg.norm(res.x[k] - xe) / np.linalg.norm(xe) < 1e-10
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_real_oracle_is_the_complex_oracle_on_real_data(dtype):
+    # A real matrix stored as complex has exactly zero imaginary parts throughout ((a+0i)(b+0i) = ab
+    # exactly), so the real-typed oracle must reproduce the (pinned) complex-typed one BITWISE.
+    cdt = np.complex128 if dtype == np.float64 else np.complex64
+    for w, fn in ((W.poisson_workload(13, 11, nshifts=5, tol=1e-9, real=True), oracle.cgm),
+                  (W.poisson_workload(13, 11, nshifts=5, tol=1e-9, real=True, drift=0.4), oracle.bicgstabm)):
+        tol = 1e-9 if dtype == np.float64 else 1e-5
+        re = fn(w.rowptr, w.colidx, w.val.astype(dtype), w.b.astype(dtype), w.shifts, tol, 3000)
+        cx = fn(w.rowptr, w.colidx, w.val.astype(cdt), w.b.astype(cdt), w.shifts, tol, 3000)
+        assert re.status == cx.status == oracle.OK and re.iterations == cx.iterations
+        assert np.array_equal(re.conv_iter, cx.conv_iter)
+        assert np.array_equal(re.x, cx.x.real) and not np.any(cx.x.imag)
+        assert np.array_equal(re.relres, cx.relres)
+
+
+def test_real_bicgstabm_dense_lu():
+    w = W.poisson_workload(9, 8, nshifts=4, tol=1e-14, real=True, drift=0.5)
+    res = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, w.shifts, 1e-14, 3000)
+    assert res.status == oracle.OK
+    A = scipy.sparse.csr_matrix((w.val, w.colidx, w.rowptr), shape=(w.n, w.n)).toarray()
+    assert np.abs(A - A.T).max() > 0.5          # genuinely non-symmetric
+    for k, s in enumerate(w.shifts):
+        xe = np.linalg.solve(A + s * np.eye(w.n), w.b)
+        assert np.linalg.norm(res.x[k] - xe) / np.linalg.norm(xe) < 1e-12
