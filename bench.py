@@ -214,6 +214,8 @@ def main():
     ap.add_argument("--profile-iters", type=int, default=20)
     ap.add_argument("--cpu-iters", type=int, default=6, help="oracle iterations timed for cpu_baseline (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--spmv", default="auto", choices=["auto", "vector", "merge"],
+                    help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
     ap.add_argument("--loop-mode", default="while", choices=["while", "chunk"],
                     help="while: device WHILE graph node (default). chunk: unrolled graph relaunched by the host; "
                          "same kernels, used for ncu (kernel nodes of conditional graphs cannot be profiled)")
@@ -250,10 +252,11 @@ def main():
         return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
     t_create = time.perf_counter()
+    flags = {"auto": ms.MSOLVE_SPMV_AUTO, "vector": ms.MSOLVE_SPMV_VECTOR, "merge": ms.MSOLVE_SPMV_MERGE}[args.spmv]
     if fmt == "bsr3":
-        A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype, copy=False)))
+        A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype, copy=False)), flags)
     else:
-        A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype, copy=False)))
+        A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype, copy=False)), flags)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
     S = int(w.shifts.size)
@@ -341,7 +344,7 @@ def main():
             "dtype": "c128" if dtype == np.complex128 else "c64", "data": "synthetic",
             "config": {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt,
                        "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.nnz), "shifts": S, "tol": w.tol,
-                       "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode,
+                       "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode, "spmv": args.spmv,
                        "l2": "inputs larger than L2 (matrix + %d vectors >> 126 MB), no flush" % (3 + 2 * S)},
             "time_to_solution_ms": ms_total / args.steps, "iterations_per_solve": iters_all / args.steps / world,
             "status": status, "conv_iter": conv_iter, "create_ms": 1e3 * t_create,
