@@ -30,6 +30,7 @@ if ROOT not in sys.path:
 
 from paper_1102_2143_b200 import workloads as W  # noqa: E402
 
+DTYPE_NAME = {np.complex128: "c128", np.complex64: "c64", np.float64: "f64", np.float32: "f32"}
 METRIC = "multishift_solver_iterations_per_s"
 UNIT = "iterations/s"
 
@@ -53,18 +54,22 @@ def make_workload(name: str, rank: int, want_csr: bool):
         w, dt, fmt = W.config5(), np.complex128, "csr"
     elif name == "config5_c64_csr":
         w, dt, fmt = W.config5(tol=1e-5), np.complex64, "csr"
+    elif name in ("poisson1000_f64_csr", "poisson1000_f32_csr"):   # the paper's own Table 1 run
+        dt = np.float64 if "f64" in name else np.float32
+        w, fmt = W.poisson_workload(1000, 1000, nshifts=15, tol=1e-5, real=True), "csr"
+        w.max_iter = 2000                                          # default_monitor(b, 2000, 1e-5)
     elif name == "config5_small_c128_csr":
         w, dt, fmt = W.config5(n=1 << 16), np.complex128, "csr"
     else:
         raise SystemExit("unknown workload %s" % name)
     if rank:
-        w.b = W.unit_rhs(W.DEFAULT_SEED + rank, w.n)
+        w.b = (W.real_unit_rhs if np.isrealobj(w.b) else W.unit_rhs)(W.DEFAULT_SEED + rank, w.n)
     return w, dt, fmt
 
 
 def algorithmic_bytes(w, dtype, fmt, s_active):
     """bytes the method must move per kernel launch (x gathered once)."""
-    e = 16 if dtype == np.complex128 else 8
+    e = np.dtype(dtype).itemsize
     n = w.n
     if fmt == "bsr3":
         nb = w.bcolidx.size
@@ -76,6 +81,11 @@ def algorithmic_bytes(w, dtype, fmt, s_active):
                 "cgm_scal1": 0, "cgm_scal2": 0}
     return {"spmv1_dot": spmv + n * e, "spmv2_dots": spmv + 2 * n * e, "bi_supdate": 3 * n * e,
             "bi_update": (7 + 4 * s_active) * n * e, "bi_scal1": 0, "bi_scal2": 0, "bi_scal3": 0}
+
+
+# The only numbers the paper publishes (Table 1): CG-M, 15 shifts, 2-D
+# Poisson 1000x1000, one Tesla T10: 12.9839 ms/iteration fp64, 8.82461 ms/iteration fp32.
+PAPER_ITERS_PER_S = {"poisson1000_f64_csr": 1e3 / 12.9839, "poisson1000_f32_csr": 1e3 / 8.82461}
 
 
 # ----------------------------------------------------------------------------------- clocks
@@ -131,15 +141,16 @@ def measured_peak_gbs():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic_bytes(kernel_regex: str):
-    """dram read+write bytes per launch of the dominant kernel from the committed ncu summary, or None."""
+def ncu_traffic_bytes(kernel_regex: str, workload: str):
+    """dram read+write bytes per launch of the dominant kernel from the committed ncu summary
+    (only if that capture was taken on this workload), or None."""
     p = os.path.join(ROOT, "profiles", "r01_ncu_dram_traffic.csv")
     if not os.path.exists(p):
         return None
     try:
         for ln in open(p):
             f = ln.strip().split(",")
-            if len(f) >= 2 and f[0] == kernel_regex:
+            if len(f) >= 6 and f[0] == kernel_regex and f[5] == workload:
                 return float(f[1])
     except Exception:
         return None
@@ -194,7 +205,7 @@ def run_reference(args, rank):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "c128" if dtype == np.complex128 else "c64", "data": "synthetic",
+            "dtype": DTYPE_NAME[dtype], "data": "synthetic",
             "config": {"workload": args.workload, "n": w.n, "nnz": int(w.nnz), "shifts": int(w.shifts.size),
                        "format": "csr", "algorithm": w.algorithm},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
@@ -244,7 +255,8 @@ def main():
 
     need_csr = args.workload.endswith("_csr") or (rank == 0 and world == 1 and args.cpu_iters > 0)
     w, dtype, fmt = make_workload(args.workload, rank, want_csr=need_csr)
-    tdt = torch.complex128 if dtype == np.complex128 else torch.complex64
+    tdt = {np.complex128: torch.complex128, np.complex64: torch.complex64,
+           np.float64: torch.float64, np.float32: torch.float32}[dtype]
     alg = ms.MSOLVE_ALG_CGM if w.algorithm == "cgm" else ms.MSOLVE_ALG_BICGSTABM
     solve = ms.msolve_cgm if w.algorithm == "cgm" else ms.msolve_bicgstabm
 
@@ -326,7 +338,7 @@ def main():
                              "GBps": round(gbs, 1), "frac_measured_peak": round(gbs / peak, 4),
                              "frac_8TBps": round(gbs / 8000.0, 4)}
         dom = "cgm_update" if w.algorithm == "cgm" else "bi_update"
-        traffic = ncu_traffic_bytes(dom)
+        traffic = ncu_traffic_bytes(dom, args.workload)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["GBps"], "peak": peak,
                     "unit": "GB/s", "frac": round(kernels[dom]["GBps"] / peak, 4), "peak_source": peak_src,
                     "traffic": traffic, "algorithmic_bytes_per_launch": ab[dom]}
@@ -340,8 +352,10 @@ def main():
         line = {
             "metric": METRIC, "value": throughput(iters_all, ms_total), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "c128" if dtype == np.complex128 else "c64", "data": "synthetic",
+            "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": (throughput(iters_all, ms_total) / world / PAPER_ITERS_PER_S[args.workload]
+                            if args.workload in PAPER_ITERS_PER_S else None),
+            "dtype": DTYPE_NAME[dtype], "data": "synthetic",
             "config": {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt,
                        "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.nnz), "shifts": S, "tol": w.tol,
                        "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode, "spmv": args.spmv,

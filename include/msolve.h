@@ -22,8 +22,9 @@
  *    msolve_last_error() gives the text of the last failure of the calling thread.
  *  - Pointers named d_* are DEVICE pointers, h_* are HOST pointers.  Device buffers are owned
  *    by the caller (e.g. torch tensors); the library never frees them.
- *  - Complex numbers are interleaved (re, im) pairs of float (MSOLVE_C64) or double
- *    (MSOLVE_C128).  Indices are int32.  All device arrays must be 16-byte aligned.
+ *  - Elements are interleaved (re, im) pairs of float (MSOLVE_C64) or double (MSOLVE_C128), or
+ *    plain float / double (MSOLVE_F32 / MSOLVE_F64).  "complex" below means "element of the
+ *    handle's dtype".  Indices are int32.  All device arrays must be 16-byte aligned.
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *  - A handle may be used by one solve at a time (it owns the device-side solver state and the
  *    cached CUDA graphs); different handles are independent.
@@ -40,7 +41,10 @@ extern "C" {
 
 typedef struct msolve_matrix msolve_matrix; /* opaque */
 
-enum { MSOLVE_C64 = 0, MSOLVE_C128 = 1 };
+/* Element type of the matrix and of every vector.  Complex = interleaved (re, im) pairs: the
+ * BASELINE lattice / unstructured configs.  Real: the paper's own measurements are real fp32 /
+ * fp64 (Table 1); CSR only. */
+enum { MSOLVE_C64 = 0, MSOLVE_C128 = 1, MSOLVE_F32 = 2, MSOLVE_F64 = 3 };
 
 enum { MSOLVE_ALG_CGM = 0, MSOLVE_ALG_BICGSTABM = 1 };
 

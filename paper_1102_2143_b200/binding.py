@@ -17,7 +17,7 @@ import torch
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmsolve.so")
 
-MSOLVE_C64, MSOLVE_C128 = 0, 1
+MSOLVE_C64, MSOLVE_C128, MSOLVE_F32, MSOLVE_F64 = 0, 1, 2, 3
 MSOLVE_ALG_CGM, MSOLVE_ALG_BICGSTABM = 0, 1
 MSOLVE_OK, MSOLVE_MAXITER, MSOLVE_BREAKDOWN = 0, 1, 2
 MSOLVE_EINVAL, MSOLVE_ECUDA, MSOLVE_ENOMEM = -1, -2, -3
@@ -91,7 +91,11 @@ def _dtype_code(t: torch.Tensor) -> int:
         return MSOLVE_C64
     if t.dtype == torch.complex128:
         return MSOLVE_C128
-    raise TypeError("expected complex64 / complex128, got %s" % t.dtype)
+    if t.dtype == torch.float32:
+        return MSOLVE_F32
+    if t.dtype == torch.float64:
+        return MSOLVE_F64
+    raise TypeError("expected complex64 / complex128 / float32 / float64, got %s" % t.dtype)
 
 
 def _dev(t: torch.Tensor, dtype=None) -> torch.Tensor:

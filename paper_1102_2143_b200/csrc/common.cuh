@@ -16,14 +16,23 @@ constexpr int kMaxPartials = 4096;  // upper bound on any reducing kernel's grid
 constexpr int kAccMax = 5;          // doubles reduced per CTA (BiCGStab-M SpMV#2 needs 5)
 constexpr int kThreads = 256;
 
-// ----------------------------------------------------------------------------- complex types
-template <typename T> struct Cx;
-template <> struct Cx<float> { typedef float2 type; };
-template <> struct Cx<double> { typedef double2 type; };
+// ----------------------------------------------------------------------------- element types
+// The kernels are templated on the ELEMENT type E of matrices and vectors: float2 / double2 are
+// interleaved complex (MSOLVE_C64 / MSOLVE_C128, the BASELINE configs), float / double are real
+// (MSOLVE_F32 / MSOLVE_F64, the paper's own runs, Table 1).  RealOf<E>::type is
+// the precision T the vector arithmetic is done in; recurrence scalars are always fp64.
+template <typename E> struct RealOf;
+template <> struct RealOf<float>   { typedef float type; };
+template <> struct RealOf<double>  { typedef double type; };
+template <> struct RealOf<float2>  { typedef float type; };
+template <> struct RealOf<double2> { typedef double type; };
 
 template <typename C> __device__ __forceinline__ C cmake(double re, double im);
 template <> __device__ __forceinline__ float2 cmake<float2>(double re, double im) { return make_float2((float)re, (float)im); }
 template <> __device__ __forceinline__ double2 cmake<double2>(double re, double im) { return make_double2(re, im); }
+// real data: every dot product is real, so the imaginary part of every scalar is exactly zero
+template <> __device__ __forceinline__ float cmake<float>(double re, double) { return (float)re; }
+template <> __device__ __forceinline__ double cmake<double>(double re, double) { return re; }
 
 template <typename C> __device__ __forceinline__ C cadd(C a, C b) { C r; r.x = a.x + b.x; r.y = a.y + b.y; return r; }
 template <typename C> __device__ __forceinline__ C csub(C a, C b) { C r; r.x = a.x - b.x; r.y = a.y - b.y; return r; }
@@ -36,6 +45,31 @@ template <typename C> __device__ __forceinline__ C cfma(C a, C b, C acc) {
 }
 // a + s*b with real s
 template <typename C, typename S> __device__ __forceinline__ C caxpy_r(C a, S s, C b) { C r; r.x = a.x + s * b.x; r.y = a.y + s * b.y; return r; }
+// s*a + t*b with real s, t
+template <typename C, typename S> __device__ __forceinline__ C clin_r(S s, C a, S t, C b) { C r; r.x = s * a.x + t * b.x; r.y = s * a.y + t * b.y; return r; }
+// fp64 pieces of the fused reductions: |v|^2, Re / Im of conj(u) v
+template <typename C> __device__ __forceinline__ double cnorm2(C v) { return (double)v.x * v.x + (double)v.y * v.y; }
+template <typename C> __device__ __forceinline__ double cdot_re(C u, C v) { return (double)u.x * (double)v.x + (double)u.y * (double)v.y; }
+template <typename C> __device__ __forceinline__ double cdot_im(C u, C v) { return (double)u.x * (double)v.y - (double)u.y * (double)v.x; }
+template <typename C> __device__ __forceinline__ C cshfl_xor_add(C v, int o) {
+    v.x += __shfl_xor_sync(0xffffffffu, v.x, o); v.y += __shfl_xor_sync(0xffffffffu, v.y, o); return v;
+}
+
+// real overloads (non-templates win overload resolution)
+#define MSOLVE_REAL_OPS(R)                                                                          \
+    __device__ __forceinline__ R cadd(R a, R b) { return a + b; }                                   \
+    __device__ __forceinline__ R csub(R a, R b) { return a - b; }                                   \
+    __device__ __forceinline__ R cmul(R a, R b) { return a * b; }                                   \
+    __device__ __forceinline__ R cfma(R a, R b, R acc) { acc += a * b; return acc; }                \
+    __device__ __forceinline__ R caxpy_r(R a, R s, R b) { return a + s * b; }                       \
+    __device__ __forceinline__ R clin_r(R s, R a, R t, R b) { return s * a + t * b; }               \
+    __device__ __forceinline__ double cnorm2(R v) { return (double)v * v; }                         \
+    __device__ __forceinline__ double cdot_re(R u, R v) { return (double)u * (double)v; }           \
+    __device__ __forceinline__ double cdot_im(R, R) { return 0.0; }                                 \
+    __device__ __forceinline__ R cshfl_xor_add(R v, int o) { return v + __shfl_xor_sync(0xffffffffu, v, o); }
+MSOLVE_REAL_OPS(float)
+MSOLVE_REAL_OPS(double)
+#undef MSOLVE_REAL_OPS
 
 // ----------------------------------------------------------------------------- memory access
 // Streaming (touched once per iteration, far larger than L2): evict-first loads / stores.

@@ -20,41 +20,36 @@
 namespace msolve {
 
 // ----------------------------------------------------------------------------- vector packs
-// Pack<T,VEC>: VEC complex<T> moved by one load/store instruction (16 bytes when possible).
-template <typename T, int VEC> struct Pack;
-template <> struct __align__(8)  Pack<float, 1>  { float2 v[1]; };
-template <> struct __align__(16) Pack<float, 2>  { float2 v[2]; };
-template <> struct __align__(16) Pack<double, 1> { double2 v[1]; };
+// Pack<E,VEC>: VEC elements of type E moved by ONE load/store instruction (16 bytes whenever the
+// vector length allows it: 1 complex128, 2 complex64 / float64, 4 float32).
+template <typename E, int VEC> struct __align__(sizeof(E) * VEC) Pack { E v[VEC]; };
 
-template <bool STREAM> __device__ __forceinline__ Pack<float, 1> ld_pack(const Pack<float, 1>* p) {
-    Pack<float, 1> r; r.v[0] = STREAM ? __ldcs((const float2*)p) : *(const float2*)p; return r;
-}
-template <bool STREAM> __device__ __forceinline__ Pack<float, 2> ld_pack(const Pack<float, 2>* p) {
-    const float4 t = STREAM ? __ldcs((const float4*)p) : *(const float4*)p;
-    Pack<float, 2> r; r.v[0] = make_float2(t.x, t.y); r.v[1] = make_float2(t.z, t.w); return r;
-}
-template <bool STREAM> __device__ __forceinline__ Pack<double, 1> ld_pack(const Pack<double, 1>* p) {
-    Pack<double, 1> r; r.v[0] = STREAM ? __ldcs((const double2*)p) : *(const double2*)p; return r;
-}
-template <bool STREAM> __device__ __forceinline__ void st_pack(Pack<float, 1>* p, const Pack<float, 1>& r) {
-    if (STREAM) __stcs((float2*)p, r.v[0]); else *(float2*)p = r.v[0];
-}
-template <bool STREAM> __device__ __forceinline__ void st_pack(Pack<float, 2>* p, const Pack<float, 2>& r) {
-    const float4 t = make_float4(r.v[0].x, r.v[0].y, r.v[1].x, r.v[1].y);
-    if (STREAM) __stcs((float4*)p, t); else *(float4*)p = t;
-}
-template <bool STREAM> __device__ __forceinline__ void st_pack(Pack<double, 1>* p, const Pack<double, 1>& r) {
-    if (STREAM) __stcs((double2*)p, r.v[0]); else *(double2*)p = r.v[0];
-}
+template <int BYTES> struct RawOf;
+template <> struct RawOf<4>  { typedef unsigned int type; };
+template <> struct RawOf<8>  { typedef uint2 type; };
+template <> struct RawOf<16> { typedef uint4 type; };
 
-template <typename C, typename T> __device__ __forceinline__ C cz(T re, T im) { C r; r.x = re; r.y = im; return r; }
+template <bool STREAM, typename E, int VEC>
+__device__ __forceinline__ Pack<E, VEC> ld_pack(const Pack<E, VEC>* p) {
+    typedef typename RawOf<sizeof(Pack<E, VEC>)>::type R;
+    union { R raw; Pack<E, VEC> pk; } u;
+    u.raw = STREAM ? __ldcs((const R*)p) : *(const R*)p;
+    return u.pk;
+}
+template <bool STREAM, typename E, int VEC>
+__device__ __forceinline__ void st_pack(Pack<E, VEC>* p, const Pack<E, VEC>& r) {
+    typedef typename RawOf<sizeof(Pack<E, VEC>)>::type R;
+    union { R raw; Pack<E, VEC> pk; } u;
+    u.pk = r;
+    if (STREAM) __stcs((R*)p, u.raw); else *(R*)p = u.raw;
+}
 
 // ----------------------------------------------------------------------------- init
 // r <- b, p <- b (Alg. 1 l.9-10); partial |b|^2 (l.13).  p_k <- b and x_k <- 0 (l.11-12) are not
 // materialised: the first update treats them as such without reading them.
-template <typename T, int VEC>
+template <typename E, int VEC>
 __global__ void __launch_bounds__(kThreads) k_init_vectors(SolveState* st) {
-    typedef Pack<T, VEC> P;
+    typedef Pack<E, VEC> P;
     const long long nvec = st->h.n / VEC;
     const P* b = (const P*)st->h.b;
     P* r = (P*)st->h.r;
@@ -66,7 +61,7 @@ __global__ void __launch_bounds__(kThreads) k_init_vectors(SolveState* st) {
         st_pack<false>(r + i, bv);
         st_pack<false>(p + i, bv);
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) acc[0] += (double)bv.v[e].x * bv.v[e].x + (double)bv.v[e].y * bv.v[e].y;
+        for (int e = 0; e < VEC; ++e) acc[0] += cnorm2(bv.v[e]);
     }
     __shared__ double red[32];
     block_sum<1>(acc, red);
@@ -107,10 +102,11 @@ __global__ void __launch_bounds__(kThreads) k_init_state(SolveState* st) {
 
 // ----------------------------------------------------------------------------- CG-M
 // A1: p <- r + alpha p  (l.27; at n = 0 p = b already)
-template <typename T, int VEC>
+template <typename E, int VEC>
 __global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
     if (st->res.done || st->res.n_iter == 0) return;
-    typedef Pack<T, VEC> P;
+    typedef typename RealOf<E>::type T;
+    typedef Pack<E, VEC> P;
     const long long nvec = st->h.n / VEC;
     const P* r = (const P*)st->h.r;
     P* p = (P*)st->h.p;
@@ -162,11 +158,12 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal1(SolveState* st) {
 
 // A5: the fused multishift update.  UNR shifts are in flight per thread (2*UNR independent
 // 16-byte loads) on top of r and Ap; x_k / p_k are streamed with evict-first hints.
-template <typename T, int VEC, int UNR>
+template <typename E, int VEC, int UNR>
 __global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
     if (st->res.done) return;
-    typedef typename Cx<T>::type C;
-    typedef Pack<T, VEC> P;
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    typedef Pack<E, VEC> P;
     __shared__ T s_zeta[kMaxShifts], s_alpha[kMaxShifts], s_beta[kMaxShifts];
     __shared__ int s_k[kMaxShifts];
     const int na = st->res.nactive;
@@ -208,14 +205,12 @@ __global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
 #pragma unroll
                     for (int e = 0; e < VEC; ++e) {
                         C pe, xe;
-                        if (first) { pe = rv.v[e]; xe = cz<C, T>(0, 0); }            // p_k = b, x_k = 0
+                        if (first) { pe = rv.v[e]; xe = cmake<C>(0.0, 0.0); }        // p_k = b, x_k = 0
                         else {
-                            pe.x = zk * rv.v[e].x + ak * pv[u].v[e].x;               // l.29 (lagged)
-                            pe.y = zk * rv.v[e].y + ak * pv[u].v[e].y;
+                            pe = clin_r(zk, rv.v[e], ak, pv[u].v[e]);                // l.29 (lagged)
                             xe = xv[u].v[e];
                         }
-                        xo.v[e].x = xe.x - bk * pe.x;                                // l.28
-                        xo.v[e].y = xe.y - bk * pe.y;
+                        xo.v[e] = caxpy_r(xe, -bk, pe);                              // l.28
                         po.v[e] = pe;
                     }
                     st_pack<true>((P*)(x + k * n) + i, xo);
@@ -226,7 +221,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
 #pragma unroll
         for (int e = 0; e < VEC; ++e) {
             rv.v[e] = caxpy_r(rv.v[e], beta, qv.v[e]);                               // l.21
-            acc[0] += (double)rv.v[e].x * rv.v[e].x + (double)rv.v[e].y * rv.v[e].y; // l.24
+            acc[0] += cnorm2(rv.v[e]);                                               // l.24
         }
         st_pack<false>(r + i, rv);
     }
@@ -322,11 +317,11 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal1(SolveState* st) {
 }
 
 // s <- r + beta q
-template <typename T, int VEC>
+template <typename E, int VEC>
 __global__ void __launch_bounds__(kThreads) k_bi_supdate(SolveState* st) {
     if (st->res.done) return;
-    typedef typename Cx<T>::type C;
-    typedef Pack<T, VEC> P;
+    typedef E C;
+    typedef Pack<E, VEC> P;
     const long long nvec = st->h.n / VEC;
     const P* r = (const P*)st->h.r;
     const P* q = (const P*)st->h.q;
@@ -397,11 +392,11 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal2(SolveState* st) {
 // The fused BiCGStab-M update: per element read r, s, t, q, p once;
 //   r' = s - chi t ; p <- r' + alpha'(p - chi q) ; |r'|^2 partials; per active shift
 //   x_k <- (x_k - beta_k p_k) + cs_k s ; p_k <- zr_k r' + alpha_k ( p_k - cb_k ( zs_k s - zo_k r ) ).
-template <typename T, int VEC, int UNR>
+template <typename E, int VEC, int UNR>
 __global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
     if (st->res.done) return;
-    typedef typename Cx<T>::type C;
-    typedef Pack<T, VEC> P;
+    typedef E C;
+    typedef Pack<E, VEC> P;
     __shared__ C s_c[kMaxShifts * 7];
     __shared__ int s_k[kMaxShifts];
     const int na = st->res.nactive;
@@ -430,7 +425,7 @@ __global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
         for (int e = 0; e < VEC; ++e) {
             rn.v[e] = csub(sv.v[e], cmul(chi, tv.v[e]));
             pv0.v[e] = cadd(rn.v[e], cmul(alpha_new, csub(pv0.v[e], cmul(chi, qv.v[e]))));
-            acc[0] += (double)rn.v[e].x * rn.v[e].x + (double)rn.v[e].y * rn.v[e].y;
+            acc[0] += cnorm2(rn.v[e]);
         }
         for (int a0 = 0; a0 < na; a0 += UNR) {
             P xv[UNR], pv[UNR];
@@ -451,7 +446,7 @@ __global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
 #pragma unroll
                     for (int e = 0; e < VEC; ++e) {
                         const C pe = first ? rv.v[e] : pv[u].v[e];                   // p_k = b = r at n = 0
-                        const C xe = first ? cz<C, T>(0, 0) : xv[u].v[e];
+                        const C xe = first ? cmake<C>(0.0, 0.0) : xv[u].v[e];
                         xo.v[e] = cadd(csub(xe, cmul(c[0], pe)), cmul(c[1], sv.v[e]));
                         const C ds = csub(cmul(c[5], sv.v[e]), cmul(c[6], rv.v[e]));
                         po.v[e] = cadd(cmul(c[2], rn.v[e]), cmul(c[3], csub(pe, cmul(c[4], ds))));

@@ -69,7 +69,12 @@ struct msolve_matrix {
 };
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
-static size_t elem_bytes(int dtype) { return dtype == MSOLVE_C64 ? 8 : 16; }
+static size_t elem_bytes(int dtype) { return dtype == MSOLVE_C128 ? 16 : dtype == MSOLVE_F32 ? 4 : 8; }
+static bool valid_dtype(int dtype) { return dtype >= MSOLVE_C64 && dtype <= MSOLVE_F64; }
+static bool complex_dtype(int dtype) { return dtype == MSOLVE_C64 || dtype == MSOLVE_C128; }
+template <typename E> struct IsComplex { static constexpr bool value = false; };
+template <> struct IsComplex<float2> { static constexpr bool value = true; };
+template <> struct IsComplex<double2> { static constexpr bool value = true; };
 
 // ------------------------------------------------------------------------------------- launch
 template <typename K>
@@ -89,7 +94,7 @@ static int grid_for(const msolve_matrix* A, K kernel, long long work_items, long
 }
 
 // TMA-staged BSR3 kernel configuration: block rows per tile, lanes per scalar row, pipeline depth
-template <typename T> struct BsrTile;
+template <typename E> struct BsrTile;
 // Tuned on B200 (profiles/r01_spmv_bsr3_tile_sweep.md): many small CTAs per SM (independent
 // tiles in flight hide the x-gather latency), a 2-deep ring is enough for the bulk copies, and a
 // small shared-memory footprint leaves L1 for the gathers.
@@ -101,8 +106,8 @@ template <typename T> struct BsrTile;
 #ifndef MSOLVE_BSR_CPS_F
 #define MSOLVE_BSR_CPS_F 4
 #endif
-template <> struct BsrTile<double> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
-template <> struct BsrTile<float>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS_F; };
+template <> struct BsrTile<double2> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
+template <> struct BsrTile<float2>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS_F; };
 
 // Merge-path CSR kernel configuration: tile capacity (non-zeros), ring depth, CTAs per SM.
 #ifndef MSOLVE_MERGE_CAP
@@ -112,13 +117,25 @@ template <> struct BsrTile<float>  { static constexpr int TB = 2 * MSOLVE_BSR_TB
 #define MSOLVE_MERGE_CPS 4
 #define MSOLVE_MERGE_CPS_F 3
 #endif
-template <typename T> struct MergeTile;
-template <> struct MergeTile<double> { static constexpr int CAP = MSOLVE_MERGE_CAP, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS; };
-template <> struct MergeTile<float>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
+template <typename E> struct MergeTile;
+template <> struct MergeTile<double2> { static constexpr int CAP = MSOLVE_MERGE_CAP, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS; };
+template <> struct MergeTile<float2>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
+template <> struct MergeTile<double>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
+template <> struct MergeTile<float>   { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
 
+// run F<E>() for the element type of `dtype`
+#define DISPATCH_ELEM(dtype, EXPR_C128, EXPR_C64, EXPR_F64, EXPR_F32) \
+    ((dtype) == MSOLVE_C128 ? (EXPR_C128) : (dtype) == MSOLVE_C64 ? (EXPR_C64) : (dtype) == MSOLVE_F64 ? (EXPR_F64) : (EXPR_F32))
+
+static int merge_cps(int dtype) {
+    return DISPATCH_ELEM(dtype, MergeTile<double2>::CPS, MergeTile<float2>::CPS, MergeTile<double>::CPS, MergeTile<float>::CPS);
+}
+static int merge_diag(int dtype) {
+    return DISPATCH_ELEM(dtype, (MergeCfg<double2, MergeTile<double2>::CAP>::kDiag), (MergeCfg<float2, MergeTile<float2>::CAP>::kDiag),
+                         (MergeCfg<double, MergeTile<double>::CAP>::kDiag), (MergeCfg<float, MergeTile<float>::CAP>::kDiag));
+}
 static int merge_grid(const msolve_matrix* A) {
-    const int cps = A->dtype == MSOLVE_C64 ? MergeTile<float>::CPS : MergeTile<double>::CPS;
-    return std::max(1, std::min(A->num_sms * cps, A->dev.aux_count));
+    return std::max(1, std::min(A->num_sms * merge_cps(A->dtype), A->dev.aux_count));
 }
 static int merge_fixup_grid(const msolve_matrix* A) {
     return std::max(1, std::min(A->num_sms, (A->dev.aux_count + kThreads - 1) / kThreads));
@@ -137,20 +154,22 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
         k_spmv_csr_merge_fixup<T, ROLE><<<merge_fixup_grid(A), kThreads, 0, s>>>(A->dev, A->d_state, grid);
         return;
     }
-    if (A->format == FMT_BSR3 && A->kernel == KERNEL_BSR_TMA) {
-        typedef BsrTile<T> B;
-        auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, B::CPS, ROLE>;
-        const int smem = BsrTmaCfg<T, B::TB>::smem_bytes(B::STAGES);
-        static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-        if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-        const int grid = std::max(1, std::min(A->num_sms * B::CPS, A->dev.aux_count));
-        k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-        return;
-    }
-    if (A->format == FMT_BSR3) {
-        auto k = k_spmv_bsr3_rows<T, ROLE>;
-        k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
-        return;
+    if constexpr (IsComplex<T>::value) {               // BSR3 = SU(3) blocks: complex only
+        if (A->format == FMT_BSR3 && A->kernel == KERNEL_BSR_TMA) {
+            typedef BsrTile<T> B;
+            auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, B::CPS, ROLE>;
+            const int smem = BsrTmaCfg<T, B::TB>::smem_bytes(B::STAGES);
+            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
+            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+            const int grid = std::max(1, std::min(A->num_sms * B::CPS, A->dev.aux_count));
+            k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+            return;
+        }
+        if (A->format == FMT_BSR3) {
+            auto k = k_spmv_bsr3_rows<T, ROLE>;
+            k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
+            return;
+        }
     }
 #define VEC_CASE(L)                                                                                     \
     case L: {                                                                                           \
@@ -167,18 +186,26 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
 
 template <int ROLE>
 static void launch_spmv(const msolve_matrix* A, cudaStream_t s) {
-    if (A->dtype == MSOLVE_C64) launch_spmv_t<float, ROLE>(A, s);
-    else launch_spmv_t<double, ROLE>(A, s);
+    switch (A->dtype) {
+        case MSOLVE_C128: launch_spmv_t<double2, ROLE>(A, s); break;
+        case MSOLVE_C64:  launch_spmv_t<float2, ROLE>(A, s); break;
+        case MSOLVE_F64:  launch_spmv_t<double, ROLE>(A, s); break;
+        default:          launch_spmv_t<float, ROLE>(A, s); break;
+    }
 }
 
-// element-wise kernels: VEC complex per 16-byte access when the length allows it
-static int vec_width(const msolve_matrix* A) { return (A->dtype == MSOLVE_C64 && (A->dev.n % 2 == 0)) ? 2 : 1; }
+// element-wise kernels: 16 bytes (1, 2 or 4 elements) per access when the length allows it
+static bool vec16(const msolve_matrix* A) { return A->dev.n % (long long)(16 / elem_bytes(A->dtype)) == 0; }
 
 #define DISPATCH_VEC(A, KERNEL, ...)                                                       \
     do {                                                                                   \
-        if ((A)->dtype == MSOLVE_C128) { KERNEL(double, 1, __VA_ARGS__); }                 \
-        else if (vec_width(A) == 2) { KERNEL(float, 2, __VA_ARGS__); }                     \
-        else { KERNEL(float, 1, __VA_ARGS__); }                                            \
+        const bool v16_ = vec16(A);                                                        \
+        switch ((A)->dtype) {                                                              \
+            case MSOLVE_C128: KERNEL(double2, 1, __VA_ARGS__); break;                      \
+            case MSOLVE_C64: if (v16_) { KERNEL(float2, 2, __VA_ARGS__); } else { KERNEL(float2, 1, __VA_ARGS__); } break; \
+            case MSOLVE_F64: if (v16_) { KERNEL(double, 2, __VA_ARGS__); } else { KERNEL(double, 1, __VA_ARGS__); } break; \
+            default:         if (v16_) { KERNEL(float, 4, __VA_ARGS__); } else { KERNEL(float, 1, __VA_ARGS__); } break;   \
+        }                                                                                  \
     } while (0)
 
 constexpr int kUnrollCgm = 4;
@@ -284,7 +311,7 @@ static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t str
 // blocks per tile, every tile starting at a block index that is a multiple of 4 (16-byte aligned
 // bulk copies for both dtypes).  Falls back to the row kernel when no such partition exists.
 static int build_bsr_tiles(msolve_matrix* A) {
-    const int TB = A->dtype == MSOLVE_C64 ? BsrTile<float>::TB : BsrTile<double>::TB;
+    const int TB = A->dtype == MSOLVE_C64 ? BsrTile<float2>::TB : BsrTile<double2>::TB;
     const int maxb = 9 * TB;
     const long long nbr = A->dev.nbrows;
     std::vector<int32_t> rp((size_t)nbr + 1);
@@ -331,8 +358,7 @@ static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int
         const double mean = (double)nnz / (double)n;
         if ((double)maxlen <= 2.0 * mean + 4.0) return MSOLVE_OK;   // regular rows: vector kernel
     }
-    const int D = A->dtype == MSOLVE_C64 ? MergeCfg<float, MergeTile<float>::CAP>::kDiag
-                                         : MergeCfg<double, MergeTile<double>::CAP>::kDiag;
+    const int D = merge_diag(A->dtype);
     const long long items = n + nnz;
     const long long ntiles = (items + D - 1) / D;
     if (ntiles >= (1ll << 31) - 1) return force ? fail(MSOLVE_EINVAL, "msolve_create_csr: too many tiles") : MSOLVE_OK;
@@ -378,7 +404,7 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
     *out = nullptr;
     if (n < 0 || nnz < 0 || nnz >= (1ll << 31) || n >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad n/nnz");
     if (!d_rowptr || (nnz > 0 && (!d_colidx || !d_val))) return fail(MSOLVE_EINVAL, "msolve_create_csr: NULL array");
-    if (dtype != MSOLVE_C64 && dtype != MSOLVE_C128) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad dtype");
+    if (!valid_dtype(dtype)) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad dtype");
     if (flags < MSOLVE_SPMV_AUTO || flags > MSOLVE_SPMV_MERGE) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad flags");
     if (!aligned16(d_val) || ((uintptr_t)d_colidx & 3u) || ((uintptr_t)d_rowptr & 3u)) return fail(MSOLVE_EINVAL, "msolve_create_csr: misaligned array");
     msolve_matrix* A = new (std::nothrow) msolve_matrix();
@@ -412,7 +438,7 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     *out = nullptr;
     if (nbrows < 0 || nblocks < 0 || nblocks >= (1ll << 31) / 9 || 3 * nbrows >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad sizes");
     if (!d_browptr || (nblocks > 0 && (!d_bcolidx || !d_blocks))) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: NULL array");
-    if (dtype != MSOLVE_C64 && dtype != MSOLVE_C128) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad dtype");
+    if (!complex_dtype(dtype)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: dtype must be MSOLVE_C64 or MSOLVE_C128 (SU(3) blocks are complex)");
     if (flags != MSOLVE_SPMV_AUTO && flags != MSOLVE_SPMV_VECTOR) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad flags");
     if (!aligned16(d_blocks)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: misaligned array");
     msolve_matrix* A = new (std::nothrow) msolve_matrix();

@@ -32,22 +32,20 @@ __device__ __forceinline__ void role_vectors(const SolveState* st, const C*& x, 
 // Fused reductions for one finished row (all accumulation in fp64, R14).
 template <typename C, int ROLE>
 __device__ __forceinline__ void role_epilogue(double* acc, long long row, C yi, const C* x, const C* u) {
-    const double yr = yi.x, ym = yi.y;
     if (ROLE == ROLE_CG) {
-        const C xi = x[row];
-        acc[0] += (double)xi.x * yr + (double)xi.y * ym;
+        acc[0] += cdot_re(x[row], yi);                          // Re <p,q>
     } else if (ROLE == ROLE_B1 || ROLE == ROLE_GEN) {
         const C ui = u[row];
-        acc[0] += (double)ui.x * yr + (double)ui.y * ym;       // conj(u) y
-        acc[1] += (double)ui.x * ym - (double)ui.y * yr;
+        acc[0] += cdot_re(ui, yi);                              // conj(u) y
+        acc[1] += cdot_im(ui, yi);
     } else {
         const C xi = x[row];
         const C ui = u[row];
-        acc[0] += yr * (double)xi.x + ym * (double)xi.y;        // conj(y) x  = <t,s>
-        acc[1] += yr * (double)xi.y - ym * (double)xi.x;
-        acc[2] += yr * yr + ym * ym;                            // <t,t>
-        acc[3] += (double)ui.x * yr + (double)ui.y * ym;        // <r0,t>
-        acc[4] += (double)ui.x * ym - (double)ui.y * yr;
+        acc[0] += cdot_re(yi, xi);                              // conj(y) x  = <t,s>
+        acc[1] += cdot_im(yi, xi);
+        acc[2] += cnorm2(yi);                                   // <t,t>
+        acc[3] += cdot_re(ui, yi);                              // <r0,t>
+        acc[4] += cdot_im(ui, yi);
     }
 }
 
@@ -67,9 +65,9 @@ __device__ __forceinline__ void write_partials(SolveState* st, double (&acc)[NAC
 // row read consecutive non-zeros (coalesced 16-byte values, 4-byte indices).  For short regular
 // lattice rows (27 nnz: LANES = 8, four passes).
 // ------------------------------------------------------------------------------------------
-template <typename T, int LANES, int ROLE>
+template <typename E, int LANES, int ROLE>
 __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveState* st) {
-    typedef typename Cx<T>::type C;
+    typedef E C;
     constexpr int NACC = RoleAcc<ROLE>::value;
     if (ROLE != ROLE_GEN && st->res.done) return;
     const C* x; C* y; const C* u;
@@ -98,10 +96,7 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
             sum = cfma(v, ld_ro(x + c), sum);
         }
 #pragma unroll
-        for (int o = LANES / 2; o > 0; o >>= 1) {
-            sum.x += __shfl_xor_sync(0xffffffffu, sum.x, o);
-            sum.y += __shfl_xor_sync(0xffffffffu, sum.y, o);
-        }
+        for (int o = LANES / 2; o > 0; o >>= 1) sum = cshfl_xor_add(sum, o);
         if (valid && sub == 0) {
             y[row] = sum;
             role_epilogue<C, ROLE>(acc, row, sum, x, u);
@@ -115,9 +110,9 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
 // block row br and multiplies row r of every 3x3 block with the 3-vector x[3*bcol .. +3].
 // The three threads of a block row read one contiguous 144-byte (c128) block between them.
 // ------------------------------------------------------------------------------------------
-template <typename T, int ROLE>
+template <typename E, int ROLE>
 __global__ void __launch_bounds__(kThreads) k_spmv_bsr3_rows(MatDev A, SolveState* st) {
-    typedef typename Cx<T>::type C;
+    typedef E C;
     constexpr int NACC = RoleAcc<ROLE>::value;
     if (ROLE != ROLE_GEN && st->res.done) return;
     const C* x; C* y; const C* u;
@@ -211,21 +206,21 @@ __device__ __forceinline__ float2 ld_hint(const float2* p, uint64_t policy) {
 // Tile table (A.aux, built at create time): int4 {row_begin, row_end, block_begin, block_end},
 // block_begin % 4 == 0 so that every bulk copy is 16-byte aligned for both dtypes.
 // ------------------------------------------------------------------------------------------
-template <typename T, int TB> struct BsrTmaCfg {
+template <typename E, int TB> struct BsrTmaCfg {
     static constexpr int kMaxBlocks = 9 * TB;
     static constexpr int kConsumers = (kMaxBlocks + 31) / 32 * 32;
     static constexpr int kThreadsTotal = kConsumers + 32;
-    static constexpr int kValBytes = kMaxBlocks * 9 * 2 * (int)sizeof(T);
+    static constexpr int kValBytes = kMaxBlocks * 9 * (int)sizeof(E);
     static constexpr int kIdxBytes = kMaxBlocks * 4;
     static constexpr int kStageBytes = kValBytes + kIdxBytes;
-    static constexpr int kPartBytes = kMaxBlocks * 3 * 2 * (int)sizeof(T);   // one partial buffer
+    static constexpr int kPartBytes = kMaxBlocks * 3 * (int)sizeof(E);       // one partial buffer
     static constexpr int smem_bytes(int stages) { return stages * kStageBytes + 2 * kPartBytes + 2 * stages * 8; }
 };
 
-template <typename T, int TB, int STAGES, int CPS, int ROLE>
-__global__ void __launch_bounds__(BsrTmaCfg<T, TB>::kThreadsTotal, CPS) k_spmv_bsr3_tma(MatDev A, SolveState* st) {
-    typedef typename Cx<T>::type C;
-    typedef BsrTmaCfg<T, TB> Cfg;
+template <typename E, int TB, int STAGES, int CPS, int ROLE>
+__global__ void __launch_bounds__(BsrTmaCfg<E, TB>::kThreadsTotal, CPS) k_spmv_bsr3_tma(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef BsrTmaCfg<E, TB> Cfg;
     constexpr int NACC = RoleAcc<ROLE>::value;
     constexpr int NCT = Cfg::kConsumers;
     constexpr int NCW = NCT / 32;

@@ -28,8 +28,8 @@
 
 namespace msolve {
 
-template <typename T, int CAP> struct MergeCfg {
-    typedef typename Cx<T>::type C;
+template <typename E, int CAP> struct MergeCfg {
+    typedef E C;
     static constexpr int kConsumers = 256;
     static constexpr int kThreadsTotal = kConsumers + 32;
     static constexpr int kDiag = CAP - 4;                 // merge items per tile (before 4-alignment of k)
@@ -55,10 +55,10 @@ __device__ __forceinline__ void write_partials_at(SolveState* st, double (&acc)[
     }
 }
 
-template <typename T, int CAP, int STAGES, int CPS, int ROLE>
-__global__ void __launch_bounds__(MergeCfg<T, CAP>::kThreadsTotal, CPS) k_spmv_csr_merge(MatDev A, SolveState* st) {
-    typedef typename Cx<T>::type C;
-    typedef MergeCfg<T, CAP> Cfg;
+template <typename E, int CAP, int STAGES, int CPS, int ROLE>
+__global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_csr_merge(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef MergeCfg<E, CAP> Cfg;
     constexpr int NACC = RoleAcc<ROLE>::value;
     constexpr int NCT = Cfg::kConsumers;
     constexpr int NCW = NCT / 32;
@@ -198,10 +198,7 @@ __global__ void __launch_bounds__(MergeCfg<T, CAP>::kThreadsTotal, CPS) k_spmv_c
                 if (valid) {
                     for (int j = lo + l; j < hi; j += g) sum = cadd(sum, vals[j]);
                 }
-                for (int o = g >> 1; o > 0; o >>= 1) {
-                    sum.x += __shfl_xor_sync(0xffffffffu, sum.x, o);
-                    sum.y += __shfl_xor_sync(0xffffffffu, sum.y, o);
-                }
+                for (int o = g >> 1; o > 0; o >>= 1) sum = cshfl_xor_add(sum, o);
                 if (valid && l == 0) {
                     if (started && ends) {
                         y[r] = sum;
@@ -227,9 +224,9 @@ __global__ void __launch_bounds__(MergeCfg<T, CAP>::kThreadsTotal, CPS) k_spmv_c
 
 // Rows cut by tile boundaries: y[row] = tail of the tile the row begins in + the heads of the
 // following tiles up to the one the row ends in, summed in tile order by one thread.
-template <typename T, int ROLE>
+template <typename E, int ROLE>
 __global__ void __launch_bounds__(kThreads) k_spmv_csr_merge_fixup(MatDev A, SolveState* st, int main_grid) {
-    typedef typename Cx<T>::type C;
+    typedef E C;
     constexpr int NACC = RoleAcc<ROLE>::value;
     if (ROLE != ROLE_GEN && st->res.done) return;
     const C* x; C* y; const C* u;
