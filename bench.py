@@ -42,6 +42,16 @@ def make_workload(name: str, rank: int, want_csr: bool):
         w, dt, fmt = W.config4(want_csr=want_csr), np.complex128, "bsr3"
     elif name == "config4_c64_bsr3":
         w, dt, fmt = W.config4(want_csr=want_csr, tol=1e-5), np.complex64, "bsr3"
+    elif name == "config4_c128_lat":                   # matrix-free operator from the link field
+        w, dt, fmt = W.config4(want_csr=want_csr), np.complex128, "lat"
+    elif name == "config4_c64_lat":
+        w, dt, fmt = W.config4(want_csr=want_csr, tol=1e-5), np.complex64, "lat"
+    elif name == "config4_small_c128_lat":
+        w, dt, fmt = W.config4(extents=(32, 8, 8, 8), want_csr=want_csr), np.complex128, "lat"
+    elif name == "config3_c128_lat":
+        w, dt, fmt = W.config3(), np.complex128, "lat"
+    elif name == "config2_c128_lat":
+        w, dt, fmt = W.config2(), np.complex128, "lat"
     elif name == "config4_c128_csr":
         w, dt, fmt = W.config4(want_csr=True), np.complex128, "csr"
     elif name == "config4_small_c128_bsr3":          # quick functional check of the bench itself
@@ -74,6 +84,8 @@ def algorithmic_bytes(w, dtype, fmt, s_active):
     if fmt == "bsr3":
         nb = w.bcolidx.size
         spmv = nb * (9 * e + 4) + (n // 3 + 1) * 4 + 2 * n * e
+    elif fmt == "lat":          # every link once (d blocks of 9 per site), x in, y out; no indices
+        spmv = w.links.size * e + 2 * n * e
     else:
         spmv = w.nnz * (e + 4) + (n + 1) * 4 + 2 * n * e
     if w.algorithm == "cgm":
@@ -267,6 +279,10 @@ def main():
     flags = {"auto": ms.MSOLVE_SPMV_AUTO, "vector": ms.MSOLVE_SPMV_VECTOR, "merge": ms.MSOLVE_SPMV_MERGE}[args.spmv]
     if fmt == "bsr3":
         A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype, copy=False)), flags)
+    elif fmt == "lat":
+        m = w.meta
+        A = ms.msolve_create_lattice_su3(m["extents"], dev(w.links.astype(dtype, copy=False)), m["diag"], m["c_f"],
+                                         m["c_b"], flags)
     else:
         A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype, copy=False)), flags)
     torch.cuda.synchronize()
@@ -357,7 +373,7 @@ def main():
                             if args.workload in PAPER_ITERS_PER_S else None),
             "dtype": DTYPE_NAME[dtype], "data": "synthetic",
             "config": {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt,
-                       "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.nnz), "shifts": S, "tol": w.tol,
+                       "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.links.size // 9 if fmt == "lat" else w.nnz), "shifts": S, "tol": w.tol,
                        "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode, "spmv": args.spmv,
                        "l2": "inputs larger than L2 (matrix + %d vectors >> 126 MB), no flush" % (3 + 2 * S)},
             "time_to_solution_ms": ms_total / args.steps, "iterations_per_solve": iters_all / args.steps / world,

@@ -89,6 +89,23 @@ int msolve_create_bsr3(msolve_matrix **A, int64_t nbrows, int64_t nblocks,
                        const int32_t *d_browptr /* nbrows+1 */, const int32_t *d_bcolidx /* nblocks */,
                        const void *d_blocks /* nblocks*9 complex */, int dtype, int flags, void *stream);
 
+/* Matrix-free handle for the gauged lattice operator with SU(3) links (the "custom linear
+ * operator" hook of PAPER.md:146 applied to the operator of BASELINE configs 2-4):
+ *
+ *   (A x)(s) = diag x(s) - sum_mu [ c_f U_mu(s) x(s+mu) + c_b U_mu(s-mu)^dagger x(s-mu) ]
+ *
+ * on a periodic lattice of `ndim` (1..4) dimensions with extents h_extents[0..ndim-1] (host), site
+ * index s = x0 + L0 (x1 + L1 (x2 + L2 x3)), scalar row = 3 s + colour, n = 3 V.  d_links holds
+ * links[mu][s] = U_mu(s): ndim * V blocks of 9 complex, row-major 3x3 (borrowed, as above).
+ * The assembled form of the same operator is what msolve_create_bsr3 takes; this handle reads 4
+ * link blocks per site instead of 9 matrix blocks + indices.  dtype: MSOLVE_C64 / MSOLVE_C128.
+ * flags: MSOLVE_SPMV_AUTO = TMA-staged tile kernel when an x0-row is a 16-byte multiple and at most
+ * 32 sites, MSOLVE_SPMV_VECTOR = thread-per-row kernel (any extents).
+ * Errors: EINVAL (ndim, extents, null / misaligned pointer, dtype, flags, 3 V >= 2^31), ECUDA. */
+int msolve_create_lattice_su3(msolve_matrix **A, int ndim, const int32_t *h_extents /* ndim */,
+                              const void *d_links /* ndim*V*9 complex */, double diag, double c_f,
+                              double c_b, int dtype, int flags, void *stream);
+
 /* Bytes of caller-provided device workspace a solve with `nshifts` shifts needs
  * (r, p, Ap [, s, t] and one search direction p_k per shift, Alg. 1 l.10-11).  0 on bad input. */
 size_t msolve_workspace_bytes(const msolve_matrix *A, int nshifts, int algorithm);

@@ -26,7 +26,7 @@ MSOLVE_MAX_SHIFTS = 128
 MSOLVE_CFG_LOOP_MODE = 0
 
 EXPORTS = (
-    "msolve_create_csr", "msolve_create_bsr3", "msolve_workspace_bytes", "msolve_cgm",
+    "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
     "msolve_bicgstabm", "msolve_solve_host", "msolve_spmv", "msolve_profile_iteration",
     "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_destroy",
     "msolve_last_error",
@@ -53,6 +53,7 @@ def load_library() -> ctypes.CDLL:
     vp, i32, i64, dbl, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64, ctypes.c_double, ctypes.c_size_t
     lib.msolve_create_csr.argtypes = [ctypes.POINTER(vp), i64, i64, vp, vp, vp, i32, i32, vp]
     lib.msolve_create_bsr3.argtypes = [ctypes.POINTER(vp), i64, i64, vp, vp, vp, i32, i32, vp]
+    lib.msolve_create_lattice_su3.argtypes = [ctypes.POINTER(vp), i32, vp, vp, dbl, dbl, dbl, i32, i32, vp]
     lib.msolve_workspace_bytes.argtypes = [vp, i32, i32]
     lib.msolve_workspace_bytes.restype = sz
     solver_args = [vp, vp, vp, i32, dbl, i32, vp, vp, sz, vp, vp, vp, vp]
@@ -69,7 +70,7 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_destroy.argtypes = [vp]
     lib.msolve_destroy.restype = None
     lib.msolve_last_error.restype = ctypes.c_char_p
-    for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_cgm", "msolve_bicgstabm",
+    for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_cgm", "msolve_bicgstabm",
                  "msolve_solve_host", "msolve_spmv", "msolve_profile_iteration", "msolve_config"):
         getattr(lib, name).restype = i32
     _lib = lib
@@ -156,6 +157,23 @@ def msolve_create_bsr3(browptr: torch.Tensor, bcolidx: torch.Tensor, blocks: tor
     _check(lib.msolve_create_bsr3(ctypes.byref(h), nbrows, bcolidx.numel(), browptr.data_ptr(), bcolidx.data_ptr(),
                                   blocks.data_ptr(), _dtype_code(blocks), flags, _stream(stream)))
     return Matrix(h.value, blocks.dtype, 3 * nbrows, (browptr, bcolidx, blocks))
+
+
+def msolve_create_lattice_su3(extents: Sequence[int], links: torch.Tensor, diag: float, c_f: float, c_b: float,
+                              flags: int = 0, stream=None) -> Matrix:
+    """Matrix-free gauged lattice operator; links[mu, s] = U_mu(s), shape (ndim, V, 3, 3)."""
+    lib = load_library()
+    links = _dev(links)
+    ext = (ctypes.c_int32 * len(extents))(*[int(e) for e in extents])
+    vol = 1
+    for e in extents:
+        vol *= int(e)
+    if links.numel() != 9 * len(extents) * vol:
+        raise ValueError("links must hold ndim * V blocks of 9 complex numbers")
+    h = ctypes.c_void_p()
+    _check(lib.msolve_create_lattice_su3(ctypes.byref(h), len(extents), ext, links.data_ptr(), float(diag),
+                                         float(c_f), float(c_b), _dtype_code(links), flags, _stream(stream)))
+    return Matrix(h.value, links.dtype, 3 * vol, (links,))
 
 
 def msolve_destroy(A: Matrix) -> None:

@@ -214,6 +214,12 @@ struct MatDev {
     const int32_t* aux;      // merge-path partition table / BSR tile table
     void* carry;             // merge-path: per-tile head / tail partial sums, 2 * aux_count complex
     int aux_count;
+    // matrix-free SU(3) lattice operator (msolve_create_lattice_su3): val = links[ndim][vol][3][3]
+    int lat_ndim;            // 0 for CSR / BSR3
+    int lat_ext[4];          // extents, dimension 0 fastest (unused dimensions = 1)
+    int lat_rows_per_tile;   // x0-rows per tile of the TMA kernel
+    long long lat_vol;       // number of sites
+    double lat_diag, lat_cf, lat_cb;
 };
 
 }  // namespace msolve

@@ -24,25 +24,27 @@ namespace msolve {
 // vector length allows it: 1 complex128, 2 complex64 / float64, 4 float32).
 template <typename E, int VEC> struct __align__(sizeof(E) * VEC) Pack { E v[VEC]; };
 
-template <int BYTES> struct RawOf;
-template <> struct RawOf<4>  { typedef unsigned int type; };
-template <> struct RawOf<8>  { typedef uint2 type; };
-template <> struct RawOf<16> { typedef uint4 type; };
-
-template <bool STREAM, typename E, int VEC>
-__device__ __forceinline__ Pack<E, VEC> ld_pack(const Pack<E, VEC>* p) {
-    typedef typename RawOf<sizeof(Pack<E, VEC>)>::type R;
-    union { R raw; Pack<E, VEC> pk; } u;
-    u.raw = STREAM ? __ldcs((const R*)p) : *(const R*)p;
-    return u.pk;
-}
-template <bool STREAM, typename E, int VEC>
-__device__ __forceinline__ void st_pack(Pack<E, VEC>* p, const Pack<E, VEC>& r) {
-    typedef typename RawOf<sizeof(Pack<E, VEC>)>::type R;
-    union { R raw; Pack<E, VEC> pk; } u;
-    u.pk = r;
-    if (STREAM) __stcs((R*)p, u.raw); else *(R*)p = u.raw;
-}
+// Loads / stores go through the CUDA vector type of the same size (no unions: type punning through
+// memory made ptxas reuse registers between the per-shift loads and serialise them).
+#define MSOLVE_PACK_IO(E, VEC, V, UNPACK, PACK)                                                     \
+    template <bool STREAM> __device__ __forceinline__ Pack<E, VEC> ld_pack(const Pack<E, VEC>* p) { \
+        const V t = STREAM ? __ldcs((const V*)p) : *(const V*)p;                                    \
+        Pack<E, VEC> r; UNPACK; return r;                                                           \
+    }                                                                                               \
+    template <bool STREAM> __device__ __forceinline__ void st_pack(Pack<E, VEC>* p, const Pack<E, VEC>& r) { \
+        const V t = PACK;                                                                           \
+        if (STREAM) __stcs((V*)p, t); else *(V*)p = t;                                              \
+    }
+MSOLVE_PACK_IO(double2, 1, double2, r.v[0] = t, r.v[0])
+MSOLVE_PACK_IO(float2, 1, float2, r.v[0] = t, r.v[0])
+MSOLVE_PACK_IO(float2, 2, float4, (r.v[0] = make_float2(t.x, t.y), r.v[1] = make_float2(t.z, t.w)),
+               make_float4(r.v[0].x, r.v[0].y, r.v[1].x, r.v[1].y))
+MSOLVE_PACK_IO(double, 1, double, r.v[0] = t, r.v[0])
+MSOLVE_PACK_IO(double, 2, double2, (r.v[0] = t.x, r.v[1] = t.y), make_double2(r.v[0], r.v[1]))
+MSOLVE_PACK_IO(float, 1, float, r.v[0] = t, r.v[0])
+MSOLVE_PACK_IO(float, 4, float4, (r.v[0] = t.x, r.v[1] = t.y, r.v[2] = t.z, r.v[3] = t.w),
+               make_float4(r.v[0], r.v[1], r.v[2], r.v[3]))
+#undef MSOLVE_PACK_IO
 
 // ----------------------------------------------------------------------------- init
 // r <- b, p <- b (Alg. 1 l.9-10); partial |b|^2 (l.13).  p_k <- b and x_k <- 0 (l.11-12) are not

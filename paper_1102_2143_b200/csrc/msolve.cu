@@ -8,6 +8,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -18,6 +19,7 @@
 #include "kernels.cuh"
 #include "spmv.cuh"
 #include "spmv_merge.cuh"
+#include "spmv_lattice.cuh"
 
 using namespace msolve;
 
@@ -41,8 +43,8 @@ static int fail(int code, const char* fmt, ...) {
     } while (0)
 
 // ------------------------------------------------------------------------------------- handle
-enum { FMT_CSR = 0, FMT_BSR3 = 1 };
-enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3, KERNEL_BSR_TMA = 4 };
+enum { FMT_CSR = 0, FMT_BSR3 = 1, FMT_LATTICE = 2 };
+enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3, KERNEL_BSR_TMA = 4, KERNEL_LAT_ROWS = 5, KERNEL_LAT_TMA = 6 };
 constexpr int kChunk = 8;  // iteration bodies per graph launch in chunked mode
 
 struct LoopGraph {
@@ -109,6 +111,17 @@ template <typename E> struct BsrTile;
 template <> struct BsrTile<double2> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
 template <> struct BsrTile<float2>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS_F; };
 
+// Matrix-free lattice kernel configuration: sites per tile, ring depth, CTAs per SM.
+#ifndef MSOLVE_LAT_NS
+#define MSOLVE_LAT_NS 32
+#define MSOLVE_LAT_STAGES 2
+#define MSOLVE_LAT_CPS 2
+#define MSOLVE_LAT_CPS_F 4
+#endif
+template <typename E> struct LatTile;
+template <> struct LatTile<double2> { static constexpr int NS = MSOLVE_LAT_NS, STAGES = MSOLVE_LAT_STAGES, CPS = MSOLVE_LAT_CPS; };
+template <> struct LatTile<float2>  { static constexpr int NS = MSOLVE_LAT_NS, STAGES = MSOLVE_LAT_STAGES, CPS = MSOLVE_LAT_CPS_F; };
+
 // Merge-path CSR kernel configuration: tile capacity (non-zeros), ring depth, CTAs per SM.
 #ifndef MSOLVE_MERGE_CAP
 #define MSOLVE_MERGE_CAP 1024
@@ -163,6 +176,21 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
             if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
             const int grid = std::max(1, std::min(A->num_sms * B::CPS, A->dev.aux_count));
             k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+            return;
+        }
+        if (A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
+            typedef LatTile<T> L;
+            auto k = k_spmv_lat_tma<T, L::NS, L::STAGES, L::CPS, ROLE>;
+            const int smem = LatCfg<T, L::NS>::smem_bytes(L::STAGES);
+            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
+            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+            const int grid = std::max(1, std::min(A->num_sms * L::CPS, A->dev.aux_count));
+            k<<<grid, LatCfg<T, L::NS>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+            return;
+        }
+        if (A->format == FMT_LATTICE) {
+            auto k = k_spmv_lat_rows<T, ROLE>;
+            k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
             return;
         }
         if (A->format == FMT_BSR3) {
@@ -450,6 +478,51 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     A->kernel = KERNEL_BSR_ROWS;
     int rc = create_common(out, A, (cudaStream_t)stream);
     if (rc == MSOLVE_OK && flags == MSOLVE_SPMV_AUTO && nbrows > 0) rc = build_bsr_tiles(A);
+    if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
+    return rc;
+}
+
+extern "C" int msolve_create_lattice_su3(msolve_matrix** out, int ndim, const int32_t* h_extents, const void* d_links,
+                                         double diag, double c_f, double c_b, int dtype, int flags, void* stream) {
+    if (!out) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: A is NULL");
+    *out = nullptr;
+    if (ndim < 1 || ndim > 4 || !h_extents) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: ndim must be in [1, 4]");
+    long long vol = 1;
+    for (int mu = 0; mu < ndim; ++mu) {
+        if (h_extents[mu] < 1) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: extents must be >= 1");
+        vol *= h_extents[mu];
+        if (3 * vol >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: lattice too large (3 V >= 2^31)");
+    }
+    if (!d_links) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: NULL array");
+    if (!complex_dtype(dtype)) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: dtype must be MSOLVE_C64 or MSOLVE_C128");
+    if (flags != MSOLVE_SPMV_AUTO && flags != MSOLVE_SPMV_VECTOR) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: bad flags");
+    if (!aligned16(d_links)) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: misaligned array");
+    if (!std::isfinite(diag) || !std::isfinite(c_f) || !std::isfinite(c_b)) return fail(MSOLVE_EINVAL, "msolve_create_lattice_su3: non-finite coefficient");
+    msolve_matrix* A = new (std::nothrow) msolve_matrix();
+    if (!A) return fail(MSOLVE_ENOMEM, "out of host memory");
+    A->format = FMT_LATTICE;
+    A->dtype = dtype;
+    A->dev.rowptr = nullptr; A->dev.colidx = nullptr; A->dev.val = d_links;
+    A->dev.n = 3 * vol; A->dev.nbrows = vol; A->dev.nnz = (long long)ndim * vol;
+    A->dev.aux = nullptr; A->dev.aux_count = 0; A->dev.carry = nullptr;
+    A->dev.lat_ndim = ndim;
+    for (int mu = 0; mu < 4; ++mu) A->dev.lat_ext[mu] = mu < ndim ? h_extents[mu] : 1;
+    A->dev.lat_vol = vol;
+    A->dev.lat_diag = diag; A->dev.lat_cf = c_f; A->dev.lat_cb = c_b;
+    A->dev.lat_rows_per_tile = 1;
+    A->kernel = KERNEL_LAT_ROWS;
+    // TMA tile kernel: every x0-row of links / x must be a 16-byte multiple and fit a tile
+    const int L0 = h_extents[0];
+    const int NS = dtype == MSOLVE_C128 ? LatTile<double2>::NS : LatTile<float2>::NS;
+    const bool row16 = ((size_t)L0 * 3 * elem_bytes(dtype)) % 16 == 0;
+    if (flags == MSOLVE_SPMV_AUTO && row16 && L0 <= NS) {
+        const int T = NS / L0;
+        const long long nrows = vol / L0;
+        A->dev.lat_rows_per_tile = T;
+        A->dev.aux_count = (int)((nrows + T - 1) / T);
+        A->kernel = KERNEL_LAT_TMA;
+    }
+    int rc = create_common(out, A, (cudaStream_t)stream);
     if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
     return rc;
 }

@@ -1,0 +1,250 @@
+// spmv_lattice.cuh -- matrix-free gauged lattice operator with SU(3) links (the
+// "custom linear operator" hook the paper advertises, applied to the operator of
+// BASELINE configs 2-4):
+//
+//   (A x)(s) = D x(s) - sum_mu [ c_f U_mu(s) x(s+mu) + c_b U_mu(s-mu)^dagger x(s-mu) ]
+//
+// read straight from the link field links[mu][s] = U_mu(s) (3x3 complex, row-major) instead of an
+// assembled BSR3 matrix: 4 x 144 B of links per site (c128) instead of 9 x 148 B of blocks and
+// indices.  Every link is used twice (forward at s, backward at s+mu); the second use is an L2 hit.
+//
+// Site index s = x0 + L0 (x1 + L1 (x2 + L2 x3)), periodic; scalar row = 3 s + colour.
+//
+// k_spmv_lat_tma: a tile is T consecutive x0-rows (T L0 <= NS sites, contiguous in memory).  All
+// operands of a tile are contiguous byte ranges, so the producer thread moves EVERYTHING with 1-D
+// bulk async copies (TMA engine) into a shared-memory ring -- there is not a single gather:
+//   * forward links U_mu(s) of the tile's sites: one range per direction;
+//   * backward links U_mu(s-mu), mu >= 1: per x0-row one range (the row at coordinate x_mu - 1);
+//     mu = 0: U_0(s-0) is the forward link of the left neighbour in the same row, already staged;
+//   * x of the tile's sites (one range), and per x0-row the 2(d-1) neighbour rows; the mu = 0
+//     neighbours are the same row rotated by one site.
+// Phase 1: one consumer thread per (direction term, site) multiplies its 3x3 link (or its conjugate
+// transpose) with the neighbour's 3-vector out of shared memory and leaves a 3-vector partial.
+// Phase 2 (one named barrier later): one thread per scalar row combines the 2d partials with the
+// diagonal term, writes y (coalesced) and feeds the fused dot products.
+#pragma once
+
+#include "spmv.cuh"
+
+namespace msolve {
+
+// acc + conj(a) * b
+template <typename C> __device__ __forceinline__ C cfma_conj(C a, C b, C acc) {
+    acc.x += a.x * b.x; acc.x += a.y * b.y;
+    acc.y += a.x * b.y; acc.y -= a.y * b.x;
+    return acc;
+}
+
+// y = D xi - (cf f + cb g)
+template <typename C, typename T>
+__device__ __forceinline__ C lat_combine(T dg, C xi, T cf, C f, T cb, C g) {
+    C r;
+    r.x = dg * xi.x - (cf * f.x + cb * g.x);
+    r.y = dg * xi.y - (cf * f.y + cb * g.y);
+    return r;
+}
+
+// ------------------------------------------------------------------------------------------
+// Fallback (any extents): one thread per scalar row, operands through L1/L2.
+// ------------------------------------------------------------------------------------------
+template <typename E, int ROLE>
+__global__ void __launch_bounds__(kThreads) k_spmv_lat_rows(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    const C* __restrict__ links = (const C*)A.val;
+    const long long vol = A.lat_vol;
+    const int nd = A.lat_ndim;
+    const T dg = (T)A.lat_diag, cf = (T)A.lat_cf, cb = (T)A.lat_cb;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long row = (long long)blockIdx.x * blockDim.x + threadIdx.x; row < A.n; row += stride) {
+        const long long s = row / 3;
+        const int r = (int)(row - 3 * s);
+        C f = cmake<C>(0.0, 0.0), g = f;
+        long long rem = s, str = 1;
+#pragma unroll
+        for (int mu = 0; mu < 4; ++mu) {
+            if (mu >= nd) break;
+            const int L = A.lat_ext[mu];
+            const int c = (int)(rem % L);
+            rem /= L;
+            const long long sf = s + (c + 1 == L ? -(long long)(L - 1) * str : str);
+            const long long sb = s + (c == 0 ? (long long)(L - 1) * str : -str);
+            const C* U = links + ((long long)mu * vol + s) * 9 + 3 * r;      // row r of U_mu(s)
+            const C* xf = x + 3 * sf;
+            f = cfma(ld_ro(U), ld_ro(xf), f);
+            f = cfma(ld_ro(U + 1), ld_ro(xf + 1), f);
+            f = cfma(ld_ro(U + 2), ld_ro(xf + 2), f);
+            const C* V = links + ((long long)mu * vol + sb) * 9 + r;         // column r of U_mu(s-mu)
+            const C* xb = x + 3 * sb;
+            g = cfma_conj(ld_ro(V), ld_ro(xb), g);
+            g = cfma_conj(ld_ro(V + 3), ld_ro(xb + 1), g);
+            g = cfma_conj(ld_ro(V + 6), ld_ro(xb + 2), g);
+            str *= L;
+        }
+        const C sum = lat_combine(dg, ld_ro(x + row), cf, f, cb, g);
+        y[row] = sum;
+        role_epilogue<C, ROLE>(acc, row, sum, x, u);
+    }
+    write_partials<NACC>(st, acc);
+}
+
+// ------------------------------------------------------------------------------------------
+// TMA-staged tile kernel.
+// ------------------------------------------------------------------------------------------
+template <typename E, int NS> struct LatCfg {
+    static constexpr int kConsumers = 8 * NS;                           // (term, site) pairs, d <= 4
+    static constexpr int kThreadsTotal = kConsumers + 32;
+    static constexpr int kLinkSlot = NS * 9 * (int)sizeof(E);           // one direction's links
+    static constexpr int kXSlot = NS * 3 * (int)sizeof(E);              // one neighbour's x
+    static constexpr int kXBase = 7 * kLinkSlot;                        // x slots behind the link slots
+    static constexpr int kStageBytes = 7 * (kLinkSlot + kXSlot);
+    static constexpr int kPartBytes = 8 * NS * 3 * (int)sizeof(E);
+    static constexpr int smem_bytes(int stages) { return stages * kStageBytes + 2 * kPartBytes + 2 * stages * 8; }
+    static_assert((NS & (NS - 1)) == 0, "NS must be a power of two");
+};
+// link slots: 0..3 = forward U_mu(s), mu = 0..3 ; 4..6 = backward U_mu(s-mu), mu = 1..3
+// x slots   : 0 = x(s) ; 1..3 = x(s+mu), mu = 1..3 ; 4..6 = x(s-mu), mu = 1..3
+
+template <typename E, int NS, int STAGES, int CPS, int ROLE>
+__global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_tma(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    typedef LatCfg<E, NS> Cfg;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    constexpr int NCT = Cfg::kConsumers;
+    constexpr int NCW = NCT / 32;
+    constexpr int SZ = (int)sizeof(C);
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    C* part = (C*)(smem + STAGES * Cfg::kStageBytes);
+    uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::kStageBytes + 2 * Cfg::kPartBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, NCW); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    const int nd = A.lat_ndim;
+    const int L0 = A.lat_ext[0];
+    const int TR = A.lat_rows_per_tile;
+    const long long vol = A.lat_vol;
+    const long long nrows = vol / L0;                                    // x0-rows of the lattice
+    const int ntiles = A.aux_count;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    int stage = 0;
+    uint32_t phase = 0;
+    if (threadIdx.x >= NCT) {
+        // ---------------- producer: one elected lane of the last warp
+        if (threadIdx.x == NCT) {
+            const C* __restrict__ links = (const C*)A.val;
+            const uint64_t pol = policy_evict_normal();
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+                mbar_wait(empty0 + 8 * stage, phase ^ 1u);
+                unsigned char* sb = smem + stage * Cfg::kStageBytes;
+                const uint32_t bar = full0 + 8 * stage;
+                const long long row0 = (long long)t * TR;
+                const int nr = (int)min((long long)TR, nrows - row0);
+                const long long site0 = row0 * L0;
+                const uint32_t ns = (uint32_t)(nr * L0);
+                const uint32_t lrow = (uint32_t)(L0 * 9 * SZ), xrow = (uint32_t)(L0 * 3 * SZ);
+                mbar_expect_tx(bar, ns * (uint32_t)SZ * (uint32_t)(9 * nd + 3 + (nd - 1) * 15));
+                for (int mu = 0; mu < nd; ++mu)
+                    bulk_g2s(smem_u32(sb + mu * Cfg::kLinkSlot), links + ((long long)mu * vol + site0) * 9, ns * 9u * SZ, bar, pol);
+                bulk_g2s(smem_u32(sb + Cfg::kXBase), x + 3 * site0, ns * 3u * SZ, bar, pol);
+                for (int rt = 0; rt < nr; ++rt) {
+                    long long rem = row0 + rt, rs = 1;                   // row index = x1 + L1 (x2 + L2 x3)
+#pragma unroll
+                    for (int mu = 1; mu < 4; ++mu) {
+                        if (mu >= nd) break;
+                        const int L = A.lat_ext[mu];
+                        const int c = (int)(rem % L);
+                        rem /= L;
+                        const long long rf = row0 + rt + (c + 1 == L ? -(long long)(L - 1) * rs : rs);
+                        const long long rb = row0 + rt + (c == 0 ? (long long)(L - 1) * rs : -rs);
+                        bulk_g2s(smem_u32(sb + (3 + mu) * Cfg::kLinkSlot + rt * lrow), links + ((long long)mu * vol + rb * L0) * 9, lrow, bar, pol);
+                        bulk_g2s(smem_u32(sb + Cfg::kXBase + mu * Cfg::kXSlot + rt * xrow), x + 3 * rf * L0, xrow, bar, pol);
+                        bulk_g2s(smem_u32(sb + Cfg::kXBase + (3 + mu) * Cfg::kXSlot + rt * xrow), x + 3 * rb * L0, xrow, bar, pol);
+                        rs *= L;
+                    }
+                }
+                if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+            }
+        }
+    } else {
+        // ---------------- consumers.  Thread (d, j): direction term d = 2 mu + (0 fwd | 1 bwd) at
+        // site slot j of the tile; its operand offsets inside a stage never change.
+        const int tid = threadIdx.x;
+        const int d = tid / NS, j = tid & (NS - 1);
+        const int mu = d >> 1;
+        const bool bwd = (d & 1) != 0;
+        int loff, xoff;                                                  // element offsets in a stage
+        if (mu == 0) {
+            const int rt = j / L0, i = j - rt * L0;
+            const int jn = rt * L0 + (bwd ? (i == 0 ? L0 - 1 : i - 1) : (i + 1 == L0 ? 0 : i + 1));
+            loff = (bwd ? jn : j) * 9;
+            xoff = Cfg::kXBase / SZ + jn * 3;
+        } else {
+            loff = ((bwd ? 3 + mu : mu) * NS + j) * 9;
+            xoff = Cfg::kXBase / SZ + ((bwd ? 3 + mu : mu) * NS + j) * 3;
+        }
+        const bool term = d < 2 * nd;
+        const T dg = (T)A.lat_diag, cf = (T)A.lat_cf, cb = (T)A.lat_cb;
+        int pbuf = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
+            const long long row0 = (long long)t * TR;
+            const int nr = (int)min((long long)TR, nrows - row0);
+            const int ns = nr * L0;
+            mbar_wait(full0 + 8 * stage, phase);
+            const C* sb = (const C*)(smem + stage * Cfg::kStageBytes);
+            C* pb = part + pbuf * (8 * NS * 3);
+            if (term && j < ns) {                                       // phase 1
+                const C* a = sb + loff;
+                const C x0 = sb[xoff], x1 = sb[xoff + 1], x2 = sb[xoff + 2];
+                C v0, v1, v2;
+                const C z = cmake<C>(0.0, 0.0);
+                if (!bwd) {
+                    v0 = cfma(a[2], x2, cfma(a[1], x1, cfma(a[0], x0, z)));
+                    v1 = cfma(a[5], x2, cfma(a[4], x1, cfma(a[3], x0, z)));
+                    v2 = cfma(a[8], x2, cfma(a[7], x1, cfma(a[6], x0, z)));
+                } else {                                                 // U^dagger: conj of the columns
+                    v0 = cfma_conj(a[6], x2, cfma_conj(a[3], x1, cfma_conj(a[0], x0, z)));
+                    v1 = cfma_conj(a[7], x2, cfma_conj(a[4], x1, cfma_conj(a[1], x0, z)));
+                    v2 = cfma_conj(a[8], x2, cfma_conj(a[5], x1, cfma_conj(a[2], x0, z)));
+                }
+                C* po = pb + (d * NS + j) * 3;
+                po[0] = v0; po[1] = v1; po[2] = v2;
+            }
+            asm volatile("bar.sync 1, %0;" ::"n"(NCT) : "memory");       // partials visible
+            if (tid < 3 * ns) {                                         // phase 2: scalar row 3 site0 + tid
+                C f = cmake<C>(0.0, 0.0), g = f;
+                for (int m = 0; m < nd; ++m) {
+                    f = cadd(f, pb[(2 * m) * NS * 3 + tid]);
+                    g = cadd(g, pb[(2 * m + 1) * NS * 3 + tid]);
+                }
+                const C xi = sb[Cfg::kXBase / SZ + tid];
+                const C sum = lat_combine(dg, xi, cf, f, cb, g);
+                const long long row = 3 * row0 * L0 + tid;
+                y[row] = sum;
+                role_epilogue<C, ROLE>(acc, row, sum, x, u);
+            }
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);        // this warp is done with the stage
+            pbuf ^= 1;
+            if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+    }
+    write_partials<NACC>(st, acc);
+}
+
+}  // namespace msolve

@@ -309,6 +309,7 @@ class Workload:
     browptr: Optional[np.ndarray] = None   # int32 [n/3+1]
     bcolidx: Optional[np.ndarray] = None   # int32 [nb]
     blocks: Optional[np.ndarray] = None    # complex128 [nb,3,3]
+    links: Optional[np.ndarray] = None     # complex128 [d,V,3,3], links[mu,s] = U_mu(s) (lattice workloads)
     meta: Dict = field(default_factory=dict)
 
     @property
@@ -331,7 +332,7 @@ def su3_workload(name: str, algorithm: str, extents: Sequence[int], diag: float,
     else:
         rowptr = colidx = val = np.zeros(0)
     return Workload(name, algorithm, n, np.asarray(shifts, dtype=np.float64), tol, max_iter,
-                    unit_rhs(seed, n), rowptr, colidx, val, browptr, bcolidx, blocks,
+                    unit_rhs(seed, n), rowptr, colidx, val, browptr, bcolidx, blocks, lk,
                     {"extents": tuple(extents), "diag": diag, "c_f": c_f, "c_b": c_b,
                      "links": links, "seed": seed})
 

@@ -31,6 +31,10 @@ def dev(a):
 def make_matrix(ms, w, dtype, fmt, flags=0):
     if fmt == "bsr3rows":   # the simple one-thread-per-row BSR3 kernel instead of the TMA-staged one
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
+    if fmt in ("lat", "latrows"):   # matrix-free operator from the link field (TMA tile kernel / row kernel)
+        m = w.meta
+        return ms.msolve_create_lattice_su3(m["extents"], dev(w.links.astype(dtype)), m["diag"], m["c_f"], m["c_b"],
+                                            ms.MSOLVE_SPMV_VECTOR if fmt == "latrows" else ms.MSOLVE_SPMV_AUTO)
     if fmt == "bsr3":
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
     if fmt == "csrmerge":   # merge-path CSR forced (AUTO picks it only for irregular rows)
