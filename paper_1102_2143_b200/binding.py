@@ -15,7 +15,8 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmsolve.so")
+# MSOLVE_LIB selects another build of the same library (kernel-tuning sweeps); default: in-tree
+LIB_PATH = os.environ.get("MSOLVE_LIB") or os.path.join(_HERE, "libmsolve.so")
 
 MSOLVE_C64, MSOLVE_C128, MSOLVE_F32, MSOLVE_F64 = 0, 1, 2, 3
 MSOLVE_ALG_CGM, MSOLVE_ALG_BICGSTABM = 0, 1

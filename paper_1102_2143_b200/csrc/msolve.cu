@@ -126,15 +126,19 @@ template <> struct LatTile<float2>  { static constexpr int NS = MSOLVE_LAT_NS, S
 #ifndef MSOLVE_MERGE_CAP
 #define MSOLVE_MERGE_CAP 1024
 #define MSOLVE_MERGE_CAP_F 2048
-#define MSOLVE_MERGE_STAGES 2
-#define MSOLVE_MERGE_CPS 4
-#define MSOLVE_MERGE_CPS_F 3
+#define MSOLVE_MERGE_STAGES 4
+#define MSOLVE_MERGE_STAGES_F 3
+#define MSOLVE_MERGE_CPS 2
+#define MSOLVE_MERGE_CPS_F 2
+#endif
+#ifndef MSOLVE_MERGE_STAGES_F
+#define MSOLVE_MERGE_STAGES_F MSOLVE_MERGE_STAGES
 #endif
 template <typename E> struct MergeTile;
 template <> struct MergeTile<double2> { static constexpr int CAP = MSOLVE_MERGE_CAP, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS; };
-template <> struct MergeTile<float2>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
-template <> struct MergeTile<double>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
-template <> struct MergeTile<float>   { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS_F; };
+template <> struct MergeTile<float2>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
+template <> struct MergeTile<double>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
+template <> struct MergeTile<float>   { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
 
 // run F<E>() for the element type of `dtype`
 #define DISPATCH_ELEM(dtype, EXPR_C128, EXPR_C64, EXPR_F64, EXPR_F32) \
@@ -384,7 +388,10 @@ static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int
     }
     if (!force) {
         const double mean = (double)nnz / (double)n;
-        if ((double)maxlen <= 2.0 * mean + 4.0) return MSOLVE_OK;   // regular rows: vector kernel
+        // Vector kernel unless single rows dwarf the mean (a sub-warp would serialise them): on
+        // config 5 (rows 5..200, mean 32) the vector kernel is the faster one on B200 (1.14 vs
+        // 1.33 ms complex128, 0.91 vs 0.90 ms complex64, profiles/r01_spmv_config5.md).
+        if ((double)maxlen <= 16.0 * mean + 64.0) return MSOLVE_OK;
     }
     const int D = merge_diag(A->dtype);
     const long long items = n + nnz;
@@ -442,6 +449,7 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
     A->dev.rowptr = d_rowptr; A->dev.colidx = d_colidx; A->dev.val = d_val;
     A->dev.n = n; A->dev.nbrows = 0; A->dev.nnz = nnz; A->dev.aux = nullptr; A->dev.aux_count = 0; A->dev.carry = nullptr;
     A->kernel = KERNEL_VECTOR;
+    A->dev.x_pin = (size_t)n * elem_bytes(dtype) <= (size_t)48 << 20;
     const double mean = n > 0 ? (double)nnz / (double)n : 0.0;
     A->lanes = mean > 48 ? 32 : mean > 20 ? 8 : mean > 6 ? 4 : 2;
     int rc = create_common(out, A, (cudaStream_t)stream);

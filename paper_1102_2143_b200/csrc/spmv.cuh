@@ -76,6 +76,7 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
     const int32_t* __restrict__ colidx = A.colidx;
     const int32_t* __restrict__ rowptr = A.rowptr;
     constexpr int RPW = 32 / LANES;  // rows per warp
+    const uint64_t polx = policy_x(A.x_pin);
     const int lane = threadIdx.x & 31;
     const int sub = lane % LANES;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -93,7 +94,7 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
         for (; j < e; j += LANES) {
             const int c = ld_stream(colidx + j);
             const C v = ld_stream(val + j);
-            sum = cfma(v, ld_ro(x + c), sum);
+            sum = cfma(v, ld_xg(x + c, polx), sum);
         }
 #pragma unroll
         for (int o = LANES / 2; o > 0; o >>= 1) sum = cshfl_xor_add(sum, o);
@@ -168,15 +169,6 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     } while (!ok);
-}
-__device__ __forceinline__ uint64_t policy_evict_first() {
-    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p)); return p;
-}
-__device__ __forceinline__ uint64_t policy_evict_normal() {
-    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p)); return p;
-}
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
 }
 // global -> shared bulk copy; bytes % 16 == 0, both addresses 16-byte aligned; completes on `bar`
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t policy) {

@@ -95,6 +95,23 @@ __global__ void __launch_bounds__(kThreads) k_spmv_lat_rows(MatDev A, SolveState
     write_partials<NACC>(st, acc);
 }
 
+// fused reductions with x_i and u_i already in registers (same sums as role_epilogue)
+template <typename C, int ROLE>
+__device__ __forceinline__ void lat_epilogue(double* acc, C yi, C xi, C ui) {
+    if (ROLE == ROLE_CG) {
+        acc[0] += cdot_re(xi, yi);
+    } else if (ROLE == ROLE_B1 || ROLE == ROLE_GEN) {
+        acc[0] += cdot_re(ui, yi);
+        acc[1] += cdot_im(ui, yi);
+    } else {
+        acc[0] += cdot_re(yi, xi);
+        acc[1] += cdot_im(yi, xi);
+        acc[2] += cnorm2(yi);
+        acc[3] += cdot_re(ui, yi);
+        acc[4] += cdot_im(ui, yi);
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // TMA-staged tile kernel.
 // ------------------------------------------------------------------------------------------
@@ -105,7 +122,7 @@ template <typename E, int NS> struct LatCfg {
     static constexpr int kXSlot = NS * 3 * (int)sizeof(E);              // one neighbour's x
     static constexpr int kXBase = 7 * kLinkSlot;                        // x slots behind the link slots
     static constexpr int kStageBytes = 7 * (kLinkSlot + kXSlot);
-    static constexpr int kPartBytes = 8 * NS * 3 * (int)sizeof(E);
+    static constexpr int kPartBytes = 9 * NS * 3 * (int)sizeof(E);      // 8 terms + a copy of x(s)
     static constexpr int smem_bytes(int stages) { return stages * kStageBytes + 2 * kPartBytes + 2 * stages * 8; }
     static_assert((NS & (NS - 1)) == 0, "NS must be a power of two");
 };
@@ -205,9 +222,12 @@ __global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_
             const long long row0 = (long long)t * TR;
             const int nr = (int)min((long long)TR, nrows - row0);
             const int ns = nr * L0;
+            const long long row = 3 * row0 * L0 + tid;
+            C ui = cmake<C>(0.0, 0.0);
+            if (ROLE != ROLE_CG && tid < 3 * ns) ui = ld_ro(u + row);     // in flight while the tile lands
             mbar_wait(full0 + 8 * stage, phase);
             const C* sb = (const C*)(smem + stage * Cfg::kStageBytes);
-            C* pb = part + pbuf * (8 * NS * 3);
+            C* pb = part + pbuf * (9 * NS * 3);
             if (term && j < ns) {                                       // phase 1
                 const C* a = sb + loff;
                 const C x0 = sb[xoff], x1 = sb[xoff + 1], x2 = sb[xoff + 2];
@@ -224,7 +244,14 @@ __global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_
                 }
                 C* po = pb + (d * NS + j) * 3;
                 po[0] = v0; po[1] = v1; po[2] = v2;
+                if (d == 0) {                                            // keep x(s) for the diagonal term
+                    const C* xs = sb + Cfg::kXBase / SZ + j * 3;
+                    C* px = pb + (8 * NS + j) * 3;
+                    px[0] = xs[0]; px[1] = xs[1]; px[2] = xs[2];
+                }
             }
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);        // this warp no longer reads the stage
             asm volatile("bar.sync 1, %0;" ::"n"(NCT) : "memory");       // partials visible
             if (tid < 3 * ns) {                                         // phase 2: scalar row 3 site0 + tid
                 C f = cmake<C>(0.0, 0.0), g = f;
@@ -232,14 +259,11 @@ __global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_
                     f = cadd(f, pb[(2 * m) * NS * 3 + tid]);
                     g = cadd(g, pb[(2 * m + 1) * NS * 3 + tid]);
                 }
-                const C xi = sb[Cfg::kXBase / SZ + tid];
+                const C xi = pb[8 * NS * 3 + tid];
                 const C sum = lat_combine(dg, xi, cf, f, cb, g);
-                const long long row = 3 * row0 * L0 + tid;
                 y[row] = sum;
-                role_epilogue<C, ROLE>(acc, row, sum, x, u);
+                lat_epilogue<C, ROLE>(acc, sum, xi, ui);
             }
-            __syncwarp();
-            if ((tid & 31) == 0) mbar_arrive(empty0 + 8 * stage);        // this warp is done with the stage
             pbuf ^= 1;
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
         }

@@ -124,6 +124,7 @@ __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_c
     } else {
         // ---------------- consumers
         const int tid = threadIdx.x;
+        const uint64_t polx = policy_x(A.x_pin);
         const int32_t* __restrict__ rowptr = A.rowptr;
         C* head = (C*)A.carry;
         C* tail = head + ntiles;
@@ -142,7 +143,7 @@ __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_c
 #pragma unroll
             for (int i = 0; i < IPT; ++i) {
                 const int j = tid + i * NCT;
-                if (j < nz) xn[i] = ld_ro(x + cols[j]);
+                if (j < nz) xn[i] = ld_xg(x + cols[j], polx);
             }
         }
         while (t < ntiles) {
@@ -161,7 +162,7 @@ __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_c
 #pragma unroll
                 for (int i = 0; i < IPT; ++i) {
                     const int j = tid + i * NCT;
-                    if (j < nzn) xn[i] = ld_ro(x + cols[j]);
+                    if (j < nzn) xn[i] = ld_xg(x + cols[j], polx);
                 }
             }
             // phase 1: products, in place

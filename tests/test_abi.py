@@ -41,6 +41,10 @@ def test_validation_without_gpu(lib):
     assert b"bad n/nnz" in lib.msolve_last_error()
     assert lib.msolve_create_csr(ctypes.byref(h), 4, 4, None, None, None, 1, 0, None) == -1
     assert lib.msolve_create_bsr3(ctypes.byref(h), 4, 4, None, None, None, 7, 0, None) == -1
+    ext = (ctypes.c_int32 * 4)(4, 4, 4, 4)
+    assert lib.msolve_create_lattice_su3(ctypes.byref(h), 5, ext, None, 8.0, 1.0, 1.0, 1, 0, None) == -1
+    assert b"ndim" in lib.msolve_last_error()
+    assert lib.msolve_create_lattice_su3(ctypes.byref(h), 4, ext, None, 8.0, 1.0, 1.0, 1, 0, None) == -1
     assert lib.msolve_workspace_bytes(None, 4, 0) == 0
     assert lib.msolve_config(99, 0) == -1
     assert lib.msolve_last_launch_count(None) == 0

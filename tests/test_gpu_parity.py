@@ -189,12 +189,12 @@ def test_config4_scaled_cgm(ms, fmt, dtype, tol):
 @pytest.mark.parametrize("fmt", ["csr", "csrvector", "csrmerge"])
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 def test_config5_scaled_cgm(ms, fmt, dtype, tol):
-    w = W.config5(n=(1 << 15) + 37, tol=tol)       # ragged size; "csr" = AUTO picks merge-path here
+    w = W.config5(n=(1 << 15) + 37, tol=tol)       # ragged size; "csr" = AUTO (vector kernel: rows <= 200)
     g = gpu_solve(ms, w, dtype, fmt)
     o = oracle_solve(w, dtype)
     check_parity(w, dtype, g, o, tol)
     assert np.all(np.diff(g[3]) <= 0)              # larger shifts never converge later
-    per_iter = 5 if fmt == "csrvector" else 6      # merge-path SpMV = tile kernel + carry fix-up
+    per_iter = 6 if fmt == "csrmerge" else 5       # merge-path SpMV = tile kernel + carry fix-up
     assert g[5] == 2 + per_iter * g[1]
 
 
