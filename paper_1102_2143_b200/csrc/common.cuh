@@ -91,20 +91,42 @@ __device__ __forceinline__ uint64_t policy_evict_last() {
 
 // Gathered x of the CSR kernels, loaded with an L2 cache hint: evict_last pins x against the matrix
 // stream when it fits in L2 comfortably (measured on config 5, B200: complex64, 34 MB of x: 0.98 ->
-// 0.91 ms; complex128, 67 MB: 1.14 -> 1.34 ms, so there the policy is evict_normal).
-__device__ __forceinline__ uint64_t policy_x(int pin) { return pin ? policy_evict_last() : policy_evict_normal(); }
-__device__ __forceinline__ double2 ld_xg(const double2* p, uint64_t policy) {
-    double2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(policy)); return r;
+// 0.91 ms; complex128, 67 MB: 1.14 -> 1.34 ms, so there it is a plain ld.global.nc -- a hinted
+// load with an evict_normal policy is slower than the plain one: 1.14 -> 1.38 ms).
+template <bool PIN> __device__ __forceinline__ double2 ld_xg(const double2* p, uint64_t policy) {
+    if (!PIN) return __ldg(p);
+    double2 r; asm("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(policy)); return r;
 }
-__device__ __forceinline__ float2 ld_xg(const float2* p, uint64_t policy) {
-    float2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(policy)); return r;
+template <bool PIN> __device__ __forceinline__ float2 ld_xg(const float2* p, uint64_t policy) {
+    if (!PIN) return __ldg(p);
+    float2 r; asm("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(policy)); return r;
 }
-__device__ __forceinline__ double ld_xg(const double* p, uint64_t policy) {
-    double r; asm volatile("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(r) : "l"(p), "l"(policy)); return r;
+template <bool PIN> __device__ __forceinline__ double ld_xg(const double* p, uint64_t policy) {
+    if (!PIN) return __ldg(p);
+    double r; asm("ld.global.nc.L2::cache_hint.f64 %0, [%1], %2;" : "=d"(r) : "l"(p), "l"(policy)); return r;
 }
-__device__ __forceinline__ float ld_xg(const float* p, uint64_t policy) {
-    float r; asm volatile("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(r) : "l"(p), "l"(policy)); return r;
+template <bool PIN> __device__ __forceinline__ float ld_xg(const float* p, uint64_t policy) {
+    if (!PIN) return __ldg(p);
+    float r; asm("ld.global.nc.L2::cache_hint.f32 %0, [%1], %2;" : "=f"(r) : "l"(p), "l"(policy)); return r;
 }
+
+// Matrix stream of the vector-CSR kernel (read once).  HINT: no L1 allocation + evict-first L2
+// policy; used for elements of <= 8 bytes, where it is faster on B200 (config 5 complex64: 0.91 ->
+// 0.73 ms); 16-byte elements are faster through a plain evict-first load (1.14 vs 1.34 ms).
+#define MSOLVE_LD_MAT(TY, PTX, CONSTRAINT)                                                              \
+    template <bool HINT> __device__ __forceinline__ TY ld_mat(const TY* p, uint64_t pol) {             \
+        if (!HINT) return __ldcs(p);                                                                    \
+        TY r; asm("ld.global.nc.L1::no_allocate.L2::cache_hint." PTX " %0, [%1], %2;" : CONSTRAINT(r) : "l"(p), "l"(pol)); return r; \
+    }
+MSOLVE_LD_MAT(int, "s32", "=r")
+MSOLVE_LD_MAT(float, "f32", "=f")
+MSOLVE_LD_MAT(double, "f64", "=d")
+#undef MSOLVE_LD_MAT
+template <bool HINT> __device__ __forceinline__ float2 ld_mat(const float2* p, uint64_t pol) {
+    if (!HINT) return __ldcs(p);
+    float2 r; asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(pol)); return r;
+}
+template <bool HINT> __device__ __forceinline__ double2 ld_mat(const double2* p, uint64_t) { return __ldcs(p); }
 
 // ----------------------------------------------------------------------------- reductions
 __device__ __forceinline__ double warp_sum(double v) {

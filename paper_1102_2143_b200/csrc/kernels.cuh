@@ -114,7 +114,20 @@ __global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
     P* p = (P*)st->h.p;
     const T alpha = (T)st->alpha.re;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+    constexpr int U = 4;                                   // 2U independent 16-byte loads in flight
+    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + (U - 1) * stride < nvec; i += U * stride) {
+        P rv[U], pv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { rv[u] = ld_pack<false>(r + i + u * stride); pv[u] = ld_pack<false>(p + i + u * stride); }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) pv[u].v[e] = caxpy_r(rv[u].v[e], alpha, pv[u].v[e]);
+            st_pack<false>(p + i + u * stride, pv[u]);
+        }
+    }
+    for (; i < nvec; i += stride) {
         const P rv = ld_pack<false>(r + i);
         P pv = ld_pack<false>(p + i);
 #pragma unroll

@@ -162,12 +162,17 @@ template <typename T, int ROLE>
 static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
     if (A->format == FMT_CSR && A->kernel == KERNEL_MERGE) {
         typedef MergeTile<T> M;
-        auto k = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE>;
+        auto kp = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE, true>;     // x pinned in L2
+        auto kn = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE, false>;
         const int smem = MergeCfg<T, M::CAP>::smem_bytes(M::STAGES);
         static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-        if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+        if (!attr_set) {
+            cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            cudaFuncSetAttribute(kn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+            attr_set = true;
+        }
         const int grid = merge_grid(A);
-        k<<<grid, MergeCfg<T, M::CAP>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+        (A->dev.x_pin ? kp : kn)<<<grid, MergeCfg<T, M::CAP>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
         k_spmv_csr_merge_fixup<T, ROLE><<<merge_fixup_grid(A), kThreads, 0, s>>>(A->dev, A->d_state, grid);
         return;
     }
@@ -205,7 +210,7 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
     }
 #define VEC_CASE(L)                                                                                     \
     case L: {                                                                                           \
-        auto k = k_spmv_csr_vector<T, L, ROLE>;                                                         \
+        auto k = A->dev.x_pin ? k_spmv_csr_vector<T, L, ROLE, true> : k_spmv_csr_vector<T, L, ROLE, false>; \
         k<<<grid_for(A, k, A->dev.n, kThreads / L), kThreads, 0, s>>>(A->dev, A->d_state);              \
         break;                                                                                          \
     }
@@ -386,6 +391,13 @@ static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int
         if (rp[i + 1] < rp[i]) return force ? fail(MSOLVE_EINVAL, "msolve_create_csr: rowptr is not non-decreasing") : MSOLVE_OK;
         maxlen = std::max<long long>(maxlen, rp[i + 1] - rp[i]);
     }
+    if (maxlen * n == nnz) {   // constant row length (stencils, lattices): lanes by the BYTES of a row (measured,
+        const long long rb = maxlen * (long long)elem_bytes(A->dtype);   // config 4 CSR c64: 4 lanes 0.59 ms, 8 lanes 0.75 ms)
+        A->lanes = rb > 768 ? 32 : rb > 320 ? 8 : rb > 96 ? 4 : 2;
+#ifdef MSOLVE_VEC_LANES
+        A->lanes = MSOLVE_VEC_LANES;
+#endif
+    }
     if (!force) {
         const double mean = (double)nnz / (double)n;
         // Vector kernel unless single rows dwarf the mean (a sub-warp would serialise them): on
@@ -449,9 +461,12 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
     A->dev.rowptr = d_rowptr; A->dev.colidx = d_colidx; A->dev.val = d_val;
     A->dev.n = n; A->dev.nbrows = 0; A->dev.nnz = nnz; A->dev.aux = nullptr; A->dev.aux_count = 0; A->dev.carry = nullptr;
     A->kernel = KERNEL_VECTOR;
-    A->dev.x_pin = (size_t)n * elem_bytes(dtype) <= (size_t)48 << 20;
+    A->dev.x_pin = elem_bytes(dtype) <= 8 && (size_t)n * elem_bytes(dtype) <= (size_t)48 << 20;
     const double mean = n > 0 ? (double)nnz / (double)n : 0.0;
     A->lanes = mean > 48 ? 32 : mean > 20 ? 8 : mean > 6 ? 4 : 2;
+#ifdef MSOLVE_VEC_LANES
+    A->lanes = MSOLVE_VEC_LANES;
+#endif
     int rc = create_common(out, A, (cudaStream_t)stream);
     if (rc == MSOLVE_OK && flags != MSOLVE_SPMV_VECTOR && n > 0) {
         const bool force = flags == MSOLVE_SPMV_MERGE;

@@ -65,7 +65,7 @@ __device__ __forceinline__ void write_partials(SolveState* st, double (&acc)[NAC
 // row read consecutive non-zeros (coalesced 16-byte values, 4-byte indices).  For short regular
 // lattice rows (27 nnz: LANES = 8, four passes).
 // ------------------------------------------------------------------------------------------
-template <typename E, int LANES, int ROLE>
+template <typename E, int LANES, int ROLE, bool PIN>
 __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveState* st) {
     typedef E C;
     constexpr int NACC = RoleAcc<ROLE>::value;
@@ -76,7 +76,8 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
     const int32_t* __restrict__ colidx = A.colidx;
     const int32_t* __restrict__ rowptr = A.rowptr;
     constexpr int RPW = 32 / LANES;  // rows per warp
-    const uint64_t polx = policy_x(A.x_pin);
+    constexpr bool HINT = sizeof(E) <= 8;
+    const uint64_t polx = policy_evict_last(), polm = policy_evict_first();
     const int lane = threadIdx.x & 31;
     const int sub = lane % LANES;
     const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
@@ -92,9 +93,9 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
         C sum = cmake<C>(0.0, 0.0);
 #pragma unroll 4
         for (; j < e; j += LANES) {
-            const int c = ld_stream(colidx + j);
-            const C v = ld_stream(val + j);
-            sum = cfma(v, ld_xg(x + c, polx), sum);
+            const int c = ld_mat<HINT>(colidx + j, polm);
+            const C v = ld_mat<HINT>(val + j, polm);
+            sum = cfma(v, ld_xg<PIN>(x + c, polx), sum);
         }
 #pragma unroll
         for (int o = LANES / 2; o > 0; o >>= 1) sum = cshfl_xor_add(sum, o);

@@ -55,7 +55,7 @@ __device__ __forceinline__ void write_partials_at(SolveState* st, double (&acc)[
     }
 }
 
-template <typename E, int CAP, int STAGES, int CPS, int ROLE>
+template <typename E, int CAP, int STAGES, int CPS, int ROLE, bool PIN>
 __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_csr_merge(MatDev A, SolveState* st) {
     typedef E C;
     typedef MergeCfg<E, CAP> Cfg;
@@ -124,7 +124,7 @@ __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_c
     } else {
         // ---------------- consumers
         const int tid = threadIdx.x;
-        const uint64_t polx = policy_x(A.x_pin);
+        const uint64_t polx = policy_evict_last();
         const int32_t* __restrict__ rowptr = A.rowptr;
         C* head = (C*)A.carry;
         C* tail = head + ntiles;
@@ -143,7 +143,7 @@ __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_c
 #pragma unroll
             for (int i = 0; i < IPT; ++i) {
                 const int j = tid + i * NCT;
-                if (j < nz) xn[i] = ld_xg(x + cols[j], polx);
+                if (j < nz) xn[i] = ld_xg<PIN>(x + cols[j], polx);
             }
         }
         while (t < ntiles) {
@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(MergeCfg<E, CAP>::kThreadsTotal, CPS) k_spmv_c
 #pragma unroll
                 for (int i = 0; i < IPT; ++i) {
                     const int j = tid + i * NCT;
-                    if (j < nzn) xn[i] = ld_xg(x + cols[j], polx);
+                    if (j < nzn) xn[i] = ld_xg<PIN>(x + cols[j], polx);
                 }
             }
             // phase 1: products, in place
