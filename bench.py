@@ -239,6 +239,8 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--spmv", default="auto", choices=["auto", "vector", "merge"],
                     help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
+    ap.add_argument("--update-kernel", default="regs", choices=["regs", "tma"],
+                    help="CG-M fused multishift update: register kernel (default) or the TMA-staged kernel")
     ap.add_argument("--loop-mode", default="while", choices=["while", "chunk"],
                     help="while: device WHILE graph node (default). chunk: unrolled graph relaunched by the host; "
                          "same kernels, used for ncu (kernel nodes of conditional graphs cannot be profiled)")
@@ -264,6 +266,7 @@ def main():
     _build.build()
     ms.load_library()
     ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 0 if args.loop_mode == "while" else 1)
+    ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, 1 if args.update_kernel == "tma" else 0)
 
     need_csr = args.workload.endswith("_csr") or (rank == 0 and world == 1 and args.cpu_iters > 0)
     w, dtype, fmt = make_workload(args.workload, rank, want_csr=need_csr)
@@ -374,7 +377,7 @@ def main():
             "dtype": DTYPE_NAME[dtype], "data": "synthetic",
             "config": {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt,
                        "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.links.size // 9 if fmt == "lat" else w.nnz), "shifts": S, "tol": w.tol,
-                       "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode, "spmv": args.spmv,
+                       "parallelism": "replicas x%d" % world, "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel,
                        "l2": "inputs larger than L2 (matrix + %d vectors >> 126 MB), no flush" % (3 + 2 * S)},
             "time_to_solution_ms": ms_total / args.steps, "iterations_per_solve": iters_all / args.steps / world,
             "status": status, "conv_iter": conv_iter, "create_ms": 1e3 * t_create,

@@ -20,12 +20,14 @@
 #include "spmv.cuh"
 #include "spmv_merge.cuh"
 #include "spmv_lattice.cuh"
+#include "update_tma.cuh"
 
 using namespace msolve;
 
 // ------------------------------------------------------------------------------------- errors
 static thread_local char g_err[512] = "";
 static int g_loop_mode = 0;
+static int g_update_kernel = 0;   // 0 = register kernel, 1 = TMA-staged fused update when the vectors allow it
 
 static int fail(int code, const char* fmt, ...) {
     va_list ap;
@@ -250,7 +252,24 @@ constexpr int kUnrollBi = 2;
 
 #define L_INIT(T, V, A, s) { auto k = k_init_vectors<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
 #define L_PUPD(T, V, A, s) { auto k = k_cgm_pupdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
-#define L_CUPD(T, V, A, s) { auto k = k_cgm_update<T, V, kUnrollCgm>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
+#ifndef MSOLVE_UPD_STAGES
+#define MSOLVE_UPD_STAGES 6
+#define MSOLVE_UPD_LAG 2
+#endif
+template <typename T>
+static void launch_cgm_update_tma(const msolve_matrix* A, cudaStream_t s) {
+    typedef UpdTmaCfg<T> U;
+    auto k = k_cgm_update_tma<T, MSOLVE_UPD_STAGES, MSOLVE_UPD_LAG>;
+    const int smem = U::smem_bytes(MSOLVE_UPD_STAGES);
+    static thread_local bool attr_set = false;   // per <T> instantiation
+    if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+    const long long ntiles = (A->dev.n / U::VEC + U::kTile - 1) / U::kTile;
+    const int grid = (int)std::max(1ll, std::min<long long>(A->num_sms, ntiles));
+    k<<<grid, U::kThreadsTotal, smem, s>>>(A->d_state);
+}
+#define L_CUPD(T, V, A, s) {                                                                            \
+    if (V * sizeof(T) == 16 && g_update_kernel == 1) launch_cgm_update_tma<T>(A, s);                      \
+    else { auto k = k_cgm_update<T, V, kUnrollCgm>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); } }
 #define L_SUPD(T, V, A, s) { auto k = k_bi_supdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
 #define L_BUPD(T, V, A, s) { auto k = k_bi_update<T, V, kUnrollBi>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
 
@@ -300,7 +319,7 @@ static int build_graph(msolve_matrix* A, int alg, int mode) {
     if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
     if (g.graph) { cudaGraphDestroy(g.graph); g.graph = nullptr; }
     const int nk = kernels_per_iter(alg);
-    if (mode == 0) {
+    if ((mode & 1) == 0) {
         CU(cudaGraphCreate(&g.graph, 0));
         cudaGraphConditionalHandle cond;
         CU(cudaGraphConditionalHandleCreate(&cond, g.graph, 1, cudaGraphCondAssignDefault));
@@ -568,6 +587,7 @@ extern "C" const char* msolve_last_error(void) { return g_err; }
 
 extern "C" int msolve_config(int key, int value) {
     if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { g_loop_mode = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { g_update_kernel = value; return MSOLVE_OK; }
     return fail(MSOLVE_EINVAL, "msolve_config: bad key/value");
 }
 
@@ -640,7 +660,7 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
         return A->dev.n == 0 ? MSOLVE_OK : MSOLVE_MAXITER;
     }
     const int mode = g_loop_mode;
-    rc = build_graph(A, alg, mode);
+    rc = build_graph(A, alg, mode | (g_update_kernel << 1));
     if (rc != MSOLVE_OK) return rc;
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
     launch_init(A, stream);

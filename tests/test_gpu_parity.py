@@ -177,6 +177,25 @@ def test_config2_cgm(ms, fmt, dtype, tol):
     check_parity(w, dtype, g, o, tol)
 
 
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+@pytest.mark.parametrize("extents", [(8, 8, 8, 8), (6, 5, 7, 9)])     # 1890 sites: tiles with a ragged tail
+def test_update_kernels_agree(ms, extents, dtype, tol):
+    # the register kernel (default) and the TMA-staged fused update do the same arithmetic
+    w = W.config2(extents=extents)
+    o = oracle_solve(w, dtype, tol=tol)
+    xs = []
+    for which in (0, 1):
+        ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, which)
+        try:
+            g = gpu_solve(ms, w, dtype, "bsr3", tol=tol)
+        finally:
+            ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, 0)
+        check_parity(w, dtype, g, o, tol)
+        xs.append(g[2])
+    d = np.linalg.norm(xs[0].astype(np.complex128) - xs[1]) / np.linalg.norm(xs[1])
+    assert d <= (1e-12 if dtype == np.complex128 else 1e-5)
+
+
 @pytest.mark.parametrize("fmt", ["csr", "bsr3"])
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 def test_config4_scaled_cgm(ms, fmt, dtype, tol):
