@@ -140,7 +140,8 @@ int msolve_bicgstabm(const msolve_matrix *A, const void *d_b, const double *h_sh
 
 /* The call of Fig. 1 with HOST vectors: copies h_b to the device, solves,
  * copies all nshifts*n solutions back to h_x (both inside the call, on `stream`).  The library
- * allocates and frees the device vectors and workspace itself.  algorithm = MSOLVE_ALG_*. */
+ * allocates the device vectors and workspace itself and keeps them in the handle for the next call
+ * (grow-only; freed by msolve_destroy).  algorithm = MSOLVE_ALG_*. */
 int msolve_solve_host(const msolve_matrix *A, int algorithm, const void *h_b, const double *h_shifts,
                       int nshifts, double tol, int max_iter, void *h_x,
                       int *h_iterations, int *h_conv_iter, double *h_relres, void *stream);

@@ -67,6 +67,8 @@ struct msolve_matrix {
     SolveState* h_stage = nullptr;      // pinned staging for header / result
     void* d_aux = nullptr;              // library-owned auxiliary matrix data
     void* d_carry = nullptr;            // merge-path carries (library-owned)
+    char* d_host_buf = nullptr;         // msolve_solve_host: device b, x and workspace, kept for the next call
+    size_t host_buf_bytes = 0;
     cudaStream_t capture_stream = nullptr;
     LoopGraph graphs[2];
     int64_t last_launches = 0;
@@ -580,6 +582,7 @@ extern "C" void msolve_destroy(msolve_matrix* A) {
     if (A->h_stage) cudaFreeHost(A->h_stage);
     if (A->d_aux) cudaFree(A->d_aux);
     if (A->d_carry) cudaFree(A->d_carry);
+    if (A->d_host_buf) cudaFree(A->d_host_buf);
     delete A;
 }
 
@@ -718,12 +721,18 @@ extern "C" int msolve_solve_host(const msolve_matrix* A, int algorithm, const vo
     cudaStream_t stream = (cudaStream_t)stream_;
     const size_t eb = elem_bytes(A->dtype);
     const size_t bbytes = (size_t)A->dev.n * eb, xbytes = bbytes * (size_t)nshifts;
-    char* d_all = nullptr;
+    msolve_matrix* Am = const_cast<msolve_matrix*>(A);
     const size_t boff = 0, xoff = align_up(bbytes, 256), woff = xoff + align_up(xbytes, 256);
-    if (cudaMalloc((void**)&d_all, woff + wsb + 256) != cudaSuccess) return fail(MSOLVE_ENOMEM, "msolve_solve_host: cudaMalloc of %zu bytes failed", woff + wsb);
+    if (Am->host_buf_bytes < woff + wsb + 256) {               // grow-only cache of the device buffers
+        if (Am->d_host_buf) cudaFree(Am->d_host_buf);
+        Am->d_host_buf = nullptr; Am->host_buf_bytes = 0;
+        if (cudaMalloc((void**)&Am->d_host_buf, woff + wsb + 256) != cudaSuccess) return fail(MSOLVE_ENOMEM, "msolve_solve_host: cudaMalloc of %zu bytes failed", woff + wsb);
+        Am->host_buf_bytes = woff + wsb + 256;
+    }
+    char* d_all = Am->d_host_buf;
     int rc;
     cudaError_t e = cudaMemcpyAsync(d_all + boff, h_b, bbytes, cudaMemcpyHostToDevice, stream);
-    if (e != cudaSuccess) { cudaFree(d_all); return fail(MSOLVE_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e)); }
+    if (e != cudaSuccess) return fail(MSOLVE_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e));
     rc = run_solver(algorithm, A, d_all + boff, h_shifts, nshifts, tol, max_iter, d_all + xoff, d_all + woff, wsb + 256,
                     h_iterations, h_conv_iter, h_relres, stream_);
     if (rc >= 0) {
@@ -731,7 +740,6 @@ extern "C" int msolve_solve_host(const msolve_matrix* A, int algorithm, const vo
         if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
         if (e != cudaSuccess) rc = fail(MSOLVE_ECUDA, "D2H copy failed: %s", cudaGetErrorString(e));
     }
-    cudaFree(d_all);
     return rc;
 }
 
