@@ -235,7 +235,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4_c128_bsr3")
     ap.add_argument("--profile-iters", type=int, default=20)
-    ap.add_argument("--cpu-iters", type=int, default=6, help="oracle iterations timed for cpu_baseline (0 = skip)")
+    ap.add_argument("--cpu-iters", type=int, default=14, help="oracle iterations timed for cpu_baseline (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--spmv", default="auto", choices=["auto", "vector", "merge"],
                     help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
