@@ -101,7 +101,7 @@ static int grid_for(const msolve_matrix* A, K kernel, long long work_items, long
 
 // TMA-staged BSR3 kernel configuration: block rows per tile, lanes per scalar row, pipeline depth
 template <typename E> struct BsrTile;
-// Tuned on B200 (profiles/r01_spmv_bsr3_tile_sweep.md): many small CTAs per SM (independent
+// Tuned on B200 (profiles/r01_sweeps.md): many small CTAs per SM (independent
 // tiles in flight hide the x-gather latency), a 2-deep ring is enough for the bulk copies, and a
 // small shared-memory footprint leaves L1 for the gathers.
 #ifndef MSOLVE_BSR_TB
@@ -423,7 +423,7 @@ static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int
         const double mean = (double)nnz / (double)n;
         // Vector kernel unless single rows dwarf the mean (a sub-warp would serialise them): on
         // config 5 (rows 5..200, mean 32) the vector kernel is the faster one on B200 (1.14 vs
-        // 1.33 ms complex128, 0.91 vs 0.90 ms complex64, profiles/r01_spmv_config5.md).
+        // 1.33 ms complex128, 0.91 vs 0.90 ms complex64, profiles/r01_sweeps.md).
         if ((double)maxlen <= 16.0 * mean + 64.0) return MSOLVE_OK;
     }
     const int D = merge_diag(A->dtype);
