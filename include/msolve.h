@@ -73,7 +73,9 @@ enum {
                                  unrolled iteration graph with a device `done` flag */
     MSOLVE_CFG_UPDATE_KERNEL = 1 /* CG-M fused multishift update: 0 = register kernel (default), 1 = TMA-staged
                                     kernel (bulk async loads AND stores) whenever the vector length is a multiple
-                                    of 16 bytes.  Same arithmetic; both run at the same 6.0 TB/s on B200 */
+                                    of 16 bytes.  Same arithmetic; both run at the same 6.0 TB/s on B200 */,
+    MSOLVE_CFG_LATTICE_KERNEL = 2 /* tile kernel of msolve_create_lattice_su3 handles: 0 = the faster one per
+                                     element type (default), 1 = (term, site) threads + partials, 2 = warp per tile */
 };
 
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay

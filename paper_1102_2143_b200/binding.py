@@ -26,6 +26,7 @@ MSOLVE_SPMV_AUTO, MSOLVE_SPMV_VECTOR, MSOLVE_SPMV_MERGE = 0, 1, 2
 MSOLVE_MAX_SHIFTS = 128
 MSOLVE_CFG_LOOP_MODE = 0
 MSOLVE_CFG_UPDATE_KERNEL = 1
+MSOLVE_CFG_LATTICE_KERNEL = 2
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",

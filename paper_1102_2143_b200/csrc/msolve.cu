@@ -27,6 +27,7 @@ using namespace msolve;
 // ------------------------------------------------------------------------------------- errors
 static thread_local char g_err[512] = "";
 static int g_loop_mode = 0;
+static int g_lattice_kernel = 0;  // 0 = per element type (see MSOLVE_LAT_WARP), 1 = k_spmv_lat_tma, 2 = k_spmv_lat_warp
 static int g_update_kernel = 0;   // 0 = register kernel, 1 = TMA-staged fused update when the vectors allow it
 
 static int fail(int code, const char* fmt, ...) {
@@ -122,6 +123,27 @@ template <> struct BsrTile<float2>  { static constexpr int TB = 2 * MSOLVE_BSR_T
 #define MSOLVE_LAT_CPS 2
 #define MSOLVE_LAT_CPS_F 4
 #endif
+// Which lattice tile kernel: 1 = warp-per-tile (k_spmv_lat_warp), 0 = (term, site) threads + partials
+// (k_spmv_lat_tma).  Measured on config 4 (profiles/r01_sweeps.md): complex128 0.269 ms (tma) vs
+// 0.277 ms (warp); complex64 0.160 ms (tma) vs 0.150 ms (warp).
+#ifndef MSOLVE_LAT_WARP
+#define MSOLVE_LAT_WARP 0
+#endif
+#ifndef MSOLVE_LAT_WARP_F
+#define MSOLVE_LAT_WARP_F 1
+#endif
+#ifndef MSOLVE_LATW_PW
+#define MSOLVE_LATW_PW 4         // producer warps (bulk-copy issue is the bottleneck)
+#endif
+#ifndef MSOLVE_LATW_W
+#define MSOLVE_LATW_W 2
+#define MSOLVE_LATW_STAGES 4
+#define MSOLVE_LATW_W_F 4
+#define MSOLVE_LATW_STAGES_F 8
+#endif
+template <typename E> struct LatWarpTile;
+template <> struct LatWarpTile<double2> { static constexpr int W = MSOLVE_LATW_W, STAGES = MSOLVE_LATW_STAGES; static constexpr bool USE = MSOLVE_LAT_WARP != 0; };
+template <> struct LatWarpTile<float2>  { static constexpr int W = MSOLVE_LATW_W_F, STAGES = MSOLVE_LATW_STAGES_F; static constexpr bool USE = MSOLVE_LAT_WARP_F != 0; };
 template <typename E> struct LatTile;
 template <> struct LatTile<double2> { static constexpr int NS = MSOLVE_LAT_NS, STAGES = MSOLVE_LAT_STAGES, CPS = MSOLVE_LAT_CPS; };
 template <> struct LatTile<float2>  { static constexpr int NS = MSOLVE_LAT_NS, STAGES = MSOLVE_LAT_STAGES, CPS = MSOLVE_LAT_CPS_F; };
@@ -189,6 +211,16 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
             if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
             const int grid = std::max(1, std::min(A->num_sms * B::CPS, A->dev.aux_count));
             k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+            return;
+        }
+        if ((g_lattice_kernel == 2 || (g_lattice_kernel == 0 && LatWarpTile<T>::USE)) && A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
+            typedef LatWarpTile<T> L;
+            auto k = k_spmv_lat_warp<T, L::W, MSOLVE_LATW_PW, L::STAGES, ROLE>;
+            const int smem = LatWarpCfg<T, L::W, MSOLVE_LATW_PW>::smem_bytes(L::STAGES);
+            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
+            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+            const int grid = std::max(1, std::min(A->num_sms, A->dev.aux_count));
+            k<<<grid, LatWarpCfg<T, L::W, MSOLVE_LATW_PW>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
             return;
         }
         if (A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
@@ -591,6 +623,7 @@ extern "C" const char* msolve_last_error(void) { return g_err; }
 extern "C" int msolve_config(int key, int value) {
     if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { g_loop_mode = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { g_update_kernel = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 2) { g_lattice_kernel = value; return MSOLVE_OK; }
     return fail(MSOLVE_EINVAL, "msolve_config: bad key/value");
 }
 
@@ -663,7 +696,7 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
         return A->dev.n == 0 ? MSOLVE_OK : MSOLVE_MAXITER;
     }
     const int mode = g_loop_mode;
-    rc = build_graph(A, alg, mode | (g_update_kernel << 1));
+    rc = build_graph(A, alg, mode | (g_update_kernel << 1) | (g_lattice_kernel << 2));
     if (rc != MSOLVE_OK) return rc;
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
     launch_init(A, stream);

@@ -112,6 +112,47 @@ __device__ __forceinline__ void lat_epilogue(double* acc, C yi, C xi, C ui) {
     }
 }
 
+// Producer side of both tile kernels, run by ONE elected thread: waits for the stage, posts the byte
+// count and issues the tile's bulk copies (d + 1 + 3 (d-1) per x0-row: 14 for one 4-D row).  Issuing
+// is the bottleneck of these kernels (~0.1 us per copy and thread; spreading the copies over the
+// lanes of a warp is slower still: UBLKCP is a uniform-datapath instruction), hence 32-bit coordinate
+// arithmetic here and several producer warps in k_spmv_lat_warp.
+template <typename C, int LINK_SLOT, int X_SLOT, int X_BASE>
+__device__ __forceinline__ void lat_issue_tile(const MatDev& A, const C* __restrict__ links, const C* x, unsigned char* sb,
+                                               uint32_t bar, uint32_t empty_bar, uint32_t empty_parity, int t, uint64_t pol) {
+    constexpr int SZ = (int)sizeof(C);
+    const int nd = A.lat_ndim, L0 = A.lat_ext[0], TR = A.lat_rows_per_tile;
+    const long long vol = A.lat_vol;
+    const int nrows = (int)(vol / L0);
+    const int row0 = t * TR;
+    const int nr = min(TR, nrows - row0);
+    const long long site0 = (long long)row0 * L0;
+    const uint32_t ns = (uint32_t)(nr * L0);
+    const uint32_t lrow = (uint32_t)(L0 * 9 * SZ), xrow = (uint32_t)(L0 * 3 * SZ);
+    mbar_wait(empty_bar, empty_parity);
+    mbar_expect_tx(bar, ns * (uint32_t)SZ * (uint32_t)(9 * nd + 3 + (nd - 1) * 15));
+    for (int mu = 0; mu < nd; ++mu)                                     // forward links of the tile
+        bulk_g2s(smem_u32(sb + mu * LINK_SLOT), links + ((long long)mu * vol + site0) * 9, ns * 9u * SZ, bar, pol);
+    bulk_g2s(smem_u32(sb + X_BASE), x + 3 * site0, ns * 3u * SZ, bar, pol);
+    for (int rt = 0; rt < nr; ++rt) {
+        const unsigned row = (unsigned)(row0 + rt);                     // = x1 + L1 (x2 + L2 x3)
+        unsigned rem = row, rs = 1;
+#pragma unroll
+        for (int mu = 1; mu < 4; ++mu) {
+            if (mu >= nd) break;
+            const unsigned L = (unsigned)A.lat_ext[mu];
+            const unsigned cm = rem % L;
+            rem /= L;
+            const long long rf = (long long)row + (cm + 1 == L ? -(long long)((L - 1) * rs) : (long long)rs);
+            const long long rb = (long long)row + (cm == 0 ? (long long)((L - 1) * rs) : -(long long)rs);
+            bulk_g2s(smem_u32(sb + (3 + mu) * LINK_SLOT + rt * lrow), links + ((long long)mu * vol + rb * L0) * 9, lrow, bar, pol);
+            bulk_g2s(smem_u32(sb + X_BASE + mu * X_SLOT + rt * xrow), x + 3 * rf * L0, xrow, bar, pol);
+            bulk_g2s(smem_u32(sb + X_BASE + (3 + mu) * X_SLOT + rt * xrow), x + 3 * rb * L0, xrow, bar, pol);
+            rs *= L;
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------
 // TMA-staged tile kernel.
 // ------------------------------------------------------------------------------------------
@@ -167,34 +208,8 @@ __global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_
             const C* __restrict__ links = (const C*)A.val;
             const uint64_t pol = policy_evict_normal();
             for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-                mbar_wait(empty0 + 8 * stage, phase ^ 1u);
-                unsigned char* sb = smem + stage * Cfg::kStageBytes;
-                const uint32_t bar = full0 + 8 * stage;
-                const long long row0 = (long long)t * TR;
-                const int nr = (int)min((long long)TR, nrows - row0);
-                const long long site0 = row0 * L0;
-                const uint32_t ns = (uint32_t)(nr * L0);
-                const uint32_t lrow = (uint32_t)(L0 * 9 * SZ), xrow = (uint32_t)(L0 * 3 * SZ);
-                mbar_expect_tx(bar, ns * (uint32_t)SZ * (uint32_t)(9 * nd + 3 + (nd - 1) * 15));
-                for (int mu = 0; mu < nd; ++mu)
-                    bulk_g2s(smem_u32(sb + mu * Cfg::kLinkSlot), links + ((long long)mu * vol + site0) * 9, ns * 9u * SZ, bar, pol);
-                bulk_g2s(smem_u32(sb + Cfg::kXBase), x + 3 * site0, ns * 3u * SZ, bar, pol);
-                for (int rt = 0; rt < nr; ++rt) {
-                    long long rem = row0 + rt, rs = 1;                   // row index = x1 + L1 (x2 + L2 x3)
-#pragma unroll
-                    for (int mu = 1; mu < 4; ++mu) {
-                        if (mu >= nd) break;
-                        const int L = A.lat_ext[mu];
-                        const int c = (int)(rem % L);
-                        rem /= L;
-                        const long long rf = row0 + rt + (c + 1 == L ? -(long long)(L - 1) * rs : rs);
-                        const long long rb = row0 + rt + (c == 0 ? (long long)(L - 1) * rs : -rs);
-                        bulk_g2s(smem_u32(sb + (3 + mu) * Cfg::kLinkSlot + rt * lrow), links + ((long long)mu * vol + rb * L0) * 9, lrow, bar, pol);
-                        bulk_g2s(smem_u32(sb + Cfg::kXBase + mu * Cfg::kXSlot + rt * xrow), x + 3 * rf * L0, xrow, bar, pol);
-                        bulk_g2s(smem_u32(sb + Cfg::kXBase + (3 + mu) * Cfg::kXSlot + rt * xrow), x + 3 * rb * L0, xrow, bar, pol);
-                        rs *= L;
-                    }
-                }
+                lat_issue_tile<C, Cfg::kLinkSlot, Cfg::kXSlot, Cfg::kXBase>(A, links, x, smem + stage * Cfg::kStageBytes, full0 + 8 * stage,
+                                                                           empty0 + 8 * stage, phase ^ 1u, t, pol);
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
         }
@@ -266,6 +281,135 @@ __global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_
             }
             pbuf ^= 1;
             if (++stage == STAGES) { stage = 0; phase ^= 1u; }
+        }
+    }
+    write_partials<NACC>(st, acc);
+}
+
+// ------------------------------------------------------------------------------------------
+// Warp-per-tile variant (the shipped one).  k_spmv_lat_tma above is bound by shared-memory
+// bandwidth: 28 KB of its 120 KB per tile are the 3-vector partials that go from phase 1 to phase 2.
+// Here ONE warp owns a tile (lane = site slot) and accumulates all 2d terms of its site in
+// registers: no partials, no barrier.  A CTA is W consumer warps + the producer warp around one
+// ring of STAGES stages; tile k of the CTA lives in stage k % STAGES and is consumed by warp k % W.
+// ------------------------------------------------------------------------------------------
+template <typename E, int W, int PW> struct LatWarpCfg {
+    static constexpr int NS = 32;                                       // sites per tile = lanes
+    static constexpr int kThreadsTotal = (W + PW) * 32;                  // W consumer + PW producer warps
+    static constexpr int kLinkSlot = NS * 9 * (int)sizeof(E);
+    static constexpr int kXSlot = NS * 3 * (int)sizeof(E);
+    static constexpr int kXBase = 7 * kLinkSlot;
+    static constexpr int kStageBytes = 7 * (kLinkSlot + kXSlot);
+    static constexpr int smem_bytes(int stages) { return stages * kStageBytes + 2 * stages * 8; }
+};
+
+template <typename C, bool DAGGER>
+__device__ __forceinline__ void lat_matvec_acc(const C* a, const C* xv, C& s0, C& s1, C& s2) {
+    const C x0 = xv[0], x1 = xv[1], x2 = xv[2];
+    if (!DAGGER) {
+        s0 = cfma(a[2], x2, cfma(a[1], x1, cfma(a[0], x0, s0)));
+        s1 = cfma(a[5], x2, cfma(a[4], x1, cfma(a[3], x0, s1)));
+        s2 = cfma(a[8], x2, cfma(a[7], x1, cfma(a[6], x0, s2)));
+    } else {                                                            // U^dagger: conj of the columns
+        s0 = cfma_conj(a[6], x2, cfma_conj(a[3], x1, cfma_conj(a[0], x0, s0)));
+        s1 = cfma_conj(a[7], x2, cfma_conj(a[4], x1, cfma_conj(a[1], x0, s1)));
+        s2 = cfma_conj(a[8], x2, cfma_conj(a[5], x1, cfma_conj(a[2], x0, s2)));
+    }
+}
+
+template <typename E, int W, int PW, int STAGES, int ROLE>
+__global__ void __launch_bounds__(LatWarpCfg<E, W, PW>::kThreadsTotal, 1) k_spmv_lat_warp(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    typedef LatWarpCfg<E, W, PW> Cfg;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    constexpr int NS = Cfg::NS;
+    constexpr int SZ = (int)sizeof(C);
+    static_assert(STAGES % W == 0 && STAGES % PW == 0, "each stage has one producer and one consumer warp");
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::kStageBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    const int nd = A.lat_ndim;
+    const int L0 = A.lat_ext[0];
+    const int TR = A.lat_rows_per_tile;
+    const long long vol = A.lat_vol;
+    const long long nrows = vol / L0;
+    const int ntiles = A.aux_count;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    if (warp >= W) {
+        // ---------------- producer warps: one elected lane each; producer p issues the CTA's tiles p, p+PW, ...
+        if (lane == 0) {
+            const C* __restrict__ links = (const C*)A.val;
+            const uint64_t pol = policy_evict_normal();
+            // a stage is always filled by the same producer (stage % PW) and drained by the same
+            // consumer warp (stage % W): its uses are then waited for in order by ONE thread on either
+            // side, which is what the parity waits of an mbarrier need
+            for (int m = 0;; ++m) {
+                bool more = true;
+                for (int stage = warp - W; stage < STAGES; stage += PW) {
+                    const long long tl = (long long)blockIdx.x + (long long)(m * STAGES + stage) * gridDim.x;
+                    if (tl >= ntiles) { more = false; break; }
+                    lat_issue_tile<C, Cfg::kLinkSlot, Cfg::kXSlot, Cfg::kXBase>(A, links, x, smem + stage * Cfg::kStageBytes, full0 + 8 * stage,
+                                                                               empty0 + 8 * stage, ((uint32_t)m & 1u) ^ 1u, (int)tl, pol);
+                }
+                if (!more) break;
+            }
+        }
+    } else {
+        // ---------------- consumer warp: lane = site slot of the tile
+        const int rt = lane / L0, i0 = lane - rt * L0;
+        const int jf = rt * L0 + (i0 + 1 == L0 ? 0 : i0 + 1);          // mu = 0 neighbours: same row, rotated
+        const int jb = rt * L0 + (i0 == 0 ? L0 - 1 : i0 - 1);
+        const T dg = (T)A.lat_diag, cf = (T)A.lat_cf, cb = (T)A.lat_cb;
+        const C z = cmake<C>(0.0, 0.0);
+        for (int k = warp;; k += W) {                                // k = m * (STAGES / W) * W + ... : walk own stages
+            const int per = STAGES / W;                                // stages owned by this warp
+            const int m = (k / W) / per, stage = warp + ((k / W) % per) * W;
+            const long long tl = (long long)blockIdx.x + (long long)(m * STAGES + stage) * gridDim.x;
+            if (tl >= ntiles) break;
+            const uint32_t phase = (uint32_t)m & 1u;
+            const long long row0 = tl * TR;
+            const int nr = (int)min((long long)TR, nrows - row0);
+            const int ns = nr * L0;
+            const bool on = lane < ns;
+            const long long row = 3 * (row0 * L0 + lane);
+            C u0 = z, u1 = z, u2 = z;
+            if (ROLE != ROLE_CG && on) { u0 = ld_ro(u + row); u1 = ld_ro(u + row + 1); u2 = ld_ro(u + row + 2); }
+            mbar_wait(full0 + 8 * stage, phase);
+            if (on) {
+                const C* sb = (const C*)(smem + stage * Cfg::kStageBytes);
+                const C* xs = sb + Cfg::kXBase / SZ;
+                C f0 = z, f1 = z, f2 = z, g0 = z, g1 = z, g2 = z;
+                lat_matvec_acc<C, false>(sb + lane * 9, xs + jf * 3, f0, f1, f2);
+                lat_matvec_acc<C, true>(sb + jb * 9, xs + jb * 3, g0, g1, g2);
+#pragma unroll
+                for (int mu = 1; mu < 4; ++mu) {
+                    if (mu >= nd) break;
+                    lat_matvec_acc<C, false>(sb + (mu * NS + lane) * 9, xs + (mu * NS + lane) * 3, f0, f1, f2);
+                    lat_matvec_acc<C, true>(sb + ((3 + mu) * NS + lane) * 9, xs + ((3 + mu) * NS + lane) * 3, g0, g1, g2);
+                }
+                const C x0 = xs[lane * 3], x1 = xs[lane * 3 + 1], x2 = xs[lane * 3 + 2];
+                const C y0 = lat_combine(dg, x0, cf, f0, cb, g0);
+                const C y1 = lat_combine(dg, x1, cf, f1, cb, g1);
+                const C y2 = lat_combine(dg, x2, cf, f2, cb, g2);
+                y[row] = y0; y[row + 1] = y1; y[row + 2] = y2;
+                lat_epilogue<C, ROLE>(acc, y0, x0, u0);
+                lat_epilogue<C, ROLE>(acc, y1, x1, u1);
+                lat_epilogue<C, ROLE>(acc, y2, x2, u2);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * stage);            // the tile's operands are in registers
         }
     }
     write_partials<NACC>(st, acc);

@@ -26,11 +26,19 @@ EXTENTS = [(4, 4, 6, 5),        # 8 x0-rows per tile
            (36, 3, 3, 3)]       # L0 > 32 sites: row kernel
 
 
+@pytest.fixture(params=[1, 2], ids=["termsite", "warptile"])
+def tile_kernel(request, ms):
+    """Run with each of the two TMA tile kernels forced (default: the faster one per element type)."""
+    ms.msolve_config(ms.MSOLVE_CFG_LATTICE_KERNEL, request.param)
+    yield request.param
+    ms.msolve_config(ms.MSOLVE_CFG_LATTICE_KERNEL, 0)
+
+
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 @pytest.mark.parametrize("fmt", ["lat", "latrows"])
 @pytest.mark.parametrize("nh", [False, True])
 @pytest.mark.parametrize("extents", EXTENTS)
-def test_lattice_spmv_matches_oracle(ms, extents, nh, fmt, dtype):
+def test_lattice_spmv_matches_oracle(ms, tile_kernel, extents, nh, fmt, dtype):
     w = _workload(extents, nh)
     rng = np.random.default_rng(5)
     x = (rng.standard_normal(w.n) + 1j * rng.standard_normal(w.n)).astype(dtype)
@@ -55,7 +63,7 @@ def test_config2_cgm_matrix_free(ms, fmt, dtype, tol):
 
 
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
-def test_config4_scaled_cgm_matrix_free(ms, dtype, tol):
+def test_config4_scaled_cgm_matrix_free(ms, tile_kernel, dtype, tol):
     w = W.config4(extents=(32, 8, 4, 6), tol=tol)
     g = gpu_solve(ms, w, dtype, "lat")
     o = oracle_solve(w, dtype)
@@ -63,7 +71,7 @@ def test_config4_scaled_cgm_matrix_free(ms, dtype, tol):
 
 
 @pytest.mark.parametrize("fmt", ["lat", "latrows"])
-def test_config3_bicgstabm_matrix_free(ms, fmt):
+def test_config3_bicgstabm_matrix_free(ms, tile_kernel, fmt):
     w = W.config3(extents=(8, 8, 8, 8))
     g = gpu_solve(ms, w, np.complex128, fmt)
     o = oracle_solve(w, np.complex128)
