@@ -54,6 +54,12 @@ def make_workload(name: str, rank: int, want_csr: bool):
         w, dt, fmt = W.config2(), np.complex128, "lat"
     elif name == "config4_c128_csr":
         w, dt, fmt = W.config4(want_csr=True), np.complex128, "csr"
+    elif name == "config4_c64_csr":
+        w, dt, fmt = W.config4(want_csr=True, tol=1e-5), np.complex64, "csr"
+    elif name == "config3_c128_csr":
+        w, dt, fmt = W.config3(), np.complex128, "csr"
+    elif name == "config2_c128_csr":
+        w, dt, fmt = W.config2(), np.complex128, "csr"
     elif name == "config4_small_c128_bsr3":          # quick functional check of the bench itself
         w, dt, fmt = W.config4(extents=(8, 8, 8, 16), want_csr=want_csr), np.complex128, "bsr3"
     elif name == "config2_c128_bsr3":
@@ -237,7 +243,7 @@ def main():
     ap.add_argument("--profile-iters", type=int, default=20)
     ap.add_argument("--cpu-iters", type=int, default=14, help="oracle iterations timed for cpu_baseline (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--spmv", default="auto", choices=["auto", "vector", "merge"],
+    ap.add_argument("--spmv", default="auto", choices=["auto", "vector", "merge", "tile"],
                     help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
     ap.add_argument("--update-kernel", default="regs", choices=["regs", "tma"],
                     help="CG-M fused multishift update: register kernel (default) or the TMA-staged kernel")
@@ -279,7 +285,7 @@ def main():
         return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
     t_create = time.perf_counter()
-    flags = {"auto": ms.MSOLVE_SPMV_AUTO, "vector": ms.MSOLVE_SPMV_VECTOR, "merge": ms.MSOLVE_SPMV_MERGE}[args.spmv]
+    flags = {"auto": ms.MSOLVE_SPMV_AUTO, "vector": ms.MSOLVE_SPMV_VECTOR, "merge": ms.MSOLVE_SPMV_MERGE, "tile": ms.MSOLVE_SPMV_TILE}[args.spmv]
     if fmt == "bsr3":
         A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype, copy=False)), flags)
     elif fmt == "lat":

@@ -60,9 +60,10 @@ enum {
 
 /* create-time flags: SpMV kernel choice for CSR (Alg. 1 l.18). */
 enum {
-    MSOLVE_SPMV_AUTO = 0,    /* vector kernel for short regular rows, merge-path otherwise */
+    MSOLVE_SPMV_AUTO = 0,    /* TMA-staged vector-CSR for short rows, else vector or merge-path */
     MSOLVE_SPMV_VECTOR = 1,  /* sub-warp-per-row vector-CSR                                 */
-    MSOLVE_SPMV_MERGE = 2    /* merge-path CSR (load-balanced over rows + non-zeros)        */
+    MSOLVE_SPMV_MERGE = 2,   /* merge-path CSR (load-balanced over rows + non-zeros)        */
+    MSOLVE_SPMV_TILE = 3     /* TMA-staged vector-CSR (rows of at most 64 non-zeros for 16-byte elements, 128 otherwise) */
 };
 
 #define MSOLVE_MAX_SHIFTS 128
@@ -81,6 +82,10 @@ enum {
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay
  * valid and unchanged until msolve_destroy.  Column indices must lie in [0, n).  May allocate
  * library-owned auxiliary device data (merge-path partition table, solver state).
+ * flags: MSOLVE_SPMV_AUTO reads d_rowptr once at create time and takes the TMA-staged vector-CSR
+ * kernel when no row is longer than MSOLVE_SPMV_TILE allows (and d_rowptr / d_colidx are 16-byte
+ * aligned), merge-path when single rows dwarf the mean, the plain vector kernel otherwise; the
+ * other values force one kernel (EINVAL when the matrix does not fit it).
  * Errors: EINVAL (null pointer, n < 0, nnz < 0, bad dtype/flags, nnz >= 2^31), ECUDA, ENOMEM. */
 int msolve_create_csr(msolve_matrix **A, int64_t n, int64_t nnz,
                       const int32_t *d_rowptr /* n+1 */, const int32_t *d_colidx /* nnz */,

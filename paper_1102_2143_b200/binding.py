@@ -22,7 +22,7 @@ MSOLVE_C64, MSOLVE_C128, MSOLVE_F32, MSOLVE_F64 = 0, 1, 2, 3
 MSOLVE_ALG_CGM, MSOLVE_ALG_BICGSTABM = 0, 1
 MSOLVE_OK, MSOLVE_MAXITER, MSOLVE_BREAKDOWN = 0, 1, 2
 MSOLVE_EINVAL, MSOLVE_ECUDA, MSOLVE_ENOMEM = -1, -2, -3
-MSOLVE_SPMV_AUTO, MSOLVE_SPMV_VECTOR, MSOLVE_SPMV_MERGE = 0, 1, 2
+MSOLVE_SPMV_AUTO, MSOLVE_SPMV_VECTOR, MSOLVE_SPMV_MERGE, MSOLVE_SPMV_TILE = 0, 1, 2, 3
 MSOLVE_MAX_SHIFTS = 128
 MSOLVE_CFG_LOOP_MODE = 0
 MSOLVE_CFG_UPDATE_KERNEL = 1

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmsolve.so")
 SOURCES = ["msolve.cu"]
-HEADERS = ["common.cuh", "kernels.cuh", "spmv.cuh", "spmv_merge.cuh", os.path.join("..", "..", "include", "msolve.h")]
+HEADERS = ["common.cuh", "kernels.cuh", "spmv.cuh", "spmv_merge.cuh", "spmv_csr_tile.cuh", "spmv_lattice.cuh", "update_tma.cuh", os.path.join("..", "..", "include", "msolve.h")]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -19,6 +19,7 @@
 #include "kernels.cuh"
 #include "spmv.cuh"
 #include "spmv_merge.cuh"
+#include "spmv_csr_tile.cuh"
 #include "spmv_lattice.cuh"
 #include "update_tma.cuh"
 
@@ -47,7 +48,7 @@ static int fail(int code, const char* fmt, ...) {
 
 // ------------------------------------------------------------------------------------- handle
 enum { FMT_CSR = 0, FMT_BSR3 = 1, FMT_LATTICE = 2 };
-enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3, KERNEL_BSR_TMA = 4, KERNEL_LAT_ROWS = 5, KERNEL_LAT_TMA = 6 };
+enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3, KERNEL_BSR_TMA = 4, KERNEL_LAT_ROWS = 5, KERNEL_LAT_TMA = 6, KERNEL_CSR_TILE = 7 };
 constexpr int kChunk = 8;  // iteration bodies per graph launch in chunked mode
 
 struct LoopGraph {
@@ -61,6 +62,7 @@ struct msolve_matrix {
     int dtype = MSOLVE_C128;
     int kernel = KERNEL_VECTOR;
     int lanes = 8;
+    int tile_u = 4;                     // KERNEL_CSR_TILE: non-zeros per lane
     MatDev dev{};
     int device = 0;
     int num_sms = 148;
@@ -166,6 +168,38 @@ template <> struct MergeTile<float2>  { static constexpr int CAP = MSOLVE_MERGE_
 template <> struct MergeTile<double>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
 template <> struct MergeTile<float>   { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
 
+// TMA-staged vector-CSR (spmv_csr_tile.cuh): ring depth and CTAs per SM; the lanes per row and
+// the non-zeros per lane U are chosen per matrix at create time (csr_tile_shape).
+// Measured on config 4 as CSR (profiles/r01_sweeps.md): complex128 8 lanes x 4 non-zeros, 3 stages,
+// 5 CTAs per SM: 0.559 ms (vector kernel 0.874); complex64 4 lanes x 8: 0.324 ms (8 x 4: 0.389; vector 0.678).
+#ifndef MSOLVE_CT_STAGES
+#define MSOLVE_CT_STAGES 3
+#define MSOLVE_CT_CPS 5
+#endif
+#ifndef MSOLVE_CT_STAGES_F
+#define MSOLVE_CT_STAGES_F 3
+#define MSOLVE_CT_CPS_F 5
+#endif
+template <typename E> struct CsrTile { static constexpr int STAGES = MSOLVE_CT_STAGES_F, CPS = MSOLVE_CT_CPS_F; };
+template <> struct CsrTile<double2> { static constexpr int STAGES = MSOLVE_CT_STAGES, CPS = MSOLVE_CT_CPS; };
+// (lanes, U) for rows of at most `maxlen` non-zeros; false when the rows are too long.
+// 16-byte elements: U = 4, 2..16 lanes (rows <= 64).  Smaller elements: U = 4 with 2 or 4 lanes
+// for rows <= 16 (the 5-point Poisson matrix: 2 x 4 0.0225 ms, 2 x 8 0.0261 ms), U = 8 with
+// 4..16 lanes for rows <= 128.
+static bool csr_tile_shape(int dtype, long long maxlen, int* lanes, int* u) {
+    if (maxlen <= 0) return false;
+    if (dtype == MSOLVE_C128 || maxlen <= 16) {
+        *u = 4;
+        *lanes = 2;
+        while (*lanes * 4 < maxlen) *lanes *= 2;
+        return *lanes <= 16;
+    }
+    *u = 8;
+    *lanes = 4;
+    while (*lanes * 8 < maxlen) *lanes *= 2;
+    return *lanes <= 16;
+}
+
 // run F<E>() for the element type of `dtype`
 #define DISPATCH_ELEM(dtype, EXPR_C128, EXPR_C64, EXPR_F64, EXPR_F32) \
     ((dtype) == MSOLVE_C128 ? (EXPR_C128) : (dtype) == MSOLVE_C64 ? (EXPR_C64) : (dtype) == MSOLVE_F64 ? (EXPR_F64) : (EXPR_F32))
@@ -184,8 +218,38 @@ static int merge_fixup_grid(const msolve_matrix* A) {
     return std::max(1, std::min(A->num_sms, (A->dev.aux_count + kThreads - 1) / kThreads));
 }
 
+template <typename T, int LANES, int U, int ROLE>
+static void launch_csr_tile(const msolve_matrix* A, cudaStream_t s) {
+    typedef CsrTile<T> P;
+    typedef CsrTileCfg<T, LANES, U> Cfg;
+    auto k = k_spmv_csr_tile<T, LANES, U, P::STAGES, P::CPS, ROLE>;
+    const int smem = Cfg::smem_bytes(P::STAGES);
+    static thread_local bool attr_set = false;   // per <T, LANES, U, ROLE> instantiation
+    if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+    const long long ntiles = (A->dev.n + Cfg::kRows - 1) / Cfg::kRows;
+    const int grid = (int)std::max(1ll, std::min<long long>((long long)A->num_sms * P::CPS, ntiles));
+    k<<<grid, Cfg::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+}
+
 template <typename T, int ROLE>
 static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
+    if (A->format == FMT_CSR && A->kernel == KERNEL_CSR_TILE) {
+        if (sizeof(T) == 16 || A->tile_u == 4) {
+            switch (A->lanes) {
+                case 2: launch_csr_tile<T, 2, 4, ROLE>(A, s); break;
+                case 4: launch_csr_tile<T, 4, 4, ROLE>(A, s); break;
+                case 8: if constexpr (sizeof(T) == 16) launch_csr_tile<T, 8, 4, ROLE>(A, s); break;
+                default: if constexpr (sizeof(T) == 16) launch_csr_tile<T, 16, 4, ROLE>(A, s); break;
+            }
+        } else if constexpr (sizeof(T) < 16) {
+            switch (A->lanes) {
+                case 4: launch_csr_tile<T, 4, 8, ROLE>(A, s); break;
+                case 8: launch_csr_tile<T, 8, 8, ROLE>(A, s); break;
+                default: launch_csr_tile<T, 16, 8, ROLE>(A, s); break;
+            }
+        }
+        return;
+    }
     if (A->format == FMT_CSR && A->kernel == KERNEL_MERGE) {
         typedef MergeTile<T> M;
         auto kp = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE, true>;     // x pinned in L2
@@ -435,7 +499,8 @@ static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 // multiple of 4 (16-byte aligned bulk copies for values and indices) and i to the first row not
 // yet finished at that k.  Tile t = {i0, i1, k0, k1}: rows i0..i1-1 end inside the tile, row i1
 // (if < n) may continue.  Also decides AUTO: merge-path when the row lengths are irregular.
-static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int32_t>& rp) {
+static int build_merge_tiles(msolve_matrix* A, int flags, const std::vector<int32_t>& rp) {
+    const bool force = flags != MSOLVE_SPMV_AUTO;      // a kernel was asked for by name: bad input is an error
     const long long n = A->dev.n, nnz = A->dev.nnz;
     if (n == 0) return MSOLVE_OK;
     if (rp[0] != 0 || rp[(size_t)n] != nnz) return force ? fail(MSOLVE_EINVAL, "msolve_create_csr: rowptr[0] != 0 or rowptr[n] != nnz") : MSOLVE_OK;
@@ -451,7 +516,23 @@ static int build_merge_tiles(msolve_matrix* A, bool force, const std::vector<int
         A->lanes = MSOLVE_VEC_LANES;
 #endif
     }
-    if (!force) {
+    // TMA-staged vector-CSR (spmv_csr_tile.cuh): every row fits LANES * U non-zeros, LANES <= 16.
+    // AUTO takes it whenever the rows allow it: it is the faster CSR kernel on every workload
+    // with short rows (config 4 as CSR, config 3, the 1000 x 1000 Poisson matrix).
+    int tl = 0, tu = 0;
+    const bool tile_ok = csr_tile_shape(A->dtype, maxlen, &tl, &tu);
+    if (flags == MSOLVE_SPMV_TILE && !tile_ok)
+        return fail(MSOLVE_EINVAL, "msolve_create_csr: MSOLVE_SPMV_TILE needs rows of 1..%d non-zeros (longest row: %lld)",
+                    A->dtype == MSOLVE_C128 ? 64 : 128, maxlen);
+    // small matrices (config 2, N = 12288: 0.0088 vs 0.0090 ms per SpMV, 37.2k vs 40.9k iterations/s)
+    // do not fill the ring; they stay with the vector kernel
+    if (flags == MSOLVE_SPMV_TILE || (flags == MSOLVE_SPMV_AUTO && tile_ok && n >= 65536)) {
+        A->lanes = tl;
+        A->tile_u = tu;
+        A->kernel = KERNEL_CSR_TILE;
+        return MSOLVE_OK;
+    }
+    if (flags != MSOLVE_SPMV_MERGE) {
         const double mean = (double)nnz / (double)n;
         // Vector kernel unless single rows dwarf the mean (a sub-warp would serialise them): on
         // config 5 (rows 5..200, mean 32) the vector kernel is the faster one on B200 (1.14 vs
@@ -505,7 +586,7 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
     if (n < 0 || nnz < 0 || nnz >= (1ll << 31) || n >= (1ll << 31)) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad n/nnz");
     if (!d_rowptr || (nnz > 0 && (!d_colidx || !d_val))) return fail(MSOLVE_EINVAL, "msolve_create_csr: NULL array");
     if (!valid_dtype(dtype)) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad dtype");
-    if (flags < MSOLVE_SPMV_AUTO || flags > MSOLVE_SPMV_MERGE) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad flags");
+    if (flags < MSOLVE_SPMV_AUTO || flags > MSOLVE_SPMV_TILE) return fail(MSOLVE_EINVAL, "msolve_create_csr: bad flags");
     if (!aligned16(d_val) || ((uintptr_t)d_colidx & 3u) || ((uintptr_t)d_rowptr & 3u)) return fail(MSOLVE_EINVAL, "msolve_create_csr: misaligned array");
     msolve_matrix* A = new (std::nothrow) msolve_matrix();
     if (!A) return fail(MSOLVE_ENOMEM, "out of host memory");
@@ -522,14 +603,14 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
 #endif
     int rc = create_common(out, A, (cudaStream_t)stream);
     if (rc == MSOLVE_OK && flags != MSOLVE_SPMV_VECTOR && n > 0) {
-        const bool force = flags == MSOLVE_SPMV_MERGE;
+        const bool force = flags != MSOLVE_SPMV_AUTO;
         if (!aligned16(d_rowptr) || !aligned16(d_colidx)) {
-            if (force) rc = fail(MSOLVE_EINVAL, "msolve_create_csr: merge-path needs 16-byte aligned rowptr / colidx");
+            if (force) rc = fail(MSOLVE_EINVAL, "msolve_create_csr: the TMA-staged kernels need 16-byte aligned rowptr / colidx");
         } else {
             std::vector<int32_t> rp((size_t)n + 1);
             cudaError_t e = cudaMemcpy(rp.data(), d_rowptr, sizeof(int32_t) * (size_t)(n + 1), cudaMemcpyDeviceToHost);
             if (e != cudaSuccess) rc = fail(MSOLVE_ECUDA, "msolve_create_csr: reading rowptr failed: %s", cudaGetErrorString(e));
-            else rc = build_merge_tiles(A, force, rp);
+            else rc = build_merge_tiles(A, flags, rp);
         }
     }
     if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }

@@ -39,6 +39,8 @@ def make_matrix(ms, w, dtype, fmt, flags=0):
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
     if fmt == "csrmerge":   # merge-path CSR forced (AUTO picks it only for irregular rows)
         return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), ms.MSOLVE_SPMV_MERGE)
+    if fmt == "csrtile":    # TMA-staged vector-CSR forced (AUTO picks it for large matrices of short rows)
+        return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), ms.MSOLVE_SPMV_TILE)
     if fmt == "csrvector":
         return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
     return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), flags)
@@ -81,7 +83,8 @@ def check_parity(w, dtype, g, o, tol):
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
 @pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c2", "bsr3rows"),
                                        ("c2big", "bsr3"), ("c5", "csr"), ("c5", "csrvector"), ("c5", "csrmerge"),
-                                       ("c1", "csrmerge"), ("c2big", "csrmerge"), ("c5big", "csrmerge")])
+                                       ("c1", "csrmerge"), ("c2big", "csrmerge"), ("c5big", "csrmerge"),
+                                       ("c1", "csrtile"), ("c2", "csrtile"), ("c2big", "csrtile")])
 def test_spmv_matches_oracle(ms, dtype, which, fmt):
     w = {"c1": lambda: W.config1(), "c2": lambda: W.config2(extents=(4, 4, 6, 5)),
          "c2big": lambda: W.config2(extents=(12, 10, 9, 11)),   # 11880 sites: many tiles per CTA, ragged tail
@@ -196,7 +199,7 @@ def test_update_kernels_agree(ms, extents, dtype, tol):
     assert d <= (1e-12 if dtype == np.complex128 else 1e-5)
 
 
-@pytest.mark.parametrize("fmt", ["csr", "bsr3"])
+@pytest.mark.parametrize("fmt", ["csr", "csrtile", "bsr3"])
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 def test_config4_scaled_cgm(ms, fmt, dtype, tol):
     w = W.config4(extents=(8, 8, 8, 16), tol=tol)
@@ -215,6 +218,76 @@ def test_config5_scaled_cgm(ms, fmt, dtype, tol):
     assert np.all(np.diff(g[3]) <= 0)              # larger shifts never converge later
     per_iter = 6 if fmt == "csrmerge" else 5       # merge-path SpMV = tile kernel + carry fix-up
     assert g[5] == 2 + per_iter * g[1]
+
+
+def test_bicgstabm_csr_tile(ms):
+    # both SpMV roles of BiCGStab-M through the TMA-staged vector-CSR kernel
+    w = W.config3(extents=(6, 6, 6, 6))
+    g = gpu_solve(ms, w, np.complex128, "csrtile")
+    o = oracle_solve(w, np.complex128)
+    check_parity(w, np.complex128, g, o, w.tol)
+    assert g[5] == 2 + 7 * g[1]
+
+
+@pytest.mark.parametrize("dtype", [np.complex128, np.complex64])
+@pytest.mark.parametrize("shape", ["ragged", "empty_rows", "max_rows", "all_empty", "single_row", "tiny", "short", "mid", "long_f"])
+def test_csr_tile_degenerate_rows(ms, dtype, shape):
+    # TMA-staged vector-CSR: rows of 0..64 non-zeros in any mix (lane counts 2..16), tiles whose
+    # non-zero range starts and ends off the 4-element alignment, matrices smaller than one tile
+    rng = np.random.default_rng(17)
+    if shape == "ragged":
+        n, lengths = 30011, rng.integers(0, 28, 30011)
+    elif shape == "empty_rows":
+        n = 20001
+        lengths = rng.integers(1, 16, n) * (rng.random(n) < 0.4)
+        lengths[3000:9000] = 0
+    elif shape == "max_rows":
+        n, lengths = 5003, rng.integers(40, 65, 5003)
+    elif shape == "all_empty":
+        n, lengths = 5000, np.zeros(5000, dtype=np.int64)
+    elif shape == "single_row":
+        n, lengths = 1, np.array([1])
+    elif shape == "tiny":
+        n, lengths = 7, np.array([0, 2, 0, 0, 5, 1, 0])
+    elif shape == "mid":
+        n, lengths = 9001, rng.integers(9, 17, 9001)              # 4 lanes x 4
+    elif shape == "long_f":
+        n, lengths = 3001, rng.integers(90, 129, 3001)            # 16 lanes x 8: elements of <= 8 bytes only
+    else:
+        n, lengths = 40007, rng.integers(1, 6, 40007)
+    rowptr, colidx, val = _random_csr(rng, lengths, n)
+    if shape == "long_f" and dtype == np.complex128:
+        with pytest.raises(Exception):                            # 16-byte elements: rows of at most 64
+            ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val.astype(dtype)), ms.MSOLVE_SPMV_TILE)
+        return
+    if colidx.size == 0:
+        colidx_d, val_d = torch.zeros(4, dtype=torch.int32, device="cuda"), torch.zeros(4, dtype=TORCH[dtype], device="cuda")
+        with pytest.raises(Exception):                            # no non-zeros: not a tile-kernel matrix
+            ms.msolve_create_csr(dev(rowptr), colidx_d[:0], val_d[:0], ms.MSOLVE_SPMV_TILE)
+        return
+    A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val.astype(dtype)), ms.MSOLVE_SPMV_TILE)
+    x = (rng.standard_normal(n) + 1j * rng.standard_normal(n)).astype(dtype)
+    y, dot = ms.msolve_spmv(A, dev(x), torch.full((n,), 7.0, dtype=TORCH[dtype], device="cuda"))
+    y = y.cpu().numpy()
+    ref = oracle.spmv(rowptr, colidx, val.astype(dtype), x)
+    eps = 1e-13 if dtype == np.complex128 else 2e-5
+    scale = max(np.linalg.norm(ref), 1e-300)
+    assert np.linalg.norm(y - ref) <= eps * scale
+    assert np.array_equal(y[lengths == 0], np.zeros(int((lengths == 0).sum()), dtype=dtype))   # every row written
+    ref_dot = np.vdot(x.astype(np.complex128), ref.astype(np.complex128))
+    assert abs(dot - ref_dot) <= eps * max(abs(ref_dot), np.linalg.norm(x) * scale)
+    y2, dot2 = ms.msolve_spmv(A, dev(x))
+    assert np.array_equal(y2.cpu().numpy(), y) and dot2 == dot
+    ms.msolve_destroy(A)
+
+
+def test_csr_tile_rejects_long_rows(ms):
+    rng = np.random.default_rng(5)
+    lengths = np.full(100, 4)
+    lengths[17] = 65
+    rowptr, colidx, val = _random_csr(rng, lengths, 100)
+    with pytest.raises(Exception):
+        ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val), ms.MSOLVE_SPMV_TILE)
 
 
 def test_bicgstabm_merge_path(ms):

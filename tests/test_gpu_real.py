@@ -50,7 +50,7 @@ def solve_both(ms, w, dtype, flags, tol):
     return g, o
 
 
-@pytest.mark.parametrize("flags", [0, 1, 2])                      # AUTO, VECTOR, MERGE
+@pytest.mark.parametrize("flags", [0, 1, 2, 3])                   # AUTO, VECTOR, MERGE, TILE
 @pytest.mark.parametrize("dtype", [np.float64, np.float32])
 def test_spmv_real(ms, dtype, flags):
     w = W.poisson_workload(67, 45, real=True)                     # n = 3015: odd, ragged tiles
@@ -64,7 +64,7 @@ def test_spmv_real(ms, dtype, flags):
     ms.msolve_destroy(A)
 
 
-@pytest.mark.parametrize("flags", [0, 2])
+@pytest.mark.parametrize("flags", [0, 2, 3])
 @pytest.mark.parametrize("dtype,shape", [(np.float64, (64, 48)), (np.float64, (37, 29)), (np.float32, (24, 20)),
                                          (np.float32, (23, 19))])
 def test_poisson_cgm_real(ms, dtype, shape, flags):
