@@ -52,8 +52,21 @@ def test_config4_full_c128_bsr3_vs_oracle(ms):
         rs = sampled_true_residual(w, x[k], s, rows)
         # ||b|| = 1: an rms residual entry of tol/sqrt(n) corresponds to ||r|| = tol
         assert np.sqrt(np.mean(np.abs(rs) ** 2) * w.n) <= 10 * w.tol, k
-    # same handle, complex64 data path at full size: properties only
     ms.msolve_destroy(A)
+    del res, x
+    # the same matrix as CSR (AUTO = TMA-staged vector-CSR kernel), element by element
+    A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val))
+    rc = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
+    assert rc.status == 0 and abs(rc.iterations - ref.iterations) <= 2
+    assert np.all(np.abs(rc.conv_iter - ref.conv_iter) <= 2)
+    xc = rc.x.cpu().numpy()
+    for k in range(len(w.shifts)):
+        d = np.linalg.norm(xc[k] - ref.x[k]) / np.linalg.norm(ref.x[k])
+        assert d <= 1e-9, (k, d)
+    ms.msolve_destroy(A)
+    del rc, xc
+    torch.cuda.empty_cache()
+    # complex64 data path at full size: properties only
     A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(np.complex64)))
     r32 = ms.msolve_cgm(A, dev(w.b.astype(np.complex64)), w.shifts, 1e-5, w.max_iter)
     assert r32.status == 0 and abs(r32.iterations - 12) <= 2
