@@ -66,6 +66,10 @@ def make_workload(name: str, rank: int, want_csr: bool):
         w, dt, fmt = W.config2(), np.complex128, "bsr3"
     elif name == "config3_c128_bsr3":
         w, dt, fmt = W.config3(), np.complex128, "bsr3"
+    elif name == "config3x_c128_bsr3":               # config 3's non-Hermitian operator on config 4's lattice:
+        w, dt, fmt = W.config3(extents=(32, 32, 32, 64)), np.complex128, "bsr3"   # BiCGStab-M kernels at HBM-bound size
+    elif name == "config3x_c128_lat":
+        w, dt, fmt = W.config3(extents=(32, 32, 32, 64)), np.complex128, "lat"
     elif name == "config5_c128_csr":
         w, dt, fmt = W.config5(), np.complex128, "csr"
     elif name == "config5_c64_csr":

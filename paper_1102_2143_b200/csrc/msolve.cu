@@ -115,8 +115,14 @@ template <typename E> struct BsrTile;
 #ifndef MSOLVE_BSR_CPS_F
 #define MSOLVE_BSR_CPS_F 4
 #endif
+#ifndef MSOLVE_BSR_TB_F
+#define MSOLVE_BSR_TB_F (2 * MSOLVE_BSR_TB)
+#endif
+#ifndef MSOLVE_BSR_STAGES_F
+#define MSOLVE_BSR_STAGES_F MSOLVE_BSR_STAGES
+#endif
 template <> struct BsrTile<double2> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
-template <> struct BsrTile<float2>  { static constexpr int TB = 2 * MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS_F; };
+template <> struct BsrTile<float2>  { static constexpr int TB = MSOLVE_BSR_TB_F, STAGES = MSOLVE_BSR_STAGES_F, CPS = MSOLVE_BSR_CPS_F; };
 
 // Matrix-free lattice kernel configuration: sites per tile, ring depth, CTAs per SM.
 #ifndef MSOLVE_LAT_NS
@@ -345,8 +351,14 @@ static bool vec16(const msolve_matrix* A) { return A->dev.n % (long long)(16 / e
         }                                                                                  \
     } while (0)
 
-constexpr int kUnrollCgm = 4;
-constexpr int kUnrollBi = 2;
+#ifndef MSOLVE_UNROLL_CGM
+#define MSOLVE_UNROLL_CGM 4
+#endif
+constexpr int kUnrollCgm = MSOLVE_UNROLL_CGM;
+#ifndef MSOLVE_UNROLL_BI
+#define MSOLVE_UNROLL_BI 4
+#endif
+constexpr int kUnrollBi = MSOLVE_UNROLL_BI;
 
 #define L_INIT(T, V, A, s) { auto k = k_init_vectors<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
 #define L_PUPD(T, V, A, s) { auto k = k_cgm_pupdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
