@@ -102,6 +102,9 @@ __global__ void __launch_bounds__(kThreads) k_init_state(SolveState* st) {
     }
 }
 
+#ifndef MSOLVE_PUPD_U
+#define MSOLVE_PUPD_U 4
+#endif
 // ----------------------------------------------------------------------------- CG-M
 // A1: p <- r + alpha p  (l.27; at n = 0 p = b already)
 template <typename E, int VEC>
@@ -114,7 +117,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
     P* p = (P*)st->h.p;
     const T alpha = (T)st->alpha.re;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    constexpr int U = 4;                                   // 2U independent 16-byte loads in flight
+    constexpr int U = MSOLVE_PUPD_U;                       // 2U independent 16-byte loads in flight
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     for (; i + (U - 1) * stride < nvec; i += U * stride) {
         P rv[U], pv[U];

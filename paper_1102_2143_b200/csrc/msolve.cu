@@ -115,6 +115,9 @@ template <typename E> struct BsrTile;
 #ifndef MSOLVE_BSR_CPS_F
 #define MSOLVE_BSR_CPS_F 4
 #endif
+#ifndef MSOLVE_BSR_CPS_B2_LESS
+#define MSOLVE_BSR_CPS_B2_LESS 1
+#endif
 #ifndef MSOLVE_BSR_TB_F
 #define MSOLVE_BSR_TB_F (2 * MSOLVE_BSR_TB)
 #endif
@@ -275,11 +278,13 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
     if constexpr (IsComplex<T>::value) {               // BSR3 = SU(3) blocks: complex only
         if (A->format == FMT_BSR3 && A->kernel == KERNEL_BSR_TMA) {
             typedef BsrTile<T> B;
-            auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, B::CPS, ROLE>;
+            // the second BiCGStab-M SpMV carries five fp64 accumulators: one CTA per SM less keeps it from spilling
+            constexpr int CPS = B::CPS - (ROLE == ROLE_B2 ? MSOLVE_BSR_CPS_B2_LESS : 0);
+            auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, CPS, ROLE>;
             const int smem = BsrTmaCfg<T, B::TB>::smem_bytes(B::STAGES);
             static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
             if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-            const int grid = std::max(1, std::min(A->num_sms * B::CPS, A->dev.aux_count));
+            const int grid = std::max(1, std::min(A->num_sms * CPS, A->dev.aux_count));
             k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
             return;
         }
