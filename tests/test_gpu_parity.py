@@ -396,3 +396,27 @@ def test_handle_reuse_and_solve_host(ms):
     rh = ms.msolve_solve_host(A, ms.MSOLVE_ALG_CGM, torch.from_numpy(w.b), w.shifts, w.tol, 500)
     assert not rh.x.is_cuda and torch.equal(rh.x, r1.x.cpu()) and rh.iterations == r1.iterations
     ms.msolve_destroy(A)
+
+
+# ------------------------------------------------------------------------------- determinism under repetition
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+@pytest.mark.parametrize("fmt", ["csrtile", "csrmerge", "csrvector", "bsr3", "lat"])
+def test_repeated_launches_bit_identical(ms, fmt, dtype, tol):
+    # every reduction has a fixed order and every mbarrier ring a fixed hand-over, so 60 SpMVs and 6 whole
+    # solves in a row must return the same bytes (a race or a stale stage would show up as a differing run)
+    w = W.config4(extents=(16, 16, 8, 12), tol=tol)
+    A = make_matrix(ms, w, dtype, fmt)
+    rng = np.random.default_rng(23)
+    x = dev((rng.standard_normal(w.n) + 1j * rng.standard_normal(w.n)).astype(dtype))
+    y0, d0 = ms.msolve_spmv(A, x)
+    y0 = y0.clone()
+    for _ in range(60):
+        y, d = ms.msolve_spmv(A, x)
+        assert d == d0 and torch.equal(y, y0)
+    b = dev(w.b.astype(dtype))
+    r0 = ms.msolve_cgm(A, b, w.shifts, tol, w.max_iter)
+    x0 = r0.x.clone()
+    for _ in range(6):
+        r = ms.msolve_cgm(A, b, w.shifts, tol, w.max_iter)
+        assert r.iterations == r0.iterations and torch.equal(r.x, x0)
+    ms.msolve_destroy(A)
