@@ -153,6 +153,18 @@ int msolve_solve_host(const msolve_matrix *A, int algorithm, const void *h_b, co
                       int nshifts, double tol, int max_iter, void *h_x,
                       int *h_iterations, int *h_conv_iter, double *h_relres, void *stream);
 
+/* The same for a batch of nrhs right-hand sides of one family (RHMC solves the same shifted family for
+ * several pseudofermion fields): h_b[i] -> h_x[i] (nshifts*n each, shift-major), solved one
+ * after the other on `stream`, software-pipelined: the device-to-host copy of solution set i runs on a
+ * library-owned copy stream while solve i+1 is running (two device slots of b and x, kept in the handle).
+ * Host vectors should be pinned, or the copies do not overlap.  h_iterations: nrhs; h_conv_iter,
+ * h_relres: nrhs*nshifts (or NULL).  Returns the largest status of the solves (MSOLVE_OK / MAXITER /
+ * BREAKDOWN) or the first error (< 0); all copies have completed on return. */
+int msolve_solve_host_batch(const msolve_matrix *A, int algorithm, int nrhs, const void *const *h_b,
+                            const double *h_shifts, int nshifts, double tol, int max_iter,
+                            void *const *h_x, int *h_iterations, int *h_conv_iter, double *h_relres,
+                            void *stream);
+
 /* One SpMV y = A x with the fused reduction of the CG-M step (Alg. 1 l.18-19):
  * h_dot[0..1] receives <x, A x> = sum_i conj(x_i) y_i (may be NULL).  d_x, d_y: n complex, device.
  * Exposed for parity tests of the SpMV kernels and for per-kernel timing. */

@@ -30,7 +30,7 @@ MSOLVE_CFG_LATTICE_KERNEL = 2
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
-    "msolve_bicgstabm", "msolve_solve_host", "msolve_spmv", "msolve_profile_iteration",
+    "msolve_bicgstabm", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
     "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_destroy",
     "msolve_last_error",
 )
@@ -63,6 +63,7 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_cgm.argtypes = solver_args
     lib.msolve_bicgstabm.argtypes = solver_args
     lib.msolve_solve_host.argtypes = [vp, i32, vp, vp, i32, dbl, i32, vp, vp, vp, vp, vp]
+    lib.msolve_solve_host_batch.argtypes = [vp, i32, i32, vp, vp, i32, dbl, i32, vp, vp, vp, vp, vp]
     lib.msolve_spmv.argtypes = [vp, vp, vp, vp, vp]
     lib.msolve_profile_iteration.argtypes = [vp, i32, vp, vp, i32, i32, vp, vp, sz, vp, vp, vp]
     lib.msolve_kernel_name.argtypes = [i32, i32]
@@ -74,7 +75,7 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_destroy.restype = None
     lib.msolve_last_error.restype = ctypes.c_char_p
     for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_cgm", "msolve_bicgstabm",
-                 "msolve_solve_host", "msolve_spmv", "msolve_profile_iteration", "msolve_config"):
+                 "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration", "msolve_config"):
         getattr(lib, name).restype = i32
     _lib = lib
     return lib
@@ -265,6 +266,34 @@ def msolve_solve_host(A: Matrix, algorithm: int, b: torch.Tensor, shifts, tol: f
                                x.data_ptr(), ctypes.addressof(it), conv.ctypes.data, rel.ctypes.data, _stream(stream))
     _check(rc)
     return SolveResult(rc, it.value, x.view(s, A.n), conv, rel)
+
+
+def msolve_solve_host_batch(A: Matrix, algorithm: int, bs, shifts, tol: float, max_iter: int, xs=None, stream=None):
+    """A batch of HOST right-hand sides `bs` (list of CPU tensors, pinned for overlap) -> list of SolveResult;
+    the D2H copy of solution set i overlaps solve i+1 (include/msolve.h: msolve_solve_host_batch)."""
+    lib = load_library()
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    s, m = sh.size, len(bs)
+    bs = [b.contiguous() for b in bs]
+    for b in bs:
+        if b.is_cuda or b.dtype != A.dtype or b.numel() != A.n:
+            raise ValueError("every b must be a CPU tensor of n elements of the matrix dtype")
+    if xs is None:
+        xs = [torch.empty((s, A.n), dtype=A.dtype, pin_memory=True) for _ in range(m)]
+    for x in xs:
+        if x.is_cuda or x.dtype != A.dtype or x.numel() != s * A.n or not x.is_contiguous():
+            raise ValueError("every x must be a contiguous CPU tensor of nshifts*n elements")
+    if len(xs) != m:
+        raise ValueError("one x per b")
+    bp = (ctypes.c_void_p * max(m, 1))(*[b.data_ptr() for b in bs])
+    xp = (ctypes.c_void_p * max(m, 1))(*[x.data_ptr() for x in xs])
+    it = np.zeros(max(m, 1), dtype=np.int32)
+    conv = np.full((max(m, 1), s), -1, dtype=np.int32)
+    rel = np.zeros((max(m, 1), s), dtype=np.float64)
+    rc = lib.msolve_solve_host_batch(A.handle, algorithm, m, bp, sh.ctypes.data, s, float(tol), int(max_iter), xp,
+                                     it.ctypes.data, conv.ctypes.data, rel.ctypes.data, _stream(stream))
+    _check(rc)
+    return [SolveResult(rc, int(it[i]), xs[i].view(s, A.n), conv[i], rel[i]) for i in range(m)]
 
 
 def msolve_spmv(A: Matrix, x: torch.Tensor, y: Optional[torch.Tensor] = None, stream=None):

@@ -72,6 +72,10 @@ struct msolve_matrix {
     void* d_carry = nullptr;            // merge-path carries (library-owned)
     char* d_host_buf = nullptr;         // msolve_solve_host: device b, x and workspace, kept for the next call
     size_t host_buf_bytes = 0;
+    char* d_batch_buf = nullptr;        // msolve_solve_host_batch: two (b, x) slots + workspace
+    size_t batch_buf_bytes = 0;
+    cudaStream_t copy_stream = nullptr; // D2H of solve i overlaps solve i+1
+    cudaEvent_t ev_solved[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
     cudaStream_t capture_stream = nullptr;
     LoopGraph graphs[2];
     int64_t last_launches = 0;
@@ -713,6 +717,12 @@ extern "C" void msolve_destroy(msolve_matrix* A) {
     if (A->d_aux) cudaFree(A->d_aux);
     if (A->d_carry) cudaFree(A->d_carry);
     if (A->d_host_buf) cudaFree(A->d_host_buf);
+    if (A->d_batch_buf) cudaFree(A->d_batch_buf);
+    for (int i = 0; i < 2; ++i) {
+        if (A->ev_solved[i]) cudaEventDestroy(A->ev_solved[i]);
+        if (A->ev_copied[i]) cudaEventDestroy(A->ev_copied[i]);
+    }
+    if (A->copy_stream) cudaStreamDestroy(A->copy_stream);
     delete A;
 }
 
@@ -872,6 +882,61 @@ extern "C" int msolve_solve_host(const msolve_matrix* A, int algorithm, const vo
         if (e != cudaSuccess) rc = fail(MSOLVE_ECUDA, "D2H copy failed: %s", cudaGetErrorString(e));
     }
     return rc;
+}
+
+// A batch of right-hand sides through the host interface, software-pipelined: the D2H copy of
+// solve i (on a copy stream, out of x slot i % 2) overlaps solve i+1 (which writes the other slot).
+extern "C" int msolve_solve_host_batch(const msolve_matrix* A, int algorithm, int nrhs, const void* const* h_b,
+                                       const double* h_shifts, int nshifts, double tol, int max_iter,
+                                       void* const* h_x, int* h_iterations, int* h_conv_iter, double* h_relres,
+                                       void* stream_) {
+    if (!A || !h_b || !h_x || nrhs < 0) return fail(MSOLVE_EINVAL, "msolve_solve_host_batch: bad argument");
+    if (algorithm != MSOLVE_ALG_CGM && algorithm != MSOLVE_ALG_BICGSTABM) return fail(MSOLVE_EINVAL, "msolve_solve_host_batch: bad algorithm");
+    for (int i = 0; i < nrhs; ++i)
+        if (!h_b[i] || !h_x[i]) return fail(MSOLVE_EINVAL, "msolve_solve_host_batch: NULL vector %d", i);
+    const size_t wsb = msolve_workspace_bytes(A, nshifts, algorithm);
+    if (!wsb) return fail(MSOLVE_EINVAL, "msolve_solve_host_batch: bad nshifts");
+    if (nrhs == 0) return MSOLVE_OK;
+    cudaStream_t stream = (cudaStream_t)stream_;
+    msolve_matrix* Am = const_cast<msolve_matrix*>(A);
+    const size_t eb = elem_bytes(A->dtype);
+    const size_t bbytes = (size_t)A->dev.n * eb, xbytes = bbytes * (size_t)nshifts;
+    const size_t slot = align_up(bbytes, 256) + align_up(xbytes, 256);
+    const size_t need = 2 * slot + wsb + 256;
+    if (Am->batch_buf_bytes < need) {
+        if (Am->d_batch_buf) cudaFree(Am->d_batch_buf);
+        Am->d_batch_buf = nullptr; Am->batch_buf_bytes = 0;
+        if (cudaMalloc((void**)&Am->d_batch_buf, need) != cudaSuccess) return fail(MSOLVE_ENOMEM, "msolve_solve_host_batch: cudaMalloc of %zu bytes failed", need);
+        Am->batch_buf_bytes = need;
+    }
+    if (!Am->copy_stream) {
+        CU(cudaStreamCreateWithFlags(&Am->copy_stream, cudaStreamNonBlocking));
+        for (int j = 0; j < 2; ++j) {
+            CU(cudaEventCreateWithFlags(&Am->ev_solved[j], cudaEventDisableTiming));
+            CU(cudaEventCreateWithFlags(&Am->ev_copied[j], cudaEventDisableTiming));
+        }
+    }
+    char* d_ws = Am->d_batch_buf + 2 * slot;
+    int worst = MSOLVE_OK;
+    for (int i = 0; i < nrhs; ++i) {
+        const int j = i & 1;
+        char* d_b = Am->d_batch_buf + (size_t)j * slot;
+        char* d_x = d_b + align_up(bbytes, 256);
+        if (i >= 2) CU(cudaStreamWaitEvent(stream, Am->ev_copied[j], 0));       // slot j has been read back
+        CU(cudaMemcpyAsync(d_b, h_b[i], bbytes, cudaMemcpyHostToDevice, stream));
+        const int rc = run_solver(algorithm, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_ws, wsb + 256,
+                                  h_iterations ? h_iterations + i : nullptr,
+                                  h_conv_iter ? h_conv_iter + (size_t)i * nshifts : nullptr,
+                                  h_relres ? h_relres + (size_t)i * nshifts : nullptr, stream_);
+        if (rc < 0) { cudaStreamSynchronize(Am->copy_stream); return rc; }
+        worst = std::max(worst, rc);
+        CU(cudaEventRecord(Am->ev_solved[j], stream));
+        CU(cudaStreamWaitEvent(Am->copy_stream, Am->ev_solved[j], 0));
+        CU(cudaMemcpyAsync(h_x[i], d_x, xbytes, cudaMemcpyDeviceToHost, Am->copy_stream));
+        CU(cudaEventRecord(Am->ev_copied[j], Am->copy_stream));
+    }
+    CU(cudaStreamSynchronize(Am->copy_stream));
+    return worst;
 }
 
 // ------------------------------------------------------------------------------------- spmv / profile

@@ -398,6 +398,32 @@ def test_handle_reuse_and_solve_host(ms):
     ms.msolve_destroy(A)
 
 
+@pytest.mark.parametrize("alg", ["cgm", "bicgstabm"])
+def test_solve_host_batch_matches_single_solves(ms, alg):
+    # five right-hand sides through the pipelined batch call (two device slots in turn, D2H of solve i
+    # overlapping solve i+1): every solution set equals the one of a single host call, bit for bit
+    w = W.config2(extents=(8, 6, 4, 6)) if alg == "cgm" else W.config3(extents=(6, 6, 4, 6))
+    A = make_matrix(ms, w, np.complex128, "bsr3")
+    code = ms.MSOLVE_ALG_CGM if alg == "cgm" else ms.MSOLVE_ALG_BICGSTABM
+    bs = [torch.from_numpy(W.unit_rhs(100 + i, w.n)).pin_memory() for i in range(5)]
+    singles = [ms.msolve_solve_host(A, code, b, w.shifts, w.tol, 500) for b in bs]
+    singles = [(r.x.clone(), r.iterations, r.conv_iter.copy(), r.relres.copy()) for r in singles]
+    batch = ms.msolve_solve_host_batch(A, code, bs, w.shifts, w.tol, 500)
+    assert len(batch) == 5
+    for r, (x, it, conv, rel) in zip(batch, singles):
+        assert r.status == 0 and r.iterations == it and torch.equal(r.x, x)
+        assert np.array_equal(r.conv_iter, conv) and np.array_equal(r.relres, rel)
+    assert not torch.equal(batch[0].x, batch[1].x)                    # different right-hand sides
+    o = oracle_solve(w, np.complex128)                                 # and one of them against the oracle
+    w2 = W.config2(extents=(8, 6, 4, 6)) if alg == "cgm" else W.config3(extents=(6, 6, 4, 6))
+    w2.b = bs[3].numpy()
+    o = oracle_solve(w2, np.complex128)
+    g = (0, batch[3].iterations, batch[3].x.numpy(), batch[3].conv_iter, batch[3].relres, 0)
+    check_parity(w2, np.complex128, g, o, w2.tol)
+    assert ms.msolve_solve_host_batch(A, code, [], w.shifts, w.tol, 500) == []
+    ms.msolve_destroy(A)
+
+
 # ------------------------------------------------------------------------------- determinism under repetition
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 @pytest.mark.parametrize("fmt", ["csrtile", "csrmerge", "csrvector", "bsr3", "lat"])
