@@ -284,7 +284,11 @@ def main():
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    _build.build()
+        if local_rank == 0:
+            _build.build()                                   # one compile per node, the other ranks wait
+        dist.barrier()
+    else:
+        _build.build()
     ms.load_library()
     ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 0 if args.loop_mode == "while" else 1)
     ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, 1 if args.update_kernel == "tma" else 0)
