@@ -76,7 +76,8 @@ enum {
                                     kernel (bulk async loads AND stores) whenever the vector length is a multiple
                                     of 16 bytes.  Same arithmetic; both run at the same 6.0 TB/s on B200 */,
     MSOLVE_CFG_LATTICE_KERNEL = 2 /* tile kernel of msolve_create_lattice_su3 handles: 0 = the faster one per
-                                     element type (default), 1 = (term, site) threads + partials, 2 = warp per tile */
+                                     element type (default), 1 = (term, site) threads + partials, 2 = warp per tile,
+                                     3 = hybrid (forward links by bulk copy, backward links and neighbours gathered) */
 };
 
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay

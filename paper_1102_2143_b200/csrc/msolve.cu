@@ -28,7 +28,7 @@ using namespace msolve;
 // ------------------------------------------------------------------------------------- errors
 static thread_local char g_err[512] = "";
 static int g_loop_mode = 0;
-static int g_lattice_kernel = 0;  // 0 = per element type (see MSOLVE_LAT_WARP), 1 = k_spmv_lat_tma, 2 = k_spmv_lat_warp
+static int g_lattice_kernel = 0;  // 0 = per element type (MSOLVE_LAT_HYB / MSOLVE_LAT_WARP), 1 = k_spmv_lat_tma, 2 = k_spmv_lat_warp, 3 = k_spmv_lat_hyb
 static int g_update_kernel = 0;   // 0 = register kernel, 1 = TMA-staged fused update when the vectors allow it
 
 static int fail(int code, const char* fmt, ...) {
@@ -155,6 +155,23 @@ template <> struct BsrTile<float2>  { static constexpr int TB = MSOLVE_BSR_TB_F,
 #define MSOLVE_LATW_STAGES 4
 #define MSOLVE_LATW_W_F 4
 #define MSOLVE_LATW_STAGES_F 8
+#endif
+// Hybrid lattice kernel (k_spmv_lat_hyb): consumer warps and ring depth.
+#ifndef MSOLVE_LATH_W
+#define MSOLVE_LATH_W 6
+#define MSOLVE_LATH_STAGES 6
+#endif
+#ifndef MSOLVE_LATH_W_F
+#define MSOLVE_LATH_W_F 8
+#define MSOLVE_LATH_STAGES_F 8
+#endif
+// Default lattice tile kernel per element type (config 4, profiles/r01_sweeps.md): complex128 hybrid 0.237 ms
+// (all-TMA kernels 0.269 / 0.277); complex64 warp-per-tile all-TMA 0.149 ms (hybrid 0.168).
+#ifndef MSOLVE_LAT_HYB
+#define MSOLVE_LAT_HYB 1
+#endif
+#ifndef MSOLVE_LAT_HYB_F
+#define MSOLVE_LAT_HYB_F 0
 #endif
 template <typename E> struct LatWarpTile;
 template <> struct LatWarpTile<double2> { static constexpr int W = MSOLVE_LATW_W, STAGES = MSOLVE_LATW_STAGES; static constexpr bool USE = MSOLVE_LAT_WARP != 0; };
@@ -290,6 +307,19 @@ static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
             if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
             const int grid = std::max(1, std::min(A->num_sms * CPS, A->dev.aux_count));
             k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
+            return;
+        }
+        // default: not for the second BiCGStab-M SpMV, whose five accumulators and two extra operands spill at 255
+        // registers (config3x: spmv2_dots 0.278 ms all-TMA, 0.320 ms hybrid)
+        if ((g_lattice_kernel == 3 || (g_lattice_kernel == 0 && ROLE != ROLE_B2 && (sizeof(T) == 16 ? MSOLVE_LAT_HYB : MSOLVE_LAT_HYB_F))) && A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
+            constexpr int HW = sizeof(T) == 16 ? MSOLVE_LATH_W : MSOLVE_LATH_W_F;
+            constexpr int HS = sizeof(T) == 16 ? MSOLVE_LATH_STAGES : MSOLVE_LATH_STAGES_F;
+            auto k = k_spmv_lat_hyb<T, HW, HS, ROLE>;
+            const int smem = LatHybCfg<T, HW>::smem_bytes(HS);
+            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
+            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
+            const int grid = std::max(1, std::min(A->num_sms, A->dev.aux_count));
+            k<<<grid, LatHybCfg<T, HW>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
             return;
         }
         if ((g_lattice_kernel == 2 || (g_lattice_kernel == 0 && LatWarpTile<T>::USE)) && A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
@@ -731,7 +761,7 @@ extern "C" const char* msolve_last_error(void) { return g_err; }
 extern "C" int msolve_config(int key, int value) {
     if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { g_loop_mode = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { g_update_kernel = value; return MSOLVE_OK; }
-    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 2) { g_lattice_kernel = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { g_lattice_kernel = value; return MSOLVE_OK; }
     return fail(MSOLVE_EINVAL, "msolve_config: bad key/value");
 }
 

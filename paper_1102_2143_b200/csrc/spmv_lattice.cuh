@@ -415,4 +415,148 @@ __global__ void __launch_bounds__(LatWarpCfg<E, W, PW>::kThreadsTotal, 1) k_spmv
     write_partials<NACC>(st, acc);
 }
 
+// ------------------------------------------------------------------------------------------
+// Hybrid tile kernel: two operand paths out of L2.  The all-TMA kernels above stop at ~10 TB/s of
+// L2 -> shared-memory traffic (every link twice, x seven times), not at HBM.  Here only the tile's
+// forward links and its own x come by bulk copy (d + 1 copies per tile instead of 14); the backward
+// links U_mu(s - mu) and the neighbours' x for mu >= 1 are loaded by the consumer lanes through
+// L1/L2 -- the neighbour of an x0-row is an x0-row, so a warp's loads cover contiguous ranges --
+// and are issued BEFORE the warp waits for its stage.  mu = 0 neighbours: the tile's own rows rotated.
+// Warp per tile, lane = site, one producer thread; a stage is owned by one consumer warp.
+// ------------------------------------------------------------------------------------------
+template <typename E, int W> struct LatHybCfg {
+    static constexpr int NS = 32;
+    static constexpr int kThreadsTotal = (W + 1) * 32;
+    static constexpr int kLinkSlot = NS * 9 * (int)sizeof(E);
+    static constexpr int kXSlot = NS * 3 * (int)sizeof(E);
+    static constexpr int kXBase = 4 * kLinkSlot;
+    static constexpr int kStageBytes = 4 * kLinkSlot + kXSlot;
+    static constexpr int smem_bytes(int stages) { return stages * kStageBytes + 2 * stages * 8; }
+};
+
+template <typename E, int W, int STAGES, int ROLE>
+__global__ void __launch_bounds__(LatHybCfg<E, W>::kThreadsTotal, 1) k_spmv_lat_hyb(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    typedef LatHybCfg<E, W> Cfg;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    constexpr int SZ = (int)sizeof(C);
+    static_assert(STAGES % W == 0, "each stage has one consumer warp");
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::kStageBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, 1); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    const C* __restrict__ links = (const C*)A.val;
+    const int nd = A.lat_ndim;
+    const int L0 = A.lat_ext[0];
+    const int TR = A.lat_rows_per_tile;
+    const long long vol = A.lat_vol;
+    const int nrows = (int)(vol / L0);
+    const int ntiles = A.aux_count;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    if (warp >= W) {
+        if (lane == 0) {                                               // producer: d + 1 bulk copies per tile
+            const uint64_t pol = policy_evict_normal();                // forward links are re-read as backward links
+            for (int m = 0;; ++m) {
+                bool more = true;
+                for (int stage = 0; stage < STAGES; ++stage) {
+                    const long long tl = (long long)blockIdx.x + (long long)(m * STAGES + stage) * gridDim.x;
+                    if (tl >= ntiles) { more = false; break; }
+                    const int row0 = (int)tl * TR;
+                    const int nr = min(TR, nrows - row0);
+                    const long long site0 = (long long)row0 * L0;
+                    const uint32_t ns = (uint32_t)(nr * L0);
+                    unsigned char* sb = smem + stage * Cfg::kStageBytes;
+                    const uint32_t bar = full0 + 8 * stage;
+                    mbar_wait(empty0 + 8 * stage, ((uint32_t)m & 1u) ^ 1u);
+                    mbar_expect_tx(bar, ns * (uint32_t)SZ * (uint32_t)(9 * nd + 3));
+                    for (int mu = 0; mu < nd; ++mu)
+                        bulk_g2s(smem_u32(sb + mu * Cfg::kLinkSlot), links + ((long long)mu * vol + site0) * 9, ns * 9u * SZ, bar, pol);
+                    bulk_g2s(smem_u32(sb + Cfg::kXBase), x + 3 * site0, ns * 3u * SZ, bar, pol);
+                }
+                if (!more) break;
+            }
+        }
+    } else {
+        const int rt = lane / L0, i0 = lane - rt * L0;
+        const int jf = rt * L0 + (i0 + 1 == L0 ? 0 : i0 + 1);
+        const int jb = rt * L0 + (i0 == 0 ? L0 - 1 : i0 - 1);
+        const T dg = (T)A.lat_diag, cf = (T)A.lat_cf, cb = (T)A.lat_cb;
+        const C z = cmake<C>(0.0, 0.0);
+        constexpr int per = STAGES / W;
+        for (int k = 0;; ++k) {
+            const int m = k / per, stage = warp + (k % per) * W;
+            const long long tl = (long long)blockIdx.x + (long long)(m * STAGES + stage) * gridDim.x;
+            if (tl >= ntiles) break;
+            const uint32_t phase = (uint32_t)m & 1u;
+            const int row0 = (int)tl * TR;
+            const int nr = min(TR, nrows - row0);
+            const int ns = nr * L0;
+            const bool on = lane < ns;
+            const long long s = (long long)row0 * L0 + lane;
+            const long long row = 3 * s;
+            C f0 = z, f1 = z, f2 = z, g0 = z, g1 = z, g2 = z;
+            C u0 = z, u1 = z, u2 = z;
+            // operands that do not come through the stage: issued before the wait
+            C xf[3][3], xb[3][3], ub[3][9];
+            if (on) {
+                if (ROLE != ROLE_CG) { u0 = ld_ro(u + row); u1 = ld_ro(u + row + 1); u2 = ld_ro(u + row + 2); }
+                unsigned rem = (unsigned)(row0 + rt);
+                long long str = L0;
+#pragma unroll
+                for (int mu = 1; mu < 4; ++mu) {
+                    if (mu >= nd) break;
+                    const unsigned L = (unsigned)A.lat_ext[mu];
+                    const unsigned c = rem % L;
+                    rem /= L;
+                    const long long sf = s + (c + 1 == L ? -(long long)(L - 1) * str : str);
+                    const long long sbk = s + (c == 0 ? (long long)(L - 1) * str : -str);
+                    const C* pf = x + 3 * sf;
+                    const C* pb = x + 3 * sbk;
+                    const C* pu = links + ((long long)mu * vol + sbk) * 9;
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) { xf[mu - 1][q] = ld_ro(pf + q); xb[mu - 1][q] = ld_ro(pb + q); }
+#pragma unroll
+                    for (int q = 0; q < 9; ++q) ub[mu - 1][q] = ld_ro(pu + q);
+                    str *= L;
+                }
+            }
+            mbar_wait(full0 + 8 * stage, phase);
+            if (on) {
+                const C* sbp = (const C*)(smem + stage * Cfg::kStageBytes);
+                const C* xs = sbp + Cfg::kXBase / SZ;
+                lat_matvec_acc<C, false>(sbp + lane * 9, xs + jf * 3, f0, f1, f2);
+                lat_matvec_acc<C, true>(sbp + jb * 9, xs + jb * 3, g0, g1, g2);
+#pragma unroll
+                for (int mu = 1; mu < 4; ++mu) {
+                    if (mu >= nd) break;
+                    lat_matvec_acc<C, false>(sbp + (mu * Cfg::NS + lane) * 9, xf[mu - 1], f0, f1, f2);
+                    lat_matvec_acc<C, true>(ub[mu - 1], xb[mu - 1], g0, g1, g2);
+                }
+                const C x0 = xs[lane * 3], x1 = xs[lane * 3 + 1], x2 = xs[lane * 3 + 2];
+                const C y0 = lat_combine(dg, x0, cf, f0, cb, g0);
+                const C y1 = lat_combine(dg, x1, cf, f1, cb, g1);
+                const C y2 = lat_combine(dg, x2, cf, f2, cb, g2);
+                y[row] = y0; y[row + 1] = y1; y[row + 2] = y2;
+                lat_epilogue<C, ROLE>(acc, y0, x0, u0);
+                lat_epilogue<C, ROLE>(acc, y1, x1, u1);
+                lat_epilogue<C, ROLE>(acc, y2, x2, u2);
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+        }
+    }
+    write_partials<NACC>(st, acc);
+}
+
 }  // namespace msolve

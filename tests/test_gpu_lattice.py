@@ -26,9 +26,9 @@ EXTENTS = [(4, 4, 6, 5),        # 8 x0-rows per tile
            (36, 3, 3, 3)]       # L0 > 32 sites: row kernel
 
 
-@pytest.fixture(params=[1, 2], ids=["termsite", "warptile"])
+@pytest.fixture(params=[1, 2, 3], ids=["termsite", "warptile", "hybrid"])
 def tile_kernel(request, ms):
-    """Run with each of the two TMA tile kernels forced (default: the faster one per element type)."""
+    """Run with each of the three tile kernels forced (default: the faster one per element type)."""
     ms.msolve_config(ms.MSOLVE_CFG_LATTICE_KERNEL, request.param)
     yield request.param
     ms.msolve_config(ms.MSOLVE_CFG_LATTICE_KERNEL, 0)
