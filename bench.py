@@ -163,20 +163,23 @@ def measured_peak_gbs():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def ncu_traffic_bytes(kernel_regex: str, workload: str):
-    """dram read+write bytes per launch of the dominant kernel from the committed ncu summary
-    (only if that capture was taken on this workload), or None."""
-    p = os.path.join(ROOT, "profiles", "r01_ncu_dram_traffic.csv")
-    if not os.path.exists(p):
-        return None
-    try:
-        for ln in open(p):
-            f = ln.strip().split(",")
-            if len(f) >= 6 and f[0] == kernel_regex and f[5] == workload:
-                return float(f[1])
-    except Exception:
-        return None
-    return None
+def ncu_traffic_bytes(kernel: str, workload: str):
+    """(dram read+write bytes per launch, source) of the dominant kernel from the newest committed ncu summary
+    that holds a capture of this kernel on this workload -- a STORED figure from one `ncu --set full` capture
+    (profiles/*.md names the command and the commit), not something measured in this run -- or (None, None)."""
+    for name in ("r02_ncu_dram_traffic.csv", "r01_ncu_dram_traffic.csv"):
+        p = os.path.join(ROOT, "profiles", name)
+        if not os.path.exists(p):
+            continue
+        try:
+            for ln in open(p):
+                f = ln.strip().split(",")
+                if len(f) >= 6 and f[0] == kernel and f[5] == workload:
+                    commit = f[6] if len(f) > 6 else "round 1 (see profiles/r01_ncu_dram_traffic.md)"
+                    return float(f[1]), "profiles/%s: stored ncu --set full capture taken at commit %s; not re-measured in this run" % (name, commit)
+        except Exception:
+            continue
+    return None, None
 
 
 # ----------------------------------------------------------------------------------- ranks
@@ -206,39 +209,73 @@ def throughput(total_iterations, max_ms):
 
 
 # ----------------------------------------------------------------------------------- oracle legs
-def oracle_sample(w, dtype, iters):
-    """The CPU oracle, as it stands, on the first `iters` iterations of the same workload."""
+def oracle_sample(w, dtype, iters, omp):
+    """The CPU oracle, as it stands, on the first `iters` iterations of the same workload (tol = 0: every shift
+    stays active).  omp=False: the single-threaded parity build; omp=True: the same source built with -fopenmp,
+    loops over rows / elements on all host cores.  The time includes the oracle's own allocation and
+    x_k <- 0, p_k <- b initialisation (2 S vectors), which is why a sample is not shorter than ~14 iterations."""
     import oracle
-    oracle.build()
+    (oracle.build_omp if omp else oracle.build)()
     fn = oracle.cgm if w.algorithm == "cgm" else oracle.bicgstabm
     t0 = time.perf_counter()
-    res = fn(w.rowptr, w.colidx, w.val.astype(dtype, copy=False), w.b.astype(dtype), w.shifts, 0.0, iters)
+    res = fn(w.rowptr, w.colidx, w.val.astype(dtype, copy=False), w.b.astype(dtype), w.shifts, 0.0, iters, omp=omp)
     dt = time.perf_counter() - t0
     return res.iterations / dt, dt, res.iterations
 
 
+def host_threads():
+    try:
+        return int(os.environ.get("OMP_NUM_THREADS", "")) or os.cpu_count()
+    except ValueError:
+        return os.cpu_count()
+
+
+def config_dict(args, w, dtype, fmt, world, S, shifts_total):
+    """`config` of the JSON line: a function of the workload and the command line only, so that the GPU arm and
+    the --impl reference arm print the same keys and values for the same command."""
+    e = np.dtype(dtype).itemsize
+    if fmt == "bsr3":
+        units, spmv = int(w.bcolidx.size), w.bcolidx.size * (9 * e + 4) + (w.n // 3 + 1) * 4 + 2 * w.n * e
+    elif fmt == "lat":
+        units, spmv = int(w.links.size // 9), w.links.size * e + 2 * w.n * e
+    else:
+        units, spmv = int(w.nnz), w.nnz * (e + 4) + (w.n + 1) * 4 + 2 * w.n * e
+    footprint_mb = (spmv + (4 + 2 * S) * w.n * e) / 1e6
+    l2_note = ("inputs larger than L2 (matrix + %d vectors = %.0f MB >> 126 MB), no flush" % (4 + 2 * S, footprint_mb)
+               if footprint_mb > 252 else
+               "working set %.0f MB (matrix + %d vectors) is not larger than 2 x L2 (126 MB) and is NOT flushed between "
+               "iterations: a solve re-reads its own vectors every iteration by construction" % (footprint_mb, 4 + 2 * S))
+    return {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
+            "shifts": S, "tol": w.tol,
+            "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world,
+            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "x_window": bool(args.x_window), "l2": l2_note}
+
+
 def run_reference(args, rank):
-    """--impl reference: the oracle on the host cores; each step = a bounded sample (2 iterations)."""
+    """--impl reference: the oracle on the host cores (all of them: the -fopenmp build of the same source).  Each
+    step = the same bounded sample the cpu_baseline leg of the GPU arm times (--cpu-iters iterations, tol = 0)."""
     if rank != 0:
         return
     w, dtype, fmt = make_workload(args.workload, 0, want_csr=True)
-    per_step = 2
+    per_step = max(args.cpu_iters, 1)
     for _ in range(args.warmup):
-        oracle_sample(w, dtype, per_step)
+        oracle_sample(w, dtype, per_step, True)
     t_tot, it_tot = 0.0, 0
     for _ in range(args.steps):
-        _, dt, it = oracle_sample(w, dtype, per_step)
+        _, dt, it = oracle_sample(w, dtype, per_step, True)
         t_tot += dt
         it_tot += it
     value = it_tot / t_tot
-    sample = "first %d iterations of %s per step (tol=0), all %d shifts active" % (per_step, w.name, w.shifts.size)
+    S = int(w.shifts.size)
+    sample = ("first %d iterations of %s per step (tol=0), all %d shifts active, OpenMP build of the oracle on %d threads"
+              % (per_step, w.name, S, host_threads()))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "higher_is_better": True, "scaling": "strong" if args.shard == "shifts" else "weak", "vs_baseline": None,
             "dtype": DTYPE_NAME[dtype], "data": "synthetic",
-            "config": {"workload": args.workload, "n": w.n, "nnz": int(w.nnz), "shifts": int(w.shifts.size),
-                       "format": "csr", "algorithm": w.algorithm},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "config": config_dict(args, w, dtype, fmt, int(os.environ.get("WORLD_SIZE", "1")), S, S),
+            "oracle_reads": "the same operator assembled as CSR (rowptr/colidx/val), whatever `format` the GPU arm takes",
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -253,12 +290,14 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="config4_c128_bsr3")
     ap.add_argument("--profile-iters", type=int, default=20)
-    ap.add_argument("--cpu-iters", type=int, default=14, help="oracle iterations timed for cpu_baseline (0 = skip)")
+    ap.add_argument("--cpu-iters", type=int, default=14, help="oracle iterations timed per cpu_baseline sample / per --impl reference step (0 = skip)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--spmv", default="auto", choices=["auto", "vector", "merge", "tile"],
                     help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
     ap.add_argument("--update-kernel", default="regs", choices=["regs", "tma"],
                     help="CG-M fused multishift update: register kernel (default) or the TMA-staged kernel")
+    ap.add_argument("--x-window", action="store_true",
+                    help="vector-CSR kernel: L2 access-policy window over the gathered vector (MSOLVE_CFG_X_WINDOW)")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "shifts"],
                     help="N > 1: replicas = every rank solves the whole family for its own right-hand side (weak "
                          "scaling, default); shifts = the ranks split the shifts of ONE system (strong scaling)")
@@ -290,8 +329,6 @@ def main():
     else:
         _build.build()
     ms.load_library()
-    ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 0 if args.loop_mode == "while" else 1)
-    ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, 1 if args.update_kernel == "tma" else 0)
 
     need_csr = args.workload.endswith("_csr") or (rank == 0 and world == 1 and args.cpu_iters > 0)
     w, dtype, fmt = make_workload(args.workload, 0 if args.shard == "shifts" else rank, want_csr=need_csr)
@@ -320,6 +357,10 @@ def main():
         A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype, copy=False)), flags)
     torch.cuda.synchronize()
     t_create = time.perf_counter() - t_create
+    ms.msolve_config(A, ms.MSOLVE_CFG_LOOP_MODE, 0 if args.loop_mode == "while" else 1)
+    ms.msolve_config(A, ms.MSOLVE_CFG_UPDATE_KERNEL, 1 if args.update_kernel == "tma" else 0)
+    if args.x_window:
+        ms.msolve_config(A, ms.MSOLVE_CFG_X_WINDOW, 1)
     S = int(w.shifts.size)
     b_host = torch.from_numpy(w.b.astype(dtype)).pin_memory()
     b_dev = b_host.cuda()
@@ -407,22 +448,21 @@ def main():
                              "GBps": round(gbs, 1), "frac_measured_peak": round(gbs / peak, 4),
                              "frac_8TBps": round(gbs / 8000.0, 4)}
         dom = "cgm_update" if w.algorithm == "cgm" else "bi_update"
-        traffic = ncu_traffic_bytes(dom, args.workload)
+        traffic, traffic_src = ncu_traffic_bytes(dom, args.workload)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["GBps"], "peak": peak,
                     "unit": "GB/s", "frac": round(kernels[dom]["GBps"] / peak, 4), "peak_source": peak_src,
-                    "traffic": traffic, "algorithmic_bytes_per_launch": ab[dom]}
+                    "traffic": traffic, "traffic_source": traffic_src, "algorithmic_bytes_per_launch": ab[dom]}
         iter_ms = sum(v["ms"] for v in kernels.values())
-        footprint_mb = (ab["spmv_dot" if w.algorithm == "cgm" else "spmv1_dot"] + (4 + 2 * S) * w.n * np.dtype(dtype).itemsize) / 1e6
-        l2_note = ("inputs larger than L2 (matrix + %d vectors = %.0f MB >> 126 MB), no flush" % (4 + 2 * S, footprint_mb)
-                   if footprint_mb > 252 else
-                   "working set %.0f MB (matrix + %d vectors) is not larger than 2 x L2 (126 MB) and is NOT flushed between "
-                   "iterations: a solve re-reads its own vectors every iteration by construction" % (footprint_mb, 4 + 2 * S))
         cpu = None
         if args.cpu_iters > 0 and world == 1:
-            v, dt, it = oracle_sample(w, dtype, args.cpu_iters)
-            cpu = {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle",
-                   "sample": "first %d iterations of %s (tol=0, all %d shifts active), %.1f s, single thread, %d host cores present"
-                             % (it, w.name, S, dt, os.cpu_count())}
+            v, dt, it = oracle_sample(w, dtype, args.cpu_iters, True)
+            v1, dt1, it1 = oracle_sample(w, dtype, max(args.cpu_iters // 2, 1), False)
+            cpu = {"value": v, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+                   "sample": "first %d iterations of %s (tol=0, all %d shifts active), %.1f s, OpenMP build of the oracle "
+                             "(same source, -fopenmp) on %d threads; allocation and p_k/x_k initialisation included"
+                             % (it, w.name, S, dt, host_threads()),
+                   "single_thread_value": v1,
+                   "single_thread_sample": "first %d iterations, %.1f s, the parity build (one thread)" % (it1, dt1)}
         line = {
             "metric": METRIC, "value": throughput(iters_all, ms_total), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
@@ -430,10 +470,7 @@ def main():
             "vs_baseline": (throughput(iters_all, ms_total) / (1 if args.shard == "shifts" else world) / PAPER_ITERS_PER_S[args.workload]
                             if args.workload in PAPER_ITERS_PER_S else None),
             "dtype": DTYPE_NAME[dtype], "data": "synthetic",
-            "config": {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt,
-                       "nnz_or_blocks": int(w.bcolidx.size if fmt == "bsr3" else w.links.size // 9 if fmt == "lat" else w.nnz), "shifts": S, "tol": w.tol,
-                       "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world, "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel,
-                       "l2": l2_note},
+            "config": config_dict(args, w, dtype, fmt, world, S, shifts_total),
             "time_to_solution_ms": ms_total / args.steps, "iterations_per_solve": iters_all / args.steps / (1 if args.shard == "shifts" else world),
             "status": status, "conv_iter": conv_iter, "create_ms": 1e3 * t_create,
             "steady_state_ms_per_iteration": round(iter_ms, 4),

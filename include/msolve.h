@@ -27,7 +27,8 @@
  *    handle's dtype".  Indices are int32.  All device arrays must be 16-byte aligned.
  *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
  *  - A handle may be used by one solve at a time (it owns the device-side solver state and the
- *    cached CUDA graphs); different handles are independent.
+ *    cached CUDA graphs); different handles are independent.  A handle belongs to the device that
+ *    was current when it was created; calls made with another current device return MSOLVE_EINVAL.
  */
 #ifndef MSOLVE_H
 #define MSOLVE_H
@@ -68,7 +69,7 @@ enum {
 
 #define MSOLVE_MAX_SHIFTS 128
 
-/* msolve_config keys */
+/* msolve_config keys (per handle) */
 enum {
     MSOLVE_CFG_LOOP_MODE = 0, /* 0 = device WHILE graph node (default), 1 = chunked relaunch of an
                                  unrolled iteration graph with a device `done` flag */
@@ -77,7 +78,15 @@ enum {
                                     of 16 bytes.  Same arithmetic; both run at the same 6.0 TB/s on B200 */,
     MSOLVE_CFG_LATTICE_KERNEL = 2 /* tile kernel of msolve_create_lattice_su3 handles: 0 = the faster one per
                                      element type (default), 1 = (term, site) threads + partials, 2 = warp per tile,
-                                     3 = hybrid (forward links by bulk copy, backward links and neighbours gathered) */
+                                     3 = hybrid (forward links by bulk copy, backward links and neighbours gathered) */,
+    MSOLVE_CFG_STOP_RULE = 3 /* 0 = per shift (default): shift k stops, and x_k is frozen, at the first iteration with
+                                |zeta_k| ||r|| <= tol ||b|| (the paper is silent on masking; R15).
+                                1 = Alg. 1 l.15 read literally ("while |r| > eps"): every shift keeps
+                                iterating until the residual of the UNSHIFTED system has ||r|| <= tol ||b||, then all
+                                stop together (conv_iter[k] = that iteration for every k) */,
+    MSOLVE_CFG_X_WINDOW = 4 /* vector-CSR kernel only: 1 = every SpMV launch carries an L2 access-policy window over the
+                               gathered vector (persisting hits; sets the device-wide persisting-L2 set-aside).
+                               Measured on B200, config 5: profiles/r02_sweeps.md; default 0 */
 };
 
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay
@@ -128,7 +137,8 @@ size_t msolve_workspace_bytes(const msolve_matrix *A, int nshifts, int algorithm
  *                     with |zeta_k| ||r|| <= tol ||b||; the solve ends when all shifts stopped.
  *   max_iter     in   limit on loop bodies (one SpMV each for CG-M, two for BiCGStab-M).
  *   d_x          out  nshifts*n complex, device, shift-major: x_k[i] at d_x[k*n + i].  Fully
- *                     overwritten (zero initial guess is part of the method).
+ *                     overwritten (zero initial guess is part of the method; a solve that stops before its
+ *                     first update -- b = 0, max_iter = 0, breakdown in the first loop body -- returns x = 0).
  *   d_workspace       device scratch of >= msolve_workspace_bytes(), 256-byte aligned.
  *   h_iterations out  loop bodies executed (may be NULL).
  *   h_conv_iter  out  nshifts ints: iteration at which shift k converged, -1 if it did not (or NULL).
@@ -184,8 +194,20 @@ const char *msolve_kernel_name(int algorithm, int j);
 /* Kernel launches issued (graph kernel nodes executed) by the last solve on this handle. */
 int64_t msolve_last_launch_count(const msolve_matrix *A);
 
-/* Process-wide options (MSOLVE_CFG_*).  Returns MSOLVE_OK or MSOLVE_EINVAL. */
-int msolve_config(int key, int value);
+/* Set option `key` (MSOLVE_CFG_*) of this handle; it holds for every later call on the handle.
+ * Returns MSOLVE_OK or MSOLVE_EINVAL (NULL handle, unknown key, value out of range). */
+int msolve_config(msolve_matrix *A, int key, int value);
+
+/* Per-iteration scalar history (the quantities of Alg. 1 l.20-26, which otherwise never
+ * leave the device): every later solve on this handle writes one row per completed iteration n = 0, 1, ...
+ * into d_hist (device, 8-byte aligned, borrowed, at least cap_rows rows), rows beyond cap_rows are dropped.
+ *   CG-M row,        3 + 3 S doubles: beta_n, alpha_{n+1}, R1 = ||r_{n+1}||^2, then zeta_{n+1,k} [S], beta_{n,k} [S],
+ *                    alpha_{n+1,k} [S];
+ *   BiCGStab-M row,  8 + 6 S doubles: beta (re, im), chi (re, im), alpha' (re, im), ||r'||^2, 0, then zeta_new_k [S],
+ *                    beta_k [S], chi_k [S] as (re, im) pairs.
+ * A shift that has stopped keeps the values of its last active iteration.  An iteration that breaks down
+ * writes no row.  cap_rows = 0 (or d_hist = NULL) switches the history off.  Returns OK / EINVAL. */
+int msolve_set_history(msolve_matrix *A, double *d_hist, int cap_rows);
 
 /* Free the handle and everything the library allocated for it (never the caller's arrays). */
 void msolve_destroy(msolve_matrix *A);

@@ -19,7 +19,9 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "msolve_oracle.cpp")
 _LIB = os.path.join(_HERE, "libmsolve_oracle.so")
+_LIB_OMP = os.path.join(_HERE, "libmsolve_oracle_omp.so")
 _lib = None
+_lib_omp = None
 
 OK, MAXITER, BREAKDOWN = 0, 1, 2
 C64, C128, F32, F64 = 0, 1, 2, 3
@@ -35,11 +37,32 @@ def build(force: bool = False) -> str:
     return _LIB
 
 
-def _load():
-    global _lib
+def build_omp(force: bool = False) -> str:
+    """The SAME source compiled with -fopenmp (loops over rows / elements on all host cores).  Used only by
+    the timing legs of bench.py (cpu_baseline, --impl reference); never by a parity test: its dot products
+    are summed per thread."""
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC):
+        tmp = _LIB_OMP + ".tmp%d" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-fopenmp", "-ffp-contract=off", "-fcx-fortran-rules", "-std=c++17",
+                               "-shared", "-fPIC", "-o", tmp, _SRC])
+        os.replace(tmp, _LIB_OMP)
+    return _LIB_OMP
+
+
+_ENTRY = ("oracle_spmv_csr", "oracle_cgm", "oracle_bicgstabm", "oracle_cg", "oracle_bicgstab")
+
+
+def _load(omp: bool = False):
+    global _lib, _lib_omp
+    if omp:
+        if _lib_omp is None:
+            _lib_omp = ctypes.CDLL(build_omp())
+            for name in _ENTRY:
+                getattr(_lib_omp, name).restype = ctypes.c_int
+        return _lib_omp
     if _lib is None:
         _lib = ctypes.CDLL(build())
-        for name in ("oracle_spmv_csr", "oracle_cgm", "oracle_bicgstabm", "oracle_cg", "oracle_bicgstab"):
+        for name in _ENTRY:
             getattr(_lib, name).restype = ctypes.c_int
     return _lib
 
@@ -89,7 +112,8 @@ class MultishiftResult:
     hist: Optional[np.ndarray]
 
 
-def _multishift(fn_name, rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule, hist_cap, hist_cols, zeta_complex):
+def _multishift(fn_name, rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule, hist_cap, hist_cols, zeta_complex,
+                omp=False):
     rowptr, colidx, val = _csr(rowptr, colidx, val)
     b = np.ascontiguousarray(b, dtype=val.dtype)
     shifts = np.ascontiguousarray(shifts, dtype=np.float64)
@@ -101,7 +125,7 @@ def _multishift(fn_name, rowptr, colidx, val, b, shifts, tol, max_iter, stop_rul
     r = np.empty(n, dtype=val.dtype)
     zeta = np.zeros(2 * s if zeta_complex else s, dtype=np.float64)
     hist = np.zeros((hist_cap, hist_cols(s)), dtype=np.float64) if hist_cap > 0 else None
-    rc = getattr(_load(), fn_name)(
+    rc = getattr(_load(omp), fn_name)(
         _dt(val), ctypes.c_int64(n), _p(rowptr), _p(colidx), _p(val), _p(b), _p(shifts), ctypes.c_int(s),
         ctypes.c_double(tol), ctypes.c_int(max_iter), ctypes.c_int(stop_rule), _p(x), ctypes.byref(it),
         _p(conv), _p(relres), _p(r), _p(zeta), _p(hist), ctypes.c_int(hist_cap))
@@ -113,17 +137,21 @@ def _multishift(fn_name, rowptr, colidx, val, b, shifts, tol, max_iter, stop_rul
     return MultishiftResult(rc, it.value, x, conv, relres, r, z, hist)
 
 
-def cgm(rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule: int = 0, hist_cap: int = 0) -> MultishiftResult:
+def cgm(rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule: int = 0, hist_cap: int = 0,
+        omp: bool = False) -> MultishiftResult:
     """CG-M (Alg. 1, read as DESIGN.md R2-R7).  hist row = beta, alpha_next, R1,
-    then zeta_new[S], beta_k[S], alpha_k[S]."""
+    then zeta_new[S], beta_k[S], alpha_k[S].  stop_rule 0 = per shift (R15), 1 = literal |r| > eps (l.15).
+    omp=True: the all-core build (timing legs only)."""
     return _multishift("oracle_cgm", rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule,
-                       hist_cap, lambda s: 3 + 3 * s, False)
+                       hist_cap, lambda s: 3 + 3 * s, False, omp)
 
 
-def bicgstabm(rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule: int = 0, hist_cap: int = 0) -> MultishiftResult:
-    """BiCGStab-M (PAPER.md:31,154; derivation in DESIGN.md)."""
+def bicgstabm(rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule: int = 0, hist_cap: int = 0,
+              omp: bool = False) -> MultishiftResult:
+    """BiCGStab-M (derivation in DESIGN.md).  hist row = beta, chi, alpha' (complex), |r'|^2, 0,
+    then zeta_new[S], beta_k[S], chi_k[S] (complex)."""
     return _multishift("oracle_bicgstabm", rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule,
-                       hist_cap, lambda s: 8 + 6 * s, True)
+                       hist_cap, lambda s: 8 + 6 * s, True, omp)
 
 
 def _single(fn_name, rowptr, colidx, val, sigma, b, tol, max_iter):

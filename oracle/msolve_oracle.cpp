@@ -30,6 +30,10 @@
 // the choice of stop/mask rule (R15) is a reading, pinned only as oracle == GPU.
 //
 // Build: g++ -O2 -ffp-contract=off -shared -fPIC (see oracle/__init__.py).
+// The `#pragma omp` lines are inert in that build (no -fopenmp): the parity oracle is single-threaded and
+// every sum has one fixed order.  oracle.build_omp() compiles the SAME source with -fopenmp into a second
+// library used only by bench.py's cpu_baseline / --impl reference timing legs (all host cores; its dot
+// products are summed per thread, so it is not the parity configuration).
 
 #include <cmath>
 #include <complex>
@@ -59,6 +63,7 @@ struct Csr {
 // y = A x   (Alg. 1 l.18).  Row sum in T, stored order.
 template <typename C>
 void spmv(const Csr<C>& A, const C* x, C* y) {
+#pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < A.n; ++i) {
         C acc(0);
         for (int32_t j = A.rowptr[i]; j < A.rowptr[i + 1]; ++j) acc += A.val[j] * x[A.colidx[j]];
@@ -69,9 +74,14 @@ void spmv(const Csr<C>& A, const C* x, C* y) {
 // <u,v> = sum_i conj(u_i) v_i, accumulated in double (r^dagger . r).
 template <typename C>
 zdouble dot(int64_t n, const C* u, const C* v) {
-    zdouble acc(0, 0);
-    for (int64_t i = 0; i < n; ++i) acc += std::conj(zdouble(u[i])) * zdouble(v[i]);
-    return acc;
+    double re = 0.0, im = 0.0;                      // the two components of one complex accumulator
+#pragma omp parallel for schedule(static) reduction(+ : re, im)
+    for (int64_t i = 0; i < n; ++i) {
+        const zdouble t = std::conj(zdouble(u[i])) * zdouble(v[i]);
+        re += t.real();
+        im += t.imag();
+    }
+    return zdouble(re, im);
 }
 
 // A recurrence scalar rounded ONCE to the vectors' element type (R14).  Real data: every dot
@@ -105,6 +115,7 @@ int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
     std::vector<C> r(b, b + n), p(b, b + n), q(n);           // l.9-10: r <- b, p <- b
     std::vector<C> pk((size_t)S * n);
     for (int k = 0; k < S; ++k)
+#pragma omp parallel for schedule(static)
         for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0); }  // l.11-12
     double alpha = 0.0, beta_prev = 1.0;                      // l.2, l.4
     std::vector<double> zeta_prev(S, 1.0), zeta(S, 1.0), zeta_new(S, 1.0), beta_k(S, 0.0), alpha_k(S, 0.0);
@@ -134,6 +145,7 @@ int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
         }
         if (status == ST_BREAKDOWN) break;
         { const C bt = rnd<C>(beta);
+#pragma omp parallel for schedule(static)
           for (int64_t i = 0; i < n; ++i) r[i] = r[i] + bt * q[i]; }   // l.21
         R1 = dot(n, r.data(), r.data()).real();               // l.24
         const double alpha_next = R1 / R0;                    // l.25
@@ -142,11 +154,14 @@ int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
             alpha_k[k] = alpha_next * ratio * ratio;          // l.26 (R5)
         }
         { const C an = rnd<C>(alpha_next);
+#pragma omp parallel for schedule(static)
           for (int64_t i = 0; i < n; ++i) p[i] = r[i] + an * p[i]; }   // l.27
         for (int k = 0; k < S; ++k) if (active[k]) {
             C* xk = x + (size_t)k * n; C* pkk = pk.data() + (size_t)k * n;
             const C bk = rnd<C>(beta_k[k]), zn = rnd<C>(zeta_new[k]), ak = rnd<C>(alpha_k[k]);
+#pragma omp parallel for schedule(static)
             for (int64_t i = 0; i < n; ++i) xk[i] = xk[i] - bk * pkk[i];            // l.28
+#pragma omp parallel for schedule(static)
             for (int64_t i = 0; i < n; ++i) pkk[i] = zn * r[i] + ak * pkk[i];       // l.29 (R6)
         }
         if (hist && it < hist_cap) {
@@ -192,6 +207,7 @@ int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double to
     std::vector<C> r(b, b + n), p(b, b + n), r0(b, b + n), q(n), s(n), t(n), rnew(n);
     std::vector<C> pk((size_t)S * n);
     for (int k = 0; k < S; ++k)
+#pragma omp parallel for schedule(static)
         for (int64_t i = 0; i < n; ++i) { pk[(size_t)k * n + i] = b[i]; x[(size_t)k * n + i] = C(0); }
     zdouble alpha(0, 0), beta_prev(1, 0);
     std::vector<zdouble> zeta_prev(S, 1.0), zeta(S, 1.0), zeta_new(S, 1.0), rho(S, 1.0), rho_new(S, 1.0),
@@ -222,6 +238,7 @@ int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double to
         }
         if (status == ST_BREAKDOWN) break;
         { const C bt = rnd<C>(beta);
+#pragma omp parallel for schedule(static)
           for (int64_t i = 0; i < n; ++i) s[i] = r[i] + bt * q[i]; }       // s = r + beta q
         spmv(A, s.data(), t.data());                                       // t = A s
         const zdouble ts = dot(n, t.data(), s.data());
@@ -237,6 +254,7 @@ int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double to
         }
         if (status == ST_BREAKDOWN) break;
         { const C ch = rnd<C>(chi);
+#pragma omp parallel for schedule(static)
           for (int64_t i = 0; i < n; ++i) rnew[i] = s[i] - ch * t[i]; }    // r' = s - chi t
         const zdouble delta_new = dot(n, r0.data(), rnew.data());           // delta' = <r0,r'>
         const zdouble alpha_new = -beta * delta_new / (delta * chi);        // alpha' = -beta delta'/(delta chi)
@@ -254,12 +272,16 @@ int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double to
             const C cb = rnd<C>(chi_k[k] / beta_k[k]);
             const C zs = rnd<C>(zeta_new[k] * rho[k]);                      // s^sigma = zs * s
             const C zo = rnd<C>(zeta[k] * rho[k]);                          // r^sigma = zo * r
+#pragma omp parallel for schedule(static)
             for (int64_t i = 0; i < n; ++i) xk[i] = (xk[i] - bk * pkk[i]) + cs * s[i];
+#pragma omp parallel for schedule(static)
             for (int64_t i = 0; i < n; ++i)
                 pkk[i] = zr * rnew[i] + ak * (pkk[i] - cb * (zs * s[i] - zo * r[i]));
         }
         { const C an = rnd<C>(alpha_new), ch = rnd<C>(chi);
+#pragma omp parallel for schedule(static)
           for (int64_t i = 0; i < n; ++i) p[i] = rnew[i] + an * (p[i] - ch * q[i]); }  // p = r' + alpha'(p - chi q)
+#pragma omp parallel for schedule(static)
         for (int64_t i = 0; i < n; ++i) r[i] = rnew[i];
         rr = dot(n, r.data(), r.data()).real();
         if (hist && it < hist_cap) {

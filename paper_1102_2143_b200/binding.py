@@ -15,8 +15,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# MSOLVE_LIB selects another build of the same library (kernel-tuning sweeps); default: in-tree
-LIB_PATH = os.environ.get("MSOLVE_LIB") or os.path.join(_HERE, "libmsolve.so")
+LIB_PATH = os.path.join(_HERE, "libmsolve.so")
 
 MSOLVE_C64, MSOLVE_C128, MSOLVE_F32, MSOLVE_F64 = 0, 1, 2, 3
 MSOLVE_ALG_CGM, MSOLVE_ALG_BICGSTABM = 0, 1
@@ -27,11 +26,13 @@ MSOLVE_MAX_SHIFTS = 128
 MSOLVE_CFG_LOOP_MODE = 0
 MSOLVE_CFG_UPDATE_KERNEL = 1
 MSOLVE_CFG_LATTICE_KERNEL = 2
+MSOLVE_CFG_STOP_RULE = 3
+MSOLVE_CFG_X_WINDOW = 4
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
     "msolve_bicgstabm", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
-    "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_destroy",
+    "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_set_history", "msolve_destroy",
     "msolve_last_error",
 )
 
@@ -70,12 +71,14 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_kernel_name.restype = ctypes.c_char_p
     lib.msolve_last_launch_count.argtypes = [vp]
     lib.msolve_last_launch_count.restype = i64
-    lib.msolve_config.argtypes = [i32, i32]
+    lib.msolve_config.argtypes = [vp, i32, i32]
+    lib.msolve_set_history.argtypes = [vp, vp, i32]
     lib.msolve_destroy.argtypes = [vp]
     lib.msolve_destroy.restype = None
     lib.msolve_last_error.restype = ctypes.c_char_p
     for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_cgm", "msolve_bicgstabm",
-                 "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration", "msolve_config"):
+                 "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration", "msolve_config",
+                 "msolve_set_history"):
         getattr(lib, name).restype = i32
     _lib = lib
     return lib
@@ -125,6 +128,7 @@ class Matrix:
         self.dtype = dtype
         self.n = n
         self._keep = keep
+        self._hist = None
 
     def destroy(self):
         if self.handle:
@@ -188,8 +192,23 @@ def msolve_workspace_bytes(A: Matrix, nshifts: int, algorithm: int) -> int:
     return int(load_library().msolve_workspace_bytes(A.handle, nshifts, algorithm))
 
 
-def msolve_config(key: int, value: int) -> None:
-    _check(load_library().msolve_config(key, value))
+def msolve_config(A: Matrix, key: int, value: int) -> None:
+    """Set option `key` (MSOLVE_CFG_*) of this handle."""
+    _check(load_library().msolve_config(A.handle, key, value))
+
+
+def msolve_set_history(A: Matrix, hist: Optional[torch.Tensor]) -> None:
+    """Per-iteration scalar history: `hist` is a contiguous float64 CUDA tensor [cap_rows, 3 + 3 S] (CG-M) or
+    [cap_rows, 8 + 6 S] (BiCGStab-M) that later solves on this handle fill row by row; None switches it off."""
+    if hist is None:
+        _check(load_library().msolve_set_history(A.handle, None, 0))
+        A._hist = None
+        return
+    hist = _dev(hist, torch.float64)
+    if hist.dim() != 2:
+        raise ValueError("hist must be [cap_rows, row_length]")
+    _check(load_library().msolve_set_history(A.handle, hist.data_ptr(), hist.shape[0]))
+    A._hist = hist
 
 
 def msolve_last_launch_count(A: Matrix) -> int:

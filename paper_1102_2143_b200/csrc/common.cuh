@@ -16,6 +16,9 @@ constexpr int kMaxPartials = 4096;  // upper bound on any reducing kernel's grid
 constexpr int kAccMax = 5;          // doubles reduced per CTA (BiCGStab-M SpMV#2 needs 5)
 constexpr int kThreads = 256;
 
+// which vectors an SpMV launch works on and which reductions it fuses (spmv.cuh)
+enum { ROLE_CG = 0, ROLE_B1 = 1, ROLE_B2 = 2, ROLE_GEN = 3 };
+
 // ----------------------------------------------------------------------------- element types
 // The kernels are templated on the ELEMENT type E of matrices and vectors: float2 / double2 are
 // interleaved complex (MSOLVE_C64 / MSOLVE_C128, the BASELINE configs), float / double are real
@@ -197,6 +200,9 @@ struct SolveHeader {
     int S;
     int max_iter;
     int force_all;   // profiling: never converge, never stop before max_iter
+    int stop_rule;   // 0 = per shift (R15), 1 = literal |r| > eps on the unshifted system (Alg. 1 l.15)
+    double* hist;    // msolve_set_history: per-iteration scalars, hist_cap rows (NULL = off)
+    int hist_cap;
     int pad0;
     double sigma[kMaxShifts];
 };

@@ -102,9 +102,7 @@ __global__ void __launch_bounds__(kThreads) k_init_state(SolveState* st) {
     }
 }
 
-#ifndef MSOLVE_PUPD_U
-#define MSOLVE_PUPD_U 4
-#endif
+constexpr int kPupdUnroll = 4;   // 2 * 4 independent 16-byte loads in flight per thread
 // ----------------------------------------------------------------------------- CG-M
 // A1: p <- r + alpha p  (l.27; at n = 0 p = b already)
 template <typename E, int VEC>
@@ -117,7 +115,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
     P* p = (P*)st->h.p;
     const T alpha = (T)st->alpha.re;
     const long long stride = (long long)gridDim.x * blockDim.x;
-    constexpr int U = MSOLVE_PUPD_U;                       // 2U independent 16-byte loads in flight
+    constexpr int U = kPupdUnroll;
     long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     for (; i + (U - 1) * stride < nvec; i += U * stride) {
         P rv[U], pv[U];
@@ -278,7 +276,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGrap
     const int na = st->res.nactive;
     const int it = st->res.n_iter + 1;
     const double rnorm = sqrt(R1), bnorm = st->bnorm, tol = st->h.tol;
-    const bool force = st->h.force_all != 0;
+    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
         const int k = st->active[a];
         const double zn = st->zeta_new[k].re, z = st->zeta[k].re;
@@ -288,7 +286,19 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGrap
         st->zeta[k].re = zn;                                            // l.31
         const double rel = fabs(zn) * rnorm / bnorm;
         st->res.relres[k] = rel;
-        if (!force && fabs(zn) * rnorm <= tol * bnorm) st->res.conv_iter[k] = it;   // l.15, per shift
+        // l.15: per shift (R15), or literally on the unshifted residual (stop_rule = 1)
+        if (!force && (base_rule ? rnorm : fabs(zn) * rnorm) <= tol * bnorm) st->res.conv_iter[k] = it;
+    }
+    // msolve_set_history: row it-1 = beta, alpha_next, R1, then zeta_new[S], beta_k[S], alpha_k[S] (frozen shifts
+    // keep the values of their last active iteration)
+    if (st->h.hist && it <= st->h.hist_cap) {
+        __syncthreads();
+        const int S = st->h.S;
+        double* h = st->h.hist + (size_t)(it - 1) * (size_t)(3 + 3 * S);
+        if (threadIdx.x == 0) { h[0] = st->beta.re; h[1] = alpha_next; h[2] = R1; }
+        for (int k = threadIdx.x; k < S; k += blockDim.x) {
+            h[3 + k] = st->zeta_new[k].re; h[3 + S + k] = st->beta_k[k].re; h[3 + 2 * S + k] = st->alpha_k[k].re;
+        }
     }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -495,7 +505,7 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraph
     const int na = st->res.nactive;
     const int it = st->res.n_iter + 1;
     const double rnorm = sqrt(rr), bnorm = st->bnorm, tol = st->h.tol;
-    const bool force = st->h.force_all != 0;
+    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
         const int k = st->active[a];
         const zd zn = st->zeta_new[k], rn = st->rho_new[k];
@@ -504,7 +514,22 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraph
         st->rho[k] = rn;
         const double zr = zabs(zmul(zn, rn));
         st->res.relres[k] = zr * rnorm / bnorm;
-        if (!force && zr * rnorm <= tol * bnorm) st->res.conv_iter[k] = it;
+        if (!force && (base_rule ? rnorm : zr * rnorm) <= tol * bnorm) st->res.conv_iter[k] = it;
+    }
+    // msolve_set_history: row it-1 = beta, chi, alpha' (complex), |r'|^2, 0, then zeta_new[S], beta_k[S], chi_k[S] (complex)
+    if (st->h.hist && it <= st->h.hist_cap) {
+        __syncthreads();
+        const int S = st->h.S;
+        double* h = st->h.hist + (size_t)(it - 1) * (size_t)(8 + 6 * S);
+        if (threadIdx.x == 0) {
+            h[0] = st->beta.re; h[1] = st->beta.im; h[2] = st->chi.re; h[3] = st->chi.im;
+            h[4] = st->alpha_new.re; h[5] = st->alpha_new.im; h[6] = rr; h[7] = 0.0;
+        }
+        for (int k = threadIdx.x; k < S; k += blockDim.x) {
+            h[8 + 2 * k] = st->zeta_new[k].re; h[8 + 2 * k + 1] = st->zeta_new[k].im;
+            h[8 + 2 * S + 2 * k] = st->beta_k[k].re; h[8 + 2 * S + 2 * k + 1] = st->beta_k[k].im;
+            h[8 + 4 * S + 2 * k] = st->chi_k[k].re; h[8 + 4 * S + 2 * k + 1] = st->chi_k[k].im;
+        }
     }
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -5,6 +5,7 @@
 // node iterates the captured kernel sequence on the device until the device-side stop test
 // clears the condition ("entire solution on the GPU"),
 // then read back a ~1.6 KB result block after a single stream synchronisation.
+// The kernels live in the other translation units (handle.h lists them).
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -15,23 +16,16 @@
 #include <new>
 #include <vector>
 
-#include "common.cuh"
-#include "kernels.cuh"
-#include "spmv.cuh"
-#include "spmv_merge.cuh"
-#include "spmv_csr_tile.cuh"
-#include "spmv_lattice.cuh"
-#include "update_tma.cuh"
+#include "handle.h"
+#include "tuning.h"
+#include "spmv_merge.cuh"      // MergeCfg (tile geometry of the merge-path partition built here)
 
 using namespace msolve;
 
 // ------------------------------------------------------------------------------------- errors
 static thread_local char g_err[512] = "";
-static int g_loop_mode = 0;
-static int g_lattice_kernel = 0;  // 0 = per element type (MSOLVE_LAT_HYB / MSOLVE_LAT_WARP), 1 = k_spmv_lat_tma, 2 = k_spmv_lat_warp, 3 = k_spmv_lat_hyb
-static int g_update_kernel = 0;   // 0 = register kernel, 1 = TMA-staged fused update when the vectors allow it
 
-static int fail(int code, const char* fmt, ...) {
+int msolve::fail(int code, const char* fmt, ...) {
     va_list ap;
     va_start(ap, fmt);
     vsnprintf(g_err, sizeof(g_err), fmt, ap);
@@ -39,181 +33,31 @@ static int fail(int code, const char* fmt, ...) {
     return code;
 }
 
-#define CU(call)                                                                                   \
-    do {                                                                                           \
-        cudaError_t e_ = (call);                                                                   \
-        if (e_ != cudaSuccess)                                                                     \
-            return fail(MSOLVE_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
-    } while (0)
+#define CU(call) MSOLVE_CU(call)
 
-// ------------------------------------------------------------------------------------- handle
-enum { FMT_CSR = 0, FMT_BSR3 = 1, FMT_LATTICE = 2 };
-enum { KERNEL_VECTOR = 1, KERNEL_MERGE = 2, KERNEL_BSR_ROWS = 3, KERNEL_BSR_TMA = 4, KERNEL_LAT_ROWS = 5, KERNEL_LAT_TMA = 6, KERNEL_CSR_TILE = 7 };
-constexpr int kChunk = 8;  // iteration bodies per graph launch in chunked mode
+int msolve::ensure_smem(const msolve_matrix* A, const void* kernel, int bytes) {
+    for (const void* k : A->smem_attr_done) if (k == kernel) return MSOLVE_OK;
+    CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    A->smem_attr_done.push_back(kernel);
+    return MSOLVE_OK;
+}
 
-struct LoopGraph {
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t exec = nullptr;
-    int mode = -1;
-};
-
-struct msolve_matrix {
-    int format = FMT_CSR;
-    int dtype = MSOLVE_C128;
-    int kernel = KERNEL_VECTOR;
-    int lanes = 8;
-    int tile_u = 4;                     // KERNEL_CSR_TILE: non-zeros per lane
-    MatDev dev{};
-    int device = 0;
-    int num_sms = 148;
-    SolveState* d_state = nullptr;      // library-owned
-    SolveState* h_stage = nullptr;      // pinned staging for header / result
-    void* d_aux = nullptr;              // library-owned auxiliary matrix data
-    void* d_carry = nullptr;            // merge-path carries (library-owned)
-    char* d_host_buf = nullptr;         // msolve_solve_host: device b, x and workspace, kept for the next call
-    size_t host_buf_bytes = 0;
-    char* d_batch_buf = nullptr;        // msolve_solve_host_batch: two (b, x) slots + workspace
-    size_t batch_buf_bytes = 0;
-    cudaStream_t copy_stream = nullptr; // D2H of solve i overlaps solve i+1
-    cudaEvent_t ev_solved[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
-    cudaStream_t capture_stream = nullptr;
-    LoopGraph graphs[2];
-    int64_t last_launches = 0;
-};
+// the handle's device must be the calling thread's current device (kernels, graphs and the function
+// attributes above belong to it)
+static int check_device(const msolve_matrix* A, const char* who) {
+    int cur = -1;
+    CU(cudaGetDevice(&cur));
+    if (cur != A->device) return fail(MSOLVE_EINVAL, "%s: the handle lives on device %d, the current device is %d", who, A->device, cur);
+    return MSOLVE_OK;
+}
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
-static size_t elem_bytes(int dtype) { return dtype == MSOLVE_C128 ? 16 : dtype == MSOLVE_F32 ? 4 : 8; }
 static bool valid_dtype(int dtype) { return dtype >= MSOLVE_C64 && dtype <= MSOLVE_F64; }
 static bool complex_dtype(int dtype) { return dtype == MSOLVE_C64 || dtype == MSOLVE_C128; }
-template <typename E> struct IsComplex { static constexpr bool value = false; };
-template <> struct IsComplex<float2> { static constexpr bool value = true; };
-template <> struct IsComplex<double2> { static constexpr bool value = true; };
+static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
-// ------------------------------------------------------------------------------------- launch
-template <typename K>
-static int blocks_per_sm(K kernel) {
-    int nb = 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, kThreads, 0) != cudaSuccess || nb < 1) nb = 1;
-    return nb;
-}
-
-// persistent grid: enough CTAs for `work_items` at `items_per_cta`, capped at full occupancy
-template <typename K>
-static int grid_for(const msolve_matrix* A, K kernel, long long work_items, long long items_per_cta) {
-    long long full = (long long)A->num_sms * blocks_per_sm(kernel);
-    long long need = (work_items + items_per_cta - 1) / items_per_cta;
-    long long g = std::max(1ll, std::min(full, need));
-    return (int)std::min<long long>(g, kMaxPartials);
-}
-
-// TMA-staged BSR3 kernel configuration: block rows per tile, lanes per scalar row, pipeline depth
-template <typename E> struct BsrTile;
-// Tuned on B200 (profiles/r01_sweeps.md): many small CTAs per SM (independent
-// tiles in flight hide the x-gather latency), a 2-deep ring is enough for the bulk copies, and a
-// small shared-memory footprint leaves L1 for the gathers.
-#ifndef MSOLVE_BSR_TB
-#define MSOLVE_BSR_TB 12
-#define MSOLVE_BSR_STAGES 2
-#define MSOLVE_BSR_CPS 5
-#endif
-#ifndef MSOLVE_BSR_CPS_F
-#define MSOLVE_BSR_CPS_F 4
-#endif
-#ifndef MSOLVE_BSR_CPS_B2_LESS
-#define MSOLVE_BSR_CPS_B2_LESS 1
-#endif
-#ifndef MSOLVE_BSR_TB_F
-#define MSOLVE_BSR_TB_F (2 * MSOLVE_BSR_TB)
-#endif
-#ifndef MSOLVE_BSR_STAGES_F
-#define MSOLVE_BSR_STAGES_F MSOLVE_BSR_STAGES
-#endif
-template <> struct BsrTile<double2> { static constexpr int TB = MSOLVE_BSR_TB, STAGES = MSOLVE_BSR_STAGES, CPS = MSOLVE_BSR_CPS; };
-template <> struct BsrTile<float2>  { static constexpr int TB = MSOLVE_BSR_TB_F, STAGES = MSOLVE_BSR_STAGES_F, CPS = MSOLVE_BSR_CPS_F; };
-
-// Matrix-free lattice kernel configuration: sites per tile, ring depth, CTAs per SM.
-#ifndef MSOLVE_LAT_NS
-#define MSOLVE_LAT_NS 32
-#define MSOLVE_LAT_STAGES 2
-#define MSOLVE_LAT_CPS 2
-#define MSOLVE_LAT_CPS_F 4
-#endif
-// Which lattice tile kernel: 1 = warp-per-tile (k_spmv_lat_warp), 0 = (term, site) threads + partials
-// (k_spmv_lat_tma).  Measured on config 4 (profiles/r01_sweeps.md): complex128 0.269 ms (tma) vs
-// 0.277 ms (warp); complex64 0.160 ms (tma) vs 0.150 ms (warp).
-#ifndef MSOLVE_LAT_WARP
-#define MSOLVE_LAT_WARP 0
-#endif
-#ifndef MSOLVE_LAT_WARP_F
-#define MSOLVE_LAT_WARP_F 1
-#endif
-#ifndef MSOLVE_LATW_PW
-#define MSOLVE_LATW_PW 4         // producer warps (bulk-copy issue is the bottleneck)
-#endif
-#ifndef MSOLVE_LATW_W
-#define MSOLVE_LATW_W 2
-#define MSOLVE_LATW_STAGES 4
-#define MSOLVE_LATW_W_F 4
-#define MSOLVE_LATW_STAGES_F 8
-#endif
-// Hybrid lattice kernel (k_spmv_lat_hyb): consumer warps and ring depth.
-#ifndef MSOLVE_LATH_W
-#define MSOLVE_LATH_W 6
-#define MSOLVE_LATH_STAGES 6
-#endif
-#ifndef MSOLVE_LATH_W_F
-#define MSOLVE_LATH_W_F 8
-#define MSOLVE_LATH_STAGES_F 8
-#endif
-// Default lattice tile kernel per element type (config 4, profiles/r01_sweeps.md): complex128 hybrid 0.237 ms
-// (all-TMA kernels 0.269 / 0.277); complex64 warp-per-tile all-TMA 0.149 ms (hybrid 0.168).
-#ifndef MSOLVE_LAT_HYB
-#define MSOLVE_LAT_HYB 1
-#endif
-#ifndef MSOLVE_LAT_HYB_F
-#define MSOLVE_LAT_HYB_F 0
-#endif
-template <typename E> struct LatWarpTile;
-template <> struct LatWarpTile<double2> { static constexpr int W = MSOLVE_LATW_W, STAGES = MSOLVE_LATW_STAGES; static constexpr bool USE = MSOLVE_LAT_WARP != 0; };
-template <> struct LatWarpTile<float2>  { static constexpr int W = MSOLVE_LATW_W_F, STAGES = MSOLVE_LATW_STAGES_F; static constexpr bool USE = MSOLVE_LAT_WARP_F != 0; };
-template <typename E> struct LatTile;
-template <> struct LatTile<double2> { static constexpr int NS = MSOLVE_LAT_NS, STAGES = MSOLVE_LAT_STAGES, CPS = MSOLVE_LAT_CPS; };
-template <> struct LatTile<float2>  { static constexpr int NS = MSOLVE_LAT_NS, STAGES = MSOLVE_LAT_STAGES, CPS = MSOLVE_LAT_CPS_F; };
-
-// Merge-path CSR kernel configuration: tile capacity (non-zeros), ring depth, CTAs per SM.
-#ifndef MSOLVE_MERGE_CAP
-#define MSOLVE_MERGE_CAP 1024
-#define MSOLVE_MERGE_CAP_F 2048
-#define MSOLVE_MERGE_STAGES 4
-#define MSOLVE_MERGE_STAGES_F 3
-#define MSOLVE_MERGE_CPS 2
-#define MSOLVE_MERGE_CPS_F 2
-#endif
-#ifndef MSOLVE_MERGE_STAGES_F
-#define MSOLVE_MERGE_STAGES_F MSOLVE_MERGE_STAGES
-#endif
-template <typename E> struct MergeTile;
-template <> struct MergeTile<double2> { static constexpr int CAP = MSOLVE_MERGE_CAP, STAGES = MSOLVE_MERGE_STAGES, CPS = MSOLVE_MERGE_CPS; };
-template <> struct MergeTile<float2>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
-template <> struct MergeTile<double>  { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
-template <> struct MergeTile<float>   { static constexpr int CAP = MSOLVE_MERGE_CAP_F, STAGES = MSOLVE_MERGE_STAGES_F, CPS = MSOLVE_MERGE_CPS_F; };
-
-// TMA-staged vector-CSR (spmv_csr_tile.cuh): ring depth and CTAs per SM; the lanes per row and
-// the non-zeros per lane U are chosen per matrix at create time (csr_tile_shape).
-// Measured on config 4 as CSR (profiles/r01_sweeps.md): complex128 8 lanes x 4 non-zeros, 3 stages,
-// 5 CTAs per SM: 0.559 ms (vector kernel 0.874); complex64 4 lanes x 8: 0.324 ms (8 x 4: 0.389; vector 0.678).
-#ifndef MSOLVE_CT_STAGES
-#define MSOLVE_CT_STAGES 3
-#define MSOLVE_CT_CPS 5
-#endif
-#ifndef MSOLVE_CT_STAGES_F
-#define MSOLVE_CT_STAGES_F 3
-#define MSOLVE_CT_CPS_F 5
-#endif
-template <typename E> struct CsrTile { static constexpr int STAGES = MSOLVE_CT_STAGES_F, CPS = MSOLVE_CT_CPS_F; };
-template <> struct CsrTile<double2> { static constexpr int STAGES = MSOLVE_CT_STAGES, CPS = MSOLVE_CT_CPS; };
-// (lanes, U) for rows of at most `maxlen` non-zeros; false when the rows are too long.
-// 16-byte elements: U = 4, 2..16 lanes (rows <= 64).  Smaller elements: U = 4 with 2 or 4 lanes
+// (lanes, U) of the TMA-staged vector-CSR kernel for rows of at most `maxlen` non-zeros; false when the rows are
+// too long.  16-byte elements: U = 4, 2..16 lanes (rows <= 64).  Smaller elements: U = 4 with 2 or 4 lanes
 // for rows <= 16 (the 5-point Poisson matrix: 2 x 4 0.0225 ms, 2 x 8 0.0261 ms), U = 8 with
 // 4..16 lanes for rows <= 128.
 static bool csr_tile_shape(int dtype, long long maxlen, int* lanes, int* u) {
@@ -230,197 +74,13 @@ static bool csr_tile_shape(int dtype, long long maxlen, int* lanes, int* u) {
     return *lanes <= 16;
 }
 
-// run F<E>() for the element type of `dtype`
 #define DISPATCH_ELEM(dtype, EXPR_C128, EXPR_C64, EXPR_F64, EXPR_F32) \
     ((dtype) == MSOLVE_C128 ? (EXPR_C128) : (dtype) == MSOLVE_C64 ? (EXPR_C64) : (dtype) == MSOLVE_F64 ? (EXPR_F64) : (EXPR_F32))
 
-static int merge_cps(int dtype) {
-    return DISPATCH_ELEM(dtype, MergeTile<double2>::CPS, MergeTile<float2>::CPS, MergeTile<double>::CPS, MergeTile<float>::CPS);
-}
 static int merge_diag(int dtype) {
     return DISPATCH_ELEM(dtype, (MergeCfg<double2, MergeTile<double2>::CAP>::kDiag), (MergeCfg<float2, MergeTile<float2>::CAP>::kDiag),
                          (MergeCfg<double, MergeTile<double>::CAP>::kDiag), (MergeCfg<float, MergeTile<float>::CAP>::kDiag));
 }
-static int merge_grid(const msolve_matrix* A) {
-    return std::max(1, std::min(A->num_sms * merge_cps(A->dtype), A->dev.aux_count));
-}
-static int merge_fixup_grid(const msolve_matrix* A) {
-    return std::max(1, std::min(A->num_sms, (A->dev.aux_count + kThreads - 1) / kThreads));
-}
-
-template <typename T, int LANES, int U, int ROLE>
-static void launch_csr_tile(const msolve_matrix* A, cudaStream_t s) {
-    typedef CsrTile<T> P;
-    typedef CsrTileCfg<T, LANES, U> Cfg;
-    auto k = k_spmv_csr_tile<T, LANES, U, P::STAGES, P::CPS, ROLE>;
-    const int smem = Cfg::smem_bytes(P::STAGES);
-    static thread_local bool attr_set = false;   // per <T, LANES, U, ROLE> instantiation
-    if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-    const long long ntiles = (A->dev.n + Cfg::kRows - 1) / Cfg::kRows;
-    const int grid = (int)std::max(1ll, std::min<long long>((long long)A->num_sms * P::CPS, ntiles));
-    k<<<grid, Cfg::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-}
-
-template <typename T, int ROLE>
-static void launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
-    if (A->format == FMT_CSR && A->kernel == KERNEL_CSR_TILE) {
-        if (sizeof(T) == 16 || A->tile_u == 4) {
-            switch (A->lanes) {
-                case 2: launch_csr_tile<T, 2, 4, ROLE>(A, s); break;
-                case 4: launch_csr_tile<T, 4, 4, ROLE>(A, s); break;
-                case 8: if constexpr (sizeof(T) == 16) launch_csr_tile<T, 8, 4, ROLE>(A, s); break;
-                default: if constexpr (sizeof(T) == 16) launch_csr_tile<T, 16, 4, ROLE>(A, s); break;
-            }
-        } else if constexpr (sizeof(T) < 16) {
-            switch (A->lanes) {
-                case 4: launch_csr_tile<T, 4, 8, ROLE>(A, s); break;
-                case 8: launch_csr_tile<T, 8, 8, ROLE>(A, s); break;
-                default: launch_csr_tile<T, 16, 8, ROLE>(A, s); break;
-            }
-        }
-        return;
-    }
-    if (A->format == FMT_CSR && A->kernel == KERNEL_MERGE) {
-        typedef MergeTile<T> M;
-        auto kp = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE, true>;     // x pinned in L2
-        auto kn = k_spmv_csr_merge<T, M::CAP, M::STAGES, M::CPS, ROLE, false>;
-        const int smem = MergeCfg<T, M::CAP>::smem_bytes(M::STAGES);
-        static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-        if (!attr_set) {
-            cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-            cudaFuncSetAttribute(kn, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-            attr_set = true;
-        }
-        const int grid = merge_grid(A);
-        (A->dev.x_pin ? kp : kn)<<<grid, MergeCfg<T, M::CAP>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-        k_spmv_csr_merge_fixup<T, ROLE><<<merge_fixup_grid(A), kThreads, 0, s>>>(A->dev, A->d_state, grid);
-        return;
-    }
-    if constexpr (IsComplex<T>::value) {               // BSR3 = SU(3) blocks: complex only
-        if (A->format == FMT_BSR3 && A->kernel == KERNEL_BSR_TMA) {
-            typedef BsrTile<T> B;
-            // the second BiCGStab-M SpMV carries five fp64 accumulators: one CTA per SM less keeps it from spilling
-            constexpr int CPS = B::CPS - (ROLE == ROLE_B2 ? MSOLVE_BSR_CPS_B2_LESS : 0);
-            auto k = k_spmv_bsr3_tma<T, B::TB, B::STAGES, CPS, ROLE>;
-            const int smem = BsrTmaCfg<T, B::TB>::smem_bytes(B::STAGES);
-            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-            const int grid = std::max(1, std::min(A->num_sms * CPS, A->dev.aux_count));
-            k<<<grid, BsrTmaCfg<T, B::TB>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-            return;
-        }
-        // default: not for the second BiCGStab-M SpMV, whose five accumulators and two extra operands spill at 255
-        // registers (config3x: spmv2_dots 0.278 ms all-TMA, 0.320 ms hybrid)
-        if ((g_lattice_kernel == 3 || (g_lattice_kernel == 0 && ROLE != ROLE_B2 && (sizeof(T) == 16 ? MSOLVE_LAT_HYB : MSOLVE_LAT_HYB_F))) && A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
-            constexpr int HW = sizeof(T) == 16 ? MSOLVE_LATH_W : MSOLVE_LATH_W_F;
-            constexpr int HS = sizeof(T) == 16 ? MSOLVE_LATH_STAGES : MSOLVE_LATH_STAGES_F;
-            auto k = k_spmv_lat_hyb<T, HW, HS, ROLE>;
-            const int smem = LatHybCfg<T, HW>::smem_bytes(HS);
-            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-            const int grid = std::max(1, std::min(A->num_sms, A->dev.aux_count));
-            k<<<grid, LatHybCfg<T, HW>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-            return;
-        }
-        if ((g_lattice_kernel == 2 || (g_lattice_kernel == 0 && LatWarpTile<T>::USE)) && A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
-            typedef LatWarpTile<T> L;
-            auto k = k_spmv_lat_warp<T, L::W, MSOLVE_LATW_PW, L::STAGES, ROLE>;
-            const int smem = LatWarpCfg<T, L::W, MSOLVE_LATW_PW>::smem_bytes(L::STAGES);
-            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-            const int grid = std::max(1, std::min(A->num_sms, A->dev.aux_count));
-            k<<<grid, LatWarpCfg<T, L::W, MSOLVE_LATW_PW>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-            return;
-        }
-        if (A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
-            typedef LatTile<T> L;
-            auto k = k_spmv_lat_tma<T, L::NS, L::STAGES, L::CPS, ROLE>;
-            const int smem = LatCfg<T, L::NS>::smem_bytes(L::STAGES);
-            static thread_local bool attr_set = false;   // per <T, ROLE> instantiation
-            if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-            const int grid = std::max(1, std::min(A->num_sms * L::CPS, A->dev.aux_count));
-            k<<<grid, LatCfg<T, L::NS>::kThreadsTotal, smem, s>>>(A->dev, A->d_state);
-            return;
-        }
-        if (A->format == FMT_LATTICE) {
-            auto k = k_spmv_lat_rows<T, ROLE>;
-            k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
-            return;
-        }
-        if (A->format == FMT_BSR3) {
-            auto k = k_spmv_bsr3_rows<T, ROLE>;
-            k<<<grid_for(A, k, A->dev.n, kThreads), kThreads, 0, s>>>(A->dev, A->d_state);
-            return;
-        }
-    }
-#define VEC_CASE(L)                                                                                     \
-    case L: {                                                                                           \
-        auto k = A->dev.x_pin ? k_spmv_csr_vector<T, L, ROLE, true> : k_spmv_csr_vector<T, L, ROLE, false>; \
-        k<<<grid_for(A, k, A->dev.n, kThreads / L), kThreads, 0, s>>>(A->dev, A->d_state);              \
-        break;                                                                                          \
-    }
-    switch (A->lanes) {
-        VEC_CASE(2) VEC_CASE(4) VEC_CASE(8) VEC_CASE(16) VEC_CASE(32)
-        default: break;
-    }
-#undef VEC_CASE
-}
-
-template <int ROLE>
-static void launch_spmv(const msolve_matrix* A, cudaStream_t s) {
-    switch (A->dtype) {
-        case MSOLVE_C128: launch_spmv_t<double2, ROLE>(A, s); break;
-        case MSOLVE_C64:  launch_spmv_t<float2, ROLE>(A, s); break;
-        case MSOLVE_F64:  launch_spmv_t<double, ROLE>(A, s); break;
-        default:          launch_spmv_t<float, ROLE>(A, s); break;
-    }
-}
-
-// element-wise kernels: 16 bytes (1, 2 or 4 elements) per access when the length allows it
-static bool vec16(const msolve_matrix* A) { return A->dev.n % (long long)(16 / elem_bytes(A->dtype)) == 0; }
-
-#define DISPATCH_VEC(A, KERNEL, ...)                                                       \
-    do {                                                                                   \
-        const bool v16_ = vec16(A);                                                        \
-        switch ((A)->dtype) {                                                              \
-            case MSOLVE_C128: KERNEL(double2, 1, __VA_ARGS__); break;                      \
-            case MSOLVE_C64: if (v16_) { KERNEL(float2, 2, __VA_ARGS__); } else { KERNEL(float2, 1, __VA_ARGS__); } break; \
-            case MSOLVE_F64: if (v16_) { KERNEL(double, 2, __VA_ARGS__); } else { KERNEL(double, 1, __VA_ARGS__); } break; \
-            default:         if (v16_) { KERNEL(float, 4, __VA_ARGS__); } else { KERNEL(float, 1, __VA_ARGS__); } break;   \
-        }                                                                                  \
-    } while (0)
-
-#ifndef MSOLVE_UNROLL_CGM
-#define MSOLVE_UNROLL_CGM 4
-#endif
-constexpr int kUnrollCgm = MSOLVE_UNROLL_CGM;
-#ifndef MSOLVE_UNROLL_BI
-#define MSOLVE_UNROLL_BI 4
-#endif
-constexpr int kUnrollBi = MSOLVE_UNROLL_BI;
-
-#define L_INIT(T, V, A, s) { auto k = k_init_vectors<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
-#define L_PUPD(T, V, A, s) { auto k = k_cgm_pupdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
-#ifndef MSOLVE_UPD_STAGES
-#define MSOLVE_UPD_STAGES 6
-#define MSOLVE_UPD_LAG 2
-#endif
-template <typename T>
-static void launch_cgm_update_tma(const msolve_matrix* A, cudaStream_t s) {
-    typedef UpdTmaCfg<T> U;
-    auto k = k_cgm_update_tma<T, MSOLVE_UPD_STAGES, MSOLVE_UPD_LAG>;
-    const int smem = U::smem_bytes(MSOLVE_UPD_STAGES);
-    static thread_local bool attr_set = false;   // per <T> instantiation
-    if (!attr_set) { cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, smem); attr_set = true; }
-    const long long ntiles = (A->dev.n / U::VEC + U::kTile - 1) / U::kTile;
-    const int grid = (int)std::max(1ll, std::min<long long>(A->num_sms, ntiles));
-    k<<<grid, U::kThreadsTotal, smem, s>>>(A->d_state);
-}
-#define L_CUPD(T, V, A, s) {                                                                            \
-    if (V * sizeof(T) == 16 && g_update_kernel == 1) launch_cgm_update_tma<T>(A, s);                      \
-    else { auto k = k_cgm_update<T, V, kUnrollCgm>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); } }
-#define L_SUPD(T, V, A, s) { auto k = k_bi_supdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
-#define L_BUPD(T, V, A, s) { auto k = k_bi_update<T, V, kUnrollBi>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
 
 static const char* kCgmNames[] = {"cgm_pupdate", "spmv_dot", "cgm_scal1", "cgm_update", "cgm_scal2"};
 static const char* kBiNames[] = {"spmv1_dot", "bi_scal1", "bi_supdate", "spmv2_dots", "bi_scal2", "bi_update", "bi_scal3"};
@@ -428,47 +88,30 @@ static int kernels_per_iter(int alg) { return alg == MSOLVE_ALG_CGM ? 5 : 7; }
 // kernel launches per iteration body: the merge-path SpMV is two launches (tiles + carry fix-up)
 static int launches_per_iter(const msolve_matrix* A, int alg) {
     const int spmvs = alg == MSOLVE_ALG_CGM ? 1 : 2;
-    return kernels_per_iter(alg) + (A->kernel == KERNEL_MERGE ? spmvs : 0);
+    return kernels_per_iter(alg) + (spmv_launches(A) - 1) * spmvs;
 }
 
 // One kernel of the iteration body.  Used for graph capture, and one-by-one for profiling.
-static void launch_body_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s,
-                               cudaGraphConditionalHandle cond, int use_cond) {
-    SolveState* st = A->d_state;
-    if (alg == MSOLVE_ALG_CGM) {
-        switch (j) {
-            case 0: DISPATCH_VEC(A, L_PUPD, A, s); break;
-            case 1: launch_spmv<ROLE_CG>(A, s); break;
-            case 2: k_cgm_scal1<<<1, kThreads, 0, s>>>(st); break;
-            case 3: DISPATCH_VEC(A, L_CUPD, A, s); break;
-            case 4: k_cgm_scal2<<<1, kThreads, 0, s>>>(st, cond, use_cond); break;
-        }
-    } else {
-        switch (j) {
-            case 0: launch_spmv<ROLE_B1>(A, s); break;
-            case 1: k_bi_scal1<<<1, kThreads, 0, s>>>(st); break;
-            case 2: DISPATCH_VEC(A, L_SUPD, A, s); break;
-            case 3: launch_spmv<ROLE_B2>(A, s); break;
-            case 4: k_bi_scal2<<<1, kThreads, 0, s>>>(st); break;
-            case 5: DISPATCH_VEC(A, L_BUPD, A, s); break;
-            case 6: k_bi_scal3<<<1, kThreads, 0, s>>>(st, cond, use_cond); break;
-        }
-    }
-}
-
-static void launch_init(const msolve_matrix* A, cudaStream_t s) {
-    DISPATCH_VEC(A, L_INIT, A, s);
-    k_init_state<<<1, kThreads, 0, s>>>(A->d_state);
+static int launch_body_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s,
+                              cudaGraphConditionalHandle cond, int use_cond) {
+    if (alg == MSOLVE_ALG_CGM && j == 1) return launch_spmv<ROLE_CG>(A, s);
+    if (alg == MSOLVE_ALG_BICGSTABM && j == 0) return launch_spmv<ROLE_B1>(A, s);
+    if (alg == MSOLVE_ALG_BICGSTABM && j == 3) return launch_spmv<ROLE_B2>(A, s);
+    return launch_vec_kernel(A, alg, j, s, cond, use_cond);
 }
 
 // ------------------------------------------------------------------------------------- graph
-static int build_graph(msolve_matrix* A, int alg, int mode) {
+static int build_graph(msolve_matrix* A, int alg) {
     LoopGraph& g = A->graphs[alg];
-    if (g.exec && g.mode == mode) return MSOLVE_OK;
+    const int key = A->opt.graph_key();
+    const SolveHeader& hh = A->h_stage->h;
+    const bool same_x = !A->opt.x_window || (g.xptr == hh.p && g.xptr2 == hh.s);
+    if (g.exec && g.key == key && same_x) return MSOLVE_OK;
     if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
     if (g.graph) { cudaGraphDestroy(g.graph); g.graph = nullptr; }
     const int nk = kernels_per_iter(alg);
-    if ((mode & 1) == 0) {
+    int lrc = MSOLVE_OK;
+    if (A->opt.loop_mode == 0) {
         CU(cudaGraphCreate(&g.graph, 0));
         cudaGraphConditionalHandle cond;
         CU(cudaGraphConditionalHandleCreate(&cond, g.graph, 1, cudaGraphCondAssignDefault));
@@ -481,21 +124,23 @@ static int build_graph(msolve_matrix* A, int alg, int mode) {
         CU(cudaGraphAddNode(&node, g.graph, nullptr, 0, &np));
         cudaGraph_t body = np.conditional.phGraph_out[0];
         CU(cudaStreamBeginCaptureToGraph(A->capture_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
-        for (int j = 0; j < nk; ++j) launch_body_kernel(A, alg, j, A->capture_stream, cond, 1);
+        for (int j = 0; j < nk && lrc == MSOLVE_OK; ++j) lrc = launch_body_kernel(A, alg, j, A->capture_stream, cond, 1);
         cudaError_t le = cudaGetLastError();
         cudaGraph_t dummy = nullptr;
         CU(cudaStreamEndCapture(A->capture_stream, &dummy));
+        if (lrc != MSOLVE_OK) return lrc;
         if (le != cudaSuccess) return fail(MSOLVE_ECUDA, "kernel launch during capture failed: %s", cudaGetErrorString(le));
     } else {
         CU(cudaStreamBeginCapture(A->capture_stream, cudaStreamCaptureModeThreadLocal));
-        for (int c = 0; c < kChunk; ++c)
-            for (int j = 0; j < nk; ++j) launch_body_kernel(A, alg, j, A->capture_stream, 0, 0);
+        for (int c = 0; c < kChunk && lrc == MSOLVE_OK; ++c)
+            for (int j = 0; j < nk && lrc == MSOLVE_OK; ++j) lrc = launch_body_kernel(A, alg, j, A->capture_stream, 0, 0);
         cudaError_t le = cudaGetLastError();
         CU(cudaStreamEndCapture(A->capture_stream, &g.graph));
+        if (lrc != MSOLVE_OK) return lrc;
         if (le != cudaSuccess) return fail(MSOLVE_ECUDA, "kernel launch during capture failed: %s", cudaGetErrorString(le));
     }
     CU(cudaGraphInstantiate(&g.exec, g.graph, 0));
-    g.mode = mode;
+    g.key = key; g.xptr = hh.p; g.xptr2 = hh.s;
     return MSOLVE_OK;
 }
 
@@ -542,7 +187,6 @@ static int build_bsr_tiles(msolve_matrix* A) {
     return MSOLVE_OK;
 }
 
-static bool aligned16(const void* p) { return ((uintptr_t)p & 15u) == 0; }
 
 // Merge-path partition (spmv_merge.cuh): the n + nnz merge items (row ends, non-zeros) are cut
 // every kDiag items.  Split point on diagonal d: i = number of row ends consumed, found by binary
@@ -563,9 +207,6 @@ static int build_merge_tiles(msolve_matrix* A, int flags, const std::vector<int3
     if (maxlen * n == nnz) {   // constant row length (stencils, lattices): lanes by the BYTES of a row (measured,
         const long long rb = maxlen * (long long)elem_bytes(A->dtype);   // config 4 CSR c64: 4 lanes 0.59 ms, 8 lanes 0.75 ms)
         A->lanes = rb > 768 ? 32 : rb > 320 ? 8 : rb > 96 ? 4 : 2;
-#ifdef MSOLVE_VEC_LANES
-        A->lanes = MSOLVE_VEC_LANES;
-#endif
     }
     // TMA-staged vector-CSR (spmv_csr_tile.cuh): every row fits LANES * U non-zeros, LANES <= 16.
     // AUTO takes it whenever the rows allow it: it is the faster CSR kernel on every workload
@@ -649,9 +290,6 @@ extern "C" int msolve_create_csr(msolve_matrix** out, int64_t n, int64_t nnz, co
     A->dev.x_pin = elem_bytes(dtype) <= 8 && (size_t)n * elem_bytes(dtype) <= (size_t)48 << 20;
     const double mean = n > 0 ? (double)nnz / (double)n : 0.0;
     A->lanes = mean > 48 ? 32 : mean > 20 ? 8 : mean > 6 ? 4 : 2;
-#ifdef MSOLVE_VEC_LANES
-    A->lanes = MSOLVE_VEC_LANES;
-#endif
     int rc = create_common(out, A, (cudaStream_t)stream);
     if (rc == MSOLVE_OK && flags != MSOLVE_SPMV_VECTOR && n > 0) {
         const bool force = flags != MSOLVE_SPMV_AUTO;
@@ -676,7 +314,7 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     if (!d_browptr || (nblocks > 0 && (!d_bcolidx || !d_blocks))) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: NULL array");
     if (!complex_dtype(dtype)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: dtype must be MSOLVE_C64 or MSOLVE_C128 (SU(3) blocks are complex)");
     if (flags != MSOLVE_SPMV_AUTO && flags != MSOLVE_SPMV_VECTOR) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: bad flags");
-    if (!aligned16(d_blocks)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: misaligned array");
+    if (!aligned16(d_blocks) || ((uintptr_t)d_bcolidx & 3u) || ((uintptr_t)d_browptr & 3u)) return fail(MSOLVE_EINVAL, "msolve_create_bsr3: misaligned array");
     msolve_matrix* A = new (std::nothrow) msolve_matrix();
     if (!A) return fail(MSOLVE_ENOMEM, "out of host memory");
     A->format = FMT_BSR3;
@@ -685,7 +323,9 @@ extern "C" int msolve_create_bsr3(msolve_matrix** out, int64_t nbrows, int64_t n
     A->dev.n = 3 * nbrows; A->dev.nbrows = nbrows; A->dev.nnz = nblocks; A->dev.aux = nullptr; A->dev.aux_count = 0; A->dev.carry = nullptr;
     A->kernel = KERNEL_BSR_ROWS;
     int rc = create_common(out, A, (cudaStream_t)stream);
-    if (rc == MSOLVE_OK && flags == MSOLVE_SPMV_AUTO && nbrows > 0) rc = build_bsr_tiles(A);
+    // the TMA-staged kernel bulk-copies the block-column indices: they must be 16-byte aligned too (a torch
+    // slice may not be); otherwise the row kernel
+    if (rc == MSOLVE_OK && flags == MSOLVE_SPMV_AUTO && nbrows > 0 && aligned16(d_bcolidx)) rc = build_bsr_tiles(A);
     if (rc != MSOLVE_OK) { msolve_destroy(A); *out = nullptr; }
     return rc;
 }
@@ -758,11 +398,36 @@ extern "C" void msolve_destroy(msolve_matrix* A) {
 
 extern "C" const char* msolve_last_error(void) { return g_err; }
 
-extern "C" int msolve_config(int key, int value) {
-    if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { g_loop_mode = value; return MSOLVE_OK; }
-    if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { g_update_kernel = value; return MSOLVE_OK; }
-    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { g_lattice_kernel = value; return MSOLVE_OK; }
+extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
+    if (!A) return fail(MSOLVE_EINVAL, "msolve_config: A is NULL");
+    if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { A->opt.loop_mode = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { A->opt.update_kernel = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { A->opt.lattice_kernel = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_STOP_RULE && (value == 0 || value == 1)) { A->opt.stop_rule = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_X_WINDOW && (value == 0 || value == 1)) {
+        if (value == 1) {
+            if (A->format != FMT_CSR || A->kernel != KERNEL_VECTOR) return fail(MSOLVE_EINVAL, "msolve_config: MSOLVE_CFG_X_WINDOW applies to the vector-CSR kernel");
+            int dev_max = 0, win_max = 0;
+            CU(cudaDeviceGetAttribute(&dev_max, cudaDevAttrMaxPersistingL2CacheSize, A->device));
+            CU(cudaDeviceGetAttribute(&win_max, cudaDevAttrMaxAccessPolicyWindowSize, A->device));
+            if (dev_max <= 0 || win_max <= 0) return fail(MSOLVE_EINVAL, "msolve_config: the device has no persisting L2");
+            const size_t want = std::min<size_t>((size_t)dev_max, (size_t)A->dev.n * elem_bytes(A->dtype));
+            CU(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want));     // device-wide set-aside
+            A->l2_persist_bytes = want;
+            A->l2_window_max = (size_t)win_max;
+        }
+        A->opt.x_window = value;
+        return MSOLVE_OK;
+    }
     return fail(MSOLVE_EINVAL, "msolve_config: bad key/value");
+}
+
+extern "C" int msolve_set_history(msolve_matrix* A, double* d_hist, int cap_rows) {
+    if (!A) return fail(MSOLVE_EINVAL, "msolve_set_history: A is NULL");
+    if (cap_rows < 0 || (cap_rows > 0 && !d_hist) || ((uintptr_t)d_hist & 7u)) return fail(MSOLVE_EINVAL, "msolve_set_history: bad buffer");
+    A->d_hist = cap_rows > 0 ? d_hist : nullptr;
+    A->hist_cap = cap_rows > 0 ? cap_rows : 0;
+    return MSOLVE_OK;
 }
 
 extern "C" int64_t msolve_last_launch_count(const msolve_matrix* A) { return A ? A->last_launches : 0; }
@@ -803,6 +468,7 @@ static int fill_header(const msolve_matrix* A, int alg, const void* d_b, const d
     h->n = A->dev.n;
     h->pk_stride = pk_stride_elems(A);
     h->tol = tol; h->S = S; h->max_iter = max_iter; h->force_all = force_all;
+    h->stop_rule = A->opt.stop_rule; h->hist = A->d_hist; h->hist_cap = A->hist_cap;
     for (int k = 0; k < S; ++k) h->sigma[k] = h_shifts[k];
     return MSOLVE_OK;
 }
@@ -818,10 +484,13 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
                       int max_iter, void* d_x, void* ws, size_t ws_bytes, int* h_iterations, int* h_conv_iter,
                       double* h_relres, void* stream_) {
     msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
+    if (!A) return fail(MSOLVE_EINVAL, "solve: A is NULL");
+    int rc = check_device(A, "solve");
+    if (rc != MSOLVE_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
     SolveHeader* hh = &A->h_stage->h;
     SolveResult* hr = &A->h_stage->res;
-    int rc = fill_header(A, alg, d_b, h_shifts, S, tol, max_iter, d_x, ws, ws_bytes, 0, hh);
+    rc = fill_header(A, alg, d_b, h_shifts, S, tol, max_iter, d_x, ws, ws_bytes, 0, hh);
     if (rc != MSOLVE_OK) return rc;
     fill_result_init(hr, S);
     const size_t xbytes = (size_t)S * (size_t)A->dev.n * elem_bytes(A->dtype);
@@ -833,14 +502,14 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
         A->last_launches = 0;
         return A->dev.n == 0 ? MSOLVE_OK : MSOLVE_MAXITER;
     }
-    const int mode = g_loop_mode;
-    rc = build_graph(A, alg, mode | (g_update_kernel << 1) | (g_lattice_kernel << 2));
+    const int mode = A->opt.loop_mode;
+    rc = build_graph(A, alg);
     if (rc != MSOLVE_OK) return rc;
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
-    launch_init(A, stream);
+    rc = launch_init(A, stream);
+    if (rc != MSOLVE_OK) return rc;
     CU(cudaGetLastError());
     int64_t launches = 2;
-    const int nk = kernels_per_iter(alg);
     if (mode == 0) {
         CU(cudaGraphLaunch(A->graphs[alg].exec, stream));
         CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
@@ -855,7 +524,9 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
             if (hr->done) break;
         }
     }
-    if (hr->zero_rhs) {
+    // x_k = 0 is substituted in registers until the first update has written it: b = 0 and a breakdown in the
+    // first loop body (before any update) leave d_x untouched, so it is zeroed here (the iterate IS x_k = 0)
+    if (hr->zero_rhs || (hr->status == MSOLVE_BREAKDOWN && hr->n_iter == 0)) {
         CU(cudaMemsetAsync(d_x, 0, xbytes, stream));
         CU(cudaStreamSynchronize(stream));
     }
@@ -973,13 +644,16 @@ extern "C" int msolve_solve_host_batch(const msolve_matrix* A, int algorithm, in
 extern "C" int msolve_spmv(const msolve_matrix* Ac, const void* d_x, void* d_y, double* h_dot, void* stream_) {
     msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
     if (!A || !d_x || !d_y) return fail(MSOLVE_EINVAL, "msolve_spmv: NULL argument");
+    if (!aligned16(d_x) || !aligned16(d_y)) return fail(MSOLVE_EINVAL, "msolve_spmv: d_x / d_y must be 16-byte aligned");
+    int rc = check_device(A, "msolve_spmv");
+    if (rc != MSOLVE_OK) return rc;
     cudaStream_t stream = (cudaStream_t)stream_;
     SolveHeader* hh = &A->h_stage->h;
     memset(hh, 0, sizeof(*hh));
     hh->sp_x = d_x; hh->sp_y = d_y; hh->sp_u = d_x; hh->n = A->dev.n; hh->S = 1;
     fill_result_init(&A->h_stage->res, 1);
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
-    if (A->dev.n > 0) launch_spmv<ROLE_GEN>(A, stream);
+    if (A->dev.n > 0 && (rc = launch_spmv<ROLE_GEN>(A, stream)) != MSOLVE_OK) return rc;
     CU(cudaGetLastError());
     if (h_dot) {
         h_dot[0] = h_dot[1] = 0.0;
@@ -1004,14 +678,17 @@ extern "C" int msolve_profile_iteration(const msolve_matrix* Ac, int alg, const 
                                         int S, int iters, void* d_x, void* ws, size_t ws_bytes, float* h_ms,
                                         int* h_launches, void* stream_) {
     msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
+    if (!A) return fail(MSOLVE_EINVAL, "profile: A is NULL");
     if (alg != MSOLVE_ALG_CGM && alg != MSOLVE_ALG_BICGSTABM) return fail(MSOLVE_EINVAL, "profile: bad algorithm");
     if (iters < 1 || !h_ms) return fail(MSOLVE_EINVAL, "profile: bad iters / h_ms");
     cudaStream_t stream = (cudaStream_t)stream_;
-    int rc = fill_header(A, alg, d_b, h_shifts, S, 0.0, iters + 1, d_x, ws, ws_bytes, 1, &A->h_stage->h);
+    int rc = check_device(A, "profile");
+    if (rc != MSOLVE_OK) return rc;
+    rc = fill_header(A, alg, d_b, h_shifts, S, 0.0, iters + 1, d_x, ws, ws_bytes, 1, &A->h_stage->h);
     if (rc != MSOLVE_OK) return rc;
     fill_result_init(&A->h_stage->res, S);
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
-    launch_init(A, stream);
+    if ((rc = launch_init(A, stream)) != MSOLVE_OK) return rc;
     const int nk = kernels_per_iter(alg);
     cudaEvent_t ev[9];
     for (int j = 0; j <= nk; ++j) CU(cudaEventCreate(&ev[j]));
@@ -1020,7 +697,7 @@ extern "C" int msolve_profile_iteration(const msolve_matrix* Ac, int alg, const 
     for (int it = 0; it <= iters; ++it) {
         for (int j = 0; j < nk; ++j) {
             CU(cudaEventRecord(ev[j], stream));
-            launch_body_kernel(A, alg, j, stream, 0, 0);
+            if ((rc = launch_body_kernel(A, alg, j, stream, 0, 0)) != MSOLVE_OK) return rc;
         }
         CU(cudaEventRecord(ev[nk], stream));
         CU(cudaStreamSynchronize(stream));

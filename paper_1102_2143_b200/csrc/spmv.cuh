@@ -17,8 +17,6 @@
 
 namespace msolve {
 
-enum { ROLE_CG = 0, ROLE_B1 = 1, ROLE_B2 = 2, ROLE_GEN = 3 };
-
 template <int ROLE> struct RoleAcc { static constexpr int value = ROLE == ROLE_CG ? 1 : (ROLE == ROLE_B2 ? 5 : 2); };
 
 template <typename C, int ROLE>
@@ -176,17 +174,8 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(policy) : "memory");
 }
-#ifndef MSOLVE_X_HINT
-#define MSOLVE_X_HINT 0
-#endif
-__device__ __forceinline__ double2 ld_hint(const double2* p, uint64_t policy) {
-    if (!MSOLVE_X_HINT) return __ldg(p);
-    double2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(r.x), "=d"(r.y) : "l"(p), "l"(policy)); return r;
-}
-__device__ __forceinline__ float2 ld_hint(const float2* p, uint64_t policy) {
-    if (!MSOLVE_X_HINT) return __ldg(p);
-    float2 r; asm volatile("ld.global.nc.L2::cache_hint.v2.f32 {%0,%1}, [%2], %3;" : "=f"(r.x), "=f"(r.y) : "l"(p), "l"(policy)); return r;
-}
+// x gathers of the BSR3 kernel: plain read-only loads (hinted 16-byte loads are slower on B200, profiles/r01_sweeps.md)
+template <typename C> __device__ __forceinline__ C ld_hint(const C* p, uint64_t) { return __ldg(p); }
 
 // ------------------------------------------------------------------------------------------
 // BSR3, TMA-staged (the SU(3) lattice kernel).  Persistent CTAs, CPS of them per SM.  A producer

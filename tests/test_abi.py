@@ -46,7 +46,17 @@ def test_validation_without_gpu(lib):
     assert b"ndim" in lib.msolve_last_error()
     assert lib.msolve_create_lattice_su3(ctypes.byref(h), 4, ext, None, 8.0, 1.0, 1.0, 1, 0, None) == -1
     assert lib.msolve_workspace_bytes(None, 4, 0) == 0
-    assert lib.msolve_config(99, 0) == -1
+    assert lib.msolve_config(None, 0, 0) == -1
+    assert lib.msolve_set_history(None, None, 0) == -1
+    # the solver entry points and the profiler check the handle before anything else
+    sh = (ctypes.c_double * 1)(0.0)
+    for fn in (lib.msolve_cgm, lib.msolve_bicgstabm):
+        assert fn(None, None, sh, 1, 1e-10, 10, None, None, 0, None, None, None, None) == -1
+        assert b"A is NULL" in lib.msolve_last_error()
+    ms_buf = (ctypes.c_float * 8)()
+    assert lib.msolve_profile_iteration(None, 0, None, sh, 1, 1, None, None, 0, ms_buf, None, None) == -1
+    assert lib.msolve_solve_host(None, 0, None, sh, 1, 1e-10, 10, None, None, None, None, None) == -1
+    assert lib.msolve_spmv(None, None, None, None, None) == -1
     assert lib.msolve_last_launch_count(None) == 0
     assert lib.msolve_kernel_name(0, 1) == b"spmv_dot"
     lib.msolve_destroy(None)  # no-op

@@ -5,6 +5,7 @@ import pytest
 
 import oracle
 from paper_1102_2143_b200 import workloads as W
+import test_gpu_parity
 from test_gpu_parity import check_parity, dev, gpu_solve, make_matrix, ms, oracle_solve  # noqa: F401
 
 pytestmark = pytest.mark.gpu
@@ -29,9 +30,9 @@ EXTENTS = [(4, 4, 6, 5),        # 8 x0-rows per tile
 @pytest.fixture(params=[1, 2, 3], ids=["termsite", "warptile", "hybrid"])
 def tile_kernel(request, ms):
     """Run with each of the three tile kernels forced (default: the faster one per element type)."""
-    ms.msolve_config(ms.MSOLVE_CFG_LATTICE_KERNEL, request.param)
+    test_gpu_parity.FORCED_CFG[ms.MSOLVE_CFG_LATTICE_KERNEL] = request.param
     yield request.param
-    ms.msolve_config(ms.MSOLVE_CFG_LATTICE_KERNEL, 0)
+    test_gpu_parity.FORCED_CFG.clear()
 
 
 @pytest.mark.parametrize("dtype", [np.complex128, np.complex64])

@@ -14,6 +14,7 @@ pytestmark = pytest.mark.gpu
 
 REL = {np.complex128: 1e-9, np.complex64: 1e-4}
 TORCH = {np.complex128: torch.complex128, np.complex64: torch.complex64}
+MAXABS_C = 4.0
 
 
 @pytest.fixture(scope="module")
@@ -28,7 +29,17 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def make_matrix(ms, w, dtype, fmt, flags=0):
+FORCED_CFG = {}     # msolve_config options applied to every handle make_matrix creates (set by fixtures)
+
+
+def make_matrix(ms, w, dtype, fmt, flags=0, cfg=None):
+    A = _create(ms, w, dtype, fmt, flags)
+    for key, value in list(FORCED_CFG.items()) + list((cfg or {}).items()):
+        ms.msolve_config(A, key, value)
+    return A
+
+
+def _create(ms, w, dtype, fmt, flags):
     if fmt == "bsr3rows":   # the simple one-thread-per-row BSR3 kernel instead of the TMA-staged one
         return ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
     if fmt in ("lat", "latrows"):   # matrix-free operator from the link field (TMA tile kernel / row kernel)
@@ -46,8 +57,8 @@ def make_matrix(ms, w, dtype, fmt, flags=0):
     return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), flags)
 
 
-def gpu_solve(ms, w, dtype, fmt, tol=None, max_iter=None, shifts=None, flags=0):
-    A = make_matrix(ms, w, dtype, fmt, flags)
+def gpu_solve(ms, w, dtype, fmt, tol=None, max_iter=None, shifts=None, flags=0, cfg=None):
+    A = make_matrix(ms, w, dtype, fmt, flags, cfg)
     fn = ms.msolve_cgm if w.algorithm == "cgm" else ms.msolve_bicgstabm
     res = fn(A, dev(w.b.astype(dtype)), w.shifts if shifts is None else shifts,
              w.tol if tol is None else tol, w.max_iter if max_iter is None else max_iter)
@@ -71,8 +82,12 @@ def check_parity(w, dtype, g, o, tol):
     assert np.all(np.abs(conv - o.conv_iter) <= 2)
     A = sp.csr_matrix((w.val, w.colidx, w.rowptr), shape=(w.n, w.n))
     for k, s in enumerate(w.shifts):
-        d = np.linalg.norm(x[k].astype(np.complex128) - o.x[k].astype(np.complex128)) / np.linalg.norm(o.x[k])
+        diff = x[k].astype(np.complex128) - o.x[k].astype(np.complex128)
+        d = np.linalg.norm(diff) / np.linalg.norm(o.x[k])
         assert d <= REL[dtype], (k, d)
+        # element by element: no single entry may be off by more than MAXABS_C bars of the largest entry (a norm
+        # alone lets one wrong element in millions through at the complex64 bar)
+        assert np.abs(diff).max() <= MAXABS_C * REL[dtype] * np.abs(o.x[k]).max(), (k, np.abs(diff).max())
         xk = x[k].astype(np.complex128)
         true = np.linalg.norm(w.b - (A @ xk + s * xk)) / np.linalg.norm(w.b)
         assert true <= 10.0 * tol, (k, true)
@@ -188,11 +203,7 @@ def test_update_kernels_agree(ms, extents, dtype, tol):
     o = oracle_solve(w, dtype, tol=tol)
     xs = []
     for which in (0, 1):
-        ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, which)
-        try:
-            g = gpu_solve(ms, w, dtype, "bsr3", tol=tol)
-        finally:
-            ms.msolve_config(ms.MSOLVE_CFG_UPDATE_KERNEL, 0)
+        g = gpu_solve(ms, w, dtype, "bsr3", tol=tol, cfg={ms.MSOLVE_CFG_UPDATE_KERNEL: which})
         check_parity(w, dtype, g, o, tol)
         xs.append(g[2])
     d = np.linalg.norm(xs[0].astype(np.complex128) - xs[1]) / np.linalg.norm(xs[1])
@@ -367,23 +378,115 @@ def test_max_shifts_and_too_many(ms):
 
 
 def test_breakdown_reported(ms):
+    # indefinite A: <p,Ap> < 0 in the first loop body (R16).  The iterate at that point is x_k = 0, which is what
+    # the oracle returns; d_x must be fully overwritten with it (include/msolve.h), not left as the caller had it.
     n = 64
     rowptr = np.arange(n + 1, dtype=np.int32)
     colidx = np.arange(n, dtype=np.int32)
-    A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(-np.ones(n, dtype=np.complex128)))
-    res = ms.msolve_cgm(A, dev(W.unit_rhs(1, n)), [0.0], 1e-10, 10)
-    assert res.status == ms.MSOLVE_BREAKDOWN
+    val = -np.ones(n, dtype=np.complex128)
+    b = W.unit_rhs(1, n)
+    A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
+    x = torch.full((2, n), 7.0, dtype=torch.complex128, device="cuda")
+    res = ms.msolve_cgm(A, dev(b), [0.0, 0.5], 1e-10, 10, x=x)
+    o = oracle.cgm(rowptr, colidx, val, b, [0.0, 0.5], 1e-10, 10)
+    assert res.status == ms.MSOLVE_BREAKDOWN == o.status and res.iterations == o.iterations == 0
+    assert np.array_equal(res.x.cpu().numpy(), o.x) and not o.x.any()
+    ms.msolve_destroy(A)
+    # BiCGStab-M on A = c I (R17): s = r + beta q = 0 after the first half step, <t,t> = 0: breakdown, x = 0
+    val = np.full(n, 2.5, dtype=np.complex128)
+    A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
+    x.fill_(7.0)
+    res = ms.msolve_bicgstabm(A, dev(b), [0.0, 0.5], 1e-10, 10, x=x)
+    o = oracle.bicgstabm(rowptr, colidx, val, b, [0.0, 0.5], 1e-10, 10)
+    assert res.status == ms.MSOLVE_BREAKDOWN == o.status and res.iterations == o.iterations == 0
+    assert np.array_equal(res.x.cpu().numpy(), o.x) and not o.x.any()
+    ms.msolve_destroy(A)
+    # a breakdown AFTER the first update keeps the iterate reached so far (same as the oracle)
+    val = np.ones(n, dtype=np.complex128)
+    val[n // 2:] = -1.0                                   # indefinite, but <b,Ab> > 0 for this b
+    bb = np.zeros(n, dtype=np.complex128)
+    bb[: n // 2] = 1.0
+    bb[n // 2:] = 0.5
+    bb /= np.linalg.norm(bb)
+    A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
+    res = ms.msolve_cgm(A, dev(bb), [0.0], 1e-10, 10)
+    o = oracle.cgm(rowptr, colidx, val, bb, [0.0], 1e-10, 10)
+    assert res.status == o.status and res.iterations == o.iterations
+    if o.status == oracle.BREAKDOWN and o.iterations > 0:
+        assert np.linalg.norm(res.x.cpu().numpy() - o.x) <= 1e-12 * np.linalg.norm(o.x)
+    ms.msolve_destroy(A)
+
+
+# ------------------------------------------------------------------------------- stop rule, scalar history
+@pytest.mark.parametrize("alg", ["cgm", "bicgstabm"])
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+def test_stop_rule_base_matches_oracle(ms, alg, dtype, tol):
+    # MSOLVE_CFG_STOP_RULE = 1: Alg. 1 l.15 read literally: iterate until the UNSHIFTED residual is
+    # below tol, no shift is frozen before that.  Shifts without sigma = 0, so the two rules really differ.
+    w = W.config2(extents=(4, 6, 4, 6)) if alg == "cgm" else W.config3(extents=(4, 6, 4, 6))
+    shifts = np.array([0.7, 0.01, 0.15, 3.0])
+    g = gpu_solve(ms, w, dtype, "bsr3", tol=tol, shifts=shifts, cfg={ms.MSOLVE_CFG_STOP_RULE: 1})
+    ofn = oracle.cgm if alg == "cgm" else oracle.bicgstabm
+    o = ofn(w.rowptr, w.colidx, w.val.astype(dtype), w.b.astype(dtype), shifts, tol, w.max_iter, stop_rule=1)
+    o0 = ofn(w.rowptr, w.colidx, w.val.astype(dtype), w.b.astype(dtype), shifts, tol, w.max_iter, stop_rule=0)
+    assert o.iterations > o0.conv_iter.min()                    # the literal rule runs longer than the fastest shift
+    assert g[0] == o.status == oracle.OK and abs(g[1] - o.iterations) <= 2
+    assert np.all(g[3] == g[1]) and np.all(o.conv_iter == o.iterations)
+    for k in range(shifts.size):
+        diff = g[2][k].astype(np.complex128) - o.x[k]
+        assert np.linalg.norm(diff) <= REL[dtype] * np.linalg.norm(o.x[k]), k
+        assert np.abs(diff).max() <= MAXABS_C * REL[dtype] * np.abs(o.x[k]).max(), k
+    if g[1] == o.iterations:
+        assert np.allclose(g[4], o.relres, rtol=1e-6 if dtype == np.complex128 else 1e-2)
+
+
+HIST_RTOL = 1e-12
+
+
+@pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "bsr3"), ("c2", "csr"), ("c3", "bsr3"), ("c3", "csr")])
+def test_scalar_history_matches_oracle(ms, which, fmt):
+    # SURVEY 8(c) C6 "brute force": the scalars of Alg. 1 l.20-26 that the scalar kernels
+    # produce -- beta, alpha, R1 and zeta / beta_k / alpha_k (chi_k) of every shift, every iteration -- against
+    # the oracle's record of the same quantities, on configs 1, 2 and the 4^4 config 3.
+    w = {"c1": W.config1, "c2": W.config2, "c3": lambda: W.config3(extents=(4, 4, 4, 4))}[which]()
+    S = w.shifts.size
+    cols = 3 + 3 * S if w.algorithm == "cgm" else 8 + 6 * S
+    cap = 64
+    A = make_matrix(ms, w, np.complex128, fmt)
+    hist = torch.zeros((cap, cols), dtype=torch.float64, device="cuda")
+    ms.msolve_set_history(A, hist)
+    fn, ofn = (ms.msolve_cgm, oracle.cgm) if w.algorithm == "cgm" else (ms.msolve_bicgstabm, oracle.bicgstabm)
+    res = fn(A, dev(w.b), w.shifts, w.tol, w.max_iter)
+    o = ofn(w.rowptr, w.colidx, w.val, w.b, w.shifts, w.tol, w.max_iter, hist_cap=cap)
+    assert res.status == o.status == 0 and res.iterations == o.iterations <= cap
+    hg = hist.cpu().numpy()[: o.iterations]
+    assert not hist.cpu().numpy()[o.iterations:].any()              # nothing written past the last iteration
+    if w.algorithm == "cgm":
+        dev_rel = np.abs(hg - o.hist) / np.abs(o.hist)
+    else:                                                           # complex pairs: relative to the modulus
+        zg = np.concatenate([hg[:, :6].copy().view(np.complex128), hg[:, 8:].copy().view(np.complex128)], axis=1)
+        zo = np.concatenate([o.hist[:, :6].copy().view(np.complex128), o.hist[:, 8:].copy().view(np.complex128)], axis=1)
+        dev_rel = np.abs(zg - zo) / np.abs(zo)
+        assert np.all(np.abs(hg[:, 6] - o.hist[:, 6]) <= 1e-9 * o.hist[:, 6]) and not hg[:, 7].any()
+    print("history %s/%s: max relative deviation per iteration" % (which, fmt), dev_rel.max(axis=1))
+    assert dev_rel.max() <= HIST_RTOL * 10 ** (o.iterations / 8.0), dev_rel.max()
+    # switching it off: the next solve leaves the buffer alone
+    ms.msolve_set_history(A, None)
+    hist.zero_()
+    fn(A, dev(w.b), w.shifts, w.tol, w.max_iter)
+    assert not hist.any().item()
+    # a short buffer: rows beyond cap are dropped, the rest is the same
+    short = torch.zeros((3, cols), dtype=torch.float64, device="cuda")
+    ms.msolve_set_history(A, short)
+    fn(A, dev(w.b), w.shifts, w.tol, w.max_iter)
+    assert np.array_equal(short.cpu().numpy(), hg[:3])
     ms.msolve_destroy(A)
 
 
 def test_chunked_loop_mode_same_result(ms):
     w = W.config2(extents=(4, 4, 4, 4))
     a = gpu_solve(ms, w, np.complex128, "bsr3")
-    ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 1)
-    try:
-        b = gpu_solve(ms, w, np.complex128, "bsr3")
-    finally:
-        ms.msolve_config(ms.MSOLVE_CFG_LOOP_MODE, 0)
+    b = gpu_solve(ms, w, np.complex128, "bsr3", cfg={ms.MSOLVE_CFG_LOOP_MODE: 1})
     assert a[1] == b[1] and np.array_equal(a[2], b[2]) and np.array_equal(a[3], b[3])
 
 

@@ -356,3 +356,147 @@ def test_real_bicgstabm_dense_lu():
     for k, s in enumerate(w.shifts):
         xe = np.linalg.solve(A + s * np.eye(w.n), w.b)
         assert np.linalg.norm(res.x[k] - xe) / np.linalg.norm(xe) < 1e-12
+
+
+# ------------------------------------------------------------------ stop_rule = 1 (Alg. 1 l.15 read literally)
+def test_stop_rule_base_cgm(cfg1, cfg2_small):
+    # "while |r| > eps" on the UNSHIFTED system.  Pins: (a) the base Krylov sequence does not
+    # depend on the shifts, so the loop runs exactly as long as textbook CG on A (same R1 bitwise, same test);
+    # (b) with sigma = 0 among the shifts the default rule ends at the same iteration (zeta_0 = 1) with the
+    # same bits in x_0; (c) the other shifts are NOT frozen: they keep converging, so their true residual is
+    # no larger than under the default rule and every conv_iter equals the exit iteration.
+    # catches: testing |zeta_k| |r| instead of |r|, freezing shifts early, wrong exit bookkeeping.
+    for w in (cfg1, cfg2_small):
+        A = _A(w)
+        sig = np.array([0.37, 0.011, 2.0])                               # sigma = 0 NOT among them
+        st, it, _, rel = oracle.cg(w.rowptr, w.colidx, w.val, 0.0, w.b, w.tol, 500)
+        m1 = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig, w.tol, 500, stop_rule=1)
+        m0 = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig, w.tol, 500, stop_rule=0)
+        assert st == oracle.OK and m1.status == oracle.OK
+        assert m1.iterations == it and np.all(m1.conv_iter == it)
+        assert m0.iterations <= it and m0.conv_iter[2] < it              # under the default rule sigma = 2 stops early
+        for k, s in enumerate(sig):
+            assert abs(m1.relres[k] - abs(m1.zeta[k]) * rel) <= 1e-14 * m1.relres[k]   # reported: |zeta_k| ||r|| / ||b|| at exit
+            assert _true_relres(A, w.b, m1.x[k], s) <= _true_relres(A, w.b, m0.x[k], s) * (1 + 1e-6)
+            assert _true_relres(A, w.b, m1.x[k], s) <= w.tol
+        sig0 = np.array([0.0, 0.37, 2.0])                                # sigma = 0 among them
+        a = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig0, w.tol, 500, stop_rule=1)
+        b = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig0, w.tol, 500, stop_rule=0)
+        assert a.iterations == b.iterations == it and np.array_equal(a.x[0], b.x[0])
+        assert np.all(a.conv_iter == it) and b.conv_iter[2] < it
+        # max_iter reached first: MAXITER, nothing converged
+        c = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig0, w.tol, 3, stop_rule=1)
+        assert c.status == oracle.MAXITER and c.iterations == 3 and np.all(c.conv_iter == -1)
+
+
+def test_stop_rule_base_bicgstabm(cfg3_small):
+    # the same for BiCGStab-M against textbook BiCGStab on the unshifted matrix
+    w = cfg3_small
+    A = _A(w)
+    sig = np.array([0.3, 0.05, 1.5])
+    st, it, _, rel = oracle.bicgstab(w.rowptr, w.colidx, w.val, 0.0, w.b, w.tol, 500)
+    m1 = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, sig, w.tol, 500, stop_rule=1)
+    m0 = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, sig, w.tol, 500, stop_rule=0)
+    assert st == oracle.OK and m1.status == oracle.OK
+    assert m1.iterations == it and np.all(m1.conv_iter == it) and m0.iterations <= it
+    for k, s in enumerate(sig):
+        assert abs(m1.relres[k] - abs(m1.zeta[k]) * rel) <= 1e-9 * m1.relres[k]
+        assert _true_relres(A, w.b, m1.x[k], s) <= 10 * w.tol
+    a = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, np.array([0.0, 0.3]), w.tol, 500, stop_rule=1)
+    b = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, np.array([0.0, 0.3]), w.tol, 500, stop_rule=0)
+    assert a.iterations == b.iterations and np.array_equal(a.x[0], b.x[0])
+
+
+# ------------------------------------------------------------------ the per-iteration scalar history
+def _textbook_bicgstab_scalars(M, b, nit):
+    """van der Vorst's BiCGStab on the dense matrix M in numpy, shadow vector b: per iteration
+    (alpha, omega, beta, ||r||^2).  An independent restatement of the textbook, not of the oracle."""
+    r = b.copy(); p = b.copy(); rhat = b.copy()
+    rho = np.vdot(rhat, r)
+    out = []
+    for _ in range(nit):
+        v = M @ p
+        a = rho / np.vdot(rhat, v)
+        s = r - a * v
+        t = M @ s
+        om = np.vdot(t, s) / np.vdot(t, t)
+        r = s - om * t
+        rho_new = np.vdot(rhat, r)
+        bt = (rho_new / rho) * (a / om)
+        p = r + bt * (p - om * v)
+        rho = rho_new
+        out.append((a, om, bt, np.vdot(r, r).real, r.copy()))
+    return out
+
+
+def test_bicgstabm_history_against_textbook_and_true_residuals(cfg3_small):
+    # Base row = textbook BiCGStab on A: beta = -alpha, chi = omega, alpha' = textbook beta, |r'|^2.
+    # Per shift: beta_k = -(the BiCG step length of the system A + sigma_k I), which textbook BiCGStab on the
+    # shifted matrix recovers whatever its own omega is; chi_k and zeta_new through the shifted residual
+    # b - (A + sigma_k) x_k (numpy, from the iterate) whose norm must equal |zeta_k rho_k| ||r|| with
+    # rho_k = prod_j chi_k[j] / chi[j] (rho' = rho / (1 + chi sigma) = rho chi_k / chi).
+    # catches: a wrong zeta / beta_k / chi_k / rho recurrence, a wrong slot in the history row.
+    w = cfg3_small
+    A = _A(w)
+    M = A.toarray()
+    sig = np.array([0.0, 0.2, 1.0])
+    nit, S = 6, 3
+    m = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, sig, 0.0, nit, hist_cap=nit)
+    assert m.hist.shape == (nit, 8 + 6 * S)
+    base = _textbook_bicgstab_scalars(M, w.b, nit)
+    per_shift = [_textbook_bicgstab_scalars(M + s * np.eye(w.n), w.b, nit) for s in sig]
+    rho = np.ones(S, dtype=np.complex128)
+    for n in range(nit):
+        h = m.hist[n]
+        beta, chi, alpha_new = h[0] + 1j * h[1], h[2] + 1j * h[3], h[4] + 1j * h[5]
+        a, om, bt, rr, _ = base[n]
+        assert abs(beta + a) <= 1e-10 * abs(a) and abs(chi - om) <= 1e-10 * abs(om)
+        assert abs(alpha_new - bt) <= 1e-9 * abs(bt) and abs(h[6] - rr) <= 1e-9 * rr and h[7] == 0.0
+        zeta_new = h[8:8 + 2 * S].view(np.complex128)
+        beta_k = h[8 + 2 * S:8 + 4 * S].view(np.complex128)
+        chi_k = h[8 + 4 * S:8 + 6 * S].view(np.complex128)
+        rho = rho * chi_k / chi
+        xn = oracle.bicgstabm(w.rowptr, w.colidx, w.val, w.b, sig, 0.0, n + 1).x
+        for k in range(S):
+            ak = per_shift[k][n][0]
+            assert abs(beta_k[k] + ak) <= 1e-8 * abs(ak), (n, k)
+            tr = np.linalg.norm(w.b - (A @ xn[k] + sig[k] * xn[k]))
+            assert abs(abs(zeta_new[k] * rho[k]) * np.sqrt(rr) - tr) <= 1e-8 * tr, (n, k)
+        assert abs(zeta_new[0] - 1.0) < 1e-13 and abs(chi_k[0] - chi) == 0.0   # sigma = 0: the base system itself
+
+
+def test_cgm_history_is_the_shifted_systems_own_cg(cfg2_small):
+    # CG-M: beta_k = -(textbook CG step length on A + sigma_k I), alpha_k = its direction coefficient,
+    # |zeta_k| = ||r^sigma|| / ||r||; base row: beta = -step length of CG on A, alpha_next = R1/R0, R1.
+    w = cfg2_small
+    M = _A(w).toarray()
+    sig = np.array([0.0, 0.3, 2.0])
+    nit, S = 7, 3
+    m = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig, 0.0, nit, hist_cap=nit)
+    assert m.hist.shape == (nit, 3 + 3 * S)
+
+    def textbook_cg(Mk):
+        r = w.b.copy(); p = w.b.copy(); rr = np.vdot(r, r).real
+        out = []
+        for _ in range(nit):
+            q = Mk @ p
+            a = rr / np.vdot(p, q).real
+            r = r - a * q
+            rr_new = np.vdot(r, r).real
+            bt = rr_new / rr
+            p = r + bt * p
+            rr = rr_new
+            out.append((a, bt, rr))
+        return out
+
+    base = textbook_cg(M)
+    shifted = [textbook_cg(M + s * np.eye(w.n)) for s in sig]
+    for n in range(nit):
+        h = m.hist[n]
+        a, bt, rr = base[n]
+        assert abs(h[0] + a) <= 1e-11 * a and abs(h[1] - bt) <= 1e-10 * bt and abs(h[2] - rr) <= 1e-10 * rr
+        for k in range(S):
+            ak, btk, rrk = shifted[k][n]
+            assert abs(h[3 + S + k] + ak) <= 1e-10 * ak, (n, k)                      # beta_k
+            assert abs(h[3 + 2 * S + k] - btk) <= 1e-9 * btk, (n, k)                 # alpha_k
+            assert abs(abs(h[3 + k]) - np.sqrt(rrk / rr)) <= 1e-9 * np.sqrt(rrk / rr), (n, k)   # zeta_new
