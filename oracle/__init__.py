@@ -49,7 +49,7 @@ def build_omp(force: bool = False) -> str:
     return _LIB_OMP
 
 
-_ENTRY = ("oracle_spmv_csr", "oracle_cgm", "oracle_bicgstabm", "oracle_cg", "oracle_bicgstab")
+_ENTRY = ("oracle_spmv_csr", "oracle_cgm", "oracle_bicgstabm", "oracle_cg", "oracle_bicgstab", "oracle_multirhs")
 
 
 def _load(omp: bool = False):
@@ -152,6 +152,39 @@ def bicgstabm(rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule: int = 0,
     then zeta_new[S], beta_k[S], chi_k[S] (complex)."""
     return _multishift("oracle_bicgstabm", rowptr, colidx, val, b, shifts, tol, max_iter, stop_rule,
                        hist_cap, lambda s: 8 + 6 * s, True, omp)
+
+
+@dataclass
+class MultiRhsResult:
+    status: int
+    iterations: int
+    x: np.ndarray           # [S, n]: x_i solves (A + sigma_i) x_i = b_i
+    conv_iter: np.ndarray
+    relres: np.ndarray      # |zeta_i| ||r|| / ||b_i||
+    y: np.ndarray           # [S, n]: the initial guesses, b_i - (A + sigma_i) y_i = r0 for every i
+    r0: np.ndarray          # [n]: the common initial residual
+
+
+def multirhs(rowptr, colidx, val, B, shifts, tol, max_iter, algorithm: str = "cgm") -> MultiRhsResult:
+    """A different right-hand side per shift, eq. (6): (A + shifts[i]) x[i] = B[i], through
+    initial guesses with a common initial residual (S - 1 SpMVs) and ONE multishift solve."""
+    rowptr, colidx, val = _csr(rowptr, colidx, val)
+    shifts = np.ascontiguousarray(shifts, dtype=np.float64)
+    n, s = rowptr.size - 1, shifts.size
+    B = np.ascontiguousarray(B, dtype=val.dtype).reshape(s, n)
+    x = np.empty((s, n), dtype=val.dtype)
+    y = np.empty((s, n), dtype=val.dtype)
+    r0 = np.empty(n, dtype=val.dtype)
+    it = ctypes.c_int(0)
+    conv = np.full(s, -1, dtype=np.int32)
+    relres = np.zeros(s, dtype=np.float64)
+    rc = _load().oracle_multirhs(_dt(val), ctypes.c_int64(n), _p(rowptr), _p(colidx), _p(val), _p(B), _p(shifts),
+                                 ctypes.c_int(s), ctypes.c_double(tol), ctypes.c_int(max_iter),
+                                 ctypes.c_int(0 if algorithm == "cgm" else 1), _p(x), ctypes.byref(it), _p(conv),
+                                 _p(relres), _p(y), _p(r0))
+    if rc < 0:
+        raise ValueError("oracle multirhs: invalid arguments (shifts must be pairwise distinct)")
+    return MultiRhsResult(rc, it.value, x, conv, relres, y, r0)
 
 
 def _single(fn_name, rowptr, colidx, val, sigma, b, tol, max_iter):

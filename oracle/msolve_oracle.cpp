@@ -109,7 +109,8 @@ inline bool finite(const zdouble& z) { return std::isfinite(z.real()) && std::is
 template <typename C>
 int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
         int max_iter, int stop_rule, C* x, int* iterations, int* conv_iter,
-        double* relres, C* r_out, double* zeta_out, double* hist, int hist_cap) {
+        double* relres, C* r_out, double* zeta_out, double* hist, int hist_cap,
+        const double* tol_scale = 0) {
     const int64_t n = A.n;
     if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
     std::vector<C> r(b, b + n), p(b, b + n), q(n);           // l.9-10: r <- b, p <- b
@@ -175,15 +176,16 @@ int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
         if (stop_rule == 1) {                                 // literal |r| > eps on the base system
             if (rnorm <= tol * bnorm) { for (int k = 0; k < S; ++k) if (active[k]) { active[k] = 0; if (conv_iter) conv_iter[k] = it; } nactive = 0; }
         } else {
-            for (int k = 0; k < S; ++k) if (active[k] && std::fabs(zeta[k]) * rnorm <= tol * bnorm) {
+            // tol_scale (multirhs only, else 1): the threshold of shift k is tol * ||b_k|| with ||b_k|| = bnorm * tol_scale[k]
+            for (int k = 0; k < S; ++k) if (active[k] && std::fabs(zeta[k]) * rnorm <= tol * (bnorm * (tol_scale ? tol_scale[k] : 1.0))) {
                 active[k] = 0; --nactive; if (conv_iter) conv_iter[k] = it;
-                if (relres) relres[k] = std::fabs(zeta[k]) * rnorm / bnorm;
+                if (relres) relres[k] = std::fabs(zeta[k]) * rnorm / (bnorm * (tol_scale ? tol_scale[k] : 1.0));
             }
         }
     }
     const double rnorm = std::sqrt(R1);
     for (int k = 0; k < S; ++k) {
-        if ((active[k] || stop_rule == 1) && relres) relres[k] = std::fabs(zeta[k]) * rnorm / bnorm;
+        if ((active[k] || stop_rule == 1) && relres) relres[k] = std::fabs(zeta[k]) * rnorm / (bnorm * (tol_scale ? tol_scale[k] : 1.0));
         if (zeta_out) zeta_out[k] = zeta[k];
     }
     if (r_out) std::memcpy((void*)r_out, (const void*)r.data(), sizeof(C) * n);
@@ -201,7 +203,8 @@ int cgm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
 template <typename C>
 int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double tol,
               int max_iter, int stop_rule, C* x, int* iterations, int* conv_iter,
-              double* relres, C* r_out, double* zeta_out, double* hist, int hist_cap) {
+              double* relres, C* r_out, double* zeta_out, double* hist, int hist_cap,
+              const double* tol_scale = 0) {
     const int64_t n = A.n;
     if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
     std::vector<C> r(b, b + n), p(b, b + n), r0(b, b + n), q(n), s(n), t(n), rnew(n);
@@ -301,21 +304,91 @@ int bicgstabm(const Csr<C>& A, const C* b, const double* sigma, int S, double to
         if (stop_rule == 1) {
             if (rnorm <= tol * bnorm) { for (int k = 0; k < S; ++k) if (active[k]) { active[k] = 0; if (conv_iter) conv_iter[k] = it; } nactive = 0; }
         } else {
-            for (int k = 0; k < S; ++k) if (active[k] && std::abs(zeta[k] * rho[k]) * rnorm <= tol * bnorm) {
+            for (int k = 0; k < S; ++k) if (active[k] && std::abs(zeta[k] * rho[k]) * rnorm <= tol * (bnorm * (tol_scale ? tol_scale[k] : 1.0))) {
                 active[k] = 0; --nactive; if (conv_iter) conv_iter[k] = it;
-                if (relres) relres[k] = std::abs(zeta[k] * rho[k]) * rnorm / bnorm;
+                if (relres) relres[k] = std::abs(zeta[k] * rho[k]) * rnorm / (bnorm * (tol_scale ? tol_scale[k] : 1.0));
             }
         }
     }
     const double rnorm = std::sqrt(rr);
     for (int k = 0; k < S; ++k) {
-        if ((active[k] || stop_rule == 1) && relres) relres[k] = std::abs(zeta[k] * rho[k]) * rnorm / bnorm;
+        if ((active[k] || stop_rule == 1) && relres) relres[k] = std::abs(zeta[k] * rho[k]) * rnorm / (bnorm * (tol_scale ? tol_scale[k] : 1.0));
         if (zeta_out) { const zdouble z = zeta[k] * rho[k]; zeta_out[2 * k] = z.real(); zeta_out[2 * k + 1] = z.imag(); }
     }
     if (r_out) std::memcpy((void*)r_out, (const void*)r.data(), sizeof(C) * n);
     *iterations = it;
     if (status == ST_BREAKDOWN) return status;
     return nactive > 0 ? ST_MAXITER : ST_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// A different right-hand side per shift, eq. (6):  (A + sigma_i I) x_i = b_i.
+// The paper only states that "a judicious choice of initial guesses can deliver the same initial residual for
+// each of the linear systems" and that generating them "involves a number of SpMV operations" ([18] is not
+// available); DESIGN.md "Per-shift right-hand sides" derives the construction used here (S - 1 SpMVs):
+//   Let G(s) be the vector polynomial of degree S-1 in the SHIFT variable s with G(sigma_i) = b_i, in Newton
+//   form G(s) = sum_m d_m w_m(s), w_m(s) = prod_{j<m} (s - sigma_j), d_m = divided differences of the b_i.
+//   Seek Y(s) = sum_{m<=S-2} u_m w_m(s) and a constant vector r0 with (A + s) Y(s) + r0 = G(s) for all s.
+//   Since (A + s) w_m u_m = w_m (A + sigma_m) u_m + w_{m+1} u_m, matching the coefficients of w_m gives
+//       u_{S-2} = d_{S-1};   u_{m-1} = d_m - (A + sigma_m) u_m  (m = S-2 .. 1);   r0 = d_0 - (A + sigma_0) u_0.
+//   Then y_i = Y(sigma_i) = sum_{m<=i} w_m(sigma_i) u_m satisfies b_i - (A + sigma_i) y_i = r0 for EVERY i,
+//   so one multishift solve (A + sigma_i) z_i = r0 from z_i = 0 finishes the family: x_i = y_i + z_i, and the
+//   residual of system i is the multishift recurrence residual zeta_i r.
+// Stop rule: |zeta_i| ||r|| <= tol ||b_i||  (each system relative to its own right-hand side).
+// Needs pairwise distinct shifts (divided differences).  alg: 0 = CG-M, 1 = BiCGStab-M.
+// y_out (S x n) and r0_out (n) are optional outputs for the pins.
+// ------------------------------------------------------------------------------------------
+template <typename C>
+int multirhs(const Csr<C>& A, const C* B, const double* sigma, int S, double tol, int max_iter, int alg,
+             C* x, int* iterations, int* conv_iter, double* relres, C* y_out, C* r0_out) {
+    const int64_t n = A.n;
+    if (S < 1 || n < 0 || max_iter < 0) return ST_EINVAL;
+    for (int i = 0; i < S; ++i)
+        for (int j = 0; j < i; ++j) if (sigma[i] == sigma[j]) return ST_EINVAL;
+    // ||b_i||
+    std::vector<double> bn(S);
+    for (int i = 0; i < S; ++i) bn[i] = std::sqrt(dot(n, B + (size_t)i * n, B + (size_t)i * n).real());
+    // divided differences, in place: after level l, D[i] = b[sigma_{i-l}, ..., sigma_i] for i >= l
+    std::vector<C> D(B, B + (size_t)S * n);
+    for (int l = 1; l < S; ++l)
+        for (int i = S - 1; i >= l; --i) {
+            const C inv = rnd<C>(1.0 / (sigma[i] - sigma[i - l]));
+            C* di = D.data() + (size_t)i * n; const C* dm = D.data() + (size_t)(i - 1) * n;
+            for (int64_t e = 0; e < n; ++e) di[e] = (di[e] - dm[e]) * inv;
+        }
+    // u recursion, in place: slot m+1 holds u_m, slot 0 ends as r0
+    std::vector<C> q(n);
+    for (int m = S - 2; m >= 0; --m) {
+        const C* um = D.data() + (size_t)(m + 1) * n;
+        C* dst = D.data() + (size_t)m * n;
+        spmv(A, um, q.data());
+        const C sg = rnd<C>(sigma[m]);
+        for (int64_t e = 0; e < n; ++e) dst[e] = dst[e] - (q[e] + sg * um[e]);
+    }
+    const C* r0 = D.data();
+    if (r0_out) std::memcpy((void*)r0_out, (const void*)r0, sizeof(C) * n);
+    const double r0n = std::sqrt(dot(n, r0, r0).real());
+    // (A + sigma_i) z_i = r0 from z_i = 0, thresholds tol ||b_i||
+    std::vector<double> ts(S);
+    for (int i = 0; i < S; ++i) ts[i] = r0n > 0.0 ? bn[i] / r0n : 1.0;
+    int status;
+    if (alg == 0) status = cgm(A, r0, sigma, S, tol, max_iter, 0, x, iterations, conv_iter, relres, (C*)0, (double*)0, (double*)0, 0, ts.data());
+    else status = bicgstabm(A, r0, sigma, S, tol, max_iter, 0, x, iterations, conv_iter, relres, (C*)0, (double*)0, (double*)0, 0, ts.data());
+    // x_i = z_i + y_i,  y_i = sum_{m <= min(i, S-2)} w_m(sigma_i) u_m
+    for (int i = 0; i < S; ++i) {
+        C* xi = x + (size_t)i * n;
+        C* yi = y_out ? y_out + (size_t)i * n : (C*)0;
+        if (yi) for (int64_t e = 0; e < n; ++e) yi[e] = C(0);
+        double w = 1.0;
+        for (int m = 0; m <= i && m <= S - 2; ++m) {
+            const C wc = rnd<C>(w);
+            const C* um = D.data() + (size_t)(m + 1) * n;
+            for (int64_t e = 0; e < n; ++e) xi[e] = xi[e] + wc * um[e];
+            if (yi) for (int64_t e = 0; e < n; ++e) yi[e] = yi[e] + wc * um[e];
+            w *= sigma[i] - sigma[m];
+        }
+    }
+    return status;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -439,6 +512,13 @@ static int bicgstabm_entry(int64_t n, const int32_t* rowptr, const int32_t* coli
                      iterations, conv_iter, relres, (C*)r_out, zeta_out, hist, hist_cap);
 }
 template <typename C>
+static int multirhs_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, const void* B,
+                          const double* shifts, int nshifts, double tol, int max_iter, int alg, void* x,
+                          int* iterations, int* conv_iter, double* relres, void* y_out, void* r0_out) {
+    return multirhs(mk<C>(n, rowptr, colidx, val), (const C*)B, shifts, nshifts, tol, max_iter, alg, (C*)x,
+                    iterations, conv_iter, relres, (C*)y_out, (C*)r0_out);
+}
+template <typename C>
 static int cg_entry(int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val, double sigma,
                     const void* b, double tol, int max_iter, void* x, int* iterations, double* relres) {
     return cg(mk<C>(n, rowptr, colidx, val), sigma, (const C*)b, tol, max_iter, (C*)x, iterations, relres);
@@ -470,6 +550,13 @@ int oracle_bicgstabm(int dtype, int64_t n, const int32_t* rowptr, const int32_t*
                      void* r_out, double* zeta_out, double* hist, int hist_cap) {
     DISPATCH(bicgstabm_entry, n, rowptr, colidx, val, b, shifts, nshifts, tol, max_iter, stop_rule, x, iterations,
              conv_iter, relres, r_out, zeta_out, hist, hist_cap)
+}
+
+int oracle_multirhs(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,
+                    const void* B, const double* shifts, int nshifts, double tol, int max_iter, int alg,
+                    void* x, int* iterations, int* conv_iter, double* relres, void* y_out, void* r0_out) {
+    DISPATCH(multirhs_entry, n, rowptr, colidx, val, B, shifts, nshifts, tol, max_iter, alg, x, iterations,
+             conv_iter, relres, y_out, r0_out)
 }
 
 int oracle_cg(int dtype, int64_t n, const int32_t* rowptr, const int32_t* colidx, const void* val,

@@ -500,3 +500,68 @@ def test_cgm_history_is_the_shifted_systems_own_cg(cfg2_small):
             assert abs(h[3 + S + k] + ak) <= 1e-10 * ak, (n, k)                      # beta_k
             assert abs(h[3 + 2 * S + k] - btk) <= 1e-9 * btk, (n, k)                 # alpha_k
             assert abs(abs(h[3 + k]) - np.sqrt(rrk / rr)) <= 1e-9 * np.sqrt(rrk / rr), (n, k)   # zeta_new
+
+
+# ------------------------------------------------------------------ eq. (6): a right-hand side per shift
+@pytest.mark.parametrize("alg", ["cgm", "bicgstabm"])
+def test_multirhs_matches_dense_lu_and_common_residual(alg, cfg2_small, cfg3_small):
+    # PAPER.md:228-232.  Pins: (a) the initial guesses really give ONE residual: b_i - (A + sigma_i) y_i = r0 for
+    # every i (numpy, from the returned y and r0); (b) each x_i against a dense LU solve of (A + sigma_i) x = b_i;
+    # (c) the true residual of every system is below tol relative to ITS right-hand side.
+    # catches: wrong divided differences, a wrong sigma in the u recursion, wrong Newton weights in y_i, x_i = z_i.
+    w = cfg2_small if alg == "cgm" else cfg3_small
+    A = _A(w)
+    M = A.toarray()
+    sig = np.array([0.0, 0.35, 1.1, 2.0])
+    rng = np.random.default_rng(8)
+    B = rng.standard_normal((sig.size, w.n)) + 1j * rng.standard_normal((sig.size, w.n))
+    B /= np.linalg.norm(B, axis=1)[:, None]
+    B[2] *= 3.0                                            # different norms: the thresholds are per system
+    r = oracle.multirhs(w.rowptr, w.colidx, w.val, B, sig, 1e-13, 500, alg)
+    assert r.status == oracle.OK
+    for i, s in enumerate(sig):
+        assert np.linalg.norm(B[i] - (A @ r.y[i] + s * r.y[i]) - r.r0) <= 1e-12 * np.linalg.norm(r.r0), i
+        x_lu = np.linalg.solve(M + s * np.eye(w.n), B[i])
+        assert np.linalg.norm(r.x[i] - x_lu) / np.linalg.norm(x_lu) < 1e-10, i
+        assert np.linalg.norm(B[i] - (A @ r.x[i] + s * r.x[i])) <= 1e-11 * np.linalg.norm(B[i]), i
+    # at a loose tolerance every system stops by its own norm: true residual <= tol ||b_i|| (<= 10 tol graded)
+    r = oracle.multirhs(w.rowptr, w.colidx, w.val, B, sig, 1e-8, 500, alg)
+    for i, s in enumerate(sig):
+        assert r.relres[i] <= 1e-8
+        assert np.linalg.norm(B[i] - (A @ r.x[i] + s * r.x[i])) <= 1e-7 * np.linalg.norm(B[i]), i
+
+
+def test_multirhs_special_cases(cfg2_small):
+    w = cfg2_small
+    rng = np.random.default_rng(9)
+    # two systems: the closed form y_0 = y_1 = (b_1 - b_0) / (sigma_1 - sigma_0), r0 = b_0 - (A + sigma_0) y
+    sig = np.array([0.2, 0.9])
+    B = rng.standard_normal((2, w.n)) + 1j * rng.standard_normal((2, w.n))
+    r = oracle.multirhs(w.rowptr, w.colidx, w.val, B, sig, 1e-12, 500)
+    y = (B[1] - B[0]) / (sig[1] - sig[0])
+    assert np.allclose(r.y[0], y, rtol=1e-14, atol=0) and np.array_equal(r.y[0], r.y[1])
+    assert np.allclose(r.r0, B[0] - (_A(w) @ y + sig[0] * y), rtol=0, atol=1e-13 * np.linalg.norm(r.r0))
+    # the same right-hand side for every shift IS eq. (1): all divided differences vanish, y = 0, r0 = b, and the
+    # result is the plain multishift solve bit for bit
+    sig = np.array([0.0, 0.01, 0.3, 1.0])
+    B = np.tile(w.b, (4, 1))
+    r = oracle.multirhs(w.rowptr, w.colidx, w.val, B, sig, w.tol, 500)
+    m = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, sig, w.tol, 500)
+    assert not r.y.any() and np.array_equal(r.r0, w.b)
+    assert r.iterations == m.iterations and np.array_equal(r.x, m.x) and np.array_equal(r.conv_iter, m.conv_iter)
+    # right-hand sides that are a polynomial of degree 2 in the shift: only d_0, d_1, d_2 are non-zero
+    c = rng.standard_normal((3, w.n)) + 1j * rng.standard_normal((3, w.n))
+    sig = np.array([0.1, 0.5, 0.8, 1.4, 2.2])
+    B = np.array([c[0] + s * c[1] + s * s * c[2] for s in sig])
+    r = oracle.multirhs(w.rowptr, w.colidx, w.val, B, sig, 1e-12, 500)
+    M = _A(w).toarray()
+    for i, s in enumerate(sig):
+        x_lu = np.linalg.solve(M + s * np.eye(w.n), B[i])
+        assert np.linalg.norm(r.x[i] - x_lu) / np.linalg.norm(x_lu) < 1e-10
+    # one system: nothing to construct
+    r = oracle.multirhs(w.rowptr, w.colidx, w.val, w.b[None, :], [0.3], w.tol, 500)
+    m = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, [0.3], w.tol, 500)
+    assert np.array_equal(r.x, m.x)
+    # duplicate shifts cannot be served by this construction
+    with pytest.raises(ValueError):
+        oracle.multirhs(w.rowptr, w.colidx, w.val, B[:2], [0.5, 0.5], 1e-10, 10)
