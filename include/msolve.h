@@ -156,6 +156,26 @@ int msolve_bicgstabm(const msolve_matrix *A, const void *d_b, const double *h_sh
                      double tol, int max_iter, void *d_x, void *d_workspace, size_t workspace_bytes,
                      int *h_iterations, int *h_conv_iter, double *h_relres, void *stream);
 
+/* A different right-hand side per shift, eq. (6):  (A + sigma_i I) x_i = b_i.
+ * "A judicious choice of initial guesses can deliver the same initial residual for each of the linear systems"
+ * (PAPER.md:232): the library builds initial guesses y_i with b_i - (A + sigma_i) y_i = r0 for every i on the
+ * device (Newton divided differences of the b_i in the shift variable, nshifts - 1 SpMVs; derivation in DESIGN.md
+ * "Per-shift right-hand sides"), runs ONE multishift solve (A + sigma_i) z_i = r0 with the unchanged CG-M /
+ * BiCGStab-M iteration and returns x_i = y_i + z_i.
+ *   d_B          in   nshifts*n complex, device, shift-major: b_i[j] at d_B[i*n + j].  Not modified.
+ *   h_shifts     in   pairwise DISTINCT (EINVAL otherwise: two systems with one shift and two right-hand sides do
+ *                     not share a Krylov space).
+ *   tol          in   system i stops at |zeta_i| ||r|| <= tol ||b_i||: relative to ITS OWN right-hand side;
+ *                     h_relres[i] is that ratio.
+ *   d_workspace       >= msolve_multirhs_workspace_bytes(): the solver's workspace plus nshifts vectors.
+ * Everything else as msolve_cgm.  The divided differences amplify rounding by 1 / prod |sigma_i - sigma_j|: the
+ * construction suits a handful of well separated shifts or right-hand sides that vary smoothly with the shift. */
+size_t msolve_multirhs_workspace_bytes(const msolve_matrix *A, int nshifts, int algorithm);
+int msolve_solve_multirhs(const msolve_matrix *A, int algorithm, const void *d_B, const double *h_shifts,
+                          int nshifts, double tol, int max_iter, void *d_x, void *d_workspace,
+                          size_t workspace_bytes, int *h_iterations, int *h_conv_iter, double *h_relres,
+                          void *stream);
+
 /* The call of Fig. 1 with HOST vectors: copies h_b to the device, solves,
  * copies all nshifts*n solutions back to h_x (both inside the call, on `stream`).  The library
  * allocates the device vectors and workspace itself and keeps them in the handle for the next call

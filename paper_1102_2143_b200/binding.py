@@ -31,7 +31,7 @@ MSOLVE_CFG_X_WINDOW = 4
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
-    "msolve_bicgstabm", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
+    "msolve_bicgstabm", "msolve_multirhs_workspace_bytes", "msolve_solve_multirhs", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
     "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_set_history", "msolve_destroy",
     "msolve_last_error",
 )
@@ -63,6 +63,9 @@ def load_library() -> ctypes.CDLL:
     solver_args = [vp, vp, vp, i32, dbl, i32, vp, vp, sz, vp, vp, vp, vp]
     lib.msolve_cgm.argtypes = solver_args
     lib.msolve_bicgstabm.argtypes = solver_args
+    lib.msolve_multirhs_workspace_bytes.argtypes = [vp, i32, i32]
+    lib.msolve_multirhs_workspace_bytes.restype = sz
+    lib.msolve_solve_multirhs.argtypes = [vp, i32, vp, vp, i32, dbl, i32, vp, vp, sz, vp, vp, vp, vp]
     lib.msolve_solve_host.argtypes = [vp, i32, vp, vp, i32, dbl, i32, vp, vp, vp, vp, vp]
     lib.msolve_solve_host_batch.argtypes = [vp, i32, i32, vp, vp, i32, dbl, i32, vp, vp, vp, vp, vp]
     lib.msolve_spmv.argtypes = [vp, vp, vp, vp, vp]
@@ -78,7 +81,7 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_last_error.restype = ctypes.c_char_p
     for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_cgm", "msolve_bicgstabm",
                  "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration", "msolve_config",
-                 "msolve_set_history"):
+                 "msolve_set_history", "msolve_solve_multirhs"):
         getattr(lib, name).restype = i32
     _lib = lib
     return lib
@@ -262,6 +265,40 @@ def msolve_bicgstabm(A: Matrix, b: torch.Tensor, shifts, tol: float, max_iter: i
                      workspace: Optional[torch.Tensor] = None, stream=None) -> SolveResult:
     """BiCGStab-M (PAPER.md:31, 154)."""
     return _solve("msolve_bicgstabm", MSOLVE_ALG_BICGSTABM, A, b, shifts, tol, max_iter, x, workspace, stream)
+
+
+def msolve_multirhs_workspace_bytes(A: Matrix, nshifts: int, algorithm: int) -> int:
+    return int(load_library().msolve_multirhs_workspace_bytes(A.handle, nshifts, algorithm))
+
+
+def msolve_solve_multirhs(A: Matrix, algorithm: int, B: torch.Tensor, shifts, tol: float, max_iter: int,
+                          x: Optional[torch.Tensor] = None, workspace: Optional[torch.Tensor] = None,
+                          stream=None) -> SolveResult:
+    """eq. (6): (A + shifts[i] I) x[i] = B[i], one right-hand side per shift (distinct shifts)."""
+    lib = load_library()
+    B = _dev(B, A.dtype)
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    s = sh.size
+    if B.numel() != s * A.n:
+        raise ValueError("B must hold nshifts*n elements")
+    if x is None:
+        x = torch.empty((s, A.n), dtype=A.dtype, device=B.device)
+    x = _dev(x, A.dtype)
+    if x.numel() != s * A.n:
+        raise ValueError("x must hold nshifts*n elements")
+    need = msolve_multirhs_workspace_bytes(A, s, algorithm)
+    if need == 0:
+        raise MsolveError(MSOLVE_EINVAL, "nshifts must be in [1, %d]" % MSOLVE_MAX_SHIFTS)
+    if workspace is None:
+        workspace = torch.empty(need, dtype=torch.uint8, device=B.device)
+    it = ctypes.c_int(0)
+    conv = np.full(s, -1, dtype=np.int32)
+    rel = np.zeros(s, dtype=np.float64)
+    rc = lib.msolve_solve_multirhs(A.handle, algorithm, B.data_ptr(), sh.ctypes.data, s, float(tol), int(max_iter),
+                                   x.data_ptr(), workspace.data_ptr(), workspace.numel() * workspace.element_size(),
+                                   ctypes.addressof(it), conv.ctypes.data, rel.ctypes.data, _stream(stream))
+    _check(rc)
+    return SolveResult(rc, it.value, x.view(s, A.n), conv, rel)
 
 
 def msolve_solve_host(A: Matrix, algorithm: int, b: torch.Tensor, shifts, tol: float, max_iter: int,

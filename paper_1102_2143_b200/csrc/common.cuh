@@ -203,7 +203,7 @@ struct SolveHeader {
     int stop_rule;   // 0 = per shift (R15), 1 = literal |r| > eps on the unshifted system (Alg. 1 l.15)
     double* hist;    // msolve_set_history: per-iteration scalars, hist_cap rows (NULL = off)
     int hist_cap;
-    int pad0;
+    int per_shift_norm;  // eq. (6): the stop test of shift k is relative to rhs_norm[k] = ||b_k|| instead of ||b||
     double sigma[kMaxShifts];
 };
 
@@ -228,6 +228,7 @@ struct SolveState {
     zd zeta_prev[kMaxShifts], zeta[kMaxShifts], zeta_new[kMaxShifts];
     zd rho[kMaxShifts], rho_new[kMaxShifts];
     zd beta_k[kMaxShifts], alpha_k[kMaxShifts], chi_k[kMaxShifts];
+    double rhs_norm[kMaxShifts]; // eq. (6) only: ||b_k|| (multirhs.cu)
     int active[kMaxShifts];      // compact list of active shift indices, length res.nactive
     // per-ACTIVE-shift coefficients consumed by the fused update kernels (index = position in
     // `active`): CG-M uses 3 reals (zeta, alpha_k, beta_k); BiCGStab-M 7 complex.

@@ -119,4 +119,12 @@ inline int spmv_launches(const msolve_matrix* A) { return A->kernel == KERNEL_ME
 int launch_vec_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s, cudaGraphConditionalHandle cond, int use_cond);
 int launch_init(const msolve_matrix* A, cudaStream_t s);
 
+// msolve.cu: pieces the other entry points (multirhs.cu, slab.cu) build on
+long long pk_stride_elems(const msolve_matrix* A);
+int check_device(const msolve_matrix* A, const char* who);
+// per_shift_norm = 1: shift k stops at |zeta_k| ||r|| <= tol * rhs_norm[k] (device array, eq. (6)) instead of tol ||b||
+int run_solver(int alg, const msolve_matrix* A, const void* d_b, const double* h_shifts, int S, double tol, int max_iter,
+               void* d_x, void* ws, size_t ws_bytes, int* h_iterations, int* h_conv_iter, double* h_relres, void* stream,
+               int per_shift_norm);
+
 }  // namespace msolve

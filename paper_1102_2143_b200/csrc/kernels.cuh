@@ -276,7 +276,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGrap
     const int na = st->res.nactive;
     const int it = st->res.n_iter + 1;
     const double rnorm = sqrt(R1), bnorm = st->bnorm, tol = st->h.tol;
-    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1;
+    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1, psn = st->h.per_shift_norm != 0;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
         const int k = st->active[a];
         const double zn = st->zeta_new[k].re, z = st->zeta[k].re;
@@ -284,10 +284,11 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGrap
         st->alpha_k[k].re = alpha_next * ratio * ratio;                 // l.26
         st->zeta_prev[k].re = z;                                        // l.30
         st->zeta[k].re = zn;                                            // l.31
-        const double rel = fabs(zn) * rnorm / bnorm;
+        const double nk = psn ? st->rhs_norm[k] : bnorm;               // eq. (6): relative to the shift's own ||b_k||
+        const double rel = fabs(zn) * rnorm / nk;
         st->res.relres[k] = rel;
         // l.15: per shift (R15), or literally on the unshifted residual (stop_rule = 1)
-        if (!force && (base_rule ? rnorm : fabs(zn) * rnorm) <= tol * bnorm) st->res.conv_iter[k] = it;
+        if (!force && (base_rule ? rnorm : fabs(zn) * rnorm) <= tol * nk) st->res.conv_iter[k] = it;
     }
     // msolve_set_history: row it-1 = beta, alpha_next, R1, then zeta_new[S], beta_k[S], alpha_k[S] (frozen shifts
     // keep the values of their last active iteration)
@@ -505,7 +506,7 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraph
     const int na = st->res.nactive;
     const int it = st->res.n_iter + 1;
     const double rnorm = sqrt(rr), bnorm = st->bnorm, tol = st->h.tol;
-    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1;
+    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1, psn = st->h.per_shift_norm != 0;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
         const int k = st->active[a];
         const zd zn = st->zeta_new[k], rn = st->rho_new[k];
@@ -513,8 +514,9 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraph
         st->zeta[k] = zn;
         st->rho[k] = rn;
         const double zr = zabs(zmul(zn, rn));
-        st->res.relres[k] = zr * rnorm / bnorm;
-        if (!force && (base_rule ? rnorm : zr * rnorm) <= tol * bnorm) st->res.conv_iter[k] = it;
+        const double nk = psn ? st->rhs_norm[k] : bnorm;
+        st->res.relres[k] = zr * rnorm / nk;
+        if (!force && (base_rule ? rnorm : zr * rnorm) <= tol * nk) st->res.conv_iter[k] = it;
     }
     // msolve_set_history: row it-1 = beta, chi, alpha' (complex), |r'|^2, 0, then zeta_new[S], beta_k[S], chi_k[S] (complex)
     if (st->h.hist && it <= st->h.hist_cap) {

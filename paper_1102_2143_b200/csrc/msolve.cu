@@ -44,7 +44,7 @@ int msolve::ensure_smem(const msolve_matrix* A, const void* kernel, int bytes) {
 
 // the handle's device must be the calling thread's current device (kernels, graphs and the function
 // attributes above belong to it)
-static int check_device(const msolve_matrix* A, const char* who) {
+int msolve::check_device(const msolve_matrix* A, const char* who) {
     int cur = -1;
     CU(cudaGetDevice(&cur));
     if (cur != A->device) return fail(MSOLVE_EINVAL, "%s: the handle lives on device %d, the current device is %d", who, A->device, cur);
@@ -439,7 +439,7 @@ extern "C" const char* msolve_kernel_name(int alg, int j) {
 }
 
 // ------------------------------------------------------------------------------------- workspace
-static long long pk_stride_elems(const msolve_matrix* A) { return (long long)align_up((size_t)A->dev.n, 16); }
+long long msolve::pk_stride_elems(const msolve_matrix* A) { return (long long)align_up((size_t)A->dev.n, 16); }
 static int base_vectors(int alg) { return alg == MSOLVE_ALG_CGM ? 3 : 5; }  // r p q [s t]
 
 extern "C" size_t msolve_workspace_bytes(const msolve_matrix* A, int nshifts, int algorithm) {
@@ -480,9 +480,9 @@ static void fill_result_init(SolveResult* r, int S) {
 }
 
 // ------------------------------------------------------------------------------------- solve
-static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const double* h_shifts, int S, double tol,
-                      int max_iter, void* d_x, void* ws, size_t ws_bytes, int* h_iterations, int* h_conv_iter,
-                      double* h_relres, void* stream_) {
+int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const double* h_shifts, int S, double tol,
+                       int max_iter, void* d_x, void* ws, size_t ws_bytes, int* h_iterations, int* h_conv_iter,
+                       double* h_relres, void* stream_, int per_shift_norm) {
     msolve_matrix* A = const_cast<msolve_matrix*>(Ac);
     if (!A) return fail(MSOLVE_EINVAL, "solve: A is NULL");
     int rc = check_device(A, "solve");
@@ -492,6 +492,7 @@ static int run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const d
     SolveResult* hr = &A->h_stage->res;
     rc = fill_header(A, alg, d_b, h_shifts, S, tol, max_iter, d_x, ws, ws_bytes, 0, hh);
     if (rc != MSOLVE_OK) return rc;
+    hh->per_shift_norm = per_shift_norm;
     fill_result_init(hr, S);
     const size_t xbytes = (size_t)S * (size_t)A->dev.n * elem_bytes(A->dtype);
     if (A->dev.n == 0 || max_iter == 0) {  // nothing to iterate: x = 0
@@ -543,14 +544,14 @@ extern "C" int msolve_cgm(const msolve_matrix* A, const void* d_b, const double*
                           int max_iter, void* d_x, void* d_workspace, size_t workspace_bytes, int* h_iterations,
                           int* h_conv_iter, double* h_relres, void* stream) {
     return run_solver(MSOLVE_ALG_CGM, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_workspace, workspace_bytes,
-                      h_iterations, h_conv_iter, h_relres, stream);
+                      h_iterations, h_conv_iter, h_relres, stream, 0);
 }
 
 extern "C" int msolve_bicgstabm(const msolve_matrix* A, const void* d_b, const double* h_shifts, int nshifts, double tol,
                                 int max_iter, void* d_x, void* d_workspace, size_t workspace_bytes, int* h_iterations,
                                 int* h_conv_iter, double* h_relres, void* stream) {
     return run_solver(MSOLVE_ALG_BICGSTABM, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_workspace, workspace_bytes,
-                      h_iterations, h_conv_iter, h_relres, stream);
+                      h_iterations, h_conv_iter, h_relres, stream, 0);
 }
 
 extern "C" int msolve_solve_host(const msolve_matrix* A, int algorithm, const void* h_b, const double* h_shifts,
@@ -576,7 +577,7 @@ extern "C" int msolve_solve_host(const msolve_matrix* A, int algorithm, const vo
     cudaError_t e = cudaMemcpyAsync(d_all + boff, h_b, bbytes, cudaMemcpyHostToDevice, stream);
     if (e != cudaSuccess) return fail(MSOLVE_ECUDA, "H2D copy failed: %s", cudaGetErrorString(e));
     rc = run_solver(algorithm, A, d_all + boff, h_shifts, nshifts, tol, max_iter, d_all + xoff, d_all + woff, wsb + 256,
-                    h_iterations, h_conv_iter, h_relres, stream_);
+                    h_iterations, h_conv_iter, h_relres, stream_, 0);
     if (rc >= 0) {
         e = cudaMemcpyAsync(h_x, d_all + xoff, xbytes, cudaMemcpyDeviceToHost, stream);
         if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
@@ -628,7 +629,7 @@ extern "C" int msolve_solve_host_batch(const msolve_matrix* A, int algorithm, in
         const int rc = run_solver(algorithm, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_ws, wsb + 256,
                                   h_iterations ? h_iterations + i : nullptr,
                                   h_conv_iter ? h_conv_iter + (size_t)i * nshifts : nullptr,
-                                  h_relres ? h_relres + (size_t)i * nshifts : nullptr, stream_);
+                                  h_relres ? h_relres + (size_t)i * nshifts : nullptr, stream_, 0);
         if (rc < 0) { cudaStreamSynchronize(Am->copy_stream); return rc; }
         worst = std::max(worst, rc);
         CU(cudaEventRecord(Am->ev_solved[j], stream));

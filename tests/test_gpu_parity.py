@@ -392,14 +392,36 @@ def test_breakdown_reported(ms):
     assert res.status == ms.MSOLVE_BREAKDOWN == o.status and res.iterations == o.iterations == 0
     assert np.array_equal(res.x.cpu().numpy(), o.x) and not o.x.any()
     ms.msolve_destroy(A)
-    # BiCGStab-M on A = c I (R17): s = r + beta q = 0 after the first half step, <t,t> = 0: breakdown, x = 0
-    val = np.full(n, 2.5, dtype=np.complex128)
+    # BiCGStab-M, <r0, A p> = 0 exactly in the first loop body (A swaps neighbouring entries, b lives on the even
+    # ones): breakdown before any update, x = 0
+    rp2 = np.arange(n + 1, dtype=np.int32)
+    ci2 = (np.arange(n) ^ 1).astype(np.int32)
+    v2 = np.ones(n, dtype=np.complex128)
+    b2 = np.zeros(n, dtype=np.complex128)
+    b2[::2] = W.unit_rhs(2, n // 2)
+    A = ms.msolve_create_csr(dev(rp2), dev(ci2), dev(v2))
+    x.fill_(7.0)
+    res = ms.msolve_bicgstabm(A, dev(b2), [0.0, 0.5], 1e-10, 10, x=x)
+    o = oracle.bicgstabm(rp2, ci2, v2, b2, [0.0, 0.5], 1e-10, 10)
+    assert res.status == ms.MSOLVE_BREAKDOWN == o.status and res.iterations == o.iterations == 0
+    assert np.array_equal(res.x.cpu().numpy(), o.x) and not o.x.any()
+    ms.msolve_destroy(A)
+    # BiCGStab-M on A = c I (R17): s = r + beta q vanishes after the first half step up to rounding.  Whether that is
+    # an exact zero (<t,t> = 0: breakdown, x = 0, what the oracle's unfused arithmetic gives) or a residual of one
+    # ulp (one more half step on rounding noise: converged, x_k = b / (c + sigma_k)) is decided by the rounding of
+    # one multiply-add; both are correct outcomes and nothing else is.
+    c = 2.5
+    val = np.full(n, c, dtype=np.complex128)
     A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
     x.fill_(7.0)
     res = ms.msolve_bicgstabm(A, dev(b), [0.0, 0.5], 1e-10, 10, x=x)
-    o = oracle.bicgstabm(rowptr, colidx, val, b, [0.0, 0.5], 1e-10, 10)
-    assert res.status == ms.MSOLVE_BREAKDOWN == o.status and res.iterations == o.iterations == 0
-    assert np.array_equal(res.x.cpu().numpy(), o.x) and not o.x.any()
+    xg = res.x.cpu().numpy()
+    if res.status == ms.MSOLVE_BREAKDOWN:
+        assert res.iterations == 0 and not xg.any()
+    else:
+        assert res.status == ms.MSOLVE_OK and res.iterations == 1
+        for k, sg in enumerate([0.0, 0.5]):
+            assert np.linalg.norm(xg[k] - b / (c + sg)) <= 1e-14 * np.linalg.norm(b)
     ms.msolve_destroy(A)
     # a breakdown AFTER the first update keeps the iterate reached so far (same as the oracle)
     val = np.ones(n, dtype=np.complex128)
@@ -441,6 +463,7 @@ def test_stop_rule_base_matches_oracle(ms, alg, dtype, tol):
 
 
 HIST_RTOL = 1e-12
+HIST_ULPS = 64.0
 
 
 @pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "bsr3"), ("c2", "csr"), ("c3", "bsr3"), ("c3", "csr")])
@@ -463,13 +486,21 @@ def test_scalar_history_matches_oracle(ms, which, fmt):
     assert not hist.cpu().numpy()[o.iterations:].any()              # nothing written past the last iteration
     if w.algorithm == "cgm":
         dev_rel = np.abs(hg - o.hist) / np.abs(o.hist)
+        rr = o.hist[:, 2]
     else:                                                           # complex pairs: relative to the modulus
         zg = np.concatenate([hg[:, :6].copy().view(np.complex128), hg[:, 8:].copy().view(np.complex128)], axis=1)
         zo = np.concatenate([o.hist[:, :6].copy().view(np.complex128), o.hist[:, 8:].copy().view(np.complex128)], axis=1)
-        dev_rel = np.abs(zg - zo) / np.abs(zo)
-        assert np.all(np.abs(hg[:, 6] - o.hist[:, 6]) <= 1e-9 * o.hist[:, 6]) and not hg[:, 7].any()
-    print("history %s/%s: max relative deviation per iteration" % (which, fmt), dev_rel.max(axis=1))
-    assert dev_rel.max() <= HIST_RTOL * 10 ** (o.iterations / 8.0), dev_rel.max()
+        rr = o.hist[:, 6]
+        dev_rel = np.concatenate([np.abs(zg - zo) / np.abs(zo), (np.abs(hg[:, 6] - rr) / rr)[:, None]], axis=1)
+        assert not hg[:, 7].any()
+    # The bar: both sides run the same recurrences; they differ in the summation order of the
+    # dots and in fused multiply-adds, i.e. by a few ulp of ||b|| per element of r and per iteration.  Relative to
+    # the shrinking residual that is (n + 1) eps ||b|| / ||r_n||, so a scalar of iteration n may deviate by
+    # HIST_RTOL + HIST_ULPS (n + 1) eps ||b|| / ||r_{n+1}|| -- 1e-12 while the residual is large, where a wrong
+    # formula shows as an O(1) deviation.
+    bar = HIST_RTOL + HIST_ULPS * np.finfo(np.float64).eps * (np.arange(o.iterations) + 1) / np.sqrt(rr)
+    print("history %s/%s: max relative deviation per iteration" % (which, fmt), dev_rel.max(axis=1), "bar", bar)
+    assert np.all(dev_rel.max(axis=1) <= bar), (dev_rel.max(axis=1) / bar).max()
     # switching it off: the next solve leaves the buffer alone
     ms.msolve_set_history(A, None)
     hist.zero_()
