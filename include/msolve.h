@@ -86,7 +86,18 @@ enum {
                                 stop together (conv_iter[k] = that iteration for every k) */,
     MSOLVE_CFG_X_WINDOW = 4 /* vector-CSR kernel only: 1 = every SpMV launch carries an L2 access-policy window over the
                                gathered vector (persisting hits; sets the device-wide persisting-L2 set-aside).
-                               Measured on B200, config 5: profiles/r02_sweeps.md; default 0 */
+                               Measured on B200, config 5: profiles/r02_sweeps.md; default 0 */,
+    MSOLVE_CFG_MATRIX_L2 = 5 /* L2 policy of the matrix stream of the TMA-staged SpMV kernels: 0 = by footprint (default:
+                                evict-last when matrix + 2 vectors fit in 96 MB of the 126 MB L2, so that the second
+                                SpMV of a BiCGStab-M iteration and the next iteration find it there; evict-first
+                                otherwise: read once per SpMV), 1 = always evict-first, 2 = always evict-last */,
+    MSOLVE_CFG_ITER_PATH = 6 /* how a solve is driven: 1 = the iteration as a CUDA graph of kernels looping on the device
+                                (one kernel per step of Alg. 1; HBM-bound sizes), 2 = the WHOLE solve as one cooperative
+                                kernel with grid-wide barriers between the steps (systems that live in L2, where kernel
+                                launches, not bytes, are the cost; vector-CSR, BSR3 and lattice handles), 0 = by
+                                footprint (default): 2 when matrix + (4 + 2 nshifts) vectors take at most 40 MB.
+                                Same arithmetic step for step; the two paths group the dot products differently
+                                (per-CTA partials of different grids), so they agree to rounding, not bit for bit */
 };
 
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay

@@ -28,6 +28,8 @@ MSOLVE_CFG_UPDATE_KERNEL = 1
 MSOLVE_CFG_LATTICE_KERNEL = 2
 MSOLVE_CFG_STOP_RULE = 3
 MSOLVE_CFG_X_WINDOW = 4
+MSOLVE_CFG_MATRIX_L2 = 5
+MSOLVE_CFG_ITER_PATH = 6
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",

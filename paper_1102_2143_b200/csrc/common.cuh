@@ -218,9 +218,10 @@ struct SolveResult {
     double relres[kMaxShifts];
 };
 
-struct SolveState {
-    SolveHeader h;
-    SolveResult res;
+// The recurrence scalars of the iteration (Alg. 1 l.2-8, 17, 20-26, 30-31).  One instance lives in the
+// device-resident SolveState (iteration as a graph of kernels); the whole-solve cooperative kernel
+// (fused_small.cuh) keeps a private copy per CTA in shared memory.
+struct Recur {
     // base scalars (CG-M uses .re only)
     zd alpha, beta, beta_prev, delta, chi, alpha_new, delta_new;
     double R0, R1, bnorm;
@@ -228,29 +229,37 @@ struct SolveState {
     zd zeta_prev[kMaxShifts], zeta[kMaxShifts], zeta_new[kMaxShifts];
     zd rho[kMaxShifts], rho_new[kMaxShifts];
     zd beta_k[kMaxShifts], alpha_k[kMaxShifts], chi_k[kMaxShifts];
-    double rhs_norm[kMaxShifts]; // eq. (6) only: ||b_k|| (multirhs.cu)
     int active[kMaxShifts];      // compact list of active shift indices, length res.nactive
     // per-ACTIVE-shift coefficients consumed by the fused update kernels (index = position in
     // `active`): CG-M uses 3 reals (zeta, alpha_k, beta_k); BiCGStab-M 7 complex.
     double coef[kMaxShifts * 14];
+};
+
+struct SolveState {
+    SolveHeader h;
+    SolveResult res;
+    Recur rc;
+    double rhs_norm[kMaxShifts]; // eq. (6) only: ||b_k|| (multirhs.cu)
     // per-CTA partial sums of the fused reductions, [kAccMax][kMaxPartials]
     double partial[kAccMax * kMaxPartials];
+    double partial2[kMaxPartials];   // fused_small.cuh: |r|^2 partials (alternates with `partial` between grid syncs)
     int partial_count;           // how many CTAs wrote partials in the last reducing kernel
 };
 
-// Fixed-order reduction of the per-CTA partials by ONE CTA (deterministic for a fixed grid).
+// Fixed-order reduction of `count` per-CTA partials (NACC rows of kMaxPartials) by ONE CTA: every thread of the
+// calling CTA gets the sums (deterministic for a fixed grid).
 template <int NACC>
-__device__ __forceinline__ void reduce_partials(const SolveState* st, double (&out)[NACC], double* smem) {
-    const int count = st->partial_count;
+__device__ __forceinline__ void reduce_partials_from(const double* partial, int count, double (&out)[NACC], double* smem) {
     double acc[NACC];
 #pragma unroll
     for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
     for (int i = threadIdx.x; i < count; i += blockDim.x) {
 #pragma unroll
-        for (int a = 0; a < NACC; ++a) acc[a] += st->partial[a * kMaxPartials + i];
+        for (int a = 0; a < NACC; ++a) acc[a] += partial[a * kMaxPartials + i];
     }
     block_sum<NACC>(acc, smem);
     __shared__ double bc[kAccMax];
+    __syncthreads();                     // bc may still be read from a previous call
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int a = 0; a < NACC; ++a) bc[a] = acc[a];
@@ -258,6 +267,10 @@ __device__ __forceinline__ void reduce_partials(const SolveState* st, double (&o
     __syncthreads();
 #pragma unroll
     for (int a = 0; a < NACC; ++a) out[a] = bc[a];
+}
+template <int NACC>
+__device__ __forceinline__ void reduce_partials(const SolveState* st, double (&out)[NACC], double* smem) {
+    reduce_partials_from<NACC>(st->partial, st->partial_count, out, smem);
 }
 
 // Matrix description passed by value to the SpMV kernels.
@@ -272,6 +285,7 @@ struct MatDev {
     void* carry;             // merge-path: per-tile head / tail partial sums, 2 * aux_count complex
     int aux_count;
     int x_pin;               // CSR kernels: gather x with L2 evict_last (x fits in L2 next to the stream)
+    int mat_keep;            // TMA-staged kernels: stream the matrix with L2 evict_last (it fits in L2 between SpMVs)
     // matrix-free SU(3) lattice operator (msolve_create_lattice_su3): val = links[ndim][vol][3][3]
     int lat_ndim;            // 0 for CSR / BSR3
     int lat_ext[4];          // extents, dimension 0 fastest (unused dimensions = 1)

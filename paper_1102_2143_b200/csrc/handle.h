@@ -30,6 +30,7 @@ struct Options {
     int stop_rule = 0;       // MSOLVE_CFG_STOP_RULE
     int iter_path = 0;       // MSOLVE_CFG_ITER_PATH
     int x_window = 0;        // MSOLVE_CFG_X_WINDOW
+    int matrix_l2 = 0;       // MSOLVE_CFG_MATRIX_L2
     int graph_key() const { return loop_mode | (update_kernel << 1) | (lattice_kernel << 2) | (iter_path << 4) | (x_window << 6); }
 };
 
@@ -118,6 +119,10 @@ inline int spmv_launches(const msolve_matrix* A) { return A->kernel == KERNEL_ME
 // vec.cu: the non-SpMV kernels of the iteration body, by position j (msolve_kernel_name), and the two init kernels
 int launch_vec_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s, cudaGraphConditionalHandle cond, int use_cond);
 int launch_init(const msolve_matrix* A, cudaStream_t s);
+
+// fused_small.cu: the whole solve as ONE cooperative kernel (systems that live in L2)
+bool fused_supported(const msolve_matrix* A);
+int launch_fused(const msolve_matrix* A, int alg, cudaStream_t s);
 
 // msolve.cu: pieces the other entry points (multirhs.cu, slab.cu) build on
 long long pk_stride_elems(const msolve_matrix* A);

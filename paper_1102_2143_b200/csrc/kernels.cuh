@@ -13,6 +13,11 @@
 //
 // The per-shift zeta/alpha/beta recurrences stay on the device; converged
 // shifts are removed from the `active` list, so the update kernels never touch their vectors.
+//
+// Every step is a __device__ function over (header, result, recurrences): the k_* kernels below run one step each
+// on the device-resident SolveState (the iteration as a graph of kernels); fused_small.cuh strings the same
+// functions together inside one cooperative kernel for systems that live in L2.  `cta` / `ncta` are the CTA's
+// index and the number of CTAs the elements are spread over.
 #pragma once
 
 #include "common.cuh"
@@ -50,21 +55,27 @@ MSOLVE_PACK_IO(float, 4, float4, (r.v[0] = t.x, r.v[1] = t.y, r.v[2] = t.z, r.v[
 // r <- b, p <- b (Alg. 1 l.9-10); partial |b|^2 (l.13).  p_k <- b and x_k <- 0 (l.11-12) are not
 // materialised: the first update treats them as such without reading them.
 template <typename E, int VEC>
-__global__ void __launch_bounds__(kThreads) k_init_vectors(SolveState* st) {
+__device__ __forceinline__ double init_vectors_fn(const SolveHeader& h, int cta, int ncta) {
     typedef Pack<E, VEC> P;
-    const long long nvec = st->h.n / VEC;
-    const P* b = (const P*)st->h.b;
-    P* r = (P*)st->h.r;
-    P* p = (P*)st->h.p;
-    double acc[1] = {0.0};
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+    const long long nvec = h.n / VEC;
+    const P* b = (const P*)h.b;
+    P* r = (P*)h.r;
+    P* p = (P*)h.p;
+    double acc = 0.0;
+    const long long stride = (long long)ncta * blockDim.x;
+    for (long long i = (long long)cta * blockDim.x + threadIdx.x; i < nvec; i += stride) {
         const P bv = ld_pack<false>(b + i);
         st_pack<false>(r + i, bv);
         st_pack<false>(p + i, bv);
 #pragma unroll
-        for (int e = 0; e < VEC; ++e) acc[0] += cnorm2(bv.v[e]);
+        for (int e = 0; e < VEC; ++e) acc += cnorm2(bv.v[e]);
     }
+    return acc;
+}
+
+template <typename E, int VEC>
+__global__ void __launch_bounds__(kThreads) k_init_vectors(SolveState* st) {
+    double acc[1] = {init_vectors_fn<E, VEC>(st->h, blockIdx.x, gridDim.x)};
     __shared__ double red[32];
     block_sum<1>(acc, red);
     if (threadIdx.x == 0) {
@@ -73,50 +84,48 @@ __global__ void __launch_bounds__(kThreads) k_init_vectors(SolveState* st) {
     }
 }
 
-// Scalars of l.2-8, 13-14 and the BiCGStab-M analogue; b = 0 ends the solve at once.
-__global__ void __launch_bounds__(kThreads) k_init_state(SolveState* st) {
-    __shared__ double red[32];
-    double s[1];
-    reduce_partials<1>(st, s, red);
-    const int S = st->h.S;
+// Scalars of l.2-8, 13-14 and the BiCGStab-M analogue from bb = <b,b>; b = 0 ends the solve at once.
+__device__ __forceinline__ void init_state_fn(const SolveHeader& h, SolveResult& res, Recur& rc, double bb) {
+    const int S = h.S;
     for (int k = threadIdx.x; k < S; k += blockDim.x) {
-        st->zeta_prev[k] = {1.0, 0.0}; st->zeta[k] = {1.0, 0.0}; st->zeta_new[k] = {1.0, 0.0};
-        st->rho[k] = {1.0, 0.0}; st->rho_new[k] = {1.0, 0.0};
-        st->beta_k[k] = {0.0, 0.0}; st->alpha_k[k] = {0.0, 0.0}; st->chi_k[k] = {0.0, 0.0};
-        st->active[k] = k;
-        st->res.conv_iter[k] = (s[0] == 0.0) ? 0 : -1;
-        st->res.relres[k] = (s[0] == 0.0) ? 0.0 : 1.0;
+        rc.zeta_prev[k] = {1.0, 0.0}; rc.zeta[k] = {1.0, 0.0}; rc.zeta_new[k] = {1.0, 0.0};
+        rc.rho[k] = {1.0, 0.0}; rc.rho_new[k] = {1.0, 0.0};
+        rc.beta_k[k] = {0.0, 0.0}; rc.alpha_k[k] = {0.0, 0.0}; rc.chi_k[k] = {0.0, 0.0};
+        rc.active[k] = k;
+        res.conv_iter[k] = (bb == 0.0) ? 0 : -1;
+        res.relres[k] = (bb == 0.0) ? 0.0 : 1.0;
     }
     if (threadIdx.x == 0) {
-        st->alpha = {0.0, 0.0}; st->beta = {0.0, 0.0}; st->beta_prev = {1.0, 0.0};
-        st->delta = {s[0], 0.0};            // <r0,r> = <b,b>
-        st->chi = {0.0, 0.0}; st->alpha_new = {0.0, 0.0}; st->delta_new = {0.0, 0.0};
-        st->R0 = s[0]; st->R1 = s[0]; st->bnorm = sqrt(s[0]);
-        st->res.n_iter = 0;
-        st->res.status = MSOLVE_OK;
-        st->res.nactive = S;
-        st->res.zero_rhs = (s[0] == 0.0);
-        st->res.done = (s[0] == 0.0) || !isfinite(s[0]) || st->h.max_iter <= 0;
-        if (!isfinite(s[0])) st->res.status = MSOLVE_BREAKDOWN;
-        else if (s[0] != 0.0 && st->h.max_iter <= 0) st->res.status = MSOLVE_MAXITER;
+        rc.alpha = {0.0, 0.0}; rc.beta = {0.0, 0.0}; rc.beta_prev = {1.0, 0.0};
+        rc.delta = {bb, 0.0};            // <r0,r> = <b,b>
+        rc.chi = {0.0, 0.0}; rc.alpha_new = {0.0, 0.0}; rc.delta_new = {0.0, 0.0};
+        rc.R0 = bb; rc.R1 = bb; rc.bnorm = sqrt(bb);
+        res.n_iter = 0;
+        res.status = MSOLVE_OK;
+        res.nactive = S;
+        res.zero_rhs = (bb == 0.0);
+        res.done = (bb == 0.0) || !isfinite(bb) || h.max_iter <= 0;
+        if (!isfinite(bb)) res.status = MSOLVE_BREAKDOWN;
+        else if (bb != 0.0 && h.max_iter <= 0) res.status = MSOLVE_MAXITER;
     }
+    __syncthreads();
 }
+
 
 constexpr int kPupdUnroll = 4;   // 2 * 4 independent 16-byte loads in flight per thread
 // ----------------------------------------------------------------------------- CG-M
 // A1: p <- r + alpha p  (l.27; at n = 0 p = b already)
 template <typename E, int VEC>
-__global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
-    if (st->res.done || st->res.n_iter == 0) return;
+__device__ __forceinline__ void cgm_pupdate_fn(const SolveHeader& h, const Recur& rc, int cta, int ncta) {
     typedef typename RealOf<E>::type T;
     typedef Pack<E, VEC> P;
-    const long long nvec = st->h.n / VEC;
-    const P* r = (const P*)st->h.r;
-    P* p = (P*)st->h.p;
-    const T alpha = (T)st->alpha.re;
-    const long long stride = (long long)gridDim.x * blockDim.x;
+    const long long nvec = h.n / VEC;
+    const P* r = (const P*)h.r;
+    P* p = (P*)h.p;
+    const T alpha = (T)rc.alpha.re;
+    const long long stride = (long long)ncta * blockDim.x;
     constexpr int U = kPupdUnroll;
-    long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    long long i = (long long)cta * blockDim.x + threadIdx.x;
     for (; i + (U - 1) * stride < nvec; i += U * stride) {
         P rv[U], pv[U];
 #pragma unroll
@@ -137,69 +146,73 @@ __global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
     }
 }
 
-// A4: one CTA.  P = sum of partials; beta = -R0/P; zeta_new_k, beta_k for active shifts.
-__global__ void __launch_bounds__(kThreads) k_cgm_scal1(SolveState* st) {
-    if (st->res.done) return;
-    __shared__ double red[32];
+template <typename E, int VEC>
+__global__ void __launch_bounds__(kThreads) k_cgm_pupdate(SolveState* st) {
+    if (st->res.done || st->res.n_iter == 0) return;
+    cgm_pupdate_fn<E, VEC>(st->h, st->rc, blockIdx.x, gridDim.x);
+}
+
+// A4: one CTA.  P = <p,Ap>; beta = -R0/P; zeta_new_k, beta_k for active shifts.
+__device__ __forceinline__ void cgm_scal1_fn(const SolveHeader& h, SolveResult& res, Recur& rc, double P) {
     __shared__ int bad;
-    double s[1];
     if (threadIdx.x == 0) bad = 0;
-    reduce_partials<1>(st, s, red);
-    const double P = s[0];
-    const double R0 = st->R1;
+    __syncthreads();
+    const double R0 = rc.R1;
     const double beta = -R0 / P;
-    const double alpha = st->alpha.re, beta_prev = st->beta_prev.re;
-    const int na = st->res.nactive;
+    const double alpha = rc.alpha.re, beta_prev = rc.beta_prev.re;
+    const int na = res.nactive;
     if (!(P > 0.0) || !isfinite(P) || !isfinite(beta)) bad = 1;   // same value from every thread
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        const int k = st->active[a];
-        const double z = st->zeta[k].re, zp = st->zeta_prev[k].re;
-        const double den = beta * alpha * (zp - z) + zp * beta_prev * (1.0 - st->h.sigma[k] * beta);
+        const int k = rc.active[a];
+        const double z = rc.zeta[k].re, zp = rc.zeta_prev[k].re;
+        const double den = beta * alpha * (zp - z) + zp * beta_prev * (1.0 - h.sigma[k] * beta);
         const double zn = z * zp * beta_prev / den;
         const double bk = beta * zn / z;
         if (den == 0.0 || !isfinite(zn) || !isfinite(bk)) bad = 1;
-        st->zeta_new[k].re = zn;
-        st->beta_k[k].re = bk;
-        st->coef[3 * a + 0] = z;                 // zeta_k of this iteration: the lagged p_k update
-        st->coef[3 * a + 1] = st->alpha_k[k].re; // alpha_k from the previous scal2
-        st->coef[3 * a + 2] = bk;
+        rc.zeta_new[k].re = zn;
+        rc.beta_k[k].re = bk;
+        rc.coef[3 * a + 0] = z;                 // zeta_k of this iteration: the lagged p_k update
+        rc.coef[3 * a + 1] = rc.alpha_k[k].re;  // alpha_k from the previous scal2
+        rc.coef[3 * a + 2] = bk;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        st->R0 = R0;
-        st->beta.re = beta;
-        if (bad) { st->res.status = MSOLVE_BREAKDOWN; st->res.done = 1; }
+        rc.R0 = R0;
+        rc.beta.re = beta;
+        if (bad) { res.status = MSOLVE_BREAKDOWN; res.done = 1; }
     }
+    __syncthreads();
 }
 
+
 // A5: the fused multishift update.  UNR shifts are in flight per thread (2*UNR independent
-// 16-byte loads) on top of r and Ap; x_k / p_k are streamed with evict-first hints.
+// 16-byte loads) on top of r and Ap; x_k / p_k are streamed with evict-first hints.  Returns the thread's |r|^2 share.
 template <typename E, int VEC, int UNR>
-__global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
-    if (st->res.done) return;
+__device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const SolveResult& res, const Recur& rc, int cta, int ncta) {
     typedef E C;
     typedef typename RealOf<E>::type T;
     typedef Pack<E, VEC> P;
     __shared__ T s_zeta[kMaxShifts], s_alpha[kMaxShifts], s_beta[kMaxShifts];
     __shared__ int s_k[kMaxShifts];
-    const int na = st->res.nactive;
-    const bool first = st->res.n_iter == 0;
+    const int na = res.nactive;
+    const bool first = res.n_iter == 0;
+    __syncthreads();                              // the arrays may still be read by a previous call (fused kernel)
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        s_k[a] = st->active[a];
-        s_zeta[a] = (T)st->coef[3 * a + 0];
-        s_alpha[a] = (T)st->coef[3 * a + 1];
-        s_beta[a] = (T)st->coef[3 * a + 2];
+        s_k[a] = rc.active[a];
+        s_zeta[a] = (T)rc.coef[3 * a + 0];
+        s_alpha[a] = (T)rc.coef[3 * a + 1];
+        s_beta[a] = (T)rc.coef[3 * a + 2];
     }
-    const T beta = (T)st->beta.re;
+    const T beta = (T)rc.beta.re;
     __syncthreads();
-    const long long n = st->h.n, nvec = n / VEC, pks = st->h.pk_stride;
-    P* r = (P*)st->h.r;
-    const P* q = (const P*)st->h.q;
-    C* x = (C*)st->h.x;
-    C* pk = (C*)st->h.pk;
-    double acc[1] = {0.0};
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+    const long long n = h.n, nvec = n / VEC, pks = h.pk_stride;
+    P* r = (P*)h.r;
+    const P* q = (const P*)h.q;
+    C* x = (C*)h.x;
+    C* pk = (C*)h.pk;
+    double acc = 0.0;
+    const long long stride = (long long)ncta * blockDim.x;
+    for (long long i = (long long)cta * blockDim.x + threadIdx.x; i < nvec; i += stride) {
         P rv = ld_pack<false>(r + i);
         const P qv = ld_pack<false>(q + i);
         for (int a0 = 0; a0 < na; a0 += UNR) {
@@ -237,10 +250,17 @@ __global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
 #pragma unroll
         for (int e = 0; e < VEC; ++e) {
             rv.v[e] = caxpy_r(rv.v[e], beta, qv.v[e]);                               // l.21
-            acc[0] += cnorm2(rv.v[e]);                                               // l.24
+            acc += cnorm2(rv.v[e]);                                                  // l.24
         }
         st_pack<false>(r + i, rv);
     }
+    return acc;
+}
+
+template <typename E, int VEC, int UNR>
+__global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
+    if (st->res.done) return;
+    double acc[1] = {cgm_update_fn<E, VEC, UNR>(st->h, st->res, st->rc, blockIdx.x, gridDim.x)};
     __shared__ double red[32];
     block_sum<1>(acc, red);
     if (threadIdx.x == 0) {
@@ -250,114 +270,108 @@ __global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
 }
 
 // Loop control shared by both algorithms: called by thread 0 after the per-shift stop test.
-__device__ __forceinline__ void finish_iteration(SolveState* st, bool bad) {
+__device__ __forceinline__ void finish_iteration(const SolveHeader& h, SolveResult& res, Recur& rc, bool bad) {
     // compact the active list in order (S <= 128: serial is fine)
-    const int na = st->res.nactive;
+    const int na = res.nactive;
     int m = 0;
     for (int a = 0; a < na; ++a) {
-        const int k = st->active[a];
-        if (st->res.conv_iter[k] < 0) st->active[m++] = k;
+        const int k = rc.active[a];
+        if (res.conv_iter[k] < 0) rc.active[m++] = k;
     }
-    st->res.nactive = m;
-    if (bad) { st->res.status = MSOLVE_BREAKDOWN; st->res.done = 1; }
-    else if (m == 0) { st->res.status = MSOLVE_OK; st->res.done = 1; }
-    else if (st->res.n_iter >= st->h.max_iter) { st->res.status = MSOLVE_MAXITER; st->res.done = 1; }
+    res.nactive = m;
+    if (bad) { res.status = MSOLVE_BREAKDOWN; res.done = 1; }
+    else if (m == 0) { res.status = MSOLVE_OK; res.done = 1; }
+    else if (res.n_iter >= h.max_iter) { res.status = MSOLVE_MAXITER; res.done = 1; }
 }
 
-// A6: one CTA.  R1 -> alpha, alpha_k; zeta shuffle; per-shift stop test; loop control.
-// `cond` is the WHILE node's handle (use_cond = 0 in chunked mode).
-__global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGraphConditionalHandle cond, int use_cond) {
-    if (st->res.done) { if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, 0); return; }
-    __shared__ double red[32];
-    double s[1];
-    reduce_partials<1>(st, s, red);
-    const double R1 = s[0], R0 = st->R0;
+// A6: one CTA.  R1 -> alpha, alpha_k; zeta shuffle; per-shift stop test; loop control.  `hist` = the history
+// buffer or NULL (in the fused kernel only CTA 0 passes it).
+__device__ __forceinline__ void cgm_scal2_fn(const SolveHeader& h, SolveResult& res, Recur& rc, const double* rhs_norm,
+                                             double R1, double* hist) {
+    const double R0 = rc.R0;
     const double alpha_next = R1 / R0;
-    const int na = st->res.nactive;
-    const int it = st->res.n_iter + 1;
-    const double rnorm = sqrt(R1), bnorm = st->bnorm, tol = st->h.tol;
-    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1, psn = st->h.per_shift_norm != 0;
+    const int na = res.nactive;
+    const int it = res.n_iter + 1;
+    const double rnorm = sqrt(R1), bnorm = rc.bnorm, tol = h.tol;
+    const bool force = h.force_all != 0, base_rule = h.stop_rule == 1, psn = h.per_shift_norm != 0;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        const int k = st->active[a];
-        const double zn = st->zeta_new[k].re, z = st->zeta[k].re;
+        const int k = rc.active[a];
+        const double zn = rc.zeta_new[k].re, z = rc.zeta[k].re;
         const double ratio = zn / z;
-        st->alpha_k[k].re = alpha_next * ratio * ratio;                 // l.26
-        st->zeta_prev[k].re = z;                                        // l.30
-        st->zeta[k].re = zn;                                            // l.31
-        const double nk = psn ? st->rhs_norm[k] : bnorm;               // eq. (6): relative to the shift's own ||b_k||
+        rc.alpha_k[k].re = alpha_next * ratio * ratio;                  // l.26
+        rc.zeta_prev[k].re = z;                                         // l.30
+        rc.zeta[k].re = zn;                                             // l.31
+        const double nk = psn ? rhs_norm[k] : bnorm;                    // eq. (6): relative to the shift's own ||b_k||
         const double rel = fabs(zn) * rnorm / nk;
-        st->res.relres[k] = rel;
+        res.relres[k] = rel;
         // l.15: per shift (R15), or literally on the unshifted residual (stop_rule = 1)
-        if (!force && (base_rule ? rnorm : fabs(zn) * rnorm) <= tol * nk) st->res.conv_iter[k] = it;
-    }
-    // msolve_set_history: row it-1 = beta, alpha_next, R1, then zeta_new[S], beta_k[S], alpha_k[S] (frozen shifts
-    // keep the values of their last active iteration)
-    if (st->h.hist && it <= st->h.hist_cap) {
-        __syncthreads();
-        const int S = st->h.S;
-        double* h = st->h.hist + (size_t)(it - 1) * (size_t)(3 + 3 * S);
-        if (threadIdx.x == 0) { h[0] = st->beta.re; h[1] = alpha_next; h[2] = R1; }
-        for (int k = threadIdx.x; k < S; k += blockDim.x) {
-            h[3 + k] = st->zeta_new[k].re; h[3 + S + k] = st->beta_k[k].re; h[3 + 2 * S + k] = st->alpha_k[k].re;
-        }
+        if (!force && (base_rule ? rnorm : fabs(zn) * rnorm) <= tol * nk) res.conv_iter[k] = it;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        st->R1 = R1;
-        st->beta_prev.re = st->beta.re;                                 // l.17
-        st->alpha.re = alpha_next;                                      // l.25
-        st->res.n_iter = it;                                            // l.32
-        finish_iteration(st, !isfinite(R1) || !isfinite(alpha_next));
-        if (use_cond) cudaGraphSetConditional(cond, st->res.done ? 0u : 1u);
+    // msolve_set_history: row it-1 = beta, alpha_next, R1, then zeta_new[S], beta_k[S], alpha_k[S] (frozen shifts
+    // keep the values of their last active iteration)
+    if (hist && it <= h.hist_cap) {
+        const int S = h.S;
+        double* hr = hist + (size_t)(it - 1) * (size_t)(3 + 3 * S);
+        if (threadIdx.x == 0) { hr[0] = rc.beta.re; hr[1] = alpha_next; hr[2] = R1; }
+        for (int k = threadIdx.x; k < S; k += blockDim.x) {
+            hr[3 + k] = rc.zeta_new[k].re; hr[3 + S + k] = rc.beta_k[k].re; hr[3 + 2 * S + k] = rc.alpha_k[k].re;
+        }
     }
+    if (threadIdx.x == 0) {
+        rc.R1 = R1;
+        rc.beta_prev.re = rc.beta.re;                                   // l.17
+        rc.alpha.re = alpha_next;                                       // l.25
+        res.n_iter = it;                                                // l.32
+        finish_iteration(h, res, rc, !isfinite(R1) || !isfinite(alpha_next));
+    }
+    __syncthreads();
 }
+
 
 // ----------------------------------------------------------------------------- BiCGStab-M
 // after SpMV#1: beta = -delta/<r0,q>; zeta_new_k, beta_k (complex).
-__global__ void __launch_bounds__(kThreads) k_bi_scal1(SolveState* st) {
-    if (st->res.done) return;
-    __shared__ double red[2 * 32];
+__device__ __forceinline__ void bi_scal1_fn(const SolveHeader& h, SolveResult& res, Recur& rc, zd r0q) {
     __shared__ int bad;
-    double s[2];
     if (threadIdx.x == 0) bad = 0;
-    reduce_partials<2>(st, s, red);
-    const zd r0q = {s[0], s[1]};
-    const zd delta = st->delta;
+    __syncthreads();
+    const zd delta = rc.delta;
     const zd beta = zneg(zdiv(delta, r0q));
-    const zd alpha = st->alpha, beta_prev = st->beta_prev;
+    const zd alpha = rc.alpha, beta_prev = rc.beta_prev;
     if (zzero(r0q) || zzero(delta) || !zfinite(r0q) || !zfinite(beta)) bad = 1;
-    const int na = st->res.nactive;
+    const int na = res.nactive;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        const int k = st->active[a];
-        const zd z = st->zeta[k], zp = st->zeta_prev[k];
-        const zd one_sb = {1.0 - st->h.sigma[k] * beta.re, -st->h.sigma[k] * beta.im};
+        const int k = rc.active[a];
+        const zd z = rc.zeta[k], zp = rc.zeta_prev[k];
+        const zd one_sb = {1.0 - h.sigma[k] * beta.re, -h.sigma[k] * beta.im};
         const zd den = zadd(zmul(zmul(beta, alpha), zsub(zp, z)), zmul(zmul(zp, beta_prev), one_sb));
         const zd zn = zdiv(zmul(zmul(z, zp), beta_prev), den);
         const zd bk = zdiv(zmul(beta, zn), z);
         if (zzero(den) || !zfinite(zn) || !zfinite(bk)) bad = 1;
-        st->zeta_new[k] = zn;
-        st->beta_k[k] = bk;
+        rc.zeta_new[k] = zn;
+        rc.beta_k[k] = bk;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        st->beta = beta;
-        if (bad) { st->res.status = MSOLVE_BREAKDOWN; st->res.done = 1; }
+        rc.beta = beta;
+        if (bad) { res.status = MSOLVE_BREAKDOWN; res.done = 1; }
     }
+    __syncthreads();
 }
+
 
 // s <- r + beta q
 template <typename E, int VEC>
-__global__ void __launch_bounds__(kThreads) k_bi_supdate(SolveState* st) {
-    if (st->res.done) return;
+__device__ __forceinline__ void bi_supdate_fn(const SolveHeader& h, const Recur& rc, int cta, int ncta) {
     typedef E C;
     typedef Pack<E, VEC> P;
-    const long long nvec = st->h.n / VEC;
-    const P* r = (const P*)st->h.r;
-    const P* q = (const P*)st->h.q;
-    P* s = (P*)st->h.s;
-    const C beta = cmake<C>(st->beta.re, st->beta.im);
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+    const long long nvec = h.n / VEC;
+    const P* r = (const P*)h.r;
+    const P* q = (const P*)h.q;
+    P* s = (P*)h.s;
+    const C beta = cmake<C>(rc.beta.re, rc.beta.im);
+    const long long stride = (long long)ncta * blockDim.x;
+    for (long long i = (long long)cta * blockDim.x + threadIdx.x; i < nvec; i += stride) {
         const P rv = ld_pack<false>(r + i), qv = ld_pack<false>(q + i);
         P sv;
 #pragma unroll
@@ -366,86 +380,91 @@ __global__ void __launch_bounds__(kThreads) k_bi_supdate(SolveState* st) {
     }
 }
 
-// after SpMV#2: chi, chi_k, rho'_k, delta' = -chi <r0,t>, alpha' = -beta delta'/(delta chi), alpha_k;
-// writes the 7 complex coefficients per active shift used by k_bi_update.
-__global__ void __launch_bounds__(kThreads) k_bi_scal2(SolveState* st) {
+template <typename E, int VEC>
+__global__ void __launch_bounds__(kThreads) k_bi_supdate(SolveState* st) {
     if (st->res.done) return;
-    __shared__ double red[5 * 32];
+    bi_supdate_fn<E, VEC>(st->h, st->rc, blockIdx.x, gridDim.x);
+}
+
+// after SpMV#2: chi, chi_k, rho'_k, delta' = -chi <r0,t>, alpha' = -beta delta'/(delta chi), alpha_k;
+// writes the 7 complex coefficients per active shift used by the fused update.  s5 = <t,s> (2), <t,t>, <r0,t> (2).
+__device__ __forceinline__ void bi_scal2_fn(const SolveHeader& h, SolveResult& res, Recur& rc, const double* s5) {
     __shared__ int bad;
-    double s[5];
     if (threadIdx.x == 0) bad = 0;
-    reduce_partials<5>(st, s, red);
-    const zd ts = {s[0], s[1]};
-    const double tt = s[2];
-    const zd r0t = {s[3], s[4]};
+    __syncthreads();
+    const zd ts = {s5[0], s5[1]};
+    const double tt = s5[2];
+    const zd r0t = {s5[3], s5[4]};
     const zd chi = {ts.re / tt, ts.im / tt};
-    const zd beta = st->beta, delta = st->delta;
+    const zd beta = rc.beta, delta = rc.delta;
     const zd delta_new = zneg(zmul(chi, r0t));               // <r0, s - chi t> with <r0,s> = 0
     const zd alpha_new = zneg(zdiv(zmul(beta, delta_new), zmul(delta, chi)));
     if (!(tt > 0.0) || !isfinite(tt) || !zfinite(ts) || zzero(chi) || !zfinite(alpha_new)) bad = 1;
-    const int na = st->res.nactive;
+    const int na = res.nactive;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        const int k = st->active[a];
-        const double sg = st->h.sigma[k];
+        const int k = rc.active[a];
+        const double sg = h.sigma[k];
         const zd one_cs = {1.0 + chi.re * sg, chi.im * sg};
         if (zzero(one_cs)) bad = 1;
         const zd chik = zdiv(chi, one_cs);
-        const zd rho = st->rho[k];
+        const zd rho = rc.rho[k];
         const zd rho_new = zdiv(rho, one_cs);
-        const zd zn = st->zeta_new[k], z = st->zeta[k], bk = st->beta_k[k];
+        const zd zn = rc.zeta_new[k], z = rc.zeta[k], bk = rc.beta_k[k];
         const zd ratio = zdiv(zn, z);
         const zd ak = zmul(alpha_new, zmul(ratio, ratio));
-        st->chi_k[k] = chik;
-        st->rho_new[k] = rho_new;
-        st->alpha_k[k] = ak;
+        rc.chi_k[k] = chik;
+        rc.rho_new[k] = rho_new;
+        rc.alpha_k[k] = ak;
         const zd cs = zmul(zmul(chik, rho), zn);             // x_k += cs * s
         const zd zr = zmul(zn, rho_new);                     // p_k = zr * r' + ...
         const zd cb = zdiv(chik, bk);
         const zd zs = zmul(zn, rho);                         // s^sigma = zs * s
         const zd zo = zmul(z, rho);                          // r^sigma = zo * r
         if (!zfinite(cs) || !zfinite(zr) || !zfinite(cb) || !zfinite(ak)) bad = 1;
-        double* c = st->coef + 14 * a;
+        double* c = rc.coef + 14 * a;
         c[0] = bk.re; c[1] = bk.im; c[2] = cs.re; c[3] = cs.im; c[4] = zr.re; c[5] = zr.im;
         c[6] = ak.re; c[7] = ak.im; c[8] = cb.re; c[9] = cb.im; c[10] = zs.re; c[11] = zs.im;
         c[12] = zo.re; c[13] = zo.im;
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        st->chi = chi;
-        st->delta_new = delta_new;
-        st->alpha_new = alpha_new;
-        if (bad) { st->res.status = MSOLVE_BREAKDOWN; st->res.done = 1; }
+        rc.chi = chi;
+        rc.delta_new = delta_new;
+        rc.alpha_new = alpha_new;
+        if (bad) { res.status = MSOLVE_BREAKDOWN; res.done = 1; }
     }
+    __syncthreads();
 }
+
 
 // The fused BiCGStab-M update: per element read r, s, t, q, p once;
 //   r' = s - chi t ; p <- r' + alpha'(p - chi q) ; |r'|^2 partials; per active shift
 //   x_k <- (x_k - beta_k p_k) + cs_k s ; p_k <- zr_k r' + alpha_k ( p_k - cb_k ( zs_k s - zo_k r ) ).
 template <typename E, int VEC, int UNR>
-__global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
-    if (st->res.done) return;
+__device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const SolveResult& res, const Recur& rc, int cta, int ncta) {
     typedef E C;
     typedef Pack<E, VEC> P;
     __shared__ C s_c[kMaxShifts * 7];
     __shared__ int s_k[kMaxShifts];
-    const int na = st->res.nactive;
-    const bool first = st->res.n_iter == 0;
-    for (int a = threadIdx.x; a < na; a += blockDim.x) s_k[a] = st->active[a];
-    for (int j = threadIdx.x; j < 7 * na; j += blockDim.x) s_c[j] = cmake<C>(st->coef[2 * j], st->coef[2 * j + 1]);
-    const C chi = cmake<C>(st->chi.re, st->chi.im);
-    const C alpha_new = cmake<C>(st->alpha_new.re, st->alpha_new.im);
+    const int na = res.nactive;
+    const bool first = res.n_iter == 0;
     __syncthreads();
-    const long long n = st->h.n, nvec = n / VEC, pks = st->h.pk_stride;
-    P* r = (P*)st->h.r;
-    P* p = (P*)st->h.p;
-    const P* s = (const P*)st->h.s;
-    const P* t = (const P*)st->h.t;
-    const P* q = (const P*)st->h.q;
-    C* x = (C*)st->h.x;
-    C* pk = (C*)st->h.pk;
-    double acc[1] = {0.0};
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+    for (int a = threadIdx.x; a < na; a += blockDim.x) s_k[a] = rc.active[a];
+    for (int j = threadIdx.x; j < 7 * na; j += blockDim.x) s_c[j] = cmake<C>(rc.coef[2 * j], rc.coef[2 * j + 1]);
+    const C chi = cmake<C>(rc.chi.re, rc.chi.im);
+    const C alpha_new = cmake<C>(rc.alpha_new.re, rc.alpha_new.im);
+    __syncthreads();
+    const long long n = h.n, nvec = n / VEC, pks = h.pk_stride;
+    P* r = (P*)h.r;
+    P* p = (P*)h.p;
+    const P* s = (const P*)h.s;
+    const P* t = (const P*)h.t;
+    const P* q = (const P*)h.q;
+    C* x = (C*)h.x;
+    C* pk = (C*)h.pk;
+    double acc = 0.0;
+    const long long stride = (long long)ncta * blockDim.x;
+    for (long long i = (long long)cta * blockDim.x + threadIdx.x; i < nvec; i += stride) {
         const P rv = ld_pack<false>(r + i), sv = ld_pack<false>(s + i), tv = ld_pack<false>(t + i);
         const P qv = ld_pack<false>(q + i);
         P pv0 = ld_pack<false>(p + i);
@@ -454,7 +473,7 @@ __global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
         for (int e = 0; e < VEC; ++e) {
             rn.v[e] = csub(sv.v[e], cmul(chi, tv.v[e]));
             pv0.v[e] = cadd(rn.v[e], cmul(alpha_new, csub(pv0.v[e], cmul(chi, qv.v[e]))));
-            acc[0] += cnorm2(rn.v[e]);
+            acc += cnorm2(rn.v[e]);
         }
         for (int a0 = 0; a0 < na; a0 += UNR) {
             P xv[UNR], pv[UNR];
@@ -488,6 +507,13 @@ __global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
         st_pack<false>(r + i, rn);
         st_pack<false>(p + i, pv0);
     }
+    return acc;
+}
+
+template <typename E, int VEC, int UNR>
+__global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
+    if (st->res.done) return;
+    double acc[1] = {bi_update_fn<E, VEC, UNR>(st->h, st->res, st->rc, blockIdx.x, gridDim.x)};
     __shared__ double red[32];
     block_sum<1>(acc, red);
     if (threadIdx.x == 0) {
@@ -497,52 +523,48 @@ __global__ void __launch_bounds__(kThreads) k_bi_update(SolveState* st) {
 }
 
 // end of iteration: |r'|^2 -> shuffle zeta/rho/delta/alpha/beta, per-shift stop test, loop control.
-__global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraphConditionalHandle cond, int use_cond) {
-    if (st->res.done) { if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, 0); return; }
-    __shared__ double red[32];
-    double s[1];
-    reduce_partials<1>(st, s, red);
-    const double rr = s[0];
-    const int na = st->res.nactive;
-    const int it = st->res.n_iter + 1;
-    const double rnorm = sqrt(rr), bnorm = st->bnorm, tol = st->h.tol;
-    const bool force = st->h.force_all != 0, base_rule = st->h.stop_rule == 1, psn = st->h.per_shift_norm != 0;
+__device__ __forceinline__ void bi_scal3_fn(const SolveHeader& h, SolveResult& res, Recur& rc, const double* rhs_norm,
+                                            double rr, double* hist) {
+    const int na = res.nactive;
+    const int it = res.n_iter + 1;
+    const double rnorm = sqrt(rr), bnorm = rc.bnorm, tol = h.tol;
+    const bool force = h.force_all != 0, base_rule = h.stop_rule == 1, psn = h.per_shift_norm != 0;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        const int k = st->active[a];
-        const zd zn = st->zeta_new[k], rn = st->rho_new[k];
-        st->zeta_prev[k] = st->zeta[k];
-        st->zeta[k] = zn;
-        st->rho[k] = rn;
+        const int k = rc.active[a];
+        const zd zn = rc.zeta_new[k], rn = rc.rho_new[k];
+        rc.zeta_prev[k] = rc.zeta[k];
+        rc.zeta[k] = zn;
+        rc.rho[k] = rn;
         const double zr = zabs(zmul(zn, rn));
-        const double nk = psn ? st->rhs_norm[k] : bnorm;
-        st->res.relres[k] = zr * rnorm / nk;
-        if (!force && (base_rule ? rnorm : zr * rnorm) <= tol * nk) st->res.conv_iter[k] = it;
-    }
-    // msolve_set_history: row it-1 = beta, chi, alpha' (complex), |r'|^2, 0, then zeta_new[S], beta_k[S], chi_k[S] (complex)
-    if (st->h.hist && it <= st->h.hist_cap) {
-        __syncthreads();
-        const int S = st->h.S;
-        double* h = st->h.hist + (size_t)(it - 1) * (size_t)(8 + 6 * S);
-        if (threadIdx.x == 0) {
-            h[0] = st->beta.re; h[1] = st->beta.im; h[2] = st->chi.re; h[3] = st->chi.im;
-            h[4] = st->alpha_new.re; h[5] = st->alpha_new.im; h[6] = rr; h[7] = 0.0;
-        }
-        for (int k = threadIdx.x; k < S; k += blockDim.x) {
-            h[8 + 2 * k] = st->zeta_new[k].re; h[8 + 2 * k + 1] = st->zeta_new[k].im;
-            h[8 + 2 * S + 2 * k] = st->beta_k[k].re; h[8 + 2 * S + 2 * k + 1] = st->beta_k[k].im;
-            h[8 + 4 * S + 2 * k] = st->chi_k[k].re; h[8 + 4 * S + 2 * k + 1] = st->chi_k[k].im;
-        }
+        const double nk = psn ? rhs_norm[k] : bnorm;
+        res.relres[k] = zr * rnorm / nk;
+        if (!force && (base_rule ? rnorm : zr * rnorm) <= tol * nk) res.conv_iter[k] = it;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        st->R1 = rr;
-        st->delta = st->delta_new;
-        st->alpha = st->alpha_new;
-        st->beta_prev = st->beta;
-        st->res.n_iter = it;
-        finish_iteration(st, !isfinite(rr));
-        if (use_cond) cudaGraphSetConditional(cond, st->res.done ? 0u : 1u);
+    // msolve_set_history: row it-1 = beta, chi, alpha' (complex), |r'|^2, 0, then zeta_new[S], beta_k[S], chi_k[S] (complex)
+    if (hist && it <= h.hist_cap) {
+        const int S = h.S;
+        double* hr = hist + (size_t)(it - 1) * (size_t)(8 + 6 * S);
+        if (threadIdx.x == 0) {
+            hr[0] = rc.beta.re; hr[1] = rc.beta.im; hr[2] = rc.chi.re; hr[3] = rc.chi.im;
+            hr[4] = rc.alpha_new.re; hr[5] = rc.alpha_new.im; hr[6] = rr; hr[7] = 0.0;
+        }
+        for (int k = threadIdx.x; k < S; k += blockDim.x) {
+            hr[8 + 2 * k] = rc.zeta_new[k].re; hr[8 + 2 * k + 1] = rc.zeta_new[k].im;
+            hr[8 + 2 * S + 2 * k] = rc.beta_k[k].re; hr[8 + 2 * S + 2 * k + 1] = rc.beta_k[k].im;
+            hr[8 + 4 * S + 2 * k] = rc.chi_k[k].re; hr[8 + 4 * S + 2 * k + 1] = rc.chi_k[k].im;
+        }
     }
+    if (threadIdx.x == 0) {
+        rc.R1 = rr;
+        rc.delta = rc.delta_new;
+        rc.alpha = rc.alpha_new;
+        rc.beta_prev = rc.beta;
+        res.n_iter = it;
+        finish_iteration(h, res, rc, !isfinite(rr));
+    }
+    __syncthreads();
 }
+
 
 }  // namespace msolve

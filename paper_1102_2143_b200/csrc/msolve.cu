@@ -144,6 +144,21 @@ static int build_graph(msolve_matrix* A, int alg) {
     return MSOLVE_OK;
 }
 
+// AUTO rule of MSOLVE_CFG_MATRIX_L2: keep the matrix in L2 (evict-last bulk copies) when the matrix and the two
+// SpMV vectors take at most kMatKeepBytes of the 126 MB L2
+constexpr size_t kMatKeepBytes = (size_t)96 << 20;
+// AUTO rule of MSOLVE_CFG_ITER_PATH: one cooperative kernel per solve up to this working set (profiles/r02_sweeps.md)
+constexpr size_t kFusedMaxBytes = (size_t)40 << 20;
+static size_t matrix_bytes(const msolve_matrix* A) {
+    const size_t e = elem_bytes(A->dtype);
+    if (A->format == FMT_BSR3) return (size_t)A->dev.nnz * (9 * e + 4) + (size_t)(A->dev.nbrows + 1) * 4;
+    if (A->format == FMT_LATTICE) return (size_t)A->dev.nnz * 9 * e;
+    return (size_t)A->dev.nnz * (e + 4) + (size_t)(A->dev.n + 1) * 4;
+}
+static bool matrix_fits_l2(const msolve_matrix* A) {
+    return matrix_bytes(A) + 2 * (size_t)A->dev.n * elem_bytes(A->dtype) <= kMatKeepBytes;
+}
+
 // ------------------------------------------------------------------------------------- create
 static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t stream) {
     (void)stream;
@@ -153,6 +168,7 @@ static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t str
     CU(cudaMemset(A->d_state, 0, sizeof(SolveState)));
     CU(cudaMallocHost((void**)&A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult)));
     CU(cudaStreamCreateWithFlags(&A->capture_stream, cudaStreamNonBlocking));
+    A->dev.mat_keep = matrix_fits_l2(A);
     *out = A;
     return MSOLVE_OK;
 }
@@ -404,6 +420,12 @@ extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
     if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { A->opt.update_kernel = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { A->opt.lattice_kernel = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_STOP_RULE && (value == 0 || value == 1)) { A->opt.stop_rule = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_ITER_PATH && value >= 0 && value <= 2) { A->opt.iter_path = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_MATRIX_L2 && value >= 0 && value <= 2) {
+        A->opt.matrix_l2 = value;
+        A->dev.mat_keep = value == 2 || (value == 0 && matrix_fits_l2(A));
+        return MSOLVE_OK;
+    }
     if (key == MSOLVE_CFG_X_WINDOW && (value == 0 || value == 1)) {
         if (value == 1) {
             if (A->format != FMT_CSR || A->kernel != KERNEL_VECTOR) return fail(MSOLVE_EINVAL, "msolve_config: MSOLVE_CFG_X_WINDOW applies to the vector-CSR kernel");
@@ -504,6 +526,30 @@ int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const 
         return A->dev.n == 0 ? MSOLVE_OK : MSOLVE_MAXITER;
     }
     const int mode = A->opt.loop_mode;
+    // Systems that live in L2 are bound by launch latency, not bytes: the whole solve runs as ONE cooperative
+    // kernel (fused_small.cu).  AUTO: matrix + (4 + 2 S) vectors at most kFusedMaxBytes.
+    const bool fused = A->opt.iter_path == 2 ||
+                       (A->opt.iter_path == 0 && fused_supported(A) &&
+                        matrix_bytes(A) + (size_t)(4 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kFusedMaxBytes);
+    if (fused) {
+        if (!fused_supported(A)) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 2 needs a vector-CSR, BSR3 or lattice handle, the register update kernel and the WHILE loop mode");
+        CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
+        rc = launch_fused(A, alg, stream);
+        if (rc != MSOLVE_OK) return rc;
+        CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
+        CU(cudaStreamSynchronize(stream));
+        if (hr->zero_rhs || (hr->status == MSOLVE_BREAKDOWN && hr->n_iter == 0)) {
+            CU(cudaMemsetAsync(d_x, 0, xbytes, stream));
+            CU(cudaStreamSynchronize(stream));
+        }
+        A->last_launches = 1;
+        if (h_iterations) *h_iterations = hr->n_iter;
+        for (int k = 0; k < S; ++k) {
+            if (h_conv_iter) h_conv_iter[k] = hr->conv_iter[k];
+            if (h_relres) h_relres[k] = hr->relres[k];
+        }
+        return hr->status;
+    }
     rc = build_graph(A, alg);
     if (rc != MSOLVE_OK) return rc;
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));

@@ -20,11 +20,15 @@ namespace msolve {
 template <int ROLE> struct RoleAcc { static constexpr int value = ROLE == ROLE_CG ? 1 : (ROLE == ROLE_B2 ? 5 : 2); };
 
 template <typename C, int ROLE>
+__device__ __forceinline__ void role_vectors_h(const SolveHeader& h, const C*& x, C*& y, const C*& u) {
+    if (ROLE == ROLE_CG)  { x = (const C*)h.p; y = (C*)h.q; u = nullptr; }
+    if (ROLE == ROLE_B1)  { x = (const C*)h.p; y = (C*)h.q; u = (const C*)h.b; }
+    if (ROLE == ROLE_B2)  { x = (const C*)h.s; y = (C*)h.t; u = (const C*)h.b; }
+    if (ROLE == ROLE_GEN) { x = (const C*)h.sp_x; y = (C*)h.sp_y; u = (const C*)h.sp_u; }
+}
+template <typename C, int ROLE>
 __device__ __forceinline__ void role_vectors(const SolveState* st, const C*& x, C*& y, const C*& u) {
-    if (ROLE == ROLE_CG)  { x = (const C*)st->h.p; y = (C*)st->h.q; u = nullptr; }
-    if (ROLE == ROLE_B1)  { x = (const C*)st->h.p; y = (C*)st->h.q; u = (const C*)st->h.b; }
-    if (ROLE == ROLE_B2)  { x = (const C*)st->h.s; y = (C*)st->h.t; u = (const C*)st->h.b; }
-    if (ROLE == ROLE_GEN) { x = (const C*)st->h.sp_x; y = (C*)st->h.sp_y; u = (const C*)st->h.sp_u; }
+    role_vectors_h<C, ROLE>(st->h, x, y, u);
 }
 
 // Fused reductions for one finished row (all accumulation in fp64, R14).
@@ -63,13 +67,11 @@ __device__ __forceinline__ void write_partials(SolveState* st, double (&acc)[NAC
 // row read consecutive non-zeros (coalesced 16-byte values, 4-byte indices).  For short regular
 // lattice rows (27 nnz: LANES = 8, four passes).
 // ------------------------------------------------------------------------------------------
-template <typename E, int LANES, int ROLE, bool PIN>
-__global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveState* st) {
+// NC = false: the gathered vector was written earlier in the SAME kernel launch (fused_small.cuh), so it must not go
+// through the non-coherent load path; the matrix arrays always may.
+template <typename E, int LANES, int ROLE, bool PIN, bool NC = true>
+__device__ __forceinline__ void csr_vector_body(const MatDev& A, const E* x, E* y, const E* u, double* acc, int cta, int ncta) {
     typedef E C;
-    constexpr int NACC = RoleAcc<ROLE>::value;
-    if (ROLE != ROLE_GEN && st->res.done) return;
-    const C* x; C* y; const C* u;
-    role_vectors<C, ROLE>(st, x, y, u);
     const C* __restrict__ val = (const C*)A.val;
     const int32_t* __restrict__ colidx = A.colidx;
     const int32_t* __restrict__ rowptr = A.rowptr;
@@ -78,11 +80,8 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
     const uint64_t polx = policy_evict_last(), polm = policy_evict_first();
     const int lane = threadIdx.x & 31;
     const int sub = lane % LANES;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
-    double acc[NACC];
-#pragma unroll
-    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    const long long warp = ((long long)cta * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)ncta * blockDim.x) >> 5;
     for (long long base = warp * RPW; base < A.n; base += nwarps * RPW) {
         const long long row = base + lane / LANES;
         const bool valid = row < A.n;
@@ -93,7 +92,7 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
         for (; j < e; j += LANES) {
             const int c = ld_mat<HINT>(colidx + j, polm);
             const C v = ld_mat<HINT>(val + j, polm);
-            sum = cfma(v, ld_xg<PIN>(x + c, polx), sum);
+            sum = cfma(v, NC ? ld_xg<PIN>(x + c, polx) : x[c], sum);
         }
 #pragma unroll
         for (int o = LANES / 2; o > 0; o >>= 1) sum = cshfl_xor_add(sum, o);
@@ -102,6 +101,19 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
             role_epilogue<C, ROLE>(acc, row, sum, x, u);
         }
     }
+}
+
+template <typename E, int LANES, int ROLE, bool PIN>
+__global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveState* st) {
+    typedef E C;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    csr_vector_body<E, LANES, ROLE, PIN>(A, x, y, u, acc, blockIdx.x, gridDim.x);
     write_partials<NACC>(st, acc);
 }
 
@@ -110,21 +122,14 @@ __global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveSta
 // block row br and multiplies row r of every 3x3 block with the 3-vector x[3*bcol .. +3].
 // The three threads of a block row read one contiguous 144-byte (c128) block between them.
 // ------------------------------------------------------------------------------------------
-template <typename E, int ROLE>
-__global__ void __launch_bounds__(kThreads) k_spmv_bsr3_rows(MatDev A, SolveState* st) {
+template <typename E, int ROLE, bool NC = true>
+__device__ __forceinline__ void bsr3_rows_body(const MatDev& A, const E* x, E* y, const E* u, double* acc, int cta, int ncta) {
     typedef E C;
-    constexpr int NACC = RoleAcc<ROLE>::value;
-    if (ROLE != ROLE_GEN && st->res.done) return;
-    const C* x; C* y; const C* u;
-    role_vectors<C, ROLE>(st, x, y, u);
     const C* __restrict__ val = (const C*)A.val;
     const int32_t* __restrict__ bcol = A.colidx;
     const int32_t* __restrict__ browptr = A.rowptr;
-    double acc[NACC];
-#pragma unroll
-    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long row = (long long)blockIdx.x * blockDim.x + threadIdx.x; row < A.n; row += stride) {
+    const long long stride = (long long)ncta * blockDim.x;
+    for (long long row = (long long)cta * blockDim.x + threadIdx.x; row < A.n; row += stride) {
         const long long br = row / 3;
         const int rr = (int)(row - 3 * br);
         const int jb = browptr[br], je = browptr[br + 1];
@@ -134,13 +139,26 @@ __global__ void __launch_bounds__(kThreads) k_spmv_bsr3_rows(MatDev A, SolveStat
             const C* blk = val + (long long)j * 9 + rr * 3;
             const C* xv = x + 3ll * bcol[j];
             const C a0 = ld_stream(blk), a1 = ld_stream(blk + 1), a2 = ld_stream(blk + 2);
-            sum = cfma(a0, ld_ro(xv), sum);
-            sum = cfma(a1, ld_ro(xv + 1), sum);
-            sum = cfma(a2, ld_ro(xv + 2), sum);
+            sum = cfma(a0, NC ? ld_ro(xv) : xv[0], sum);
+            sum = cfma(a1, NC ? ld_ro(xv + 1) : xv[1], sum);
+            sum = cfma(a2, NC ? ld_ro(xv + 2) : xv[2], sum);
         }
         y[row] = sum;
         role_epilogue<C, ROLE>(acc, row, sum, x, u);
     }
+}
+
+template <typename E, int ROLE>
+__global__ void __launch_bounds__(kThreads) k_spmv_bsr3_rows(MatDev A, SolveState* st) {
+    typedef E C;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    bsr3_rows_body<E, ROLE>(A, x, y, u, acc, blockIdx.x, gridDim.x);
     write_partials<NACC>(st, acc);
 }
 
@@ -231,7 +249,8 @@ __global__ void __launch_bounds__(BsrTmaCfg<E, TB>::kThreadsTotal, CPS) k_spmv_b
     if (threadIdx.x >= NCT) {
         // ---------------- producer: one elected lane of the last warp
         if (threadIdx.x == NCT) {
-            const uint64_t pol = policy_evict_first();
+            // the matrix is read once per SpMV: evict-first, unless it is small enough to stay in L2 between SpMVs
+            const uint64_t pol = A.mat_keep ? policy_evict_last() : policy_evict_first();
             const C* __restrict__ val = (const C*)A.val;
             int t = blockIdx.x;
             int4 e = t < ntiles ? tiles[t] : make_int4(0, 0, 0, 0);

@@ -47,23 +47,16 @@ __device__ __forceinline__ C lat_combine(T dg, C xi, T cf, C f, T cb, C g) {
 // ------------------------------------------------------------------------------------------
 // Fallback (any extents): one thread per scalar row, operands through L1/L2.
 // ------------------------------------------------------------------------------------------
-template <typename E, int ROLE>
-__global__ void __launch_bounds__(kThreads) k_spmv_lat_rows(MatDev A, SolveState* st) {
+template <typename E, int ROLE, bool NC = true>
+__device__ __forceinline__ void lat_rows_body(const MatDev& A, const E* x, E* y, const E* u, double* acc, int cta, int ncta) {
     typedef E C;
     typedef typename RealOf<E>::type T;
-    constexpr int NACC = RoleAcc<ROLE>::value;
-    if (ROLE != ROLE_GEN && st->res.done) return;
-    const C* x; C* y; const C* u;
-    role_vectors<C, ROLE>(st, x, y, u);
     const C* __restrict__ links = (const C*)A.val;
     const long long vol = A.lat_vol;
     const int nd = A.lat_ndim;
     const T dg = (T)A.lat_diag, cf = (T)A.lat_cf, cb = (T)A.lat_cb;
-    double acc[NACC];
-#pragma unroll
-    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long row = (long long)blockIdx.x * blockDim.x + threadIdx.x; row < A.n; row += stride) {
+    const long long stride = (long long)ncta * blockDim.x;
+    for (long long row = (long long)cta * blockDim.x + threadIdx.x; row < A.n; row += stride) {
         const long long s = row / 3;
         const int r = (int)(row - 3 * s);
         C f = cmake<C>(0.0, 0.0), g = f;
@@ -78,20 +71,33 @@ __global__ void __launch_bounds__(kThreads) k_spmv_lat_rows(MatDev A, SolveState
             const long long sb = s + (c == 0 ? (long long)(L - 1) * str : -str);
             const C* U = links + ((long long)mu * vol + s) * 9 + 3 * r;      // row r of U_mu(s)
             const C* xf = x + 3 * sf;
-            f = cfma(ld_ro(U), ld_ro(xf), f);
-            f = cfma(ld_ro(U + 1), ld_ro(xf + 1), f);
-            f = cfma(ld_ro(U + 2), ld_ro(xf + 2), f);
+            f = cfma(ld_ro(U), NC ? ld_ro(xf) : xf[0], f);
+            f = cfma(ld_ro(U + 1), NC ? ld_ro(xf + 1) : xf[1], f);
+            f = cfma(ld_ro(U + 2), NC ? ld_ro(xf + 2) : xf[2], f);
             const C* V = links + ((long long)mu * vol + sb) * 9 + r;         // column r of U_mu(s-mu)
             const C* xb = x + 3 * sb;
-            g = cfma_conj(ld_ro(V), ld_ro(xb), g);
-            g = cfma_conj(ld_ro(V + 3), ld_ro(xb + 1), g);
-            g = cfma_conj(ld_ro(V + 6), ld_ro(xb + 2), g);
+            g = cfma_conj(ld_ro(V), NC ? ld_ro(xb) : xb[0], g);
+            g = cfma_conj(ld_ro(V + 3), NC ? ld_ro(xb + 1) : xb[1], g);
+            g = cfma_conj(ld_ro(V + 6), NC ? ld_ro(xb + 2) : xb[2], g);
             str *= L;
         }
-        const C sum = lat_combine(dg, ld_ro(x + row), cf, f, cb, g);
+        const C sum = lat_combine(dg, NC ? ld_ro(x + row) : x[row], cf, f, cb, g);
         y[row] = sum;
         role_epilogue<C, ROLE>(acc, row, sum, x, u);
     }
+}
+
+template <typename E, int ROLE>
+__global__ void __launch_bounds__(kThreads) k_spmv_lat_rows(MatDev A, SolveState* st) {
+    typedef E C;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    lat_rows_body<E, ROLE>(A, x, y, u, acc, blockIdx.x, gridDim.x);
     write_partials<NACC>(st, acc);
 }
 

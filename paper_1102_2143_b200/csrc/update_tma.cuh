@@ -64,10 +64,10 @@ __global__ void __launch_bounds__(UpdTmaCfg<E>::kThreadsTotal, 1) k_cgm_update_t
     const int na = st->res.nactive;
     const bool first = st->res.n_iter == 0;
     for (int a = threadIdx.x; a < na; a += blockDim.x) {
-        s_k[a] = st->active[a];
-        s_zeta[a] = (T)st->coef[3 * a + 0];
-        s_alpha[a] = (T)st->coef[3 * a + 1];
-        s_beta[a] = (T)st->coef[3 * a + 2];
+        s_k[a] = st->rc.active[a];
+        s_zeta[a] = (T)st->rc.coef[3 * a + 0];
+        s_alpha[a] = (T)st->rc.coef[3 * a + 1];
+        s_beta[a] = (T)st->rc.coef[3 * a + 2];
     }
     if (threadIdx.x == 0) {
         for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, Cfg::kWarps); }
@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(UpdTmaCfg<E>::kThreadsTotal, 1) k_cgm_update_t
         constexpr int SL = Cfg::kTile / Cfg::kWarps;              // packs per warp slice
         constexpr int PPL = SL / 32;                              // packs per lane
         const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-        const T beta = (T)st->beta.re;
+        const T beta = (T)st->rc.beta.re;
         const uint64_t pol = policy_evict_first(), polr = policy_evict_normal();
         int rel_stage = 0;                                        // next stage to hand back (LAG items behind)
         long long items = 0;

@@ -7,6 +7,57 @@
 
 namespace msolve {
 
+// ---- the one-CTA scalar kernels: fixed-order sum of the per-CTA partials, then the recurrence step (kernels.cuh).
+// `cond` is the WHILE node's handle (use_cond = 0 in chunked mode).
+__global__ void __launch_bounds__(kThreads) k_init_state(SolveState* st) {
+    __shared__ double red[32];
+    double s[1];
+    reduce_partials<1>(st, s, red);
+    init_state_fn(st->h, st->res, st->rc, s[0]);
+}
+
+__global__ void __launch_bounds__(kThreads) k_cgm_scal1(SolveState* st) {
+    if (st->res.done) return;
+    __shared__ double red[32];
+    double s[1];
+    reduce_partials<1>(st, s, red);
+    cgm_scal1_fn(st->h, st->res, st->rc, s[0]);
+}
+
+__global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGraphConditionalHandle cond, int use_cond) {
+    if (st->res.done) { if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, 0); return; }
+    __shared__ double red[32];
+    double s[1];
+    reduce_partials<1>(st, s, red);
+    cgm_scal2_fn(st->h, st->res, st->rc, st->rhs_norm, s[0], st->h.hist);
+    if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, st->res.done ? 0u : 1u);
+}
+
+__global__ void __launch_bounds__(kThreads) k_bi_scal1(SolveState* st) {
+    if (st->res.done) return;
+    __shared__ double red[2 * 32];
+    double s[2];
+    reduce_partials<2>(st, s, red);
+    bi_scal1_fn(st->h, st->res, st->rc, zd{s[0], s[1]});
+}
+
+__global__ void __launch_bounds__(kThreads) k_bi_scal2(SolveState* st) {
+    if (st->res.done) return;
+    __shared__ double red[5 * 32];
+    double s[5];
+    reduce_partials<5>(st, s, red);
+    bi_scal2_fn(st->h, st->res, st->rc, s);
+}
+
+__global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraphConditionalHandle cond, int use_cond) {
+    if (st->res.done) { if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, 0); return; }
+    __shared__ double red[32];
+    double s[1];
+    reduce_partials<1>(st, s, red);
+    bi_scal3_fn(st->h, st->res, st->rc, st->rhs_norm, s[0], st->h.hist);
+    if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, st->res.done ? 0u : 1u);
+}
+
 // element-wise kernels: 16 bytes (1, 2 or 4 elements) per access when the length allows it
 static bool vec16(const msolve_matrix* A) { return A->dev.n % (long long)(16 / elem_bytes(A->dtype)) == 0; }
 

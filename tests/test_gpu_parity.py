@@ -34,7 +34,10 @@ FORCED_CFG = {}     # msolve_config options applied to every handle make_matrix 
 
 def make_matrix(ms, w, dtype, fmt, flags=0, cfg=None):
     A = _create(ms, w, dtype, fmt, flags)
-    for key, value in list(FORCED_CFG.items()) + list((cfg or {}).items()):
+    # The tests of this file exercise the iteration as a graph of kernels at every size (by default the library
+    # would run systems this small as one cooperative kernel: tests/test_gpu_fused.py covers that path).
+    base = {ms.MSOLVE_CFG_ITER_PATH: 1}
+    for key, value in list(base.items()) + list(FORCED_CFG.items()) + list((cfg or {}).items()):
         ms.msolve_config(A, key, value)
     return A
 
@@ -377,7 +380,8 @@ def test_max_shifts_and_too_many(ms):
     ms.msolve_destroy(A)
 
 
-def test_breakdown_reported(ms):
+@pytest.mark.parametrize("path", [1, 2], ids=["graph", "fused"])
+def test_breakdown_reported(ms, path):
     # indefinite A: <p,Ap> < 0 in the first loop body (R16).  The iterate at that point is x_k = 0, which is what
     # the oracle returns; d_x must be fully overwritten with it (include/msolve.h), not left as the caller had it.
     n = 64
@@ -386,6 +390,7 @@ def test_breakdown_reported(ms):
     val = -np.ones(n, dtype=np.complex128)
     b = W.unit_rhs(1, n)
     A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, path)
     x = torch.full((2, n), 7.0, dtype=torch.complex128, device="cuda")
     res = ms.msolve_cgm(A, dev(b), [0.0, 0.5], 1e-10, 10, x=x)
     o = oracle.cgm(rowptr, colidx, val, b, [0.0, 0.5], 1e-10, 10)
@@ -400,6 +405,7 @@ def test_breakdown_reported(ms):
     b2 = np.zeros(n, dtype=np.complex128)
     b2[::2] = W.unit_rhs(2, n // 2)
     A = ms.msolve_create_csr(dev(rp2), dev(ci2), dev(v2))
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, path)
     x.fill_(7.0)
     res = ms.msolve_bicgstabm(A, dev(b2), [0.0, 0.5], 1e-10, 10, x=x)
     o = oracle.bicgstabm(rp2, ci2, v2, b2, [0.0, 0.5], 1e-10, 10)
@@ -413,6 +419,7 @@ def test_breakdown_reported(ms):
     c = 2.5
     val = np.full(n, c, dtype=np.complex128)
     A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, path)
     x.fill_(7.0)
     res = ms.msolve_bicgstabm(A, dev(b), [0.0, 0.5], 1e-10, 10, x=x)
     xg = res.x.cpu().numpy()
@@ -431,6 +438,7 @@ def test_breakdown_reported(ms):
     bb[n // 2:] = 0.5
     bb /= np.linalg.norm(bb)
     A = ms.msolve_create_csr(dev(rowptr), dev(colidx), dev(val))
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, path)
     res = ms.msolve_cgm(A, dev(bb), [0.0], 1e-10, 10)
     o = oracle.cgm(rowptr, colidx, val, bb, [0.0], 1e-10, 10)
     assert res.status == o.status and res.iterations == o.iterations

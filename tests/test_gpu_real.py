@@ -31,6 +31,8 @@ def dev(a):
 
 def solve_both(ms, w, dtype, flags, tol):
     A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), flags)
+    if flags == 1:      # VECTOR by name: through the graph of kernels (AUTO, flags = 0, takes the one-kernel path at these sizes)
+        ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, 1)
     fn, ofn = (ms.msolve_cgm, oracle.cgm) if w.algorithm == "cgm" else (ms.msolve_bicgstabm, oracle.bicgstabm)
     g = fn(A, dev(w.b.astype(dtype)), w.shifts, tol, w.max_iter)
     x = g.x.cpu().numpy()
@@ -64,7 +66,7 @@ def test_spmv_real(ms, dtype, flags):
     ms.msolve_destroy(A)
 
 
-@pytest.mark.parametrize("flags", [0, 2, 3])
+@pytest.mark.parametrize("flags", [0, 1, 2, 3])
 @pytest.mark.parametrize("dtype,shape", [(np.float64, (64, 48)), (np.float64, (37, 29)), (np.float32, (24, 20)),
                                          (np.float32, (23, 19))])
 def test_poisson_cgm_real(ms, dtype, shape, flags):
