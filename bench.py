@@ -248,7 +248,7 @@ def config_dict(args, w, dtype, fmt, world, S, shifts_total):
     return {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
             "shifts": S, "tol": w.tol,
             "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world,
-            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "iter_path": args.iter_path, "l2": l2_note}
+            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
 
 
 def run_reference(args, rank):
@@ -301,6 +301,7 @@ def main():
     ap.add_argument("--iter-path", default="auto", choices=["auto", "graph", "fused"],
                     help="graph: iteration as a CUDA graph of kernels; fused: whole solve in one cooperative kernel "
                          "(L2-resident systems); auto: by footprint (MSOLVE_CFG_ITER_PATH)")
+    ap.add_argument("--fused-ctas", type=int, default=0, help="CTAs of the one-kernel path (0 = by problem size)")
     ap.add_argument("--matrix-l2", default="auto", choices=["auto", "stream", "keep"],
                     help="L2 policy of the matrix stream (MSOLVE_CFG_MATRIX_L2)")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "shifts"],
@@ -367,6 +368,7 @@ def main():
     if args.x_window:
         ms.msolve_config(A, ms.MSOLVE_CFG_X_WINDOW, 1)
     ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, {"auto": 0, "graph": 1, "fused": 2}[args.iter_path])
+    ms.msolve_config(A, ms.MSOLVE_CFG_FUSED_CTAS, args.fused_ctas)
     ms.msolve_config(A, ms.MSOLVE_CFG_MATRIX_L2, {"auto": 0, "stream": 1, "keep": 2}[args.matrix_l2])
     S = int(w.shifts.size)
     b_host = torch.from_numpy(w.b.astype(dtype)).pin_memory()

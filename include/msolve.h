@@ -87,17 +87,19 @@ enum {
     MSOLVE_CFG_X_WINDOW = 4 /* vector-CSR kernel only: 1 = every SpMV launch carries an L2 access-policy window over the
                                gathered vector (persisting hits; sets the device-wide persisting-L2 set-aside).
                                Measured on B200, config 5: profiles/r02_sweeps.md; default 0 */,
-    MSOLVE_CFG_MATRIX_L2 = 5 /* L2 policy of the matrix stream of the TMA-staged SpMV kernels: 0 = by footprint (default:
-                                evict-last when matrix + 2 vectors fit in 96 MB of the 126 MB L2, so that the second
-                                SpMV of a BiCGStab-M iteration and the next iteration find it there; evict-first
-                                otherwise: read once per SpMV), 1 = always evict-first, 2 = always evict-last */,
+    MSOLVE_CFG_MATRIX_L2 = 5 /* L2 policy of the matrix stream of the TMA-staged SpMV kernels: 0 / 1 = evict-first (default:
+                                the matrix is read once per SpMV), 2 = evict-last.  Keeping a matrix that fits in L2
+                                (config 3: 88 MB of 126 MB) was measured and is slower: 11.4k -> 9.9k iterations/s
+                                (profiles/r02_sweeps.md); the option stays for that measurement */,
     MSOLVE_CFG_ITER_PATH = 6 /* how a solve is driven: 1 = the iteration as a CUDA graph of kernels looping on the device
                                 (one kernel per step of Alg. 1; HBM-bound sizes), 2 = the WHOLE solve as one cooperative
                                 kernel with grid-wide barriers between the steps (systems that live in L2, where kernel
                                 launches, not bytes, are the cost; vector-CSR, BSR3 and lattice handles), 0 = by
                                 footprint (default): 2 when matrix + (4 + 2 nshifts) vectors take at most 40 MB.
                                 Same arithmetic step for step; the two paths group the dot products differently
-                                (per-CTA partials of different grids), so they agree to rounding, not bit for bit */
+                                (per-CTA partials of different grids), so they agree to rounding, not bit for bit */,
+    MSOLVE_CFG_FUSED_CTAS = 7 /* CTAs of the cooperative kernel of MSOLVE_CFG_ITER_PATH = 2: 0 = by problem size
+                                 (default), else that many (at most one per SM) */
 };
 
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay
@@ -239,6 +241,64 @@ int msolve_config(msolve_matrix *A, int key, int value);
  * A shift that has stopped keeps the values of its last active iteration.  An iteration that breaks down
  * writes no row.  cap_rows = 0 (or d_hist = NULL) switches the history off.  Returns OK / EINVAL. */
 int msolve_set_history(msolve_matrix *A, double *d_hist, int cap_rows);
+
+/* ---------------------------------------------------------------------------------------------------------------
+ * Row (site) partition: every slab owns a contiguous range of rows of A and the same range of r, p
+ * and of every x_k, p_k.  Per iteration the halo of the gathered vector (p; BiCGStab-M also s) is exchanged before
+ * each SpMV and the fused dot products are summed over the slabs; the fused multishift update (Alg. 1 l.28-29,
+ * PAPER.md:129-131) needs no communication.  (The paper itself used one of its four GPUs.)
+ *
+ * msolve_slab_plan_*: HOST ONLY, no CUDA call.  The plan of slab `rank` of `nslabs`: rows [h_splits[rank],
+ * h_splits[rank+1]) of an n x n matrix, given as the slab's own rows in CSR form (h_rowptr rebased to 0, GLOBAL
+ * column indices).  It holds the off-slab columns the slab needs, grouped by owning slab (ascending) and sorted
+ * within a slab -- halo entry j, at position nlocal + j of the slab's vectors -- and the slab's column indices
+ * renumbered [own rows 0..nlocal-1 | halo nlocal..nlocal+nhalo-1].  What slab p must SEND to slab q is slab q's
+ * list for peer p; ranks of a multi-process run exchange those lists once at set-up.
+ * For BSR3 matrices the plan is built on block rows / block columns (indices count 3x3 blocks).
+ * Errors: EINVAL (bad splits, column out of range, NULL), ENOMEM. */
+typedef struct msolve_slab_plan msolve_slab_plan;
+int msolve_slab_plan_create(msolve_slab_plan **plan, int64_t n, int nslabs, const int64_t *h_splits /* nslabs+1 */,
+                            int rank, const int32_t *h_rowptr /* nlocal+1 */, const int32_t *h_colidx);
+int64_t msolve_slab_plan_nlocal(const msolve_slab_plan *plan);
+int64_t msolve_slab_plan_nhalo(const msolve_slab_plan *plan);
+int msolve_slab_plan_npeers(const msolve_slab_plan *plan);
+/* peer j (0 <= j < npeers): its rank, where its entries start in the halo, how many, and their GLOBAL column
+ * indices (ascending; owned by the plan).  Any output pointer may be NULL. */
+int msolve_slab_plan_peer(const msolve_slab_plan *plan, int j, int *peer_rank, int64_t *halo_offset, int64_t *count,
+                          const int32_t **h_global_ids);
+const int32_t *msolve_slab_plan_colidx(const msolve_slab_plan *plan); /* nnz renumbered columns (owned by the plan) */
+void msolve_slab_plan_destroy(msolve_slab_plan *plan);
+
+/* msolve_slabs_*: `nslabs` slabs of one matrix on the CURRENT device, in one process.  The matrix comes as HOST
+ * arrays (the partitioner is host logic); the library keeps device copies of every slab's renumbered rows and one
+ * ordinary handle per slab (same kernels as msolve_create_csr / msolve_create_bsr3 with the same `flags`).
+ * h_splits: nslabs+1 row boundaries (block rows for BSR3), 16-byte aligned in the vectors, or NULL for an even
+ * split.  The halo travels by a gather kernel that stores straight into the receiving slab's vector; the dot
+ * products are summed over the slabs' per-CTA partials in fixed slab order; every slab repeats the scalar
+ * recurrences on the same sums; the whole multi-slab iteration is one WHILE graph.  Arguments of the solvers as
+ * msolve_cgm / msolve_bicgstabm with GLOBAL vectors (d_b: n, d_x: nshifts*n shift-major) and a workspace of
+ * msolve_slabs_workspace_bytes().  Results agree with the unpartitioned solve to rounding (the dot products are
+ * grouped by slab), and are bit-reproducible for a given number of slabs. */
+typedef struct msolve_slabs msolve_slabs;
+int msolve_slabs_create_csr(msolve_slabs **S, int64_t n, int64_t nnz, const int32_t *h_rowptr, const int32_t *h_colidx,
+                            const void *h_val, int dtype, int nslabs, const int64_t *h_splits, int flags, void *stream);
+int msolve_slabs_create_bsr3(msolve_slabs **S, int64_t nbrows, int64_t nblocks, const int32_t *h_browptr,
+                             const int32_t *h_bcolidx, const void *h_blocks, int dtype, int nslabs,
+                             const int64_t *h_splits, int flags, void *stream);
+int msolve_slabs_count(const msolve_slabs *S);
+int64_t msolve_slabs_halo_elements(const msolve_slabs *S, int slab); /* elements slab `slab` receives per exchange */
+size_t msolve_slabs_workspace_bytes(const msolve_slabs *S, int nshifts, int algorithm);
+int msolve_slabs_cgm(msolve_slabs *S, const void *d_b, const double *h_shifts, int nshifts, double tol, int max_iter,
+                     void *d_x, void *d_workspace, size_t workspace_bytes, int *h_iterations, int *h_conv_iter,
+                     double *h_relres, void *stream);
+int msolve_slabs_bicgstabm(msolve_slabs *S, const void *d_b, const double *h_shifts, int nshifts, double tol,
+                           int max_iter, void *d_x, void *d_workspace, size_t workspace_bytes, int *h_iterations,
+                           int *h_conv_iter, double *h_relres, void *stream);
+/* y = A x over the slabs (halo exchange + every slab's SpMV), h_dot = <x, A x>; workspace as for one shift of CG-M */
+int msolve_slabs_spmv(msolve_slabs *S, const void *d_x, void *d_y, void *d_workspace, size_t workspace_bytes,
+                      double *h_dot, void *stream);
+int64_t msolve_slabs_last_launch_count(const msolve_slabs *S);
+void msolve_slabs_destroy(msolve_slabs *S);
 
 /* Free the handle and everything the library allocated for it (never the caller's arrays). */
 void msolve_destroy(msolve_matrix *A);

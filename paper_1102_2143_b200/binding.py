@@ -30,12 +30,18 @@ MSOLVE_CFG_STOP_RULE = 3
 MSOLVE_CFG_X_WINDOW = 4
 MSOLVE_CFG_MATRIX_L2 = 5
 MSOLVE_CFG_ITER_PATH = 6
+MSOLVE_CFG_FUSED_CTAS = 7
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
     "msolve_bicgstabm", "msolve_multirhs_workspace_bytes", "msolve_solve_multirhs", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
     "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_set_history", "msolve_destroy",
     "msolve_last_error",
+    "msolve_slab_plan_create", "msolve_slab_plan_nlocal", "msolve_slab_plan_nhalo", "msolve_slab_plan_npeers",
+    "msolve_slab_plan_peer", "msolve_slab_plan_colidx", "msolve_slab_plan_destroy",
+    "msolve_slabs_create_csr", "msolve_slabs_create_bsr3", "msolve_slabs_count", "msolve_slabs_halo_elements",
+    "msolve_slabs_workspace_bytes", "msolve_slabs_cgm", "msolve_slabs_bicgstabm", "msolve_slabs_spmv",
+    "msolve_slabs_last_launch_count", "msolve_slabs_destroy",
 )
 
 _lib = None
@@ -81,6 +87,36 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_destroy.argtypes = [vp]
     lib.msolve_destroy.restype = None
     lib.msolve_last_error.restype = ctypes.c_char_p
+    lib.msolve_slab_plan_create.argtypes = [ctypes.POINTER(vp), i64, i32, vp, i32, vp, vp]
+    lib.msolve_slab_plan_create.restype = i32
+    for name in ("msolve_slab_plan_nlocal", "msolve_slab_plan_nhalo"):
+        getattr(lib, name).argtypes = [vp]
+        getattr(lib, name).restype = i64
+    lib.msolve_slab_plan_npeers.argtypes = [vp]
+    lib.msolve_slab_plan_npeers.restype = i32
+    lib.msolve_slab_plan_peer.argtypes = [vp, i32, vp, vp, vp, vp]
+    lib.msolve_slab_plan_peer.restype = i32
+    lib.msolve_slab_plan_colidx.argtypes = [vp]
+    lib.msolve_slab_plan_colidx.restype = vp
+    lib.msolve_slab_plan_destroy.argtypes = [vp]
+    lib.msolve_slab_plan_destroy.restype = None
+    lib.msolve_slabs_create_csr.argtypes = [ctypes.POINTER(vp), i64, i64, vp, vp, vp, i32, i32, vp, i32, vp]
+    lib.msolve_slabs_create_bsr3.argtypes = [ctypes.POINTER(vp), i64, i64, vp, vp, vp, i32, i32, vp, i32, vp]
+    lib.msolve_slabs_count.argtypes = [vp]
+    lib.msolve_slabs_halo_elements.argtypes = [vp, i32]
+    lib.msolve_slabs_halo_elements.restype = i64
+    lib.msolve_slabs_workspace_bytes.argtypes = [vp, i32, i32]
+    lib.msolve_slabs_workspace_bytes.restype = sz
+    lib.msolve_slabs_cgm.argtypes = solver_args
+    lib.msolve_slabs_bicgstabm.argtypes = solver_args
+    lib.msolve_slabs_spmv.argtypes = [vp, vp, vp, vp, sz, vp, vp]
+    lib.msolve_slabs_last_launch_count.argtypes = [vp]
+    lib.msolve_slabs_last_launch_count.restype = i64
+    lib.msolve_slabs_destroy.argtypes = [vp]
+    lib.msolve_slabs_destroy.restype = None
+    for name in ("msolve_slabs_create_csr", "msolve_slabs_create_bsr3", "msolve_slabs_count", "msolve_slabs_cgm",
+                 "msolve_slabs_bicgstabm", "msolve_slabs_spmv"):
+        getattr(lib, name).restype = i32
     for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_cgm", "msolve_bicgstabm",
                  "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration", "msolve_config",
                  "msolve_set_history", "msolve_solve_multirhs"):
@@ -383,3 +419,133 @@ def msolve_profile_iteration(A: Matrix, algorithm: int, b: torch.Tensor, shifts,
                                              x.data_ptr(), workspace.data_ptr(), workspace.numel(),
                                              ms.ctypes.data, nl.ctypes.data, _stream(stream)))
     return {lib.msolve_kernel_name(algorithm, j).decode(): float(ms[j]) for j in range(nk)}
+
+
+# ----------------------------------------------------------------------------------- row partition (slabs)
+class SlabPlan:
+    """Host-only plan of one slab (msolve_slab_plan_*): halo lists and renumbered columns.  No GPU involved."""
+
+    def __init__(self, n: int, splits, rank: int, rowptr_local: np.ndarray, colidx_global: np.ndarray):
+        lib = load_library()
+        self._splits = np.ascontiguousarray(splits, dtype=np.int64)
+        rp = np.ascontiguousarray(rowptr_local, dtype=np.int32)
+        ci = np.ascontiguousarray(colidx_global, dtype=np.int32)
+        h = ctypes.c_void_p()
+        _check(lib.msolve_slab_plan_create(ctypes.byref(h), int(n), self._splits.size - 1, self._splits.ctypes.data,
+                                           int(rank), rp.ctypes.data, ci.ctypes.data))
+        self.handle = h
+        self.rank = rank
+        self.nlocal = int(lib.msolve_slab_plan_nlocal(h))
+        self.nhalo = int(lib.msolve_slab_plan_nhalo(h))
+        self.peers = []                                    # (peer rank, halo offset, global ids)
+        for j in range(lib.msolve_slab_plan_npeers(h)):
+            pr, off, cnt, ids = ctypes.c_int(), ctypes.c_int64(), ctypes.c_int64(), ctypes.c_void_p()
+            _check(lib.msolve_slab_plan_peer(h, j, ctypes.byref(pr), ctypes.byref(off), ctypes.byref(cnt), ctypes.byref(ids)))
+            arr = np.ctypeslib.as_array(ctypes.cast(ids.value, ctypes.POINTER(ctypes.c_int32)), shape=(cnt.value,)).copy() if cnt.value else np.zeros(0, np.int32)
+            self.peers.append((pr.value, off.value, arr))
+        nnz = int(rp[-1])
+        ptr = lib.msolve_slab_plan_colidx(h)
+        self.colidx = np.ctypeslib.as_array(ctypes.cast(ptr, ctypes.POINTER(ctypes.c_int32)), shape=(nnz,)).copy() if nnz else np.zeros(0, np.int32)
+        lib.msolve_slab_plan_destroy(h)
+        self.handle = None
+
+
+class Slabs:
+    """Owner of an `msolve_slabs*`: `nslabs` slabs of one matrix on the current device."""
+
+    def __init__(self, handle, dtype, n):
+        self.handle, self.dtype, self.n = ctypes.c_void_p(handle), dtype, n
+
+    def destroy(self):
+        if self.handle:
+            load_library().msolve_slabs_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):  # pragma: no cover
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+_NP2TORCH = {np.dtype(np.complex64): torch.complex64, np.dtype(np.complex128): torch.complex128,
+             np.dtype(np.float32): torch.float32, np.dtype(np.float64): torch.float64}
+_NP2CODE = {np.dtype(np.complex64): MSOLVE_C64, np.dtype(np.complex128): MSOLVE_C128,
+            np.dtype(np.float32): MSOLVE_F32, np.dtype(np.float64): MSOLVE_F64}
+
+
+def msolve_slabs_create_csr(rowptr: np.ndarray, colidx: np.ndarray, val: np.ndarray, nslabs: int, splits=None,
+                            flags: int = MSOLVE_SPMV_AUTO, stream=None) -> Slabs:
+    """HOST numpy arrays of the whole matrix -> `nslabs` row slabs on the current device."""
+    lib = load_library()
+    rp, ci, v = (np.ascontiguousarray(rowptr, dtype=np.int32), np.ascontiguousarray(colidx, dtype=np.int32),
+                 np.ascontiguousarray(val))
+    sp = None if splits is None else np.ascontiguousarray(splits, dtype=np.int64)
+    h = ctypes.c_void_p()
+    _check(lib.msolve_slabs_create_csr(ctypes.byref(h), rp.size - 1, ci.size, rp.ctypes.data, ci.ctypes.data, v.ctypes.data,
+                                       _NP2CODE[v.dtype], int(nslabs), None if sp is None else sp.ctypes.data, flags, _stream(stream)))
+    return Slabs(h.value, _NP2TORCH[v.dtype], rp.size - 1)
+
+
+def msolve_slabs_create_bsr3(browptr: np.ndarray, bcolidx: np.ndarray, blocks: np.ndarray, nslabs: int, splits=None,
+                             flags: int = MSOLVE_SPMV_AUTO, stream=None) -> Slabs:
+    lib = load_library()
+    rp, ci, v = (np.ascontiguousarray(browptr, dtype=np.int32), np.ascontiguousarray(bcolidx, dtype=np.int32),
+                 np.ascontiguousarray(blocks))
+    sp = None if splits is None else np.ascontiguousarray(splits, dtype=np.int64)
+    h = ctypes.c_void_p()
+    _check(lib.msolve_slabs_create_bsr3(ctypes.byref(h), rp.size - 1, ci.size, rp.ctypes.data, ci.ctypes.data, v.ctypes.data,
+                                        _NP2CODE[v.dtype], int(nslabs), None if sp is None else sp.ctypes.data, flags, _stream(stream)))
+    return Slabs(h.value, _NP2TORCH[v.dtype], 3 * (rp.size - 1))
+
+
+def msolve_slabs_destroy(S: Slabs) -> None:
+    S.destroy()
+
+
+def msolve_slabs_halo_elements(S: Slabs):
+    lib = load_library()
+    return [int(lib.msolve_slabs_halo_elements(S.handle, p)) for p in range(lib.msolve_slabs_count(S.handle))]
+
+
+def msolve_slabs_last_launch_count(S: Slabs) -> int:
+    return int(load_library().msolve_slabs_last_launch_count(S.handle))
+
+
+def _slabs_solve(fn_name: str, algorithm: int, S: Slabs, b, shifts, tol, max_iter, x, stream) -> SolveResult:
+    lib = load_library()
+    b = _dev(b, S.dtype)
+    sh = np.ascontiguousarray(shifts, dtype=np.float64)
+    s = sh.size
+    if x is None:
+        x = torch.empty((s, S.n), dtype=S.dtype, device=b.device)
+    need = int(lib.msolve_slabs_workspace_bytes(S.handle, s, algorithm))
+    if need == 0:
+        raise MsolveError(MSOLVE_EINVAL, "nshifts must be in [1, %d]" % MSOLVE_MAX_SHIFTS)
+    ws = torch.empty(need, dtype=torch.uint8, device=b.device)
+    it = ctypes.c_int(0)
+    conv = np.full(s, -1, dtype=np.int32)
+    rel = np.zeros(s, dtype=np.float64)
+    rc = getattr(lib, fn_name)(S.handle, b.data_ptr(), sh.ctypes.data, s, float(tol), int(max_iter), x.data_ptr(),
+                               ws.data_ptr(), need, ctypes.addressof(it), conv.ctypes.data, rel.ctypes.data, _stream(stream))
+    _check(rc)
+    return SolveResult(rc, it.value, x.view(s, S.n), conv, rel)
+
+
+def msolve_slabs_cgm(S: Slabs, b, shifts, tol, max_iter, x=None, stream=None) -> SolveResult:
+    return _slabs_solve("msolve_slabs_cgm", MSOLVE_ALG_CGM, S, b, shifts, tol, max_iter, x, stream)
+
+
+def msolve_slabs_bicgstabm(S: Slabs, b, shifts, tol, max_iter, x=None, stream=None) -> SolveResult:
+    return _slabs_solve("msolve_slabs_bicgstabm", MSOLVE_ALG_BICGSTABM, S, b, shifts, tol, max_iter, x, stream)
+
+
+def msolve_slabs_spmv(S: Slabs, x: torch.Tensor, stream=None):
+    lib = load_library()
+    x = _dev(x, S.dtype)
+    y = torch.empty_like(x)
+    need = int(lib.msolve_slabs_workspace_bytes(S.handle, 1, MSOLVE_ALG_CGM))
+    ws = torch.empty(need, dtype=torch.uint8, device=x.device)
+    dot = np.zeros(2, dtype=np.float64)
+    _check(lib.msolve_slabs_spmv(S.handle, x.data_ptr(), y.data_ptr(), ws.data_ptr(), need, dot.ctypes.data, _stream(stream)))
+    return y, complex(dot[0], dot[1])

@@ -196,6 +196,7 @@ struct SolveHeader {
     const void* sp_x; void* sp_y; const void* sp_u;
     long long n;
     long long pk_stride;
+    long long x_stride;  // elements between x_k and x_{k+1} (n for a single handle; the global n for a slab, slab.cu)
     double tol;
     int S;
     int max_iter;
@@ -235,6 +236,10 @@ struct Recur {
     double coef[kMaxShifts * 14];
 };
 
+// one CTA's contribution to a grid-wide sum of the one-kernel path (fused_small.cu): values + generation tag
+constexpr int kFusedMaxCtas = 160;
+struct alignas(64) FusedSlot { double v[kAccMax]; unsigned long long tag; };
+
 struct SolveState {
     SolveHeader h;
     SolveResult res;
@@ -242,8 +247,11 @@ struct SolveState {
     double rhs_norm[kMaxShifts]; // eq. (6) only: ||b_k|| (multirhs.cu)
     // per-CTA partial sums of the fused reductions, [kAccMax][kMaxPartials]
     double partial[kAccMax * kMaxPartials];
-    double partial2[kMaxPartials];   // fused_small.cuh: |r|^2 partials (alternates with `partial` between grid syncs)
     int partial_count;           // how many CTAs wrote partials in the last reducing kernel
+    // fused_small.cu: slots of the combined grid barrier + sum, double-buffered by the parity of the generation
+    // counter, which runs on from solve to solve (fused_gen)
+    FusedSlot fslot[2][kFusedMaxCtas];
+    unsigned long long fused_gen;
 };
 
 // Fixed-order reduction of `count` per-CTA partials (NACC rows of kMaxPartials) by ONE CTA: every thread of the

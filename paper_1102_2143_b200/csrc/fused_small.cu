@@ -2,23 +2,20 @@
 // (BASELINE configs 1-2: 31 KB and 16.5 MB per iteration).  There the iteration as a graph of 5 (CG-M) / 7
 // (BiCGStab-M) kernels is bound by launch latency, not by bytes (SURVEY.md section 7 "tiny configs are
 // launch-latency bound": config 2 spends 24.6 us per iteration on 2.7 us of traffic).  Here one persistent grid
-// (one CTA per SM at most) runs init and every iteration, with a grid-wide barrier wherever the graph path has a
-// kernel boundary that carries a dependency across rows:
+// (one CTA per SM at most, launched cooperatively so that all CTAs are resident) runs init and every iteration, with
+// a grid-wide barrier wherever the graph path has a kernel boundary that carries a dependency across rows; a barrier
+// that follows a reducing step carries the sum with it (fused_allreduce):
 //   CG-M       p <- r + alpha p | SpMV + <p,Ap> | scalars #1, fused multishift update + |r|^2 | scalars #2      (3 barriers)
 //   BiCGStab-M SpMV#1 + <r0,q> | scalars, s <- r + beta q | SpMV#2 + dots | scalars, fused update | scalars    (4 barriers)
 // The steps are the SAME device functions the graph path runs as separate kernels (kernels.cuh, spmv.cuh row
 // bodies).  Every CTA keeps its own copy of the recurrence scalars in shared memory and runs the scalar steps
 // redundantly on the fixed-order sum of the per-CTA partials, so no CTA ever waits for a scalar another one
 // computes, and the results are bit-reproducible for a given grid.  Alg. 1 step for step.
-#include <cooperative_groups.h>
-
 #include "handle.h"
 #include "tuning.h"
 #include "kernels.cuh"
 #include "spmv.cuh"
 #include "spmv_lattice.cuh"
-
-namespace cg = cooperative_groups;
 
 namespace msolve {
 
@@ -34,20 +31,71 @@ __device__ __forceinline__ void fused_spmv(const MatDev& A, const SolveHeader& h
     else csr_vector_body<E, SEL, ROLE, false, false>(A, x, y, u, acc, blockIdx.x, gridDim.x);
 }
 
-// one partial per CTA and accumulator into `dst` ([NACC][kMaxPartials])
+// ---- grid-wide barrier and sum in ONE round trip.  Every CTA publishes its share of the sum together with a
+// generation tag (values first, then the tag with release semantics); every CTA polls the tags of all CTAs (thread t
+// polls CTA t, acquire loads), and once all carry the current generation it reads the values and adds them up in
+// CTA order -- the same fixed-order tree in every CTA, so every CTA holds the same bits.  There is no atomic and no
+// single counter all CTAs serialise on (148 CTAs on one L2 atomic cost ~2 us per barrier).  Slots are
+// double-buffered by the parity of the generation: a CTA can only overwrite its slot of generation g at generation
+// g + 2, which it reaches only after every CTA has passed g + 1, i.e. has finished reading generation g.
+__device__ __forceinline__ void st_release_u64(unsigned long long* p, unsigned long long v) {
+    asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ double ld_relaxed_f64(const double* p) {
+    double v;
+    asm volatile("ld.relaxed.gpu.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+
+// NACC = 0: barrier only.  acc: this thread's share (in); out: the grid-wide sums (the same in every thread).
 template <int NACC>
-__device__ __forceinline__ void fused_write_partials(double* dst, double (&acc)[NACC], double* red) {
-    __syncthreads();                                    // `red` may still be read by the previous reduction
-    block_sum<NACC>(acc, red);
-    if (threadIdx.x == 0) {
+__device__ __forceinline__ void fused_allreduce(SolveState* st, unsigned long long& gen, double* acc, double* out, double* red) {
+    ++gen;
+    FusedSlot* slots = st->fslot[gen & 1ull];
+    __shared__ double bc[kAccMax];
+    __syncthreads();                         // everything this CTA wrote so far is ordered before the release below
+    if constexpr (NACC > 0) {
+        double a[NACC];
 #pragma unroll
-        for (int a = 0; a < NACC; ++a) dst[a * kMaxPartials + blockIdx.x] = acc[a];
+        for (int i = 0; i < NACC; ++i) a[i] = acc[i];
+        block_sum<NACC>(a, red);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) slots[blockIdx.x].v[i] = a[i];
+        }
+    }
+    if (threadIdx.x == 0) st_release_u64(&slots[blockIdx.x].tag, gen);
+    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x)
+        while (ld_acquire_u64(&slots[i].tag) != gen) {}
+    __syncthreads();                         // every CTA has arrived; their writes are visible to this CTA
+    if constexpr (NACC > 0) {
+        double a[NACC];
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) a[i] = 0.0;
+        for (int c = threadIdx.x; c < (int)gridDim.x; c += blockDim.x) {
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) a[i] += ld_relaxed_f64(&slots[c].v[i]);
+        }
+        block_sum<NACC>(a, red);
+        if (threadIdx.x == 0) {
+#pragma unroll
+            for (int i = 0; i < NACC; ++i) bc[i] = a[i];
+        }
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < NACC; ++i) out[i] = bc[i];
     }
 }
 
-__device__ __forceinline__ void fused_publish(SolveState* st, const SolveResult& res) {
+__device__ __forceinline__ void fused_publish(SolveState* st, const SolveResult& res, unsigned long long gen) {
     if (blockIdx.x != 0) return;
     __syncthreads();
+    if (threadIdx.x == 0) st->fused_gen = gen;
     const int* src = (const int*)&res;
     int* dst = (int*)&st->res;
     for (int i = threadIdx.x; i < (int)(sizeof(SolveResult) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
@@ -55,102 +103,67 @@ __device__ __forceinline__ void fused_publish(SolveState* st, const SolveResult&
 
 template <typename E, int VEC, int SEL>
 __global__ void __launch_bounds__(kFusedThreads, 1) k_cgm_fused(MatDev A, SolveState* st) {
-    cg::grid_group grid = cg::this_grid();
     extern __shared__ __align__(16) unsigned char dyn[];
     Recur& rc = *(Recur*)dyn;
     SolveResult& res = *(SolveResult*)(dyn + sizeof(Recur));
     __shared__ double red[kAccMax * 32];
     const SolveHeader& h = st->h;
     const int cta = blockIdx.x, ncta = gridDim.x;
-    double s[1];
-    {   // l.9-10, 13: r <- b, p <- b, <b,b>
-        double acc[1] = {init_vectors_fn<E, VEC>(h, cta, ncta)};
-        fused_write_partials<1>(st->partial2, acc, red);
-    }
-    grid.sync();
-    reduce_partials_from<1>(st->partial2, ncta, s, red);
+    unsigned long long gen = st->fused_gen;                                           // written back by CTA 0 at the end
+    double acc[1], s[1];
+    acc[0] = init_vectors_fn<E, VEC>(h, cta, ncta);                                  // l.9-10, 13: r <- b, p <- b, <b,b>
+    fused_allreduce<1>(st, gen, acc, s, red);
     init_state_fn(h, res, rc, s[0]);
     while (!res.done) {
-        if (res.n_iter > 0) cgm_pupdate_fn<E, VEC>(h, rc, cta, ncta);                 // l.27
-        grid.sync();                                                                  // p complete before it is gathered
-        {
-            double acc[1] = {0.0};
-            fused_spmv<E, SEL, ROLE_CG>(A, h, acc);                                   // l.18-19
-            fused_write_partials<1>(st->partial, acc, red);
+        if (res.n_iter > 0) {
+            cgm_pupdate_fn<E, VEC>(h, rc, cta, ncta);                                 // l.27
+            fused_allreduce<0>(st, gen, nullptr, nullptr, red);                       // p complete before it is gathered
         }
-        grid.sync();
-        reduce_partials_from<1>(st->partial, ncta, s, red);
+        acc[0] = 0.0;
+        fused_spmv<E, SEL, ROLE_CG>(A, h, acc);                                       // l.18-19
+        fused_allreduce<1>(st, gen, acc, s, red);
         cgm_scal1_fn(h, res, rc, s[0]);                                               // l.20, 22, 23
         if (res.done) break;                                                          // breakdown: the same in every CTA
-        {
-            double acc[1] = {cgm_update_fn<E, VEC, kUnrollCgm>(h, res, rc, cta, ncta)};   // l.21, 24, 28, 29
-            fused_write_partials<1>(st->partial2, acc, red);
-        }
-        grid.sync();
-        reduce_partials_from<1>(st->partial2, ncta, s, red);
+        acc[0] = cgm_update_fn<E, VEC, kUnrollCgm>(h, res, rc, cta, ncta);            // l.21, 24, 28, 29
+        fused_allreduce<1>(st, gen, acc, s, red);
         cgm_scal2_fn(h, res, rc, st->rhs_norm, s[0], cta == 0 ? h.hist : nullptr);   // l.25, 26, 30, 31, 15
     }
-    fused_publish(st, res);
+    fused_publish(st, res, gen);
 }
 
 template <typename E, int VEC, int SEL>
 __global__ void __launch_bounds__(kFusedThreads, 1) k_bi_fused(MatDev A, SolveState* st) {
-    cg::grid_group grid = cg::this_grid();
     extern __shared__ __align__(16) unsigned char dyn[];
     Recur& rc = *(Recur*)dyn;
     SolveResult& res = *(SolveResult*)(dyn + sizeof(Recur));
     __shared__ double red[kAccMax * 32];
     const SolveHeader& h = st->h;
     const int cta = blockIdx.x, ncta = gridDim.x;
-    {
-        double acc[1] = {init_vectors_fn<E, VEC>(h, cta, ncta)};
-        fused_write_partials<1>(st->partial2, acc, red);
-    }
-    grid.sync();
-    {
-        double s[1];
-        reduce_partials_from<1>(st->partial2, ncta, s, red);
-        init_state_fn(h, res, rc, s[0]);
-    }
+    unsigned long long gen = st->fused_gen;
+    double acc[5], s[5];
+    acc[0] = init_vectors_fn<E, VEC>(h, cta, ncta);
+    fused_allreduce<1>(st, gen, acc, s, red);
+    init_state_fn(h, res, rc, s[0]);
     while (!res.done) {
-        {
-            double acc[2] = {0.0, 0.0};
-            fused_spmv<E, SEL, ROLE_B1>(A, h, acc);                                   // q = A p, <r0,q>
-            fused_write_partials<2>(st->partial, acc, red);
-        }
-        grid.sync();
-        {
-            double s[2];
-            reduce_partials_from<2>(st->partial, ncta, s, red);
-            bi_scal1_fn(h, res, rc, zd{s[0], s[1]});
-        }
+#pragma unroll
+        for (int a = 0; a < 5; ++a) acc[a] = 0.0;
+        fused_spmv<E, SEL, ROLE_B1>(A, h, acc);                                       // q = A p, <r0,q>
+        fused_allreduce<2>(st, gen, acc, s, red);
+        bi_scal1_fn(h, res, rc, zd{s[0], s[1]});
         if (res.done) break;
         bi_supdate_fn<E, VEC>(h, rc, cta, ncta);                                      // s = r + beta q
-        grid.sync();                                                                  // s complete before it is gathered
-        {
-            double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-            fused_spmv<E, SEL, ROLE_B2>(A, h, acc);                                   // t = A s, <t,s>, <t,t>, <r0,t>
-            fused_write_partials<5>(st->partial, acc, red);
-        }
-        grid.sync();
-        {
-            double s[5];
-            reduce_partials_from<5>(st->partial, ncta, s, red);
-            bi_scal2_fn(h, res, rc, s);
-        }
+        fused_allreduce<0>(st, gen, nullptr, nullptr, red);                           // s complete before it is gathered
+#pragma unroll
+        for (int a = 0; a < 5; ++a) acc[a] = 0.0;
+        fused_spmv<E, SEL, ROLE_B2>(A, h, acc);                                       // t = A s, <t,s>, <t,t>, <r0,t>
+        fused_allreduce<5>(st, gen, acc, s, red);
+        bi_scal2_fn(h, res, rc, s);
         if (res.done) break;
-        {
-            double acc[1] = {bi_update_fn<E, VEC, kUnrollBi>(h, res, rc, cta, ncta)}; // r', p, x_k, p_k, |r'|^2
-            fused_write_partials<1>(st->partial2, acc, red);
-        }
-        grid.sync();                                                                  // also: p complete before SpMV#1
-        {
-            double s[1];
-            reduce_partials_from<1>(st->partial2, ncta, s, red);
-            bi_scal3_fn(h, res, rc, st->rhs_norm, s[0], cta == 0 ? h.hist : nullptr);
-        }
+        acc[0] = bi_update_fn<E, VEC, kUnrollBi>(h, res, rc, cta, ncta);              // r', p, x_k, p_k, |r'|^2
+        fused_allreduce<1>(st, gen, acc, s, red);                                     // also: p complete before SpMV#1
+        bi_scal3_fn(h, res, rc, st->rhs_norm, s[0], cta == 0 ? h.hist : nullptr);
     }
-    fused_publish(st, res);
+    fused_publish(st, res, gen);
 }
 
 // ------------------------------------------------------------------------------------------- host side
@@ -177,7 +190,9 @@ static int launch_coop(const msolve_matrix* A, K kernel, long long work_threads,
     MSOLVE_CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, kFusedThreads, smem));
     if (per_sm < 1) return fail(MSOLVE_ECUDA, "fused kernel does not fit on an SM");
     const long long need = (work_threads + kFusedThreads - 1) / kFusedThreads;
-    const int grid = (int)std::max(1ll, std::min<long long>(A->num_sms, need));
+    const int cap = std::min(A->num_sms, kFusedMaxCtas);
+    int grid = (int)std::max(1ll, std::min<long long>(cap, need));
+    if (A->opt.fused_ctas > 0) grid = std::min(cap, A->opt.fused_ctas);
     MatDev dev = A->dev;
     SolveState* st = A->d_state;
     void* args[2] = {&dev, &st};

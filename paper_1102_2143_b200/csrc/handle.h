@@ -31,6 +31,7 @@ struct Options {
     int iter_path = 0;       // MSOLVE_CFG_ITER_PATH
     int x_window = 0;        // MSOLVE_CFG_X_WINDOW
     int matrix_l2 = 0;       // MSOLVE_CFG_MATRIX_L2
+    int fused_ctas = 0;      // MSOLVE_CFG_FUSED_CTAS
     int graph_key() const { return loop_mode | (update_kernel << 1) | (lattice_kernel << 2) | (iter_path << 4) | (x_window << 6); }
 };
 
@@ -71,6 +72,7 @@ struct msolve_matrix {
     cudaStream_t capture_stream = nullptr;
     msolve::LoopGraph graphs[2];
     int64_t last_launches = 0;
+    long long x_stride = 0;             // slab handles: elements between x_k and x_{k+1} in the caller's array (0 = n)
     size_t l2_persist_bytes = 0;        // MSOLVE_CFG_X_WINDOW: persisting L2 set-aside / largest window of the device
     size_t l2_window_max = 0;
     mutable std::vector<const void*> smem_attr_done;   // kernels whose dynamic shared-memory limit is raised on `device`
@@ -118,7 +120,9 @@ inline int spmv_launches(const msolve_matrix* A) { return A->kernel == KERNEL_ME
 
 // vec.cu: the non-SpMV kernels of the iteration body, by position j (msolve_kernel_name), and the two init kernels
 int launch_vec_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s, cudaGraphConditionalHandle cond, int use_cond);
-int launch_init(const msolve_matrix* A, cudaStream_t s);
+int launch_init(const msolve_matrix* A, cudaStream_t s);             // both init kernels
+int launch_init_vectors(const msolve_matrix* A, cudaStream_t s);     // r <- b, p <- b, partial <b,b>
+int launch_init_state(const msolve_matrix* A, cudaStream_t s);       // scalars from the summed partials
 
 // fused_small.cu: the whole solve as ONE cooperative kernel (systems that live in L2)
 bool fused_supported(const msolve_matrix* A);

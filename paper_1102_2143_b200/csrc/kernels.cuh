@@ -205,7 +205,7 @@ __device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const Solv
     }
     const T beta = (T)rc.beta.re;
     __syncthreads();
-    const long long n = h.n, nvec = n / VEC, pks = h.pk_stride;
+    const long long n = h.n, nvec = n / VEC, pks = h.pk_stride, xs = h.x_stride;
     P* r = (P*)h.r;
     const P* q = (const P*)h.q;
     C* x = (C*)h.x;
@@ -221,7 +221,7 @@ __device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const Solv
             for (int u = 0; u < UNR; ++u) {
                 if (a0 + u < na && !first) {
                     const int k = s_k[a0 + u];
-                    xv[u] = ld_pack<true>((const P*)(x + k * n) + i);
+                    xv[u] = ld_pack<true>((const P*)(x + k * xs) + i);
                     pv[u] = ld_pack<true>((const P*)(pk + k * pks) + i);
                 }
             }
@@ -242,7 +242,7 @@ __device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const Solv
                         xo.v[e] = caxpy_r(xe, -bk, pe);                              // l.28
                         po.v[e] = pe;
                     }
-                    st_pack<true>((P*)(x + k * n) + i, xo);
+                    st_pack<true>((P*)(x + k * xs) + i, xo);
                     st_pack<true>((P*)(pk + k * pks) + i, po);
                 }
             }
@@ -454,7 +454,7 @@ __device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const Solve
     const C chi = cmake<C>(rc.chi.re, rc.chi.im);
     const C alpha_new = cmake<C>(rc.alpha_new.re, rc.alpha_new.im);
     __syncthreads();
-    const long long n = h.n, nvec = n / VEC, pks = h.pk_stride;
+    const long long n = h.n, nvec = n / VEC, pks = h.pk_stride, xs = h.x_stride;
     P* r = (P*)h.r;
     P* p = (P*)h.p;
     const P* s = (const P*)h.s;
@@ -481,7 +481,7 @@ __device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const Solve
             for (int u = 0; u < UNR; ++u) {
                 if (a0 + u < na && !first) {
                     const int k = s_k[a0 + u];
-                    xv[u] = ld_pack<true>((const P*)(x + k * n) + i);
+                    xv[u] = ld_pack<true>((const P*)(x + k * xs) + i);
                     pv[u] = ld_pack<true>((const P*)(pk + k * pks) + i);
                 }
             }
@@ -499,7 +499,7 @@ __device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const Solve
                         const C ds = csub(cmul(c[5], sv.v[e]), cmul(c[6], rv.v[e]));
                         po.v[e] = cadd(cmul(c[2], rn.v[e]), cmul(c[3], csub(pe, cmul(c[4], ds))));
                     }
-                    st_pack<true>((P*)(x + k * n) + i, xo);
+                    st_pack<true>((P*)(x + k * xs) + i, xo);
                     st_pack<true>((P*)(pk + k * pks) + i, po);
                 }
             }

@@ -144,9 +144,6 @@ static int build_graph(msolve_matrix* A, int alg) {
     return MSOLVE_OK;
 }
 
-// AUTO rule of MSOLVE_CFG_MATRIX_L2: keep the matrix in L2 (evict-last bulk copies) when the matrix and the two
-// SpMV vectors take at most kMatKeepBytes of the 126 MB L2
-constexpr size_t kMatKeepBytes = (size_t)96 << 20;
 // AUTO rule of MSOLVE_CFG_ITER_PATH: one cooperative kernel per solve up to this working set (profiles/r02_sweeps.md)
 constexpr size_t kFusedMaxBytes = (size_t)40 << 20;
 static size_t matrix_bytes(const msolve_matrix* A) {
@@ -155,10 +152,6 @@ static size_t matrix_bytes(const msolve_matrix* A) {
     if (A->format == FMT_LATTICE) return (size_t)A->dev.nnz * 9 * e;
     return (size_t)A->dev.nnz * (e + 4) + (size_t)(A->dev.n + 1) * 4;
 }
-static bool matrix_fits_l2(const msolve_matrix* A) {
-    return matrix_bytes(A) + 2 * (size_t)A->dev.n * elem_bytes(A->dtype) <= kMatKeepBytes;
-}
-
 // ------------------------------------------------------------------------------------- create
 static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t stream) {
     (void)stream;
@@ -168,7 +161,7 @@ static int create_common(msolve_matrix** out, msolve_matrix* A, cudaStream_t str
     CU(cudaMemset(A->d_state, 0, sizeof(SolveState)));
     CU(cudaMallocHost((void**)&A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult)));
     CU(cudaStreamCreateWithFlags(&A->capture_stream, cudaStreamNonBlocking));
-    A->dev.mat_keep = matrix_fits_l2(A);
+    A->dev.mat_keep = 0;
     *out = A;
     return MSOLVE_OK;
 }
@@ -421,9 +414,10 @@ extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
     if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { A->opt.lattice_kernel = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_STOP_RULE && (value == 0 || value == 1)) { A->opt.stop_rule = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_ITER_PATH && value >= 0 && value <= 2) { A->opt.iter_path = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_FUSED_CTAS && value >= 0 && value <= kFusedMaxCtas) { A->opt.fused_ctas = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_MATRIX_L2 && value >= 0 && value <= 2) {
         A->opt.matrix_l2 = value;
-        A->dev.mat_keep = value == 2 || (value == 0 && matrix_fits_l2(A));
+        A->dev.mat_keep = value == 2;
         return MSOLVE_OK;
     }
     if (key == MSOLVE_CFG_X_WINDOW && (value == 0 || value == 1)) {
@@ -489,6 +483,7 @@ static int fill_header(const msolve_matrix* A, int alg, const void* d_b, const d
     h->pk = next;
     h->n = A->dev.n;
     h->pk_stride = pk_stride_elems(A);
+    h->x_stride = A->dev.n;
     h->tol = tol; h->S = S; h->max_iter = max_iter; h->force_all = force_all;
     h->stop_rule = A->opt.stop_rule; h->hist = A->d_hist; h->hist_cap = A->hist_cap;
     for (int k = 0; k < S; ++k) h->sigma[k] = h_shifts[k];

@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(UpdTmaCfg<E>::kThreadsTotal, 1) k_cgm_update_t
     const unsigned char* q = (const unsigned char*)st->h.q;
     unsigned char* x = (unsigned char*)st->h.x;
     unsigned char* pk = (unsigned char*)st->h.pk;
-    const long long xstride = n * (long long)sizeof(E), pstride = pks * (long long)sizeof(E);
+    const long long xstride = st->h.x_stride * (long long)sizeof(E), pstride = pks * (long long)sizeof(E);
     double acc[1] = {0.0};
     int stage = 0;
     uint32_t phase = 0;

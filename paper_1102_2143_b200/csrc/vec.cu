@@ -59,7 +59,10 @@ __global__ void __launch_bounds__(kThreads) k_bi_scal3(SolveState* st, cudaGraph
 }
 
 // element-wise kernels: 16 bytes (1, 2 or 4 elements) per access when the length allows it
-static bool vec16(const msolve_matrix* A) { return A->dev.n % (long long)(16 / elem_bytes(A->dtype)) == 0; }
+static bool vec16(const msolve_matrix* A) {
+    const long long m = (long long)(16 / elem_bytes(A->dtype));
+    return A->dev.n % m == 0 && A->x_stride % m == 0;
+}
 
 #define DISPATCH_VEC(A, KERNEL, ...)                                                       \
     do {                                                                                   \
@@ -117,10 +120,17 @@ int launch_vec_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s, cu
     return rc;
 }
 
-int launch_init(const msolve_matrix* A, cudaStream_t s) {
+int launch_init_vectors(const msolve_matrix* A, cudaStream_t s) {
     DISPATCH_VEC(A, L_INIT, A, s);
+    return MSOLVE_OK;
+}
+int launch_init_state(const msolve_matrix* A, cudaStream_t s) {
     k_init_state<<<1, kThreads, 0, s>>>(A->d_state);
     return MSOLVE_OK;
+}
+int launch_init(const msolve_matrix* A, cudaStream_t s) {
+    launch_init_vectors(A, s);
+    return launch_init_state(A, s);
 }
 
 }  // namespace msolve

@@ -31,7 +31,7 @@ def test_fused_matches_oracle_and_graph(ms, which, fmt, dtype, tol):
     assert abs(gg[1] - g[1]) <= 1
     for k in range(w.shifts.size):
         d = np.linalg.norm(g[2][k].astype(np.complex128) - gg[2][k]) / np.linalg.norm(gg[2][k])
-        assert d <= (1e-11 if dtype == np.complex128 else 2e-5), (k, d)
+        assert d <= REL[dtype], (k, d)          # two groupings of the same dot products: rounding, amplified by the iteration
     # bit-reproducible: the same solve again returns the same bytes
     g2 = gpu_solve(ms, w, dtype, fmt, cfg=fused(ms))
     assert g2[1] == g[1] and np.array_equal(g2[2], g[2]) and np.array_equal(g2[3], g[3])
