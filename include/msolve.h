@@ -95,7 +95,7 @@ enum {
                                 (one kernel per step of Alg. 1; HBM-bound sizes), 2 = the WHOLE solve as one cooperative
                                 kernel with grid-wide barriers between the steps (systems that live in L2, where kernel
                                 launches, not bytes, are the cost; vector-CSR, BSR3 and lattice handles), 0 = by
-                                footprint (default): 2 when matrix + (4 + 2 nshifts) vectors take at most 40 MB.
+                                footprint (default): 2 when matrix + (4 + 2 nshifts) vectors take at most 256 MB.
                                 Same arithmetic step for step; the two paths group the dot products differently
                                 (per-CTA partials of different grids), so they agree to rounding, not bit for bit */,
     MSOLVE_CFG_FUSED_CTAS = 7 /* CTAs of the cooperative kernel of MSOLVE_CFG_ITER_PATH = 2: 0 = by problem size
@@ -181,8 +181,12 @@ int msolve_bicgstabm(const msolve_matrix *A, const void *d_b, const double *h_sh
  *   tol          in   system i stops at |zeta_i| ||r|| <= tol ||b_i||: relative to ITS OWN right-hand side;
  *                     h_relres[i] is that ratio.
  *   d_workspace       >= msolve_multirhs_workspace_bytes(): the solver's workspace plus nshifts vectors.
- * Everything else as msolve_cgm.  The divided differences amplify rounding by 1 / prod |sigma_i - sigma_j|: the
- * construction suits a handful of well separated shifts or right-hand sides that vary smoothly with the shift. */
+ * Everything else as msolve_cgm.
+ * Numerical range: r0 is the interpolant of the b_i over the shifts, EXTRAPOLATED to s = -spec(A).  For right-hand
+ * sides that vary smoothly with the shift that is harmless; for independent ones ||r0|| / ||b|| grows like
+ * ||A||^(nshifts-1) / prod |sigma_i - sigma_j|, and tol is reachable only while eps ||r0|| < tol ||b_i|| (eps of the
+ * element type).  A handful of well separated shifts is the practical range (tests: 3 smooth systems in both
+ * precisions, 5 independent ones in complex128, 20 for an operator that is small against the shift spacing). */
 size_t msolve_multirhs_workspace_bytes(const msolve_matrix *A, int nshifts, int algorithm);
 int msolve_solve_multirhs(const msolve_matrix *A, int algorithm, const void *d_B, const double *h_shifts,
                           int nshifts, double tol, int max_iter, void *d_x, void *d_workspace,

@@ -238,7 +238,7 @@ struct Recur {
 
 // one CTA's contribution to a grid-wide sum of the one-kernel path (fused_small.cu): values + generation tag
 constexpr int kFusedMaxCtas = 160;
-struct alignas(64) FusedSlot { double v[kAccMax]; unsigned long long tag; };
+struct alignas(128) FusedSlot { unsigned long long w[2 * kAccMax]; unsigned long long tag; };
 
 struct SolveState {
     SolveHeader h;

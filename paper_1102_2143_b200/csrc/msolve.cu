@@ -144,8 +144,10 @@ static int build_graph(msolve_matrix* A, int alg) {
     return MSOLVE_OK;
 }
 
-// AUTO rule of MSOLVE_CFG_ITER_PATH: one cooperative kernel per solve up to this working set (profiles/r02_sweeps.md)
-constexpr size_t kFusedMaxBytes = (size_t)40 << 20;
+// AUTO rule of MSOLVE_CFG_ITER_PATH: one cooperative kernel per solve up to this working set.  Measured per-iteration
+// times, graph / one kernel (profiles/r02_sweeps.md): 11 MB 23.6 / 18.2 us, 150 MB 86 / 76 us, 200 MB 71 / 63 us,
+// 400 MB 119 / 115 us, 800 MB 218 / 223 us.
+constexpr size_t kFusedMaxBytes = (size_t)256 << 20;
 static size_t matrix_bytes(const msolve_matrix* A) {
     const size_t e = elem_bytes(A->dtype);
     if (A->format == FMT_BSR3) return (size_t)A->dev.nnz * (9 * e + 4) + (size_t)(A->dev.nbrows + 1) * 4;

@@ -39,7 +39,7 @@ def test_fused_matches_oracle_and_graph(ms, which, fmt, dtype, tol):
 
 def test_auto_picks_by_footprint(ms):
     # AUTO (the library default): one kernel for config 2 (16.5 MB per iteration), the graph of kernels for a
-    # system whose vectors alone exceed the 40 MB bound
+    # system beyond the 256 MB bound
     w = W.config2()
     A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks))
     r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
@@ -48,7 +48,7 @@ def test_auto_picks_by_footprint(ms):
     r1 = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
     assert ms.msolve_last_launch_count(A) == 2 + 5 * r1.iterations
     ms.msolve_destroy(A)
-    w = W.config4(extents=(16, 16, 16, 16))                # 196608 rows, 16 shifts: 36 vectors of 3 MB + 88 MB of matrix
+    w = W.config4(extents=(16, 16, 16, 32))                # 393216 rows, 16 shifts: 36 vectors of 6.3 MB + 175 MB of matrix
     A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks))
     r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
     assert r.status == 0 and ms.msolve_last_launch_count(A) == 2 + 5 * r.iterations
@@ -111,6 +111,7 @@ def test_fused_multirhs_and_real(ms):
     shifts = np.array([0.0, 0.4, 1.0, 1.7])
     rng = np.random.default_rng(41)
     B = rng.standard_normal((4, w.n)) + 1j * rng.standard_normal((4, w.n))
+    B = B[0] + shifts[:, None] * B[1] + 0.05 * B
     A = make_matrix(ms, w, np.complex128, "bsr3", cfg=fused(ms))
     g = ms.msolve_solve_multirhs(A, ms.MSOLVE_ALG_CGM, dev(B), shifts, 1e-10, w.max_iter)
     o = oracle.multirhs(w.rowptr, w.colidx, w.val, B, shifts, 1e-10, w.max_iter)
