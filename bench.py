@@ -298,9 +298,10 @@ def main():
                     help="CG-M fused multishift update: register kernel (default) or the TMA-staged kernel")
     ap.add_argument("--x-window", action="store_true",
                     help="vector-CSR kernel: L2 access-policy window over the gathered vector (MSOLVE_CFG_X_WINDOW)")
-    ap.add_argument("--iter-path", default="auto", choices=["auto", "graph", "fused"],
+    ap.add_argument("--iter-path", default="auto", choices=["auto", "graph", "fused", "resident"],
                     help="graph: iteration as a CUDA graph of kernels; fused: whole solve in one cooperative kernel "
-                         "(L2-resident systems); auto: by footprint (MSOLVE_CFG_ITER_PATH)")
+                         "(L2-resident systems); resident: one kernel, matrix and vectors in shared memory (CG-M, a few "
+                         "MB); auto: by footprint (MSOLVE_CFG_ITER_PATH)")
     ap.add_argument("--fused-ctas", type=int, default=0, help="CTAs of the one-kernel path (0 = by problem size)")
     ap.add_argument("--matrix-l2", default="auto", choices=["auto", "stream", "keep"],
                     help="L2 policy of the matrix stream (MSOLVE_CFG_MATRIX_L2)")
@@ -367,7 +368,7 @@ def main():
     ms.msolve_config(A, ms.MSOLVE_CFG_UPDATE_KERNEL, 1 if args.update_kernel == "tma" else 0)
     if args.x_window:
         ms.msolve_config(A, ms.MSOLVE_CFG_X_WINDOW, 1)
-    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, {"auto": 0, "graph": 1, "fused": 2}[args.iter_path])
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, {"auto": 0, "graph": 1, "fused": 2, "resident": 3}[args.iter_path])
     ms.msolve_config(A, ms.MSOLVE_CFG_FUSED_CTAS, args.fused_ctas)
     ms.msolve_config(A, ms.MSOLVE_CFG_MATRIX_L2, {"auto": 0, "stream": 1, "keep": 2}[args.matrix_l2])
     S = int(w.shifts.size)

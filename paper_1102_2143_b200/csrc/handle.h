@@ -3,7 +3,9 @@
 //   msolve.cu      C ABI, create/destroy, graph capture, solver drivers
 //   spmv_role.cu   SpMV launches, compiled once per ROLE (the fused reductions differ per role)
 //   vec.cu         vector-update and scalar-recurrence kernels
-//   fused_small.cu whole-iteration cooperative kernel for systems that live in L2
+//   fused_small.cu whole solve as one cooperative kernel for systems that live in L2
+//   resident.cu    whole solve with matrix and vectors resident in shared memory (systems of a few MB)
+//   multirhs.cu    a right-hand side per shift, eq. (6)
 //   slab.cu        row-partitioned operator (halo exchange between slabs)
 #pragma once
 
@@ -75,6 +77,7 @@ struct msolve_matrix {
     long long x_stride = 0;             // slab handles: elements between x_k and x_{k+1} in the caller's array (0 = n)
     size_t l2_persist_bytes = 0;        // MSOLVE_CFG_X_WINDOW: persisting L2 set-aside / largest window of the device
     size_t l2_window_max = 0;
+    mutable std::vector<int32_t> h_rowptr;   // host copy of rowptr / browptr (resident.cu sizes its ranges from it), filled on demand
     mutable std::vector<const void*> smem_attr_done;   // kernels whose dynamic shared-memory limit is raised on `device`
     msolve_slab_set* slabs = nullptr;   // row-partitioned form (msolve_create_*_slabs)
 };
@@ -127,6 +130,10 @@ int launch_init_state(const msolve_matrix* A, cudaStream_t s);       // scalars 
 // fused_small.cu: the whole solve as ONE cooperative kernel (systems that live in L2)
 bool fused_supported(const msolve_matrix* A);
 int launch_fused(const msolve_matrix* A, int alg, cudaStream_t s);
+
+// resident.cu: CG-M with matrix and vectors resident in shared memory (systems of a few MB)
+bool resident_supported(const msolve_matrix* A, int S, int alg);
+int launch_resident(const msolve_matrix* A, int S, int alg, cudaStream_t s);
 
 // msolve.cu: pieces the other entry points (multirhs.cu, slab.cu) build on
 long long pk_stride_elems(const msolve_matrix* A);

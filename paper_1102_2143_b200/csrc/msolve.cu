@@ -148,6 +148,9 @@ static int build_graph(msolve_matrix* A, int alg) {
 // times, graph / one kernel (profiles/r02_sweeps.md): 11 MB 23.6 / 18.2 us, 150 MB 86 / 76 us, 200 MB 71 / 63 us,
 // 400 MB 119 / 115 us, 800 MB 218 / 223 us.
 constexpr size_t kFusedMaxBytes = (size_t)256 << 20;
+// ... and with everything resident in shared memory while it fits there (148 x ~200 KB; resident.cu checks the exact
+// per-CTA layout, this bound only saves the host copy of rowptr for matrices that cannot fit)
+constexpr size_t kResidentMaxBytes = (size_t)28 << 20;
 static size_t matrix_bytes(const msolve_matrix* A) {
     const size_t e = elem_bytes(A->dtype);
     if (A->format == FMT_BSR3) return (size_t)A->dev.nnz * (9 * e + 4) + (size_t)(A->dev.nbrows + 1) * 4;
@@ -415,7 +418,7 @@ extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
     if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { A->opt.update_kernel = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { A->opt.lattice_kernel = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_STOP_RULE && (value == 0 || value == 1)) { A->opt.stop_rule = value; return MSOLVE_OK; }
-    if (key == MSOLVE_CFG_ITER_PATH && value >= 0 && value <= 2) { A->opt.iter_path = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_ITER_PATH && value >= 0 && value <= 3) { A->opt.iter_path = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_FUSED_CTAS && value >= 0 && value <= kFusedMaxCtas) { A->opt.fused_ctas = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_MATRIX_L2 && value >= 0 && value <= 2) {
         A->opt.matrix_l2 = value;
@@ -525,13 +528,26 @@ int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const 
     const int mode = A->opt.loop_mode;
     // Systems that live in L2 are bound by launch latency, not bytes: the whole solve runs as ONE cooperative
     // kernel (fused_small.cu).  AUTO: matrix + (4 + 2 S) vectors at most kFusedMaxBytes.
-    const bool fused = A->opt.iter_path == 2 ||
+    // the smallest systems (a few MB) even fit in the shared memory of the 148 SMs: resident.cu (CG-M, CSR / BSR3)
+    bool resident = false;
+    if (alg == MSOLVE_ALG_CGM && (A->opt.iter_path == 3 || A->opt.iter_path == 0) && (A->format == FMT_CSR || A->format == FMT_BSR3) &&
+        matrix_bytes(A) + (size_t)(3 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kResidentMaxBytes) {
+        const size_t units = A->format == FMT_BSR3 ? (size_t)A->dev.nbrows : (size_t)A->dev.n;
+        if (A->h_rowptr.size() != units + 1) {
+            A->h_rowptr.resize(units + 1);
+            CU(cudaMemcpyAsync(A->h_rowptr.data(), A->dev.rowptr, sizeof(int32_t) * (units + 1), cudaMemcpyDeviceToHost, stream));
+            CU(cudaStreamSynchronize(stream));
+        }
+        resident = resident_supported(A, S, alg);
+    }
+    if (A->opt.iter_path == 3 && !resident) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 3 needs CG-M on a CSR / BSR3 handle whose matrix and 3 + 2 nshifts vectors fit in shared memory");
+    const bool fused = resident || A->opt.iter_path == 2 ||
                        (A->opt.iter_path == 0 && fused_supported(A) &&
                         matrix_bytes(A) + (size_t)(4 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kFusedMaxBytes);
     if (fused) {
-        if (!fused_supported(A)) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 2 needs a vector-CSR, BSR3 or lattice handle, the register update kernel and the WHILE loop mode");
+        if (!resident && !fused_supported(A)) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 2 needs a vector-CSR, BSR3 or lattice handle, the register update kernel and the WHILE loop mode");
         CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
-        rc = launch_fused(A, alg, stream);
+        rc = resident ? launch_resident(A, S, alg, stream) : launch_fused(A, alg, stream);
         if (rc != MSOLVE_OK) return rc;
         CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));
         CU(cudaStreamSynchronize(stream));

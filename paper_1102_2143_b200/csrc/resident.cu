@@ -1,0 +1,220 @@
+// resident.cu -- CG-M with the whole problem resident in SHARED MEMORY (BASELINE configs 1-2 and the like).
+//
+// A B200 has 148 SMs x 227 KB = 33 MB of shared memory.  When the matrix and all 3 + 2S vectors of the solve fit
+// there, one persistent cooperative kernel gives every CTA a contiguous range of rows and keeps, for the whole
+// solve, that range of the matrix and of r, p, Ap and every x_k, p_k in its shared memory.  Per iteration the only
+// global-memory traffic is the exchange the method itself needs: the search direction p (written by its owner,
+// gathered by the rows that reference it: the "halo") and the two dot products (fused_allreduce: one round trip to
+// L2 each, no atomics).  Everything else -- the matrix stream and the 4S + 3 vector passes of the fused multishift
+// update (Alg. 1 l.21, 24, 28, 29) -- runs out of shared memory.  x_k is written to the caller's
+// array once, at the end.
+//
+// Same steps, same per-element arithmetic and the same scalar functions (kernels.cuh) as the other two paths; the
+// dot products are grouped by row owner, so results agree with them to rounding and are bit-reproducible.
+// One thread per scalar row of the CTA's range (CSR: the row's non-zeros in stored order; BSR3: row r of each 3x3
+// block of the block row).
+#include "handle.h"
+#include "tuning.h"
+#include "kernels.cuh"
+#include "fused_sync.cuh"
+
+namespace msolve {
+
+constexpr int kResThreads = 256;
+
+// layout of a CTA's dynamic shared memory (byte offsets, the same in every CTA: sized for the largest range)
+struct ResLayout {
+    int max_rows;        // scalar rows per CTA (upper bound)
+    int max_units;       // index rows per CTA: scalar rows (CSR) or block rows (BSR3)
+    int max_entries;     // non-zeros (CSR) or blocks (BSR3) per CTA
+    int off_rowptr, off_col, off_val, off_r, off_p, off_q, off_xk, off_pk;
+    int S;
+    int total;
+};
+
+template <typename E, int DOF>
+__global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, SolveState* st, ResLayout L) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    extern __shared__ __align__(16) unsigned char dyn[];
+    Recur& rc = *(Recur*)dyn;
+    SolveResult& res = *(SolveResult*)(dyn + kFusedOffRes);
+    const SolveHeader& h = *(const SolveHeader*)(dyn + kFusedOffHdr);
+    double* rhs_norm = (double*)(dyn + kFusedOffNorm);
+    unsigned char* base = dyn + kFusedFixedBytes;
+    __shared__ double red[kAccMax * 32];
+    fused_stage_header(st, dyn + kFusedOffHdr, rhs_norm);
+    const int cta = blockIdx.x, ncta = gridDim.x, tid = threadIdx.x;
+    // this CTA's range of index rows (units) and scalar rows
+    const long long units = DOF == 3 ? A.nbrows : A.n;
+    const long long u0 = units * cta / ncta, u1 = units * (cta + 1) / ncta;
+    const int nu = (int)(u1 - u0), nloc = nu * DOF;
+    const long long row0 = u0 * DOF;
+    int* s_rowptr = (int*)(base + L.off_rowptr);
+    int* s_col = (int*)(base + L.off_col);
+    C* s_val = (C*)(base + L.off_val);
+    C* s_r = (C*)(base + L.off_r);
+    C* s_p = (C*)(base + L.off_p);
+    C* s_q = (C*)(base + L.off_q);
+    C* s_xk = (C*)(base + L.off_xk);     // [S][max_rows]
+    C* s_pk = (C*)(base + L.off_pk);
+    const int ld = L.max_rows;
+    const int S = h.S;
+    C* pg = (C*)h.p;                     // the one vector that lives in global memory: gathered across CTAs
+    // ---- load the matrix range (once) and the vectors: r <- b, p <- b, x_k <- 0, p_k <- b  (l.9-12)
+    const int e0 = A.rowptr[u0];
+    const int ne = A.rowptr[u1] - e0;
+    for (int i = tid; i <= nu; i += blockDim.x) s_rowptr[i] = A.rowptr[u0 + i] - e0;
+    for (int j = tid; j < ne; j += blockDim.x) s_col[j] = A.colidx[e0 + j];
+    {
+        const C* gv = (const C*)A.val + (long long)e0 * (DOF == 3 ? 9 : 1);
+        const int nv = ne * (DOF == 3 ? 9 : 1);
+        for (int j = tid; j < nv; j += blockDim.x) s_val[j] = gv[j];
+    }
+    double acc[1] = {0.0}, s[1];
+    for (int i = tid; i < nloc; i += blockDim.x) {
+        const C bv = ((const C*)h.b)[row0 + i];
+        s_r[i] = bv; s_p[i] = bv;
+        pg[row0 + i] = bv;
+        for (int k = 0; k < S; ++k) { s_xk[k * ld + i] = cmake<C>(0.0, 0.0); s_pk[k * ld + i] = bv; }
+        acc[0] += cnorm2(bv);
+    }
+    unsigned long long gen = st->fused_gen;
+    fused_allreduce<1>(st, gen, acc, s, red);                                        // <b,b> (l.13); p visible to all
+    init_state_fn(h, res, rc, s[0]);
+    while (!res.done) {
+        if (res.n_iter > 0) {
+            const T alpha = (T)rc.alpha.re;
+            for (int i = tid; i < nloc; i += blockDim.x) {                           // l.27, own rows
+                const C pv = caxpy_r(s_r[i], alpha, s_p[i]);
+                s_p[i] = pv;
+                pg[row0 + i] = pv;
+            }
+            fused_allreduce<0>(st, gen, nullptr, nullptr, red);                      // p complete before it is gathered
+        }
+        acc[0] = 0.0;
+        for (int i = tid; i < nloc; i += blockDim.x) {                               // l.18-19, matrix out of shared memory
+            C sum = cmake<C>(0.0, 0.0);
+            if (DOF == 3) {
+                const int lbr = i / 3, rr = i - 3 * lbr;
+                for (int j = s_rowptr[lbr]; j < s_rowptr[lbr + 1]; ++j) {
+                    const C* blk = s_val + j * 9 + rr * 3;
+                    const C* xv = pg + 3ll * s_col[j];
+                    sum = cfma(blk[0], xv[0], sum);
+                    sum = cfma(blk[1], xv[1], sum);
+                    sum = cfma(blk[2], xv[2], sum);
+                }
+            } else {
+#pragma unroll 4
+                for (int j = s_rowptr[i]; j < s_rowptr[i + 1]; ++j) sum = cfma(s_val[j], pg[s_col[j]], sum);
+            }
+            s_q[i] = sum;
+            acc[0] += cdot_re(s_p[i], sum);
+        }
+        fused_allreduce<1>(st, gen, acc, s, red);
+        cgm_scal1_fn(h, res, rc, s[0]);                                               // l.20, 22, 23
+        if (res.done) break;
+        {                                                                             // l.21, 24, 28, 29 out of shared memory
+            const int na = res.nactive;
+            const T beta = (T)rc.beta.re;
+            acc[0] = 0.0;
+            for (int i = tid; i < nloc; i += blockDim.x) {
+                C rv = s_r[i];
+                for (int a = 0; a < na; ++a) {
+                    const int k = rc.active[a];
+                    const T zk = (T)rc.coef[3 * a + 0], ak = (T)rc.coef[3 * a + 1], bk = (T)rc.coef[3 * a + 2];
+                    const C pe = clin_r(zk, rv, ak, s_pk[k * ld + i]);                // l.29 (lagged); n = 0: zk = 1, ak = 0
+                    s_xk[k * ld + i] = caxpy_r(s_xk[k * ld + i], -bk, pe);            // l.28
+                    s_pk[k * ld + i] = pe;
+                }
+                rv = caxpy_r(rv, beta, s_q[i]);                                       // l.21
+                s_r[i] = rv;
+                acc[0] += cnorm2(rv);                                                 // l.24
+            }
+        }
+        fused_allreduce<1>(st, gen, acc, s, red);
+        cgm_scal2_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);        // l.25, 26, 30, 31, 15
+    }
+    // ---- the solutions leave shared memory once
+    {
+        C* x = (C*)h.x;
+        const long long xs = h.x_stride;
+        const bool none = res.n_iter == 0;              // stopped before the first update: x_k = 0 (the host zeroes it too)
+        for (int i = tid; i < nloc; i += blockDim.x)
+            for (int k = 0; k < S; ++k) x[k * xs + row0 + i] = none ? cmake<C>(0.0, 0.0) : s_xk[k * ld + i];
+    }
+    fused_publish(st, res, gen);
+}
+
+// ------------------------------------------------------------------------------------------- host side
+static int res_dof(const msolve_matrix* A) { return A->format == FMT_BSR3 ? 3 : 1; }
+
+// Sizes the shared-memory layout for `ncta` CTAs; false when a CTA's range does not fit.
+static bool resident_layout(const msolve_matrix* A, int S, int ncta, ResLayout* L) {
+    const int dof = res_dof(A);
+    const long long units = dof == 3 ? A->dev.nbrows : A->dev.n;
+    if ((long long)A->h_rowptr.size() != units + 1) return false;
+    long long max_units = 0, max_entries = 0;
+    for (int c = 0; c < ncta; ++c) {
+        const long long u0 = units * c / ncta, u1 = units * (c + 1) / ncta;
+        max_units = std::max(max_units, u1 - u0);
+        max_entries = std::max<long long>(max_entries, A->h_rowptr[u1] - A->h_rowptr[u0]);
+    }
+    const size_t e = elem_bytes(A->dtype);
+    auto up = [](size_t v) { return (v + 15) / 16 * 16; };
+    size_t off = 0;
+    L->max_units = (int)max_units; L->max_rows = (int)(max_units * dof); L->max_entries = (int)max_entries; L->S = S;
+    L->off_rowptr = (int)off; off += up(sizeof(int) * (size_t)(max_units + 1));
+    L->off_col = (int)off; off += up(sizeof(int) * (size_t)max_entries);
+    L->off_val = (int)off; off += up(e * (size_t)max_entries * (dof == 3 ? 9 : 1));
+    const size_t vec = up(e * (size_t)L->max_rows);
+    L->off_r = (int)off; off += vec;
+    L->off_p = (int)off; off += vec;
+    L->off_q = (int)off; off += vec;
+    L->off_xk = (int)off; off += (size_t)S * e * (size_t)L->max_rows;
+    off = up(off);
+    L->off_pk = (int)off; off += (size_t)S * e * (size_t)L->max_rows;
+    const size_t fixed = (size_t)kFusedFixedBytes;
+    if (off + fixed > (size_t)200 * 1024) return false;
+    L->total = (int)(off + fixed);
+    return true;
+}
+
+bool resident_supported(const msolve_matrix* A, int S, int alg) {
+    if (alg != MSOLVE_ALG_CGM) return false;
+    if (A->format != FMT_CSR && A->format != FMT_BSR3) return false;
+    if (A->opt.update_kernel != 0 || A->opt.loop_mode != 0 || A->dev.n == 0) return false;
+    int coop = 0;
+    if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, A->device) != cudaSuccess || !coop) return false;
+    ResLayout L;
+    return resident_layout(A, S, std::min(A->num_sms, kFusedMaxCtas), &L);
+}
+
+template <typename E, int DOF>
+static int launch_resident_t(const msolve_matrix* A, const ResLayout& L, int ncta, cudaStream_t s) {
+    auto kernel = k_cgm_resident<E, DOF>;
+    int rc = ensure_smem(A, (const void*)kernel, L.total);
+    if (rc != MSOLVE_OK) return rc;
+    MatDev dev = A->dev;
+    SolveState* st = A->d_state;
+    ResLayout lay = L;
+    void* args[3] = {&dev, &st, &lay};
+    MSOLVE_CU(cudaLaunchCooperativeKernel((const void*)kernel, dim3(ncta), dim3(kResThreads), args, (size_t)L.total, s));
+    return MSOLVE_OK;
+}
+
+int launch_resident(const msolve_matrix* A, int S, int alg, cudaStream_t s) {
+    (void)alg;
+    const int ncta = std::min(A->num_sms, kFusedMaxCtas);
+    ResLayout L;
+    if (!resident_layout(A, S, ncta, &L)) return fail(MSOLVE_EINVAL, "resident path: the problem does not fit in shared memory");
+    const bool bsr = A->format == FMT_BSR3;
+    switch (A->dtype) {
+        case MSOLVE_C128: return bsr ? launch_resident_t<double2, 3>(A, L, ncta, s) : launch_resident_t<double2, 1>(A, L, ncta, s);
+        case MSOLVE_C64:  return bsr ? launch_resident_t<float2, 3>(A, L, ncta, s) : launch_resident_t<float2, 1>(A, L, ncta, s);
+        case MSOLVE_F64:  return launch_resident_t<double, 1>(A, L, ncta, s);
+        default:          return launch_resident_t<float, 1>(A, L, ncta, s);
+    }
+}
+
+}  // namespace msolve

@@ -16,6 +16,31 @@ def fused(ms):
     return {ms.MSOLVE_CFG_ITER_PATH: 2}
 
 
+def resident(ms):
+    return {ms.MSOLVE_CFG_ITER_PATH: 3}
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
+@pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c2", "csrtile"), ("c5", "csrvector"), ("c2odd", "bsr3"),
+                                       ("c4s", "bsr3")])
+def test_resident_matches_oracle_and_graph(ms, which, fmt, dtype, tol):
+    # MSOLVE_CFG_ITER_PATH = 3 (csrc/resident.cu): matrix and all vectors in shared memory for the whole solve
+    w = {"c1": W.config1, "c2": W.config2, "c2odd": lambda: W.config2(extents=(5, 3, 7, 3)),
+         "c5": lambda: W.config5(n=(1 << 13) + 13), "c4s": lambda: W.config4(extents=(8, 8, 8, 16), want_csr=True)}[which]()
+    w.tol = tol
+    g = gpu_solve(ms, w, dtype, fmt, cfg=resident(ms))
+    o = oracle_solve(w, dtype)
+    check_parity(w, dtype, g, o, w.tol)
+    assert g[5] == 1
+    gg = gpu_solve(ms, w, dtype, fmt)
+    assert abs(gg[1] - g[1]) <= 1
+    for k in range(w.shifts.size):
+        d = np.linalg.norm(g[2][k].astype(np.complex128) - gg[2][k]) / np.linalg.norm(gg[2][k])
+        assert d <= REL[dtype], (k, d)
+    g2 = gpu_solve(ms, w, dtype, fmt, cfg=resident(ms))
+    assert g2[1] == g[1] and np.array_equal(g2[2], g[2]) and np.array_equal(g2[3], g[3])
+
+
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 @pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c2", "bsr3rows"), ("c2", "lat"), ("c2", "latrows"),
                                        ("c5", "csrvector"), ("c3", "csr"), ("c3", "bsr3"), ("c3", "lat"), ("c2odd", "bsr3")])
@@ -37,9 +62,23 @@ def test_fused_matches_oracle_and_graph(ms, which, fmt, dtype, tol):
     assert g2[1] == g[1] and np.array_equal(g2[2], g[2]) and np.array_equal(g2[3], g[3])
 
 
+def test_resident_needs_the_problem_to_fit(ms):
+    # 16 shifts x 49152 rows x 16 B: 35 vectors + matrix = 49 MB do not fit in 148 x 200 KB; asking for the path by
+    # name is an error, AUTO falls back to the L2 one-kernel path
+    w = W.config4(extents=(8, 8, 16, 16))
+    A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks))
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, 3)
+    with pytest.raises(ms.MsolveError):
+        ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
+    ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, 0)
+    r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
+    assert r.status == 0 and ms.msolve_last_launch_count(A) == 1
+    ms.msolve_destroy(A)
+
+
 def test_auto_picks_by_footprint(ms):
-    # AUTO (the library default): one kernel for config 2 (16.5 MB per iteration), the graph of kernels for a
-    # system beyond the 256 MB bound
+    # AUTO (the library default): one kernel for config 2 (11 MB: resident in shared memory; BiCGStab-M: the L2 path),
+    # the graph of kernels for a system beyond the 256 MB bound
     w = W.config2()
     A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks))
     r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
@@ -53,8 +92,9 @@ def test_auto_picks_by_footprint(ms):
     r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
     assert r.status == 0 and ms.msolve_last_launch_count(A) == 2 + 5 * r.iterations
     ms.msolve_destroy(A)
-    # kernels the one-kernel path does not cover stay on the graph path; asking for it by name is an error
-    w = W.config2()
+    # kernels the L2 one-kernel path does not cover stay on the graph path (here a system too large for shared
+    # memory); asking for the one-kernel path by name is an error
+    w = W.config4(extents=(8, 8, 8, 16), want_csr=True)
     A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val), ms.MSOLVE_SPMV_MERGE)
     r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
     assert ms.msolve_last_launch_count(A) == 2 + 6 * r.iterations
@@ -64,11 +104,11 @@ def test_auto_picks_by_footprint(ms):
     ms.msolve_destroy(A)
 
 
-@pytest.mark.parametrize("alg", ["cgm", "bicgstabm"])
-def test_fused_edge_cases(ms, alg):
+@pytest.mark.parametrize("alg,path", [("cgm", 2), ("bicgstabm", 2), ("cgm", 3)])
+def test_fused_edge_cases(ms, alg, path):
     w = W.config2(extents=(4, 4, 4, 4)) if alg == "cgm" else W.config3(extents=(4, 4, 4, 4))
     fn = ms.msolve_cgm if alg == "cgm" else ms.msolve_bicgstabm
-    A = make_matrix(ms, w, np.complex128, "bsr3", cfg=fused(ms))
+    A = make_matrix(ms, w, np.complex128, "bsr3", cfg={ms.MSOLVE_CFG_ITER_PATH: path})
     S = w.shifts.size
     x = torch.full((S, w.n), 7.0, dtype=torch.complex128, device="cuda")
     r = fn(A, torch.zeros(w.n, dtype=torch.complex128, device="cuda"), w.shifts, 1e-10, 100, x=x)       # b = 0
@@ -106,13 +146,14 @@ def test_fused_edge_cases(ms, alg):
     ms.msolve_destroy(A)
 
 
-def test_fused_multirhs_and_real(ms):
+@pytest.mark.parametrize("path", [2, 3])
+def test_fused_multirhs_and_real(ms, path):
     w = W.config2(extents=(4, 6, 4, 6))
     shifts = np.array([0.0, 0.4, 1.0, 1.7])
     rng = np.random.default_rng(41)
     B = rng.standard_normal((4, w.n)) + 1j * rng.standard_normal((4, w.n))
     B = B[0] + shifts[:, None] * B[1] + 0.05 * B
-    A = make_matrix(ms, w, np.complex128, "bsr3", cfg=fused(ms))
+    A = make_matrix(ms, w, np.complex128, "bsr3", cfg={ms.MSOLVE_CFG_ITER_PATH: path})
     g = ms.msolve_solve_multirhs(A, ms.MSOLVE_ALG_CGM, dev(B), shifts, 1e-10, w.max_iter)
     o = oracle.multirhs(w.rowptr, w.colidx, w.val, B, shifts, 1e-10, w.max_iter)
     assert g.status == o.status == 0 and abs(g.iterations - o.iterations) <= 2
@@ -124,7 +165,7 @@ def test_fused_multirhs_and_real(ms):
     w = W.poisson_workload(37, 29, nshifts=15, real=True)
     for dtype, tol, bar in ((np.float64, 1e-10, 1e-9), (np.float32, 1e-5, 1e-4)):
         A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)), ms.MSOLVE_SPMV_VECTOR)
-        ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, 2)
+        ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, path)
         g = ms.msolve_cgm(A, dev(w.b.astype(dtype)), w.shifts, tol, w.max_iter)
         o = oracle.cgm(w.rowptr, w.colidx, w.val.astype(dtype), w.b.astype(dtype), w.shifts, tol, w.max_iter)
         assert g.status == o.status == 0 and abs(g.iterations - o.iterations) <= 2 and ms.msolve_last_launch_count(A) == 1
