@@ -281,6 +281,48 @@ def run_reference(args, rank):
     print(json.dumps(line))
 
 
+def run_slabs(args, ms, torch, w, dtype, fmt):
+    """--slabs P: the same solves through P row slabs on one device (no per-kernel table, no e2e leg)."""
+    if fmt == "lat":
+        raise SystemExit("--slabs takes the assembled forms (bsr3 / csr)")
+    tdt = {np.complex128: torch.complex128, np.complex64: torch.complex64, np.float64: torch.float64, np.float32: torch.float32}[dtype]
+    t0 = time.perf_counter()
+    if fmt == "bsr3":
+        S_ = ms.msolve_slabs_create_bsr3(w.browptr, w.bcolidx, w.blocks.astype(dtype, copy=False), args.slabs)
+    else:
+        S_ = ms.msolve_slabs_create_csr(w.rowptr, w.colidx, w.val.astype(dtype, copy=False), args.slabs)
+    torch.cuda.synchronize()
+    t_create = time.perf_counter() - t0
+    solve = ms.msolve_slabs_cgm if w.algorithm == "cgm" else ms.msolve_slabs_bicgstabm
+    b_dev = torch.from_numpy(w.b.astype(dtype)).cuda()
+    nS = int(w.shifts.size)
+    x_dev = torch.empty((nS, w.n), dtype=tdt, device="cuda")
+    for _ in range(args.warmup):
+        res = solve(S_, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    iters, launches = 0, 0
+    ev0.record()
+    for _ in range(args.steps):
+        res = solve(S_, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev)
+        iters += res.iterations
+        launches += ms.msolve_slabs_last_launch_count(S_)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms_total = ev0.elapsed_time(ev1)
+    halo = ms.msolve_slabs_halo_elements(S_)
+    cfg = config_dict(args, w, dtype, fmt, 1, nS, nS)
+    cfg["parallelism"] = "%d row slabs on one device (halo exchange + summed dot products, csrc/slab.cu)" % args.slabs
+    line = {"metric": METRIC, "value": throughput(iters, ms_total), "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": DTYPE_NAME[dtype], "data": "synthetic", "config": cfg,
+            "iterations_per_solve": iters / args.steps, "status": res.status, "create_ms": 1e3 * t_create,
+            "halo_elements_per_slab": halo, "halo_bytes_per_exchange": int(sum(halo)) * np.dtype(dtype).itemsize,
+            "gpu_launches": int(launches)}
+    print(json.dumps(line))
+    ms.msolve_slabs_destroy(S_)
+
+
 # ----------------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -305,6 +347,9 @@ def main():
     ap.add_argument("--fused-ctas", type=int, default=0, help="CTAs of the one-kernel path (0 = by problem size)")
     ap.add_argument("--matrix-l2", default="auto", choices=["auto", "stream", "keep"],
                     help="L2 policy of the matrix stream (MSOLVE_CFG_MATRIX_L2)")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="row partition on ONE device (msolve_slabs_*, SURVEY 8(f)-3): P slabs with halo exchange and "
+                         "summed dot products; measures what the partition costs against the unpartitioned solve")
     ap.add_argument("--shard", default="replicas", choices=["replicas", "shifts"],
                     help="N > 1: replicas = every rank solves the whole family for its own right-hand side (weak "
                          "scaling, default); shifts = the ranks split the shifts of ONE system (strong scaling)")
@@ -352,6 +397,9 @@ def main():
     def dev(a):
         return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
+    if args.slabs > 0:
+        run_slabs(args, ms, torch, w, dtype, fmt)
+        return
     t_create = time.perf_counter()
     flags = {"auto": ms.MSOLVE_SPMV_AUTO, "vector": ms.MSOLVE_SPMV_VECTOR, "merge": ms.MSOLVE_SPMV_MERGE, "tile": ms.MSOLVE_SPMV_TILE}[args.spmv]
     if fmt == "bsr3":

@@ -95,9 +95,10 @@ enum {
                                 (one kernel per step of Alg. 1; HBM-bound sizes), 2 = the WHOLE solve as one cooperative
                                 kernel with grid-wide barriers between the steps (systems that live in L2, where kernel
                                 launches, not bytes, are the cost; vector-CSR, BSR3 and lattice handles), 3 = one
-                                cooperative kernel with the matrix and every vector RESIDENT IN SHARED MEMORY (CG-M on
-                                CSR / BSR3 handles whose matrix and 3 + 2 nshifts vectors fit in the shared memory of
-                                the SMs, a few MB: only p and the dot products touch global memory per iteration),
+                                cooperative kernel with the matrix and every vector RESIDENT IN SHARED MEMORY (CSR / BSR3
+                                handles whose matrix and 3 + 2 nshifts (BiCGStab-M: 6 + 2 nshifts) vectors fit in the
+                                shared memory of the SMs, a few MB: only the gathered vector and the dot products touch
+                                global memory per iteration),
                                 0 = by footprint (default): 3 when it fits, else 2 when matrix + (4 + 2 nshifts) vectors
                                 take at most 256 MB, else 1.
                                 Same arithmetic step for step; the paths group the dot products differently (per-CTA

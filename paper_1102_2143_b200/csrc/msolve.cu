@@ -530,7 +530,7 @@ int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const 
     // kernel (fused_small.cu).  AUTO: matrix + (4 + 2 S) vectors at most kFusedMaxBytes.
     // the smallest systems (a few MB) even fit in the shared memory of the 148 SMs: resident.cu (CG-M, CSR / BSR3)
     bool resident = false;
-    if (alg == MSOLVE_ALG_CGM && (A->opt.iter_path == 3 || A->opt.iter_path == 0) && (A->format == FMT_CSR || A->format == FMT_BSR3) &&
+    if ((A->opt.iter_path == 3 || A->opt.iter_path == 0) && (A->format == FMT_CSR || A->format == FMT_BSR3) &&
         matrix_bytes(A) + (size_t)(3 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kResidentMaxBytes) {
         const size_t units = A->format == FMT_BSR3 ? (size_t)A->dev.nbrows : (size_t)A->dev.n;
         if (A->h_rowptr.size() != units + 1) {
@@ -540,7 +540,7 @@ int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const 
         }
         resident = resident_supported(A, S, alg);
     }
-    if (A->opt.iter_path == 3 && !resident) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 3 needs CG-M on a CSR / BSR3 handle whose matrix and 3 + 2 nshifts vectors fit in shared memory");
+    if (A->opt.iter_path == 3 && !resident) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 3 needs a CSR / BSR3 handle whose matrix and vectors fit in shared memory");
     const bool fused = resident || A->opt.iter_path == 2 ||
                        (A->opt.iter_path == 0 && fused_supported(A) &&
                         matrix_bytes(A) + (size_t)(4 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kFusedMaxBytes);

@@ -1,4 +1,4 @@
-// resident.cu -- CG-M with the whole problem resident in SHARED MEMORY (BASELINE configs 1-2 and the like).
+// resident.cu -- CG-M and BiCGStab-M with the whole problem resident in SHARED MEMORY (BASELINE configs 1-2 and the like).
 //
 // A B200 has 148 SMs x 227 KB = 33 MB of shared memory.  When the matrix and all 3 + 2S vectors of the solve fit
 // there, one persistent cooperative kernel gives every CTA a contiguous range of rows and keeps, for the whole
@@ -27,50 +27,85 @@ struct ResLayout {
     int max_rows;        // scalar rows per CTA (upper bound)
     int max_units;       // index rows per CTA: scalar rows (CSR) or block rows (BSR3)
     int max_entries;     // non-zeros (CSR) or blocks (BSR3) per CTA
-    int off_rowptr, off_col, off_val, off_r, off_p, off_q, off_xk, off_pk;
+    int off_rowptr, off_col, off_val, off_r, off_p, off_q, off_s, off_t, off_b, off_xk, off_pk;   // s, t, b: BiCGStab-M only
     int S;
     int total;
 };
 
+// (A x)_i for local scalar row i: matrix out of shared memory, x gathered from global memory
+template <typename C, int DOF>
+__device__ __forceinline__ C res_row_product(int i, const int* s_rowptr, const int* s_col, const C* s_val, const C* xg) {
+    C sum = cmake<C>(0.0, 0.0);
+    if (DOF == 3) {
+        const int lbr = i / 3, rr = i - 3 * lbr;
+        for (int j = s_rowptr[lbr]; j < s_rowptr[lbr + 1]; ++j) {
+            const C* blk = s_val + j * 9 + rr * 3;
+            const C* xv = xg + 3ll * s_col[j];
+            sum = cfma(blk[0], xv[0], sum);
+            sum = cfma(blk[1], xv[1], sum);
+            sum = cfma(blk[2], xv[2], sum);
+        }
+    } else {
+#pragma unroll 4
+        for (int j = s_rowptr[i]; j < s_rowptr[i + 1]; ++j) sum = cfma(s_val[j], xg[s_col[j]], sum);
+    }
+    return sum;
+}
+
+// what both kernels start with: private state, the CTA's range, its slice of the matrix into shared memory
+#define MSOLVE_RESIDENT_PROLOGUE                                                                        \
+    typedef E C;                                                                                        \
+    typedef typename RealOf<E>::type T;                                                                 \
+    extern __shared__ __align__(16) unsigned char dyn[];                                                \
+    Recur& rc = *(Recur*)dyn;                                                                           \
+    SolveResult& res = *(SolveResult*)(dyn + kFusedOffRes);                                             \
+    const SolveHeader& h = *(const SolveHeader*)(dyn + kFusedOffHdr);                                   \
+    double* rhs_norm = (double*)(dyn + kFusedOffNorm);                                                  \
+    unsigned char* base = dyn + kFusedFixedBytes;                                                       \
+    __shared__ double red[kAccMax * 32];                                                                \
+    fused_stage_header(st, dyn + kFusedOffHdr, rhs_norm);                                               \
+    const int cta = blockIdx.x, ncta = gridDim.x, tid = threadIdx.x;                                    \
+    const long long units = DOF == 3 ? A.nbrows : A.n;                                                  \
+    const long long u0 = units * cta / ncta, u1 = units * (cta + 1) / ncta;                             \
+    const int nu = (int)(u1 - u0), nloc = nu * DOF;                                                     \
+    const long long row0 = u0 * DOF;                                                                    \
+    int* s_rowptr = (int*)(base + L.off_rowptr);                                                        \
+    int* s_col = (int*)(base + L.off_col);                                                              \
+    C* s_val = (C*)(base + L.off_val);                                                                  \
+    C* s_r = (C*)(base + L.off_r);                                                                      \
+    C* s_p = (C*)(base + L.off_p);                                                                      \
+    C* s_q = (C*)(base + L.off_q);                                                                      \
+    C* s_xk = (C*)(base + L.off_xk);     /* [S][max_rows] */                                            \
+    C* s_pk = (C*)(base + L.off_pk);                                                                    \
+    const int ld = L.max_rows;                                                                          \
+    const int S = h.S;                                                                                  \
+    C* pg = (C*)h.p;                     /* lives in global memory: gathered across CTAs */              \
+    {                                                                                                   \
+        const int e0 = A.rowptr[u0];                                                                    \
+        const int ne = A.rowptr[u1] - e0;                                                               \
+        for (int i = tid; i <= nu; i += blockDim.x) s_rowptr[i] = A.rowptr[u0 + i] - e0;                \
+        for (int j = tid; j < ne; j += blockDim.x) s_col[j] = A.colidx[e0 + j];                         \
+        const C* gv = (const C*)A.val + (long long)e0 * (DOF == 3 ? 9 : 1);                             \
+        const int nv = ne * (DOF == 3 ? 9 : 1);                                                         \
+        for (int j = tid; j < nv; j += blockDim.x) s_val[j] = gv[j];                                    \
+    }                                                                                                   \
+    (void)sizeof(T); (void)cta
+
+// the solutions leave shared memory once
+#define MSOLVE_RESIDENT_EPILOGUE                                                                        \
+    {                                                                                                   \
+        C* x = (C*)h.x;                                                                                 \
+        const long long xs = h.x_stride;                                                                \
+        const bool none = res.n_iter == 0;   /* stopped before the first update: x_k = 0 */             \
+        for (int i = tid; i < nloc; i += blockDim.x)                                                    \
+            for (int k = 0; k < S; ++k) x[k * xs + row0 + i] = none ? cmake<C>(0.0, 0.0) : s_xk[k * ld + i]; \
+    }                                                                                                   \
+    fused_publish(st, res, gen)
+
 template <typename E, int DOF>
 __global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, SolveState* st, ResLayout L) {
-    typedef E C;
-    typedef typename RealOf<E>::type T;
-    extern __shared__ __align__(16) unsigned char dyn[];
-    Recur& rc = *(Recur*)dyn;
-    SolveResult& res = *(SolveResult*)(dyn + kFusedOffRes);
-    const SolveHeader& h = *(const SolveHeader*)(dyn + kFusedOffHdr);
-    double* rhs_norm = (double*)(dyn + kFusedOffNorm);
-    unsigned char* base = dyn + kFusedFixedBytes;
-    __shared__ double red[kAccMax * 32];
-    fused_stage_header(st, dyn + kFusedOffHdr, rhs_norm);
-    const int cta = blockIdx.x, ncta = gridDim.x, tid = threadIdx.x;
-    // this CTA's range of index rows (units) and scalar rows
-    const long long units = DOF == 3 ? A.nbrows : A.n;
-    const long long u0 = units * cta / ncta, u1 = units * (cta + 1) / ncta;
-    const int nu = (int)(u1 - u0), nloc = nu * DOF;
-    const long long row0 = u0 * DOF;
-    int* s_rowptr = (int*)(base + L.off_rowptr);
-    int* s_col = (int*)(base + L.off_col);
-    C* s_val = (C*)(base + L.off_val);
-    C* s_r = (C*)(base + L.off_r);
-    C* s_p = (C*)(base + L.off_p);
-    C* s_q = (C*)(base + L.off_q);
-    C* s_xk = (C*)(base + L.off_xk);     // [S][max_rows]
-    C* s_pk = (C*)(base + L.off_pk);
-    const int ld = L.max_rows;
-    const int S = h.S;
-    C* pg = (C*)h.p;                     // the one vector that lives in global memory: gathered across CTAs
-    // ---- load the matrix range (once) and the vectors: r <- b, p <- b, x_k <- 0, p_k <- b  (l.9-12)
-    const int e0 = A.rowptr[u0];
-    const int ne = A.rowptr[u1] - e0;
-    for (int i = tid; i <= nu; i += blockDim.x) s_rowptr[i] = A.rowptr[u0 + i] - e0;
-    for (int j = tid; j < ne; j += blockDim.x) s_col[j] = A.colidx[e0 + j];
-    {
-        const C* gv = (const C*)A.val + (long long)e0 * (DOF == 3 ? 9 : 1);
-        const int nv = ne * (DOF == 3 ? 9 : 1);
-        for (int j = tid; j < nv; j += blockDim.x) s_val[j] = gv[j];
-    }
+    MSOLVE_RESIDENT_PROLOGUE;
+    // r <- b, p <- b, x_k <- 0, p_k <- b  (l.9-12)
     double acc[1] = {0.0}, s[1];
     for (int i = tid; i < nloc; i += blockDim.x) {
         const C bv = ((const C*)h.b)[row0 + i];
@@ -94,20 +129,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, Solve
         }
         acc[0] = 0.0;
         for (int i = tid; i < nloc; i += blockDim.x) {                               // l.18-19, matrix out of shared memory
-            C sum = cmake<C>(0.0, 0.0);
-            if (DOF == 3) {
-                const int lbr = i / 3, rr = i - 3 * lbr;
-                for (int j = s_rowptr[lbr]; j < s_rowptr[lbr + 1]; ++j) {
-                    const C* blk = s_val + j * 9 + rr * 3;
-                    const C* xv = pg + 3ll * s_col[j];
-                    sum = cfma(blk[0], xv[0], sum);
-                    sum = cfma(blk[1], xv[1], sum);
-                    sum = cfma(blk[2], xv[2], sum);
-                }
-            } else {
-#pragma unroll 4
-                for (int j = s_rowptr[i]; j < s_rowptr[i + 1]; ++j) sum = cfma(s_val[j], pg[s_col[j]], sum);
-            }
+            const C sum = res_row_product<C, DOF>(i, s_rowptr, s_col, s_val, pg);
             s_q[i] = sum;
             acc[0] += cdot_re(s_p[i], sum);
         }
@@ -135,22 +157,101 @@ __global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, Solve
         fused_allreduce<1>(st, gen, acc, s, red);
         cgm_scal2_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);        // l.25, 26, 30, 31, 15
     }
-    // ---- the solutions leave shared memory once
-    {
-        C* x = (C*)h.x;
-        const long long xs = h.x_stride;
-        const bool none = res.n_iter == 0;              // stopped before the first update: x_k = 0 (the host zeroes it too)
-        for (int i = tid; i < nloc; i += blockDim.x)
-            for (int k = 0; k < S; ++k) x[k * xs + row0 + i] = none ? cmake<C>(0.0, 0.0) : s_xk[k * ld + i];
+    MSOLVE_RESIDENT_EPILOGUE;
+}
+
+// BiCGStab-M, same residency: r, p, q, s, t, b and every x_k, p_k in shared memory; p and s are the two vectors the
+// SpMVs gather, so they are mirrored in global memory.  Steps and per-element arithmetic of k_bi_fused / bi_update_fn.
+template <typename E, int DOF>
+__global__ void __launch_bounds__(kResThreads, 1) k_bi_resident(MatDev A, SolveState* st, ResLayout L) {
+    MSOLVE_RESIDENT_PROLOGUE;
+    C* s_s = (C*)(base + L.off_s);
+    C* s_t = (C*)(base + L.off_t);
+    C* s_b = (C*)(base + L.off_b);
+    C* sg = (C*)h.s;
+    __shared__ C s_c[kMaxShifts * 7];
+    double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0}, s[5];
+    for (int i = tid; i < nloc; i += blockDim.x) {
+        const C bv = ((const C*)h.b)[row0 + i];
+        s_r[i] = bv; s_p[i] = bv; s_b[i] = bv;
+        pg[row0 + i] = bv;
+        for (int k = 0; k < S; ++k) { s_xk[k * ld + i] = cmake<C>(0.0, 0.0); s_pk[k * ld + i] = bv; }
+        acc[0] += cnorm2(bv);
     }
-    fused_publish(st, res, gen);
+    unsigned long long gen = st->fused_gen;
+    fused_allreduce<1>(st, gen, acc, s, red);
+    init_state_fn(h, res, rc, s[0]);
+    while (!res.done) {
+        acc[0] = acc[1] = 0.0;
+        for (int i = tid; i < nloc; i += blockDim.x) {                               // q = A p, <r0,q>
+            const C sum = res_row_product<C, DOF>(i, s_rowptr, s_col, s_val, pg);
+            s_q[i] = sum;
+            acc[0] += cdot_re(s_b[i], sum);
+            acc[1] += cdot_im(s_b[i], sum);
+        }
+        fused_allreduce<2>(st, gen, acc, s, red);
+        bi_scal1_fn(h, res, rc, zd{s[0], s[1]});
+        if (res.done) break;
+        {
+            const C beta = cmake<C>(rc.beta.re, rc.beta.im);
+            for (int i = tid; i < nloc; i += blockDim.x) {                           // s = r + beta q
+                const C sv = cfma(beta, s_q[i], s_r[i]);
+                s_s[i] = sv;
+                sg[row0 + i] = sv;
+            }
+        }
+        fused_allreduce<0>(st, gen, nullptr, nullptr, red);                          // s complete before it is gathered
+#pragma unroll
+        for (int a = 0; a < 5; ++a) acc[a] = 0.0;
+        for (int i = tid; i < nloc; i += blockDim.x) {                               // t = A s, <t,s>, <t,t>, <r0,t>
+            const C sum = res_row_product<C, DOF>(i, s_rowptr, s_col, s_val, sg);
+            s_t[i] = sum;
+            const C xi = s_s[i], ui = s_b[i];
+            acc[0] += cdot_re(sum, xi);
+            acc[1] += cdot_im(sum, xi);
+            acc[2] += cnorm2(sum);
+            acc[3] += cdot_re(ui, sum);
+            acc[4] += cdot_im(ui, sum);
+        }
+        fused_allreduce<5>(st, gen, acc, s, red);
+        bi_scal2_fn(h, res, rc, s);
+        if (res.done) break;
+        {
+            const int na = res.nactive;
+            for (int j = tid; j < 7 * na; j += blockDim.x) s_c[j] = cmake<C>(rc.coef[2 * j], rc.coef[2 * j + 1]);
+            const C chi = cmake<C>(rc.chi.re, rc.chi.im);
+            const C alpha_new = cmake<C>(rc.alpha_new.re, rc.alpha_new.im);
+            __syncthreads();
+            acc[0] = 0.0;
+            for (int i = tid; i < nloc; i += blockDim.x) {                           // r', p, x_k, p_k, |r'|^2
+                const C rv = s_r[i], sv = s_s[i];
+                const C rn = csub(sv, cmul(chi, s_t[i]));
+                const C pn = cadd(rn, cmul(alpha_new, csub(s_p[i], cmul(chi, s_q[i]))));
+                acc[0] += cnorm2(rn);
+                for (int a = 0; a < na; ++a) {
+                    const int k = rc.active[a];
+                    const C* c = s_c + 7 * a;
+                    const C pe = s_pk[k * ld + i];
+                    s_xk[k * ld + i] = cadd(csub(s_xk[k * ld + i], cmul(c[0], pe)), cmul(c[1], sv));
+                    const C ds = csub(cmul(c[5], sv), cmul(c[6], rv));
+                    s_pk[k * ld + i] = cadd(cmul(c[2], rn), cmul(c[3], csub(pe, cmul(c[4], ds))));
+                }
+                s_r[i] = rn;
+                s_p[i] = pn;
+                pg[row0 + i] = pn;
+            }
+        }
+        fused_allreduce<1>(st, gen, acc, s, red);                                    // also: p complete before SpMV#1
+        bi_scal3_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);
+    }
+    MSOLVE_RESIDENT_EPILOGUE;
 }
 
 // ------------------------------------------------------------------------------------------- host side
 static int res_dof(const msolve_matrix* A) { return A->format == FMT_BSR3 ? 3 : 1; }
 
 // Sizes the shared-memory layout for `ncta` CTAs; false when a CTA's range does not fit.
-static bool resident_layout(const msolve_matrix* A, int S, int ncta, ResLayout* L) {
+static bool resident_layout(const msolve_matrix* A, int S, int alg, int ncta, ResLayout* L) {
     const int dof = res_dof(A);
     const long long units = dof == 3 ? A->dev.nbrows : A->dev.n;
     if ((long long)A->h_rowptr.size() != units + 1) return false;
@@ -171,6 +272,12 @@ static bool resident_layout(const msolve_matrix* A, int S, int ncta, ResLayout* 
     L->off_r = (int)off; off += vec;
     L->off_p = (int)off; off += vec;
     L->off_q = (int)off; off += vec;
+    L->off_s = L->off_t = L->off_b = 0;
+    if (alg == MSOLVE_ALG_BICGSTABM) {
+        L->off_s = (int)off; off += vec;
+        L->off_t = (int)off; off += vec;
+        L->off_b = (int)off; off += vec;
+    }
     L->off_xk = (int)off; off += (size_t)S * e * (size_t)L->max_rows;
     off = up(off);
     L->off_pk = (int)off; off += (size_t)S * e * (size_t)L->max_rows;
@@ -181,18 +288,17 @@ static bool resident_layout(const msolve_matrix* A, int S, int ncta, ResLayout* 
 }
 
 bool resident_supported(const msolve_matrix* A, int S, int alg) {
-    if (alg != MSOLVE_ALG_CGM) return false;
     if (A->format != FMT_CSR && A->format != FMT_BSR3) return false;
     if (A->opt.update_kernel != 0 || A->opt.loop_mode != 0 || A->dev.n == 0) return false;
     int coop = 0;
     if (cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, A->device) != cudaSuccess || !coop) return false;
     ResLayout L;
-    return resident_layout(A, S, std::min(A->num_sms, kFusedMaxCtas), &L);
+    return resident_layout(A, S, alg, std::min(A->num_sms, kFusedMaxCtas), &L);
 }
 
 template <typename E, int DOF>
-static int launch_resident_t(const msolve_matrix* A, const ResLayout& L, int ncta, cudaStream_t s) {
-    auto kernel = k_cgm_resident<E, DOF>;
+static int launch_resident_t(const msolve_matrix* A, int alg, const ResLayout& L, int ncta, cudaStream_t s) {
+    auto kernel = alg == MSOLVE_ALG_CGM ? k_cgm_resident<E, DOF> : k_bi_resident<E, DOF>;
     int rc = ensure_smem(A, (const void*)kernel, L.total);
     if (rc != MSOLVE_OK) return rc;
     MatDev dev = A->dev;
@@ -204,16 +310,15 @@ static int launch_resident_t(const msolve_matrix* A, const ResLayout& L, int nct
 }
 
 int launch_resident(const msolve_matrix* A, int S, int alg, cudaStream_t s) {
-    (void)alg;
     const int ncta = std::min(A->num_sms, kFusedMaxCtas);
     ResLayout L;
-    if (!resident_layout(A, S, ncta, &L)) return fail(MSOLVE_EINVAL, "resident path: the problem does not fit in shared memory");
+    if (!resident_layout(A, S, alg, ncta, &L)) return fail(MSOLVE_EINVAL, "resident path: the problem does not fit in shared memory");
     const bool bsr = A->format == FMT_BSR3;
     switch (A->dtype) {
-        case MSOLVE_C128: return bsr ? launch_resident_t<double2, 3>(A, L, ncta, s) : launch_resident_t<double2, 1>(A, L, ncta, s);
-        case MSOLVE_C64:  return bsr ? launch_resident_t<float2, 3>(A, L, ncta, s) : launch_resident_t<float2, 1>(A, L, ncta, s);
-        case MSOLVE_F64:  return launch_resident_t<double, 1>(A, L, ncta, s);
-        default:          return launch_resident_t<float, 1>(A, L, ncta, s);
+        case MSOLVE_C128: return bsr ? launch_resident_t<double2, 3>(A, alg, L, ncta, s) : launch_resident_t<double2, 1>(A, alg, L, ncta, s);
+        case MSOLVE_C64:  return bsr ? launch_resident_t<float2, 3>(A, alg, L, ncta, s) : launch_resident_t<float2, 1>(A, alg, L, ncta, s);
+        case MSOLVE_F64:  return launch_resident_t<double, 1>(A, alg, L, ncta, s);
+        default:          return launch_resident_t<float, 1>(A, alg, L, ncta, s);
     }
 }
 

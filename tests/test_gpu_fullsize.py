@@ -78,10 +78,14 @@ def c4():
     return w, refs
 
 
-C4_VARIANTS = ["bsr3", "csr", "csrmerge", "lat", "lat1", "lat2", "lat3", "bsr3_updtma"]
+C4_VARIANTS = ["bsr3", "csr", "csrmerge", "lat", "lat1", "lat2", "lat3", "bsr3_updtma", "slabs8_bsr3", "slabs3_csr"]
 
 
 def _c4_matrix(ms, w, dtype, variant):
+    if variant == "slabs8_bsr3":        # row partition: 8 slabs along t (2 x 32^3 sites of halo per slab), csrc/slab.cu
+        return ms.msolve_slabs_create_bsr3(w.browptr, w.bcolidx, w.blocks.astype(dtype), 8)
+    if variant == "slabs3_csr":         # three slabs that do not divide the lattice evenly, TMA-staged vector-CSR per slab
+        return ms.msolve_slabs_create_csr(w.rowptr, w.colidx, w.val.astype(dtype), 3)
     if variant in ("bsr3", "bsr3_updtma"):
         A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
         if variant == "bsr3_updtma":
@@ -102,12 +106,45 @@ def _c4_matrix(ms, w, dtype, variant):
 def test_config4_full_vs_oracle(ms, c4, dtype, tol, variant):
     w, refs = c4
     A = _c4_matrix(ms, w, dtype, variant)
-    res = ms.msolve_cgm(A, dev(w.b.astype(dtype)), w.shifts, tol, w.max_iter)
+    if variant.startswith("slabs"):
+        res = ms.msolve_slabs_cgm(A, dev(w.b.astype(dtype)), w.shifts, tol, w.max_iter)
+        if variant == "slabs8_bsr3":     # every slab receives the two neighbouring time slices: 2 x 32^3 sites x 3 colours
+            assert ms.msolve_slabs_halo_elements(A) == [2 * 32 * 32 * 32 * 3] * 8
+    else:
+        res = ms.msolve_cgm(A, dev(w.b.astype(dtype)), w.shifts, tol, w.max_iter)
     worst = compare_full(w, dtype, tol, res, refs[dtype], residual_shifts=(0, 7, 15))
     print("config 4 %s %s: %d iterations, worst relative L2 difference %.2e" % (np.dtype(dtype).name, variant, res.iterations, worst))
-    ms.msolve_destroy(A)
+    (ms.msolve_slabs_destroy if variant.startswith("slabs") else ms.msolve_destroy)(A)
     del res, A
     torch.cuda.empty_cache()
+
+
+def test_config4_full_multirhs_vs_oracle(ms, c4):
+    # eq. (6) at the size bench.py times: three systems whose right-hand sides vary smoothly with the shift
+    w, _ = c4
+    shifts = np.array([0.0, 0.3, 1.0])
+    rng = np.random.default_rng(51)
+    c = rng.standard_normal((2, w.n)) + 1j * rng.standard_normal((2, w.n))
+    g = rng.standard_normal((3, w.n)) + 1j * rng.standard_normal((3, w.n))
+    B = np.array([c[0] + t * c[1] + 0.05 * g[i] for i, t in enumerate(shifts)])
+    B /= np.linalg.norm(B[0])
+    del c, g
+    A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks))
+    res = ms.msolve_solve_multirhs(A, ms.MSOLVE_ALG_CGM, dev(B), shifts, 1e-10, w.max_iter)
+    ref = oracle.multirhs(w.rowptr, w.colidx, w.val, B, shifts, 1e-10, w.max_iter)
+    assert res.status == ref.status == 0 and abs(res.iterations - ref.iterations) <= 2
+    rows = np.random.default_rng(0).integers(0, w.n, 2000)
+    for k, s in enumerate(shifts):
+        xk = res.x[k].cpu().numpy()
+        diff = xk - ref.x[k]
+        assert np.linalg.norm(diff) <= 1e-9 * np.linalg.norm(ref.x[k]), k
+        assert np.abs(diff).max() <= MAXABS_C * 1e-9 * np.abs(ref.x[k]).max(), k
+        out = np.empty(rows.size, dtype=np.complex128)
+        for t, i in enumerate(rows):
+            lo, hi = w.rowptr[i], w.rowptr[i + 1]
+            out[t] = B[k, i] - (np.dot(w.val[lo:hi], xk[w.colidx[lo:hi]]) + s * xk[i])
+        assert np.sqrt(np.mean(np.abs(out) ** 2) * w.n) <= 10 * 1e-10 * np.linalg.norm(B[k]), k
+    ms.msolve_destroy(A)
 
 
 # ------------------------------------------------------------------------------------------ config 5

@@ -22,12 +22,13 @@ def resident(ms):
 
 @pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-10), (np.complex64, 1e-5)])
 @pytest.mark.parametrize("which,fmt", [("c1", "csr"), ("c2", "csr"), ("c2", "bsr3"), ("c2", "csrtile"), ("c5", "csrvector"), ("c2odd", "bsr3"),
-                                       ("c4s", "bsr3")])
+                                       ("c4s", "bsr3"), ("c3s", "bsr3"), ("c3s", "csr")])
 def test_resident_matches_oracle_and_graph(ms, which, fmt, dtype, tol):
     # MSOLVE_CFG_ITER_PATH = 3 (csrc/resident.cu): matrix and all vectors in shared memory for the whole solve
     w = {"c1": W.config1, "c2": W.config2, "c2odd": lambda: W.config2(extents=(5, 3, 7, 3)),
-         "c5": lambda: W.config5(n=(1 << 13) + 13), "c4s": lambda: W.config4(extents=(8, 8, 8, 16), want_csr=True)}[which]()
-    w.tol = tol
+         "c5": lambda: W.config5(n=(1 << 13) + 13), "c4s": lambda: W.config4(extents=(8, 8, 8, 16), want_csr=True),
+         "c3s": lambda: W.config3(extents=(8, 8, 6, 6))}[which]()          # BiCGStab-M
+    w.tol = 10 * tol if which == "c3s" else tol
     g = gpu_solve(ms, w, dtype, fmt, cfg=resident(ms))
     o = oracle_solve(w, dtype)
     check_parity(w, dtype, g, o, w.tol)
@@ -104,7 +105,7 @@ def test_auto_picks_by_footprint(ms):
     ms.msolve_destroy(A)
 
 
-@pytest.mark.parametrize("alg,path", [("cgm", 2), ("bicgstabm", 2), ("cgm", 3)])
+@pytest.mark.parametrize("alg,path", [("cgm", 2), ("bicgstabm", 2), ("cgm", 3), ("bicgstabm", 3)])
 def test_fused_edge_cases(ms, alg, path):
     w = W.config2(extents=(4, 4, 4, 4)) if alg == "cgm" else W.config3(extents=(4, 4, 4, 4))
     fn = ms.msolve_cgm if alg == "cgm" else ms.msolve_bicgstabm
