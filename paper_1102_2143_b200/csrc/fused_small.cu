@@ -33,14 +33,14 @@ __device__ __forceinline__ void fused_spmv(const MatDev& A, const SolveHeader& h
 }
 
 template <typename E, int VEC, int SEL>
-__global__ void __launch_bounds__(kFusedThreads, 1) k_cgm_fused(MatDev A, SolveState* st) {
+__global__ void __launch_bounds__(kFusedThreads, 1) k_cgm_fused(MatDev A, SolveState* st, const __grid_constant__ SolveHeader hp) {
     extern __shared__ __align__(16) unsigned char dyn[];
     Recur& rc = *(Recur*)dyn;
     SolveResult& res = *(SolveResult*)(dyn + kFusedOffRes);
     const SolveHeader& h = *(const SolveHeader*)(dyn + kFusedOffHdr);
     double* rhs_norm = (double*)(dyn + kFusedOffNorm);
     __shared__ double red[kAccMax * 32];
-    fused_stage_header(st, dyn + kFusedOffHdr, rhs_norm);
+    fused_stage_header(hp, st, dyn + kFusedOffHdr, rhs_norm);
     const int cta = blockIdx.x, ncta = gridDim.x;
     unsigned long long gen = st->fused_gen;                                           // written back by CTA 0 at the end
     double acc[1], s[1];
@@ -65,14 +65,14 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_cgm_fused(MatDev A, SolveS
 }
 
 template <typename E, int VEC, int SEL>
-__global__ void __launch_bounds__(kFusedThreads, 1) k_bi_fused(MatDev A, SolveState* st) {
+__global__ void __launch_bounds__(kFusedThreads, 1) k_bi_fused(MatDev A, SolveState* st, const __grid_constant__ SolveHeader hp) {
     extern __shared__ __align__(16) unsigned char dyn[];
     Recur& rc = *(Recur*)dyn;
     SolveResult& res = *(SolveResult*)(dyn + kFusedOffRes);
     const SolveHeader& h = *(const SolveHeader*)(dyn + kFusedOffHdr);
     double* rhs_norm = (double*)(dyn + kFusedOffNorm);
     __shared__ double red[kAccMax * 32];
-    fused_stage_header(st, dyn + kFusedOffHdr, rhs_norm);
+    fused_stage_header(hp, st, dyn + kFusedOffHdr, rhs_norm);
     const int cta = blockIdx.x, ncta = gridDim.x;
     unsigned long long gen = st->fused_gen;
     double acc[5], s[5];
@@ -130,7 +130,8 @@ static int launch_coop(const msolve_matrix* A, K kernel, long long work_threads,
     if (A->opt.fused_ctas > 0) grid = std::min(cap, A->opt.fused_ctas);
     MatDev dev = A->dev;
     SolveState* st = A->d_state;
-    void* args[2] = {&dev, &st};
+    SolveHeader hdr = A->h_stage->h;
+    void* args[3] = {&dev, &st, &hdr};
     MSOLVE_CU(cudaLaunchCooperativeKernel((const void*)kernel, dim3(grid), dim3(kFusedThreads), args, (size_t)smem, s));
     return MSOLVE_OK;
 }

@@ -90,8 +90,9 @@ __device__ __forceinline__ void fused_allreduce(SolveState* st, unsigned long lo
 
 // The header (pointers, sizes, shifts) and the per-system norms of eq. (6) are read in every phase; every barrier
 // invalidates L1, so they live in shared memory for the whole solve.
-__device__ __forceinline__ void fused_stage_header(const SolveState* st, unsigned char* dst, double* rhs_norm) {
-    const int* src = (const int*)&st->h;
+// The header arrives as a KERNEL ARGUMENT (no host-to-device copy before the launch).
+__device__ __forceinline__ void fused_stage_header(const SolveHeader& hp, const SolveState* st, unsigned char* dst, double* rhs_norm) {
+    const int* src = (const int*)&hp;
     int* d = (int*)dst;
     for (int i = threadIdx.x; i < (int)(sizeof(SolveHeader) / sizeof(int)); i += blockDim.x) d[i] = src[i];
     for (int k = threadIdx.x; k < kMaxShifts; k += blockDim.x) rhs_norm[k] = st->rhs_norm[k];

@@ -546,7 +546,7 @@ int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const 
                         matrix_bytes(A) + (size_t)(4 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kFusedMaxBytes);
     if (fused) {
         if (!resident && !fused_supported(A)) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 2 needs a vector-CSR, BSR3 or lattice handle, the register update kernel and the WHILE loop mode");
-        CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
+        // the header travels as a kernel argument and the kernel initialises the result block itself: no H2D copy
         rc = resident ? launch_resident(A, S, alg, stream) : launch_fused(A, alg, stream);
         if (rc != MSOLVE_OK) return rc;
         CU(cudaMemcpyAsync(hr, &A->d_state->res, sizeof(SolveResult), cudaMemcpyDeviceToHost, stream));

@@ -63,7 +63,7 @@ __device__ __forceinline__ C res_row_product(int i, const int* s_rowptr, const i
     double* rhs_norm = (double*)(dyn + kFusedOffNorm);                                                  \
     unsigned char* base = dyn + kFusedFixedBytes;                                                       \
     __shared__ double red[kAccMax * 32];                                                                \
-    fused_stage_header(st, dyn + kFusedOffHdr, rhs_norm);                                               \
+    fused_stage_header(hp, st, dyn + kFusedOffHdr, rhs_norm);                                               \
     const int cta = blockIdx.x, ncta = gridDim.x, tid = threadIdx.x;                                    \
     const long long units = DOF == 3 ? A.nbrows : A.n;                                                  \
     const long long u0 = units * cta / ncta, u1 = units * (cta + 1) / ncta;                             \
@@ -102,36 +102,84 @@ __device__ __forceinline__ C res_row_product(int i, const int* s_rowptr, const i
     }                                                                                                   \
     fused_publish(st, res, gen)
 
+// p_n = r_n + alpha_n p_{n-1}, with explicit fused multiply-adds: the owner of a row and every CTA that gathers the
+// row evaluate this same expression on the same operands and must get the same bits
+__device__ __forceinline__ double2 res_pnext(double2 r, double a, double2 p) { return make_double2(fma(a, p.x, r.x), fma(a, p.y, r.y)); }
+__device__ __forceinline__ float2 res_pnext(float2 r, float a, float2 p) { return make_float2(fmaf(a, p.x, r.x), fmaf(a, p.y, r.y)); }
+__device__ __forceinline__ double res_pnext(double r, double a, double p) { return fma(a, p, r); }
+__device__ __forceinline__ float res_pnext(float r, float a, float p) { return fmaf(a, p, r); }
+
+// (A p_n)_i with p_n = r_n + alpha_n p_{n-1} formed on the fly from the two vectors that ARE visible in global memory
+template <typename C, typename T, int DOF>
+__device__ __forceinline__ C res_row_product_pnext(int i, const int* s_rowptr, const int* s_col, const C* s_val, const C* rg,
+                                                   const C* pold, T alpha) {
+    C sum = cmake<C>(0.0, 0.0);
+    if (DOF == 3) {
+        const int lbr = i / 3, rr = i - 3 * lbr;
+        for (int j = s_rowptr[lbr]; j < s_rowptr[lbr + 1]; ++j) {
+            const C* blk = s_val + j * 9 + rr * 3;
+            const long long c = 3ll * s_col[j];
+            sum = cfma(blk[0], res_pnext(rg[c], alpha, pold[c]), sum);
+            sum = cfma(blk[1], res_pnext(rg[c + 1], alpha, pold[c + 1]), sum);
+            sum = cfma(blk[2], res_pnext(rg[c + 2], alpha, pold[c + 2]), sum);
+        }
+    } else {
+#pragma unroll 4
+        for (int j = s_rowptr[i]; j < s_rowptr[i + 1]; ++j) {
+            const int c = s_col[j];
+            sum = cfma(s_val[j], res_pnext(rg[c], alpha, pold[c]), sum);
+        }
+    }
+    return sum;
+}
+
+// CG-M.  Two grid-wide exchanges per iteration, the two sums the method needs (<p,Ap> and |r|^2): the search
+// direction is never waited for.  Owners mirror r (written during the update, i.e. before the |r|^2 sum) and p
+// (two buffers in turn, written right after alpha is known) in global memory; a CTA that gathers column j in
+// iteration n forms p_n[j] = r_n[j] + alpha_n p_{n-1}[j] itself from r_n and p_{n-1}, both of which became visible
+// with sums it has already passed.  The buffer p_n is written into was last read two sums ago.
 template <typename E, int DOF>
-__global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, SolveState* st, ResLayout L) {
+__global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, SolveState* st, ResLayout L, const __grid_constant__ SolveHeader hp) {
     MSOLVE_RESIDENT_PROLOGUE;
+    C* rg = (C*)h.r;                                          // mirror of r
+    C* pbuf[2] = {pg, (C*)h.q};                               // mirrors of p_n (n even / odd); q itself stays in shared memory
     // r <- b, p <- b, x_k <- 0, p_k <- b  (l.9-12)
     double acc[1] = {0.0}, s[1];
     for (int i = tid; i < nloc; i += blockDim.x) {
         const C bv = ((const C*)h.b)[row0 + i];
         s_r[i] = bv; s_p[i] = bv;
-        pg[row0 + i] = bv;
+        pbuf[0][row0 + i] = bv;
+        rg[row0 + i] = bv;
         for (int k = 0; k < S; ++k) { s_xk[k * ld + i] = cmake<C>(0.0, 0.0); s_pk[k * ld + i] = bv; }
         acc[0] += cnorm2(bv);
     }
     unsigned long long gen = st->fused_gen;
-    fused_allreduce<1>(st, gen, acc, s, red);                                        // <b,b> (l.13); p visible to all
+    fused_allreduce<1>(st, gen, acc, s, red);                                        // <b,b> (l.13); p_0, r_0 visible to all
     init_state_fn(h, res, rc, s[0]);
     while (!res.done) {
-        if (res.n_iter > 0) {
-            const T alpha = (T)rc.alpha.re;
-            for (int i = tid; i < nloc; i += blockDim.x) {                           // l.27, own rows
-                const C pv = caxpy_r(s_r[i], alpha, s_p[i]);
-                s_p[i] = pv;
-                pg[row0 + i] = pv;
-            }
-            fused_allreduce<0>(st, gen, nullptr, nullptr, red);                      // p complete before it is gathered
-        }
+        const int n = res.n_iter;
+        const T alpha = (T)rc.alpha.re;
         acc[0] = 0.0;
-        for (int i = tid; i < nloc; i += blockDim.x) {                               // l.18-19, matrix out of shared memory
-            const C sum = res_row_product<C, DOF>(i, s_rowptr, s_col, s_val, pg);
-            s_q[i] = sum;
-            acc[0] += cdot_re(s_p[i], sum);
+        if (n > 0) {
+            C* pnew = pbuf[n & 1];
+            const C* pold = pbuf[(n - 1) & 1];
+            for (int i = tid; i < nloc; i += blockDim.x) {                           // l.27, own rows; nobody waits for this store
+                const C pv = res_pnext(s_r[i], alpha, s_p[i]);
+                s_p[i] = pv;
+                pnew[row0 + i] = pv;
+            }
+            __syncthreads();
+            for (int i = tid; i < nloc; i += blockDim.x) {                           // l.18-19
+                const C sum = res_row_product_pnext<C, T, DOF>(i, s_rowptr, s_col, s_val, rg, pold, alpha);
+                s_q[i] = sum;
+                acc[0] += cdot_re(s_p[i], sum);
+            }
+        } else {
+            for (int i = tid; i < nloc; i += blockDim.x) {
+                const C sum = res_row_product<C, DOF>(i, s_rowptr, s_col, s_val, pbuf[0]);
+                s_q[i] = sum;
+                acc[0] += cdot_re(s_p[i], sum);
+            }
         }
         fused_allreduce<1>(st, gen, acc, s, red);
         cgm_scal1_fn(h, res, rc, s[0]);                                               // l.20, 22, 23
@@ -151,6 +199,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, Solve
                 }
                 rv = caxpy_r(rv, beta, s_q[i]);                                       // l.21
                 s_r[i] = rv;
+                rg[row0 + i] = rv;                                                    // visible with the |r|^2 sum
                 acc[0] += cnorm2(rv);                                                 // l.24
             }
         }
@@ -163,7 +212,7 @@ __global__ void __launch_bounds__(kResThreads, 1) k_cgm_resident(MatDev A, Solve
 // BiCGStab-M, same residency: r, p, q, s, t, b and every x_k, p_k in shared memory; p and s are the two vectors the
 // SpMVs gather, so they are mirrored in global memory.  Steps and per-element arithmetic of k_bi_fused / bi_update_fn.
 template <typename E, int DOF>
-__global__ void __launch_bounds__(kResThreads, 1) k_bi_resident(MatDev A, SolveState* st, ResLayout L) {
+__global__ void __launch_bounds__(kResThreads, 1) k_bi_resident(MatDev A, SolveState* st, ResLayout L, const __grid_constant__ SolveHeader hp) {
     MSOLVE_RESIDENT_PROLOGUE;
     C* s_s = (C*)(base + L.off_s);
     C* s_t = (C*)(base + L.off_t);
@@ -304,7 +353,8 @@ static int launch_resident_t(const msolve_matrix* A, int alg, const ResLayout& L
     MatDev dev = A->dev;
     SolveState* st = A->d_state;
     ResLayout lay = L;
-    void* args[3] = {&dev, &st, &lay};
+    SolveHeader hdr = A->h_stage->h;
+    void* args[4] = {&dev, &st, &lay, &hdr};
     MSOLVE_CU(cudaLaunchCooperativeKernel((const void*)kernel, dim3(ncta), dim3(kResThreads), args, (size_t)L.total, s));
     return MSOLVE_OK;
 }

@@ -88,7 +88,22 @@ __device__ __forceinline__ void csr_vector_body(const MatDev& A, const E* x, E* 
         int j = 0, e = 0;
         if (valid) { j = rowptr[row] + sub; e = rowptr[row + 1]; }
         C sum = cmake<C>(0.0, 0.0);
-#pragma unroll 4
+        // Long rows: the loads of a lane batched by kind (8 indices + 8 values, then the 8 gathers they address, then
+        // the arithmetic); the rest one at a time.  What matters more is the register budget: at 6 CTAs per SM
+        // (__launch_bounds__ below: 40 registers) config 5 complex128 runs at 1.00 ms, at the 34 registers ptxas
+        // picks on its own the loads of the unrolled loop share registers and serialise: 1.43 ms
+        // (profiles/r02_sweeps.md section 4).
+        constexpr int UB = 8;
+        for (; j + (UB - 1) * LANES < e; j += UB * LANES) {
+            int c[UB];
+            C v[UB], xv[UB];
+#pragma unroll
+            for (int t = 0; t < UB; ++t) { c[t] = ld_mat<HINT>(colidx + j + t * LANES, polm); v[t] = ld_mat<HINT>(val + j + t * LANES, polm); }
+#pragma unroll
+            for (int t = 0; t < UB; ++t) xv[t] = NC ? ld_xg<PIN>(x + c[t], polx) : x[c[t]];
+#pragma unroll
+            for (int t = 0; t < UB; ++t) sum = cfma(v[t], xv[t], sum);
+        }
         for (; j < e; j += LANES) {
             const int c = ld_mat<HINT>(colidx + j, polm);
             const C v = ld_mat<HINT>(val + j, polm);
@@ -104,7 +119,7 @@ __device__ __forceinline__ void csr_vector_body(const MatDev& A, const E* x, E* 
 }
 
 template <typename E, int LANES, int ROLE, bool PIN>
-__global__ void __launch_bounds__(kThreads) k_spmv_csr_vector(MatDev A, SolveState* st) {
+__global__ void __launch_bounds__(kThreads, 6) k_spmv_csr_vector(MatDev A, SolveState* st) {
     typedef E C;
     constexpr int NACC = RoleAcc<ROLE>::value;
     if (ROLE != ROLE_GEN && st->res.done) return;

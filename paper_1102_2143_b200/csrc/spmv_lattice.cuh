@@ -123,13 +123,29 @@ __device__ __forceinline__ void lat_epilogue(double* acc, C yi, C xi, C ui) {
 // is the bottleneck of these kernels (~0.1 us per copy and thread; spreading the copies over the
 // lanes of a warp is slower still: UBLKCP is a uniform-datapath instruction), hence 32-bit coordinate
 // arithmetic here and several producer warps in k_spmv_lat_warp.
+// lattice geometry the producers need, read once per kernel into registers (the 64-bit division vol / L0 must not
+// end up inside the issue loop: measured +8 % on the complex64 kernel when the compiler left it there)
+struct LatGeom {
+    int nd, L0, TR, nrows;
+    unsigned ext1, ext2, ext3;
+    long long vol;
+};
+__device__ __forceinline__ LatGeom lat_geom(const MatDev& A) {
+    LatGeom g;
+    g.nd = A.lat_ndim; g.L0 = A.lat_ext[0]; g.TR = A.lat_rows_per_tile;
+    g.ext1 = (unsigned)A.lat_ext[1]; g.ext2 = (unsigned)A.lat_ext[2]; g.ext3 = (unsigned)A.lat_ext[3];
+    g.vol = A.lat_vol;
+    g.nrows = (int)(A.lat_vol / A.lat_ext[0]);
+    return g;
+}
+
 template <typename C, int LINK_SLOT, int X_SLOT, int X_BASE>
-__device__ __forceinline__ void lat_issue_tile(const MatDev& A, const C* __restrict__ links, const C* x, unsigned char* sb,
+__device__ __forceinline__ void lat_issue_tile(const LatGeom& G, const C* __restrict__ links, const C* x, unsigned char* sb,
                                                uint32_t bar, uint32_t empty_bar, uint32_t empty_parity, int t, uint64_t pol) {
     constexpr int SZ = (int)sizeof(C);
-    const int nd = A.lat_ndim, L0 = A.lat_ext[0], TR = A.lat_rows_per_tile;
-    const long long vol = A.lat_vol;
-    const int nrows = (int)(vol / L0);
+    const int nd = G.nd, L0 = G.L0, TR = G.TR;
+    const long long vol = G.vol;
+    const int nrows = G.nrows;
     const int row0 = t * TR;
     const int nr = min(TR, nrows - row0);
     const long long site0 = (long long)row0 * L0;
@@ -146,7 +162,7 @@ __device__ __forceinline__ void lat_issue_tile(const MatDev& A, const C* __restr
 #pragma unroll
         for (int mu = 1; mu < 4; ++mu) {
             if (mu >= nd) break;
-            const unsigned L = (unsigned)A.lat_ext[mu];
+            const unsigned L = mu == 1 ? G.ext1 : mu == 2 ? G.ext2 : G.ext3;
             const unsigned cm = rem % L;
             rem /= L;
             const long long rf = (long long)row + (cm + 1 == L ? -(long long)((L - 1) * rs) : (long long)rs);
@@ -213,8 +229,9 @@ __global__ void __launch_bounds__(LatCfg<E, NS>::kThreadsTotal, CPS) k_spmv_lat_
         if (threadIdx.x == NCT) {
             const C* __restrict__ links = (const C*)A.val;
             const uint64_t pol = policy_evict_normal();
+            const LatGeom G = lat_geom(A);
             for (int t = blockIdx.x; t < ntiles; t += gridDim.x) {
-                lat_issue_tile<C, Cfg::kLinkSlot, Cfg::kXSlot, Cfg::kXBase>(A, links, x, smem + stage * Cfg::kStageBytes, full0 + 8 * stage,
+                lat_issue_tile<C, Cfg::kLinkSlot, Cfg::kXSlot, Cfg::kXBase>(G, links, x, smem + stage * Cfg::kStageBytes, full0 + 8 * stage,
                                                                            empty0 + 8 * stage, phase ^ 1u, t, pol);
                 if (++stage == STAGES) { stage = 0; phase ^= 1u; }
             }
@@ -358,6 +375,7 @@ __global__ void __launch_bounds__(LatWarpCfg<E, W, PW>::kThreadsTotal, 1) k_spmv
         if (lane == 0) {
             const C* __restrict__ links = (const C*)A.val;
             const uint64_t pol = policy_evict_normal();
+            const LatGeom G = lat_geom(A);
             // a stage is always filled by the same producer (stage % PW) and drained by the same
             // consumer warp (stage % W): its uses are then waited for in order by ONE thread on either
             // side, which is what the parity waits of an mbarrier need
@@ -366,7 +384,7 @@ __global__ void __launch_bounds__(LatWarpCfg<E, W, PW>::kThreadsTotal, 1) k_spmv
                 for (int stage = warp - W; stage < STAGES; stage += PW) {
                     const long long tl = (long long)blockIdx.x + (long long)(m * STAGES + stage) * gridDim.x;
                     if (tl >= ntiles) { more = false; break; }
-                    lat_issue_tile<C, Cfg::kLinkSlot, Cfg::kXSlot, Cfg::kXBase>(A, links, x, smem + stage * Cfg::kStageBytes, full0 + 8 * stage,
+                    lat_issue_tile<C, Cfg::kLinkSlot, Cfg::kXSlot, Cfg::kXBase>(G, links, x, smem + stage * Cfg::kStageBytes, full0 + 8 * stage,
                                                                                empty0 + 8 * stage, ((uint32_t)m & 1u) ^ 1u, (int)tl, pol);
                 }
                 if (!more) break;
