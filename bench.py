@@ -60,6 +60,8 @@ def make_workload(name: str, rank: int, want_csr: bool):
         w, dt, fmt = W.config3(), np.complex128, "csr"
     elif name == "config2_c128_csr":
         w, dt, fmt = W.config2(), np.complex128, "csr"
+    elif name == "config1_c128_csr":                 # BASELINE configs[0]: 8x8 U(1) lattice, N = 64
+        w, dt, fmt = W.config1(), np.complex128, "csr"
     elif name == "config4_small_c128_bsr3":          # quick functional check of the bench itself
         w, dt, fmt = W.config4(extents=(8, 8, 8, 16), want_csr=want_csr), np.complex128, "bsr3"
     elif name == "config2_c128_bsr3":
