@@ -308,6 +308,7 @@ static bool resident_layout(const msolve_matrix* A, int S, int alg, int ncta, Re
     for (int c = 0; c < ncta; ++c) {
         const long long u0 = units * c / ncta, u1 = units * (c + 1) / ncta;
         max_units = std::max(max_units, u1 - u0);
+        if (A->h_rowptr[u1] < A->h_rowptr[u0]) return false;             // not a CSR row pointer: leave it to the other paths
         max_entries = std::max<long long>(max_entries, A->h_rowptr[u1] - A->h_rowptr[u0]);
     }
     const size_t e = elem_bytes(A->dtype);

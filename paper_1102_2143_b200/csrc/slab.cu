@@ -212,6 +212,9 @@ static int slabs_create(msolve_slabs** out, int dof, int64_t nrows, int64_t nnz,
     std::vector<int64_t> isplits;                      // in index rows (block rows for BSR3)
     if (h_splits) isplits.assign(h_splits, h_splits + nslabs + 1); else even_splits(nrows, nslabs, isplits);
     const size_t eb = elem_bytes(dtype), vb = (dof == 3 ? 9 : 1) * eb;
+    if (isplits[0] != 0 || isplits[nslabs] != nrows) { slabs_free(S); return fail(MSOLVE_EINVAL, "msolve_slabs_create: splits must run from 0 to the number of rows"); }
+    for (int p = 0; p < nslabs; ++p)
+        if (isplits[p + 1] < isplits[p]) { slabs_free(S); return fail(MSOLVE_EINVAL, "msolve_slabs_create: splits must not decrease"); }
     for (int p = 0; p <= nslabs; ++p) {
         if ((isplits[p] * dof * (int64_t)eb) % 16 != 0 && p < nslabs && p > 0) { slabs_free(S); return fail(MSOLVE_EINVAL, "msolve_slabs_create: split %d is not 16-byte aligned in the vectors", p); }
         S->splits.push_back(isplits[p] * dof);
@@ -230,11 +233,10 @@ static int slabs_create(msolve_slabs** out, int dof, int64_t nrows, int64_t nnz,
         if (cudaMalloc((void**)&d.d_rowptr, sizeof(int32_t) * (size_t)(nloc + 1)) != cudaSuccess ||
             cudaMalloc((void**)&d.d_colidx, sizeof(int32_t) * (size_t)std::max<int64_t>(lnnz, 4)) != cudaSuccess ||
             cudaMalloc(&d.d_val, vb * (size_t)std::max<int64_t>(lnnz, 1)) != cudaSuccess) { rc = fail(MSOLVE_ENOMEM, "msolve_slabs_create: cudaMalloc failed"); break; }
-        cudaMemcpy(d.d_rowptr, rp.data(), sizeof(int32_t) * (size_t)(nloc + 1), cudaMemcpyHostToDevice);
-        if (lnnz > 0) {
-            cudaMemcpy(d.d_colidx, d.plan->colidx.data(), sizeof(int32_t) * (size_t)lnnz, cudaMemcpyHostToDevice);
-            cudaMemcpy(d.d_val, (const char*)h_val + vb * (size_t)h_rowptr[rb], vb * (size_t)lnnz, cudaMemcpyHostToDevice);
-        }
+        cudaError_t ce = cudaMemcpy(d.d_rowptr, rp.data(), sizeof(int32_t) * (size_t)(nloc + 1), cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess && lnnz > 0) ce = cudaMemcpy(d.d_colidx, d.plan->colidx.data(), sizeof(int32_t) * (size_t)lnnz, cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess && lnnz > 0) ce = cudaMemcpy(d.d_val, (const char*)h_val + vb * (size_t)h_rowptr[rb], vb * (size_t)lnnz, cudaMemcpyHostToDevice);
+        if (ce != cudaSuccess) { rc = fail(MSOLVE_ECUDA, "msolve_slabs_create: copy of slab %d failed: %s", p, cudaGetErrorString(ce)); break; }
         if (dof == 3) rc = msolve_create_bsr3(&d.A, nloc, lnnz, d.d_rowptr, d.d_colidx, d.d_val, dtype, flags, stream);
         else rc = msolve_create_csr(&d.A, nloc, lnnz, d.d_rowptr, d.d_colidx, d.d_val, dtype, flags, stream);
         if (rc != MSOLVE_OK) break;

@@ -106,3 +106,7 @@ def test_slabs_uneven_splits_real_and_edge_cases(ms):
     ms.msolve_slabs_destroy(S)
     with pytest.raises(ms.MsolveError):                               # a split that is not 16-byte aligned in the vectors
         ms.msolve_slabs_create_csr(w.rowptr, w.colidx, w.val, 2, splits=np.array([0, 401, w.n], dtype=np.int64))
+    with pytest.raises(ms.MsolveError):                               # splits that do not cover the rows / run backwards
+        ms.msolve_slabs_create_csr(w.rowptr, w.colidx, w.val, 2, splits=np.array([0, 400, w.n + 4], dtype=np.int64))
+    with pytest.raises(ms.MsolveError):
+        ms.msolve_slabs_create_csr(w.rowptr, w.colidx, w.val, 3, splits=np.array([0, 800, 400, w.n], dtype=np.int64))
