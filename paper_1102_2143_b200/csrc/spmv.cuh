@@ -90,7 +90,7 @@ __device__ __forceinline__ void csr_vector_body(const MatDev& A, const E* x, E* 
         C sum = cmake<C>(0.0, 0.0);
         // Long rows: the loads of a lane batched by kind (8 indices + 8 values, then the 8 gathers they address, then
         // the arithmetic); the rest one at a time.  What matters more is the register budget: at 6 CTAs per SM
-        // (__launch_bounds__ below: 40 registers) config 5 complex128 runs at 1.00 ms, at the 34 registers ptxas
+        // (__launch_bounds__ below: 40 registers) config 5 complex128 runs at 1.20 ms, at the 34 registers ptxas
         // picks on its own the loads of the unrolled loop share registers and serialise: 1.43 ms
         // (profiles/r02_sweeps.md section 4).
         constexpr int UB = 8;
@@ -119,7 +119,7 @@ __device__ __forceinline__ void csr_vector_body(const MatDev& A, const E* x, E* 
 }
 
 template <typename E, int LANES, int ROLE, bool PIN>
-__global__ void __launch_bounds__(kThreads, 6) k_spmv_csr_vector(MatDev A, SolveState* st) {
+__global__ void __launch_bounds__(kThreads, ROLE == ROLE_B2 ? 5 : 6) k_spmv_csr_vector(MatDev A, SolveState* st) {
     typedef E C;
     constexpr int NACC = RoleAcc<ROLE>::value;
     if (ROLE != ROLE_GEN && st->res.done) return;
