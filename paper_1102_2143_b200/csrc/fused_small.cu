@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_cgm_fused(MatDev A, SolveS
         fused_allreduce<1>(st, gen, acc, s, red);
         cgm_scal1_fn(h, res, rc, s[0]);                                               // l.20, 22, 23
         if (res.done) break;                                                          // breakdown: the same in every CTA
-        acc[0] = cgm_update_fn<E, VEC, kUnrollCgm>(h, res, rc, cta, ncta);            // l.21, 24, 28, 29
+        acc[0] = cgm_update_fn<E, VEC, kUnrollCgm, false>(h, res, rc, cta, ncta);            // l.21, 24, 28, 29
         fused_allreduce<1>(st, gen, acc, s, red);
         cgm_scal2_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);   // l.25, 26, 30, 31, 15
     }
@@ -94,7 +94,7 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_bi_fused(MatDev A, SolveSt
         fused_allreduce<5>(st, gen, acc, s, red);
         bi_scal2_fn(h, res, rc, s);
         if (res.done) break;
-        acc[0] = bi_update_fn<E, VEC, kUnrollBi>(h, res, rc, cta, ncta);              // r', p, x_k, p_k, |r'|^2
+        acc[0] = bi_update_fn<E, VEC, kUnrollBi, false>(h, res, rc, cta, ncta);              // r', p, x_k, p_k, |r'|^2
         fused_allreduce<1>(st, gen, acc, s, red);                                     // also: p complete before SpMV#1
         bi_scal3_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);
     }

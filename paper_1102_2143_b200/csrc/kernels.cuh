@@ -187,7 +187,9 @@ __device__ __forceinline__ void cgm_scal1_fn(const SolveHeader& h, SolveResult& 
 
 // A5: the fused multishift update.  UNR shifts are in flight per thread (2*UNR independent
 // 16-byte loads) on top of r and Ap; x_k / p_k are streamed with evict-first hints.  Returns the thread's |r|^2 share.
-template <typename E, int VEC, int UNR>
+// STREAM: x_k / p_k with evict-first hints (working sets far beyond L2: every byte is touched once per iteration);
+// the whole-solve kernel for systems around the size of L2 passes false so that the vectors stay there.
+template <typename E, int VEC, int UNR, bool STREAM = true>
 __device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const SolveResult& res, const Recur& rc, int cta, int ncta) {
     typedef E C;
     typedef typename RealOf<E>::type T;
@@ -221,8 +223,8 @@ __device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const Solv
             for (int u = 0; u < UNR; ++u) {
                 if (a0 + u < na && !first) {
                     const int k = s_k[a0 + u];
-                    xv[u] = ld_pack<true>((const P*)(x + k * xs) + i);
-                    pv[u] = ld_pack<true>((const P*)(pk + k * pks) + i);
+                    xv[u] = ld_pack<STREAM>((const P*)(x + k * xs) + i);
+                    pv[u] = ld_pack<STREAM>((const P*)(pk + k * pks) + i);
                 }
             }
 #pragma unroll
@@ -242,8 +244,8 @@ __device__ __forceinline__ double cgm_update_fn(const SolveHeader& h, const Solv
                         xo.v[e] = caxpy_r(xe, -bk, pe);                              // l.28
                         po.v[e] = pe;
                     }
-                    st_pack<true>((P*)(x + k * xs) + i, xo);
-                    st_pack<true>((P*)(pk + k * pks) + i, po);
+                    st_pack<STREAM>((P*)(x + k * xs) + i, xo);
+                    st_pack<STREAM>((P*)(pk + k * pks) + i, po);
                 }
             }
         }
@@ -440,7 +442,7 @@ __device__ __forceinline__ void bi_scal2_fn(const SolveHeader& h, SolveResult& r
 // The fused BiCGStab-M update: per element read r, s, t, q, p once;
 //   r' = s - chi t ; p <- r' + alpha'(p - chi q) ; |r'|^2 partials; per active shift
 //   x_k <- (x_k - beta_k p_k) + cs_k s ; p_k <- zr_k r' + alpha_k ( p_k - cb_k ( zs_k s - zo_k r ) ).
-template <typename E, int VEC, int UNR>
+template <typename E, int VEC, int UNR, bool STREAM = true>
 __device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const SolveResult& res, const Recur& rc, int cta, int ncta) {
     typedef E C;
     typedef Pack<E, VEC> P;
@@ -481,8 +483,8 @@ __device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const Solve
             for (int u = 0; u < UNR; ++u) {
                 if (a0 + u < na && !first) {
                     const int k = s_k[a0 + u];
-                    xv[u] = ld_pack<true>((const P*)(x + k * xs) + i);
-                    pv[u] = ld_pack<true>((const P*)(pk + k * pks) + i);
+                    xv[u] = ld_pack<STREAM>((const P*)(x + k * xs) + i);
+                    pv[u] = ld_pack<STREAM>((const P*)(pk + k * pks) + i);
                 }
             }
 #pragma unroll
@@ -499,8 +501,8 @@ __device__ __forceinline__ double bi_update_fn(const SolveHeader& h, const Solve
                         const C ds = csub(cmul(c[5], sv.v[e]), cmul(c[6], rv.v[e]));
                         po.v[e] = cadd(cmul(c[2], rn.v[e]), cmul(c[3], csub(pe, cmul(c[4], ds))));
                     }
-                    st_pack<true>((P*)(x + k * xs) + i, xo);
-                    st_pack<true>((P*)(pk + k * pks) + i, po);
+                    st_pack<STREAM>((P*)(x + k * xs) + i, xo);
+                    st_pack<STREAM>((P*)(pk + k * pks) + i, po);
                 }
             }
         }
