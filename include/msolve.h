@@ -287,7 +287,8 @@ void msolve_slab_plan_destroy(msolve_slab_plan *plan);
  * recurrences on the same sums; the whole multi-slab iteration is one WHILE graph.  Arguments of the solvers as
  * msolve_cgm / msolve_bicgstabm with GLOBAL vectors (d_b: n, d_x: nshifts*n shift-major) and a workspace of
  * msolve_slabs_workspace_bytes().  Results agree with the unpartitioned solve to rounding (the dot products are
- * grouped by slab), and are bit-reproducible for a given number of slabs. */
+ * grouped by slab), and are bit-reproducible for a given number of slabs.  The slab set has no options: per-shift
+ * stop rule, graph of kernels, no scalar history. */
 typedef struct msolve_slabs msolve_slabs;
 int msolve_slabs_create_csr(msolve_slabs **S, int64_t n, int64_t nnz, const int32_t *h_rowptr, const int32_t *h_colidx,
                             const void *h_val, int dtype, int nslabs, const int64_t *h_splits, int flags, void *stream);
