@@ -250,7 +250,7 @@ def config_dict(args, w, dtype, fmt, world, S, shifts_total):
     return {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
             "shifts": S, "tol": w.tol,
             "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world,
-            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
+            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "matrix_l2_keep_percent": args.matrix_l2_keep, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
 
 
 def run_reference(args, rank):
@@ -349,6 +349,11 @@ def main():
     ap.add_argument("--fused-ctas", type=int, default=0, help="CTAs of the one-kernel path (0 = by problem size)")
     ap.add_argument("--matrix-l2", default="auto", choices=["auto", "stream", "keep"],
                     help="L2 policy of the matrix stream (MSOLVE_CFG_MATRIX_L2)")
+    ap.add_argument("--phase-clock", action="store_true",
+                    help="one-kernel path: also report the microseconds per iteration CTA 0 spends in every phase "
+                         "(msolve_set_phase_clock; extra solves after the timed region)")
+    ap.add_argument("--matrix-l2-keep", type=int, default=0,
+                    help="percent of the matrix stream loaded evict-last (MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT)")
     ap.add_argument("--slabs", type=int, default=0,
                     help="row partition on ONE device (msolve_slabs_*, SURVEY 8(f)-3): P slabs with halo exchange and "
                          "summed dot products; measures what the partition costs against the unpartitioned solve")
@@ -421,6 +426,8 @@ def main():
     ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, {"auto": 0, "graph": 1, "fused": 2, "resident": 3}[args.iter_path])
     ms.msolve_config(A, ms.MSOLVE_CFG_FUSED_CTAS, args.fused_ctas)
     ms.msolve_config(A, ms.MSOLVE_CFG_MATRIX_L2, {"auto": 0, "stream": 1, "keep": 2}[args.matrix_l2])
+    if args.matrix_l2_keep:
+        ms.msolve_config(A, ms.MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT, args.matrix_l2_keep)
     S = int(w.shifts.size)
     b_host = torch.from_numpy(w.b.astype(dtype)).pin_memory()
     b_dev = b_host.cuda()
@@ -450,6 +457,21 @@ def main():
     clocks = sampler.stop()
     ms_total = ev0.elapsed_time(ev1)
     status, conv_iter = res.status, res.conv_iter.tolist()
+    phases = None
+    if args.phase_clock:
+        # one-kernel path only: where CTA 0 spends an iteration (msolve_set_phase_clock), over `steps` more solves
+        ns = torch.zeros(16, dtype=torch.int64, device="cuda")
+        ms.msolve_set_phase_clock(A, ns)
+        for _ in range(args.steps):
+            solve(A, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev, workspace=ws)
+        ms.msolve_set_phase_clock(A, None)
+        t = ns.cpu().numpy().astype(np.float64)
+        names = (["p_update", "barrier", "spmv_dot", "barrier_sum", "scalars_update", "barrier_sum2"] if alg == ms.MSOLVE_ALG_CGM else
+                 ["spmv1_dot", "barrier_sum", "scalars_s_update", "barrier", "spmv2_dots", "barrier_sum5", "scalars_update", "barrier_sum1"])
+        if t[15] > 0:
+            phases = {k: round(v / t[15] / 1e3, 2) for k, v in zip(names, t)}
+            phases["sum"] = round(float(t[:len(names)].sum()) / t[15] / 1e3, 2)
+            phases["iterations"] = int(t[15])
 
     # ---- end to end: host b in, host x out, every step.  The K steps go through ONE call of the public
     # batch interface (msolve_solve_host_batch: K right-hand sides of the same family), which overlaps the
@@ -544,6 +566,8 @@ def main():
                                              "single_call_api": "msolve_solve_host per step, nothing overlapped"},
             "gpu_launches": int(launches_all), "clocks": clocks,
         }
+        if phases is not None:
+            line["one_kernel_phases_us_per_iteration"] = phases
         print(json.dumps(line))
     ms.msolve_destroy(A)
     if world > 1:

@@ -104,7 +104,12 @@ enum {
                                 Same arithmetic step for step; the paths group the dot products differently (per-CTA
                                 partials of different grids), so they agree to rounding, not bit for bit */,
     MSOLVE_CFG_FUSED_CTAS = 7 /* CTAs of the cooperative kernel of MSOLVE_CFG_ITER_PATH = 2: 0 = by problem size
-                                 (default), else that many (at most one per SM) */
+                                 (default), else that many (at most one per SM) */,
+    MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT = 8 /* 0 .. 100: that share of the matrix stream (cache lines picked by the
+                                 hardware from the address, createpolicy.fractional) is loaded evict-last, the rest
+                                 evict-first -- for a matrix of which a part fits in L2 next to the vectors.  Applies to
+                                 the TMA-staged kernels and to the BSR3 SpMV of the one-kernel path;
+                                 MSOLVE_CFG_MATRIX_L2 = 1 / 2 set it to 0 / 100.  Default 0; profiles/r02_sweeps.md */
 };
 
 /* Build a handle for a CSR matrix (n x n).  Borrows the three device arrays: they must stay
@@ -250,6 +255,18 @@ int msolve_config(msolve_matrix *A, int key, int value);
  * A shift that has stopped keeps the values of its last active iteration.  An iteration that breaks down
  * writes no row.  cap_rows = 0 (or d_hist = NULL) switches the history off.  Returns OK / EINVAL. */
 int msolve_set_history(msolve_matrix *A, double *d_hist, int cap_rows);
+
+/* Where the time of the one-kernel path (MSOLVE_CFG_ITER_PATH = 2) goes: while d_ns is set, thread 0 of CTA 0 reads
+ * %globaltimer at every phase boundary of every later solve on this handle and ADDS the nanoseconds into
+ * d_ns[0 .. 15] (device, uint64, 8-byte aligned, borrowed; the caller zeroes it):
+ *   CG-M:        [0] p update, [1] its barrier, [2] SpMV + <p,Ap>, [3] barrier + sum, [4] scalars + fused update,
+ *                [5] barrier + sum;
+ *   BiCGStab-M:  [0] SpMV#1 + <r0,q>, [1] barrier + sum, [2] scalars + s update, [3] barrier, [4] SpMV#2 + dots,
+ *                [5] barrier + sum, [6] scalars + fused update, [7] barrier + sum;
+ *   [15] iterations counted.  A barrier entry is what CTA 0 waits: the barrier itself plus the skew of the other
+ * CTAs.  The other paths ignore it (msolve_profile_iteration times the kernels of the graph path).
+ * d_ns = NULL switches it off (default).  Returns OK / EINVAL.  Table: profiles/r02_sweeps.md section 3. */
+int msolve_set_phase_clock(msolve_matrix *A, uint64_t *d_ns);
 
 /* ---------------------------------------------------------------------------------------------------------------
  * Row (site) partition: every slab owns a contiguous range of rows of A and the same range of r, p

@@ -31,11 +31,12 @@ MSOLVE_CFG_X_WINDOW = 4
 MSOLVE_CFG_MATRIX_L2 = 5
 MSOLVE_CFG_ITER_PATH = 6
 MSOLVE_CFG_FUSED_CTAS = 7
+MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT = 8
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
     "msolve_bicgstabm", "msolve_multirhs_workspace_bytes", "msolve_solve_multirhs", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
-    "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_set_history", "msolve_destroy",
+    "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_set_history", "msolve_set_phase_clock", "msolve_destroy",
     "msolve_last_error",
     "msolve_slab_plan_create", "msolve_slab_plan_nlocal", "msolve_slab_plan_nhalo", "msolve_slab_plan_npeers",
     "msolve_slab_plan_peer", "msolve_slab_plan_colidx", "msolve_slab_plan_destroy",
@@ -84,6 +85,7 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_last_launch_count.restype = i64
     lib.msolve_config.argtypes = [vp, i32, i32]
     lib.msolve_set_history.argtypes = [vp, vp, i32]
+    lib.msolve_set_phase_clock.argtypes = [vp, vp]
     lib.msolve_destroy.argtypes = [vp]
     lib.msolve_destroy.restype = None
     lib.msolve_last_error.restype = ctypes.c_char_p
@@ -119,7 +121,7 @@ def load_library() -> ctypes.CDLL:
         getattr(lib, name).restype = i32
     for name in ("msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_cgm", "msolve_bicgstabm",
                  "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration", "msolve_config",
-                 "msolve_set_history", "msolve_solve_multirhs"):
+                 "msolve_set_history", "msolve_set_phase_clock", "msolve_solve_multirhs"):
         getattr(lib, name).restype = i32
     _lib = lib
     return lib
@@ -170,6 +172,7 @@ class Matrix:
         self.n = n
         self._keep = keep
         self._hist = None
+        self._phase_ns = None
 
     def destroy(self):
         if self.handle:
@@ -250,6 +253,17 @@ def msolve_set_history(A: Matrix, hist: Optional[torch.Tensor]) -> None:
         raise ValueError("hist must be [cap_rows, row_length]")
     _check(load_library().msolve_set_history(A.handle, hist.data_ptr(), hist.shape[0]))
     A._hist = hist
+
+
+def msolve_set_phase_clock(A: Matrix, ns: Optional[torch.Tensor]) -> None:
+    """One-kernel path: `ns` is a contiguous int64 CUDA tensor of 16 entries that later solves on this handle add
+    their per-phase nanoseconds to (include/msolve.h); None switches it off."""
+    if ns is not None:
+        ns = _dev(ns, torch.int64)
+        if ns.numel() < 16:
+            raise ValueError("ns must hold 16 entries")
+    _check(load_library().msolve_set_phase_clock(A.handle, None if ns is None else ns.data_ptr()))
+    A._phase_ns = ns
 
 
 def msolve_last_launch_count(A: Matrix) -> int:

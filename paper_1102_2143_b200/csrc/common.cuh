@@ -91,6 +91,17 @@ __device__ __forceinline__ uint64_t policy_evict_normal() {
 __device__ __forceinline__ uint64_t policy_evict_last() {
     uint64_t p; asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p)); return p;
 }
+// Matrix stream: evict-first (read once per SpMV), or evict-last for `keep_pct` percent of the lines (chosen by the
+// hardware from the address) and evict-first for the rest -- for a matrix of which only a part fits in L2 next to
+// the vectors (MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT).
+__device__ __forceinline__ uint64_t policy_matrix(int keep_pct) {
+    if (keep_pct <= 0) return policy_evict_first();
+    if (keep_pct >= 100) return policy_evict_last();
+    uint64_t p;
+    const float f = 0.01f * (float)keep_pct;
+    asm volatile("createpolicy.fractional.L2::evict_last.L2::evict_first.b64 %0, %1;" : "=l"(p) : "f"(f));
+    return p;
+}
 
 // Gathered x of the CSR kernels, loaded with an L2 cache hint: evict_last pins x against the matrix
 // stream when it fits in L2 comfortably (measured on config 5, B200: complex64, 34 MB of x: 0.98 ->
@@ -204,6 +215,7 @@ struct SolveHeader {
     int stop_rule;   // 0 = per shift (R15), 1 = literal |r| > eps on the unshifted system (Alg. 1 l.15)
     double* hist;    // msolve_set_history: per-iteration scalars, hist_cap rows (NULL = off)
     int hist_cap;
+    unsigned long long* phase_ns;   // msolve_set_phase_clock (one-kernel path), NULL = off
     int per_shift_norm;  // eq. (6): the stop test of shift k is relative to rhs_norm[k] = ||b_k|| instead of ||b||
     double sigma[kMaxShifts];
 };
@@ -293,7 +305,7 @@ struct MatDev {
     void* carry;             // merge-path: per-tile head / tail partial sums, 2 * aux_count complex
     int aux_count;
     int x_pin;               // CSR kernels: gather x with L2 evict_last (x fits in L2 next to the stream)
-    int mat_keep;            // TMA-staged kernels: stream the matrix with L2 evict_last (it fits in L2 between SpMVs)
+    int mat_keep;            // percent of the matrix stream loaded with L2 evict_last (0: all evict-first), policy_matrix()
     // matrix-free SU(3) lattice operator (msolve_create_lattice_su3): val = links[ndim][vol][3][3]
     int lat_ndim;            // 0 for CSR / BSR3
     int lat_ext[4];          // extents, dimension 0 fastest (unused dimensions = 1)

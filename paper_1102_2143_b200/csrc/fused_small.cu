@@ -47,20 +47,28 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_cgm_fused(MatDev A, SolveS
     acc[0] = init_vectors_fn<E, VEC>(h, cta, ncta);                                  // l.9-10, 13: r <- b, p <- b, <b,b>
     fused_allreduce<1>(st, gen, acc, s, red);
     init_state_fn(h, res, rc, s[0]);
+    PhaseClock clk(h.phase_ns);
     while (!res.done) {
         if (res.n_iter > 0) {
             cgm_pupdate_fn<E, VEC>(h, rc, cta, ncta);                                 // l.27
+            clk.mark(0);
             fused_allreduce<0>(st, gen, nullptr, nullptr, red);                       // p complete before it is gathered
+            clk.mark(1);
         }
         acc[0] = 0.0;
         fused_spmv<E, SEL, ROLE_CG>(A, h, acc);                                       // l.18-19
+        clk.mark(2);
         fused_allreduce<1>(st, gen, acc, s, red);
+        clk.mark(3);
         cgm_scal1_fn(h, res, rc, s[0]);                                               // l.20, 22, 23
         if (res.done) break;                                                          // breakdown: the same in every CTA
         acc[0] = cgm_update_fn<E, VEC, kUnrollCgm, false>(h, res, rc, cta, ncta);            // l.21, 24, 28, 29
+        clk.mark(4);
         fused_allreduce<1>(st, gen, acc, s, red);
+        clk.mark(5);
         cgm_scal2_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);   // l.25, 26, 30, 31, 15
     }
+    if (clk.ns) clk.ns[15] += (unsigned long long)res.n_iter;
     fused_publish(st, res, gen);
 }
 
@@ -79,25 +87,35 @@ __global__ void __launch_bounds__(kFusedThreads, 1) k_bi_fused(MatDev A, SolveSt
     acc[0] = init_vectors_fn<E, VEC>(h, cta, ncta);
     fused_allreduce<1>(st, gen, acc, s, red);
     init_state_fn(h, res, rc, s[0]);
+    PhaseClock clk(h.phase_ns);
     while (!res.done) {
 #pragma unroll
         for (int a = 0; a < 5; ++a) acc[a] = 0.0;
         fused_spmv<E, SEL, ROLE_B1>(A, h, acc);                                       // q = A p, <r0,q>
+        clk.mark(0);
         fused_allreduce<2>(st, gen, acc, s, red);
+        clk.mark(1);
         bi_scal1_fn(h, res, rc, zd{s[0], s[1]});
         if (res.done) break;
         bi_supdate_fn<E, VEC>(h, rc, cta, ncta);                                      // s = r + beta q
+        clk.mark(2);
         fused_allreduce<0>(st, gen, nullptr, nullptr, red);                           // s complete before it is gathered
+        clk.mark(3);
 #pragma unroll
         for (int a = 0; a < 5; ++a) acc[a] = 0.0;
         fused_spmv<E, SEL, ROLE_B2>(A, h, acc);                                       // t = A s, <t,s>, <t,t>, <r0,t>
+        clk.mark(4);
         fused_allreduce<5>(st, gen, acc, s, red);
+        clk.mark(5);
         bi_scal2_fn(h, res, rc, s);
         if (res.done) break;
         acc[0] = bi_update_fn<E, VEC, kUnrollBi, false>(h, res, rc, cta, ncta);              // r', p, x_k, p_k, |r'|^2
+        clk.mark(6);
         fused_allreduce<1>(st, gen, acc, s, red);                                     // also: p complete before SpMV#1
+        clk.mark(7);
         bi_scal3_fn(h, res, rc, rhs_norm, s[0], cta == 0 ? h.hist : nullptr);
     }
+    if (clk.ns) clk.ns[15] += (unsigned long long)res.n_iter;
     fused_publish(st, res, gen);
 }
 

@@ -108,4 +108,19 @@ __device__ __forceinline__ void fused_publish(SolveState* st, const SolveResult&
     for (int i = threadIdx.x; i < (int)(sizeof(SolveResult) / sizeof(int)); i += blockDim.x) dst[i] = src[i];
 }
 
+// msolve_set_phase_clock: thread 0 of CTA 0 adds the time since the previous mark to slot i (off: one uniform branch)
+struct PhaseClock {
+    unsigned long long* ns;
+    unsigned long long t0;
+    __device__ __forceinline__ static unsigned long long now() {
+        unsigned long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); return t;
+    }
+    __device__ __forceinline__ explicit PhaseClock(unsigned long long* p) : ns(blockIdx.x == 0 && threadIdx.x == 0 ? p : nullptr), t0(0) {
+        if (ns) t0 = now();
+    }
+    __device__ __forceinline__ void mark(int i) {
+        if (ns) { const unsigned long long t = now(); ns[i] += t - t0; t0 = t; }
+    }
+};
+
 }  // namespace msolve

@@ -65,6 +65,7 @@ struct msolve_matrix {
     void* d_carry = nullptr;            // merge-path carries (library-owned)
     double* d_hist = nullptr;           // msolve_set_history: caller's device buffer (borrowed)
     int hist_cap = 0;
+    unsigned long long* d_phase_ns = nullptr;   // msolve_set_phase_clock (borrowed)
     char* d_host_buf = nullptr;         // msolve_solve_host: device b, x and workspace, kept for the next call
     size_t host_buf_bytes = 0;
     char* d_batch_buf = nullptr;        // msolve_solve_host_batch: two (b, x) slots + workspace

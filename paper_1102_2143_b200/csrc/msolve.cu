@@ -422,9 +422,10 @@ extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
     if (key == MSOLVE_CFG_FUSED_CTAS && value >= 0 && value <= kFusedMaxCtas) { A->opt.fused_ctas = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_MATRIX_L2 && value >= 0 && value <= 2) {
         A->opt.matrix_l2 = value;
-        A->dev.mat_keep = value == 2;
+        A->dev.mat_keep = value == 2 ? 100 : 0;
         return MSOLVE_OK;
     }
+    if (key == MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT && value >= 0 && value <= 100) { A->dev.mat_keep = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_X_WINDOW && (value == 0 || value == 1)) {
         if (value == 1) {
             if (A->format != FMT_CSR || A->kernel != KERNEL_VECTOR) return fail(MSOLVE_EINVAL, "msolve_config: MSOLVE_CFG_X_WINDOW applies to the vector-CSR kernel");
@@ -448,6 +449,13 @@ extern "C" int msolve_set_history(msolve_matrix* A, double* d_hist, int cap_rows
     if (cap_rows < 0 || (cap_rows > 0 && !d_hist) || ((uintptr_t)d_hist & 7u)) return fail(MSOLVE_EINVAL, "msolve_set_history: bad buffer");
     A->d_hist = cap_rows > 0 ? d_hist : nullptr;
     A->hist_cap = cap_rows > 0 ? cap_rows : 0;
+    return MSOLVE_OK;
+}
+
+extern "C" int msolve_set_phase_clock(msolve_matrix* A, uint64_t* d_ns) {
+    if (!A) return fail(MSOLVE_EINVAL, "msolve_set_phase_clock: A is NULL");
+    if ((uintptr_t)d_ns & 7u) return fail(MSOLVE_EINVAL, "msolve_set_phase_clock: d_ns must be 8-byte aligned");
+    A->d_phase_ns = (unsigned long long*)d_ns;
     return MSOLVE_OK;
 }
 
@@ -490,7 +498,7 @@ static int fill_header(const msolve_matrix* A, int alg, const void* d_b, const d
     h->pk_stride = pk_stride_elems(A);
     h->x_stride = A->dev.n;
     h->tol = tol; h->S = S; h->max_iter = max_iter; h->force_all = force_all;
-    h->stop_rule = A->opt.stop_rule; h->hist = A->d_hist; h->hist_cap = A->hist_cap;
+    h->stop_rule = A->opt.stop_rule; h->hist = A->d_hist; h->hist_cap = A->hist_cap; h->phase_ns = A->d_phase_ns;
     for (int k = 0; k < S; ++k) h->sigma[k] = h_shifts[k];
     return MSOLVE_OK;
 }

@@ -144,6 +144,8 @@ __device__ __forceinline__ void bsr3_rows_body(const MatDev& A, const E* x, E* y
     const int32_t* __restrict__ bcol = A.colidx;
     const int32_t* __restrict__ browptr = A.rowptr;
     const long long stride = (long long)ncta * blockDim.x;
+    const bool keep = A.mat_keep > 0;            // MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT: hinted loads (policy_matrix)
+    const uint64_t polm = policy_matrix(A.mat_keep);
     for (long long row = (long long)cta * blockDim.x + threadIdx.x; row < A.n; row += stride) {
         const long long br = row / 3;
         const int rr = (int)(row - 3 * br);
@@ -153,7 +155,9 @@ __device__ __forceinline__ void bsr3_rows_body(const MatDev& A, const E* x, E* y
         for (int j = jb; j < je; ++j) {
             const C* blk = val + (long long)j * 9 + rr * 3;
             const C* xv = x + 3ll * bcol[j];
-            const C a0 = ld_stream(blk), a1 = ld_stream(blk + 1), a2 = ld_stream(blk + 2);
+            const C a0 = keep ? ld_xg<true>(blk, polm) : ld_stream(blk);
+            const C a1 = keep ? ld_xg<true>(blk + 1, polm) : ld_stream(blk + 1);
+            const C a2 = keep ? ld_xg<true>(blk + 2, polm) : ld_stream(blk + 2);
             sum = cfma(a0, NC ? ld_ro(xv) : xv[0], sum);
             sum = cfma(a1, NC ? ld_ro(xv + 1) : xv[1], sum);
             sum = cfma(a2, NC ? ld_ro(xv + 2) : xv[2], sum);
@@ -265,7 +269,7 @@ __global__ void __launch_bounds__(BsrTmaCfg<E, TB>::kThreadsTotal, CPS) k_spmv_b
         // ---------------- producer: one elected lane of the last warp
         if (threadIdx.x == NCT) {
             // the matrix is read once per SpMV: evict-first, unless it is small enough to stay in L2 between SpMVs
-            const uint64_t pol = A.mat_keep ? policy_evict_last() : policy_evict_first();
+            const uint64_t pol = policy_matrix(A.mat_keep);
             const C* __restrict__ val = (const C*)A.val;
             int t = blockIdx.x;
             int4 e = t < ntiles ? tiles[t] : make_int4(0, 0, 0, 0);

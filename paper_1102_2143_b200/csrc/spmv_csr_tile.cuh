@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(CsrTileCfg<E, LANES, U>::kThreadsTotal, CPS) k
         // ---------------- producer: one elected lane of the last warp
         if (threadIdx.x == NCT) {
             // the matrix is read once per SpMV: evict-first, unless it is small enough to stay in L2 between SpMVs
-            const uint64_t pol = A.mat_keep ? policy_evict_last() : policy_evict_first();
+            const uint64_t pol = policy_matrix(A.mat_keep);
             const C* __restrict__ val = (const C*)A.val;
             int t = blockIdx.x;
             int ka = 0, kb = 0;

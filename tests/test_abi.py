@@ -48,6 +48,7 @@ def test_validation_without_gpu(lib):
     assert lib.msolve_workspace_bytes(None, 4, 0) == 0
     assert lib.msolve_config(None, 0, 0) == -1
     assert lib.msolve_set_history(None, None, 0) == -1
+    assert lib.msolve_set_phase_clock(None, None) == -1
     # the solver entry points and the profiler check the handle before anything else
     sh = (ctypes.c_double * 1)(0.0)
     for fn in (lib.msolve_cgm, lib.msolve_bicgstabm):

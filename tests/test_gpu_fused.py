@@ -63,6 +63,31 @@ def test_fused_matches_oracle_and_graph(ms, which, fmt, dtype, tol):
     assert g2[1] == g[1] and np.array_equal(g2[2], g[2]) and np.array_equal(g2[3], g[3])
 
 
+@pytest.mark.parametrize("which,fmt", [("c2", "bsr3"), ("c3", "lat")])
+def test_phase_clock_counts_iterations_and_changes_nothing(ms, which, fmt):
+    # msolve_set_phase_clock: slot 15 counts the iterations of every solve, the phase slots of the algorithm are all
+    # non-zero, the rest stay zero, and the solve returns the same bytes with the clock on and off
+    w = W.config2() if which == "c2" else W.config3(extents=(8, 8, 8, 8))
+    g = gpu_solve(ms, w, np.complex128, fmt, cfg=fused(ms))
+    A = make_matrix(ms, w, np.complex128, fmt, cfg=fused(ms))
+    ns = torch.zeros(16, dtype=torch.int64, device="cuda")
+    ms.msolve_set_phase_clock(A, ns)
+    solve = ms.msolve_cgm if w.algorithm == "cgm" else ms.msolve_bicgstabm
+    b = dev(w.b)
+    for _ in range(2):
+        res = solve(A, b, w.shifts, w.tol, w.max_iter)
+    t = ns.cpu().numpy()
+    nph = 6 if w.algorithm == "cgm" else 8
+    assert t[15] == 2 * res.iterations == 2 * g[1]
+    assert np.all(t[:nph] > 0) and np.all(t[nph:15] == 0)
+    assert t[:nph].sum() < 1e9                              # two small solves: well under a second
+    assert np.array_equal(res.x.cpu().numpy(), g[2])
+    ms.msolve_set_phase_clock(A, None)
+    solve(A, b, w.shifts, w.tol, w.max_iter)
+    assert ns.cpu().numpy()[15] == t[15]
+    ms.msolve_destroy(A)
+
+
 def test_resident_needs_the_problem_to_fit(ms):
     # 16 shifts x 49152 rows x 16 B: 35 vectors + matrix = 49 MB do not fit in 148 x 200 KB; asking for the path by
     # name is an error, AUTO falls back to the L2 one-kernel path
