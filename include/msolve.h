@@ -78,7 +78,10 @@ enum {
                                     of 16 bytes.  Same arithmetic; both run at the same 6.0 TB/s on B200 */,
     MSOLVE_CFG_LATTICE_KERNEL = 2 /* tile kernel of msolve_create_lattice_su3 handles: 0 = the faster one per
                                      element type (default), 1 = (term, site) threads + partials, 2 = warp per tile,
-                                     3 = hybrid (forward links by bulk copy, backward links and neighbours gathered) */,
+                                     3 = hybrid (forward links by bulk copy, backward links and neighbours gathered),
+                                     4 = blocked (a tile is a block of x0-rows in the (x1, x2) plane whose interior
+                                     neighbours are staged once; 4-D lattices with L0 = 32 whose extents the block
+                                     divides, any other handle takes the default instead) */,
     MSOLVE_CFG_STOP_RULE = 3 /* 0 = per shift (default): shift k stops, and x_k is frozen, at the first iteration with
                                 |zeta_k| ||r|| <= tol ||b|| (the paper is silent on masking; R15).
                                 1 = Alg. 1 l.15 read literally ("while |r| > eps"): every shift keeps

@@ -416,7 +416,7 @@ extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
     if (!A) return fail(MSOLVE_EINVAL, "msolve_config: A is NULL");
     if (key == MSOLVE_CFG_LOOP_MODE && (value == 0 || value == 1)) { A->opt.loop_mode = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_UPDATE_KERNEL && (value == 0 || value == 1)) { A->opt.update_kernel = value; return MSOLVE_OK; }
-    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 3) { A->opt.lattice_kernel = value; return MSOLVE_OK; }
+    if (key == MSOLVE_CFG_LATTICE_KERNEL && value >= 0 && value <= 4) { A->opt.lattice_kernel = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_STOP_RULE && (value == 0 || value == 1)) { A->opt.stop_rule = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_ITER_PATH && value >= 0 && value <= 3) { A->opt.iter_path = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_FUSED_CTAS && value >= 0 && value <= kFusedMaxCtas) { A->opt.fused_ctas = value; return MSOLVE_OK; }

@@ -583,4 +583,154 @@ __global__ void __launch_bounds__(LatHybCfg<E, W>::kThreadsTotal, 1) k_spmv_lat_
     write_partials<NACC>(st, acc);
 }
 
+// ------------------------------------------------------------------------------------------
+// Blocked tile kernel (round 2).  The all-TMA kernels above move 84 elements per site from L2 into shared memory
+// (7 link rows and 7 x rows per x0-row) and stop at the L2 -> SM rate, not at HBM.  Here a tile is a block of
+// R1 x R2 x0-rows in the (x1, x2) plane at fixed x3: inside the block the backward link U_mu(s - mu) of a row is
+// the forward link of the neighbouring row and the neighbours' x are the neighbouring rows' own x, both already
+// staged, so only the block's surface comes in addition:
+//   link rows per tile: 4 R1 R2 (forward) + R2 (mu = 1, row x1 - 1) + R1 (mu = 2, row x2 - 1) + R1 R2 (mu = 3)
+//   x rows per tile:    R1 R2 (own) + 2 R2 (x1 -+ 1) + 2 R1 (x2 -+ 1) + 2 R1 R2 (x3 -+ 1)
+// 2 x 2: 69 elements per site instead of 84, and 25 bulk copies per 128 sites instead of 56 (R1 consecutive
+// x1-rows are one contiguous range).  One consumer warp per row of the block (lane = x0, so L0 = 32), every
+// operand out of shared memory, the same order of multiply-adds as k_spmv_lat_warp (bit-identical y); a stage is
+// filled by one producer warp (one per stage) and drained by all R1 R2 consumer warps.
+// Needs 4 dimensions, L0 = 32, R1 | L1, R2 | L2 (lat_blk_supported, spmv_role.cu).
+// ------------------------------------------------------------------------------------------
+template <typename E, int R1, int R2, int STAGES> struct LatBlkCfg {
+    static constexpr int L0 = 32;
+    static constexpr int NR = R1 * R2;                                   // rows per tile = consumer warps
+    static constexpr int kThreadsTotal = (NR + STAGES) * 32;             // + one producer warp per stage
+    static constexpr int kLinkRow = L0 * 9 * (int)sizeof(E), kXRow = L0 * 3 * (int)sizeof(E);
+    // link rows: F[mu][j][i] (4 NR), B1[j], B2[i], B3[j][i];   x rows: X[j][i], XF1[j], XB1[j], XF2[i], XB2[i], XF3, XB3
+    static constexpr int oB1 = 4 * NR, oB2 = oB1 + R2, oB3 = oB2 + R1, kLinkRows = oB3 + NR;
+    static constexpr int oXF1 = NR, oXB1 = oXF1 + R2, oXF2 = oXB1 + R2, oXB2 = oXF2 + R1, oXF3 = oXB2 + R1, oXB3 = oXF3 + NR,
+                         kXRows = oXB3 + NR;
+    static constexpr int kXBase = kLinkRows * kLinkRow;
+    static constexpr int kStageBytes = kXBase + kXRows * kXRow;
+    static constexpr int smem_bytes() { return STAGES * kStageBytes + 2 * STAGES * 8; }
+};
+
+template <typename E, int R1, int R2, int STAGES, int ROLE>
+__global__ void __launch_bounds__((LatBlkCfg<E, R1, R2, STAGES>::kThreadsTotal), 1) k_spmv_lat_blk(MatDev A, SolveState* st) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    typedef LatBlkCfg<E, R1, R2, STAGES> Cfg;
+    constexpr int NACC = RoleAcc<ROLE>::value;
+    constexpr int NR = Cfg::NR, L0 = Cfg::L0;
+    constexpr int SZ = (int)sizeof(C);
+    if (ROLE != ROLE_GEN && st->res.done) return;
+    extern __shared__ __align__(128) unsigned char smem[];
+    uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::kStageBytes);
+    const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < STAGES; ++s) { mbar_init(full0 + 8 * s, 1); mbar_init(empty0 + 8 * s, NR); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    const C* x; C* y; const C* u;
+    role_vectors<C, ROLE>(st, x, y, u);
+    const int L1 = A.lat_ext[1], L2 = A.lat_ext[2], L3 = A.lat_ext[3];
+    const int nA = L1 / R1, nB = L2 / R2;
+    const int ntiles = nA * nB * L3;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    if (warp >= NR) {
+        // ---------------- producer warp p fills stage p: tiles blockIdx.x + (m STAGES + p) gridDim.x
+        if (lane == 0) {
+            const int stage = warp - NR;
+            const C* __restrict__ links = (const C*)A.val;
+            const uint64_t pol = policy_evict_normal();
+            const long long vol = A.lat_vol;
+            unsigned char* sb = smem + stage * Cfg::kStageBytes;
+            const uint32_t bar = full0 + 8 * stage, ebar = empty0 + 8 * stage;
+            const uint32_t lrows = (uint32_t)(R1 * Cfg::kLinkRow), xrows = (uint32_t)(R1 * Cfg::kXRow);
+            for (int m = 0;; ++m) {
+                const long long tl = (long long)blockIdx.x + (long long)(m * STAGES + stage) * gridDim.x;
+                if (tl >= ntiles) break;
+                const int a = (int)(tl % nA), b = (int)((tl / nA) % nB), x3 = (int)(tl / ((long long)nA * nB));
+                const int x1 = a * R1, x2 = b * R2;
+                const int x1m = x1 == 0 ? L1 - 1 : x1 - 1, x1p = x1 + R1 == L1 ? 0 : x1 + R1;
+                const int x2m = x2 == 0 ? L2 - 1 : x2 - 1, x2p = x2 + R2 == L2 ? 0 : x2 + R2;
+                const int x3m = x3 == 0 ? L3 - 1 : x3 - 1, x3p = x3 + 1 == L3 ? 0 : x3 + 1;
+                // first site of x0-row (c1, c2, c3); link / x row `slot` of the stage
+#define MSOLVE_SITE0(c1, c2, c3) ((long long)L0 * ((c1) + (long long)L1 * ((c2) + (long long)L2 * (c3))))
+#define MSOLVE_LROW(slot) smem_u32(sb + (slot) * Cfg::kLinkRow)
+#define MSOLVE_XROW(slot) smem_u32(sb + Cfg::kXBase + (slot) * Cfg::kXRow)
+                mbar_wait(ebar, ((uint32_t)m & 1u) ^ 1u);
+                mbar_expect_tx(bar, (uint32_t)Cfg::kStageBytes);
+#pragma unroll
+                for (int j = 0; j < R2; ++j) {
+                    const long long s0 = MSOLVE_SITE0(x1, x2 + j, x3);
+#pragma unroll
+                    for (int mu = 0; mu < 4; ++mu)
+                        bulk_g2s(MSOLVE_LROW(mu * NR + j * R1), links + ((long long)mu * vol + s0) * 9, lrows, bar, pol);
+                    bulk_g2s(MSOLVE_XROW(j * R1), x + 3 * s0, xrows, bar, pol);
+                    const long long s1m = MSOLVE_SITE0(x1m, x2 + j, x3), s1p = MSOLVE_SITE0(x1p, x2 + j, x3);
+                    bulk_g2s(MSOLVE_LROW(Cfg::oB1 + j), links + (1ll * vol + s1m) * 9, (uint32_t)Cfg::kLinkRow, bar, pol);
+                    bulk_g2s(MSOLVE_XROW(Cfg::oXF1 + j), x + 3 * s1p, (uint32_t)Cfg::kXRow, bar, pol);
+                    bulk_g2s(MSOLVE_XROW(Cfg::oXB1 + j), x + 3 * s1m, (uint32_t)Cfg::kXRow, bar, pol);
+                    const long long s3m = MSOLVE_SITE0(x1, x2 + j, x3m), s3p = MSOLVE_SITE0(x1, x2 + j, x3p);
+                    bulk_g2s(MSOLVE_LROW(Cfg::oB3 + j * R1), links + (3ll * vol + s3m) * 9, lrows, bar, pol);
+                    bulk_g2s(MSOLVE_XROW(Cfg::oXF3 + j * R1), x + 3 * s3p, xrows, bar, pol);
+                    bulk_g2s(MSOLVE_XROW(Cfg::oXB3 + j * R1), x + 3 * s3m, xrows, bar, pol);
+                }
+                const long long s2m = MSOLVE_SITE0(x1, x2m, x3), s2p = MSOLVE_SITE0(x1, x2p, x3);
+                bulk_g2s(MSOLVE_LROW(Cfg::oB2), links + (2ll * vol + s2m) * 9, lrows, bar, pol);
+                bulk_g2s(MSOLVE_XROW(Cfg::oXF2), x + 3 * s2p, xrows, bar, pol);
+                bulk_g2s(MSOLVE_XROW(Cfg::oXB2), x + 3 * s2m, xrows, bar, pol);
+#undef MSOLVE_SITE0
+#undef MSOLVE_LROW
+#undef MSOLVE_XROW
+            }
+        }
+    } else {
+        // ---------------- consumer warp = row (i, j) of the block, lane = x0
+        const int i = warp % R1, j = warp / R1, r = warp;
+        const int jf = lane + 1 == L0 ? 0 : lane + 1, jb = lane == 0 ? L0 - 1 : lane - 1;
+        const T dg = (T)A.lat_diag, cf = (T)A.lat_cf, cb = (T)A.lat_cb;
+        const C z = cmake<C>(0.0, 0.0);
+        // operand rows of this warp inside a stage (in units of C): a neighbour inside the block, else the surface row
+        constexpr int LR = L0 * 9, XR = L0 * 3, XB = Cfg::kXBase / SZ;
+        const int l1b = (i > 0 ? (1 * NR + r - 1) : (Cfg::oB1 + j)) * LR;
+        const int l2b = (j > 0 ? (2 * NR + r - R1) : (Cfg::oB2 + i)) * LR;
+        const int x1f = XB + (i + 1 < R1 ? r + 1 : Cfg::oXF1 + j) * XR, x1b = XB + (i > 0 ? r - 1 : Cfg::oXB1 + j) * XR;
+        const int x2f = XB + (j + 1 < R2 ? r + R1 : Cfg::oXF2 + i) * XR, x2b = XB + (j > 0 ? r - R1 : Cfg::oXB2 + i) * XR;
+        for (int k = 0;; ++k) {
+            const int stage = k % STAGES, m = k / STAGES;
+            const long long tl = (long long)blockIdx.x + (long long)k * gridDim.x;
+            if (tl >= ntiles) break;
+            const int a = (int)(tl % nA), b = (int)((tl / nA) % nB), x3 = (int)(tl / ((long long)nA * nB));
+            const long long row = 3 * ((long long)L0 * ((a * R1 + i) + (long long)L1 * ((b * R2 + j) + (long long)L2 * x3)) + lane);
+            C u0 = z, u1 = z, u2 = z;
+            if (ROLE != ROLE_CG) { u0 = ld_ro(u + row); u1 = ld_ro(u + row + 1); u2 = ld_ro(u + row + 2); }
+            mbar_wait(full0 + 8 * stage, (uint32_t)m & 1u);
+            const C* sb = (const C*)(smem + stage * Cfg::kStageBytes);
+            C f0 = z, f1 = z, f2 = z, g0 = z, g1 = z, g2 = z;
+            lat_matvec_acc<C, false>(sb + r * LR + lane * 9, sb + XB + r * XR + jf * 3, f0, f1, f2);
+            lat_matvec_acc<C, true>(sb + r * LR + jb * 9, sb + XB + r * XR + jb * 3, g0, g1, g2);
+            lat_matvec_acc<C, false>(sb + (1 * NR + r) * LR + lane * 9, sb + x1f + lane * 3, f0, f1, f2);
+            lat_matvec_acc<C, true>(sb + l1b + lane * 9, sb + x1b + lane * 3, g0, g1, g2);
+            lat_matvec_acc<C, false>(sb + (2 * NR + r) * LR + lane * 9, sb + x2f + lane * 3, f0, f1, f2);
+            lat_matvec_acc<C, true>(sb + l2b + lane * 9, sb + x2b + lane * 3, g0, g1, g2);
+            lat_matvec_acc<C, false>(sb + (3 * NR + r) * LR + lane * 9, sb + XB + (Cfg::oXF3 + r) * XR + lane * 3, f0, f1, f2);
+            lat_matvec_acc<C, true>(sb + (Cfg::oB3 + r) * LR + lane * 9, sb + XB + (Cfg::oXB3 + r) * XR + lane * 3, g0, g1, g2);
+            const C* xo = sb + XB + r * XR + lane * 3;
+            const C x0 = xo[0], x1 = xo[1], x2 = xo[2];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty0 + 8 * stage);            // the tile's operands are in registers
+            const C y0 = lat_combine(dg, x0, cf, f0, cb, g0);
+            const C y1 = lat_combine(dg, x1, cf, f1, cb, g1);
+            const C y2 = lat_combine(dg, x2, cf, f2, cb, g2);
+            y[row] = y0; y[row + 1] = y1; y[row + 2] = y2;
+            lat_epilogue<C, ROLE>(acc, y0, x0, u0);
+            lat_epilogue<C, ROLE>(acc, y1, x1, u1);
+            lat_epilogue<C, ROLE>(acc, y2, x2, u2);
+        }
+    }
+    write_partials<NACC>(st, acc);
+}
+
 }  // namespace msolve

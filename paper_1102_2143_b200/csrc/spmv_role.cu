@@ -35,10 +35,22 @@ static int launch_csr_tile(const msolve_matrix* A, cudaStream_t s) {
     return MSOLVE_OK;
 }
 
-// which lattice tile kernel this launch takes (1 = (term, site), 2 = warp per tile, 3 = hybrid)
+// the blocked kernel's geometry: 4-D, x0-rows of 32 sites (lane = x0), extents the block divides
+template <typename T>
+static bool lat_blk_supported(const msolve_matrix* A) {
+    if constexpr (sizeof(T) == 2 * sizeof(typename RealOf<T>::type)) {
+        typedef LatBlkTile<T> B;
+        const MatDev& d = A->dev;
+        return d.lat_ndim == 4 && d.lat_ext[0] == 32 && d.lat_ext[1] % B::R1 == 0 && d.lat_ext[2] % B::R2 == 0;
+    }
+    return false;
+}
+
+// which lattice tile kernel this launch takes (1 = (term, site), 2 = warp per tile, 3 = hybrid, 4 = blocked)
 template <typename T, int ROLE>
 static int lattice_choice(const msolve_matrix* A) {
-    if (A->opt.lattice_kernel != 0) return A->opt.lattice_kernel;
+    if (A->opt.lattice_kernel == 4 && lat_blk_supported<T>(A)) return 4;
+    if (A->opt.lattice_kernel != 0 && A->opt.lattice_kernel != 4) return A->opt.lattice_kernel;
     // the second BiCGStab-M SpMV (five accumulators, two extra operands) spills in the hybrid kernel at 255
     // registers (config3x: spmv2_dots 0.278 ms all-TMA, 0.320 ms hybrid): it stays on the all-TMA kernels
     if (ROLE == ROLE_B2 && LatDefault<T>::kernel == 3) return sizeof(T) == 16 ? 1 : 2;
@@ -113,6 +125,16 @@ static int launch_spmv_t(const msolve_matrix* A, cudaStream_t s) {
         }
         if (A->format == FMT_LATTICE && A->kernel == KERNEL_LAT_TMA) {
             const int which = lattice_choice<T, ROLE>(A);
+            if (which == 4) {
+                typedef LatBlkTile<T> B;
+                typedef LatBlkCfg<T, B::R1, B::R2, B::STAGES> Cfg;
+                auto k = k_spmv_lat_blk<T, B::R1, B::R2, B::STAGES, ROLE>;
+                if ((rc = ensure_smem(A, (const void*)k, Cfg::smem_bytes())) != MSOLVE_OK) return rc;
+                const long long ntiles = (long long)(A->dev.lat_ext[1] / B::R1) * (A->dev.lat_ext[2] / B::R2) * A->dev.lat_ext[3];
+                const int grid = (int)std::max(1ll, std::min<long long>(A->num_sms, ntiles));
+                k<<<grid, Cfg::kThreadsTotal, Cfg::smem_bytes(), s>>>(A->dev, A->d_state);
+                return MSOLVE_OK;
+            }
             if (which == 3) {
                 typedef LatHybTile<T> H;
                 auto k = k_spmv_lat_hyb<T, H::W, H::STAGES, ROLE>;

@@ -32,6 +32,11 @@ constexpr int kLatWarpProducers = 4;
 template <typename E> struct LatHybTile;
 template <> struct LatHybTile<double2> { static constexpr int W = 6, STAGES = 6; };
 template <> struct LatHybTile<float2>  { static constexpr int W = 8, STAGES = 8; };
+// blocked kernel k_spmv_lat_blk: block of R1 x R2 x0-rows per tile, ring depth (= producer warps); the stage of a
+// 2 x 2 block is 70.7 KB in complex64 (three fit), 141 KB in complex128 (hence 2 x 1 there: 78.3 KB, two stages)
+template <typename E> struct LatBlkTile;
+template <> struct LatBlkTile<double2> { static constexpr int R1 = 2, R2 = 1, STAGES = 2; };
+template <> struct LatBlkTile<float2>  { static constexpr int R1 = 2, R2 = 2, STAGES = 3; };
 // default lattice tile kernel per element type (MSOLVE_CFG_LATTICE_KERNEL = 0): 1 = (term, site), 2 = warp, 3 = hybrid
 template <typename E> struct LatDefault;
 template <> struct LatDefault<double2> { static constexpr int kernel = 3; };   // 0.238 ms (all-TMA 0.269 / 0.277)

@@ -78,7 +78,7 @@ def c4():
     return w, refs
 
 
-C4_VARIANTS = ["bsr3", "csr", "csrmerge", "lat", "lat1", "lat2", "lat3", "bsr3_updtma", "slabs8_bsr3", "slabs3_csr"]
+C4_VARIANTS = ["bsr3", "csr", "csrmerge", "lat", "lat1", "lat2", "lat3", "lat4", "bsr3_updtma", "slabs8_bsr3", "slabs3_csr"]
 
 
 def _c4_matrix(ms, w, dtype, variant):

@@ -20,16 +20,19 @@ def _workload(extents, nonhermitian=False):
 
 EXTENTS = [(4, 4, 6, 5),        # 8 x0-rows per tile
            (12, 10, 9, 11),     # 2 rows per tile, odd row count: ragged last tile, many tiles per CTA
-           (32, 4, 3, 3),       # one row per tile (the config-4 shape)
+           (32, 4, 3, 3),       # one row per tile (the config-4 shape); blocked kernel: complex128 only (2 x 1 block)
+           (32, 6, 4, 3),       # blocked kernel in both precisions: 3 x 2 blocks per x3-slice, several tiles per stage
+           (32, 4, 4, 3),       # blocked kernel, two blocks per direction: both neighbours of a block are the same block
            (5, 3, 4),           # 3-D, odd L0: complex64 rows are not 16-byte multiples -> row kernel
            (3, 3),              # 2-D, smallest legal extents
            (16,),               # 1-D
            (36, 3, 3, 3)]       # L0 > 32 sites: row kernel
 
 
-@pytest.fixture(params=[1, 2, 3], ids=["termsite", "warptile", "hybrid"])
+@pytest.fixture(params=[1, 2, 3, 4], ids=["termsite", "warptile", "hybrid", "blocked"])
 def tile_kernel(request, ms):
-    """Run with each of the three tile kernels forced (default: the faster one per element type)."""
+    """Run with each of the tile kernels forced (default: the faster one per element type; the blocked kernel
+    leaves lattices it does not cover -- L0 != 32, fewer than 4 dimensions, odd extents -- to the default)."""
     test_gpu_parity.FORCED_CFG[ms.MSOLVE_CFG_LATTICE_KERNEL] = request.param
     yield request.param
     test_gpu_parity.FORCED_CFG.clear()
@@ -67,6 +70,32 @@ def test_config2_cgm_matrix_free(ms, fmt, dtype, tol):
 def test_config4_scaled_cgm_matrix_free(ms, tile_kernel, dtype, tol):
     w = W.config4(extents=(32, 8, 4, 6), tol=tol)
     g = gpu_solve(ms, w, dtype, "lat")
+    o = oracle_solve(w, dtype)
+    check_parity(w, dtype, g, o, tol)
+
+
+def test_blocked_kernel_is_bit_identical_to_the_warp_kernel(ms):
+    # same operands, same order of multiply-adds per site: only where the operands come from differs
+    for nh in (False, True):
+        w = _workload((32, 6, 4, 3), nh)
+        rng = np.random.default_rng(7)
+        for dtype in (np.complex128, np.complex64):
+            x = (rng.standard_normal(w.n) + 1j * rng.standard_normal(w.n)).astype(dtype)
+            ys = []
+            for kern in (2, 4):
+                A = make_matrix(ms, w, dtype, "lat", cfg={ms.MSOLVE_CFG_LATTICE_KERNEL: kern})
+                y, _ = ms.msolve_spmv(A, dev(x))
+                ys.append(y.cpu().numpy())
+                ms.msolve_destroy(A)
+            assert np.array_equal(ys[0], ys[1])
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.complex128, 1e-9), (np.complex64, 1e-4)])
+def test_bicgstabm_on_the_blocked_kernel(ms, dtype, tol):
+    # both BiCGStab-M SpMV roles (two and five fused dot products) on a lattice the blocked kernel covers
+    w = W.config3(extents=(32, 4, 4, 3))
+    w.tol = tol
+    g = gpu_solve(ms, w, dtype, "lat", cfg={ms.MSOLVE_CFG_LATTICE_KERNEL: 4})
     o = oracle_solve(w, dtype)
     check_parity(w, dtype, g, o, tol)
 
