@@ -76,8 +76,9 @@ enum {
     MSOLVE_CFG_UPDATE_KERNEL = 1 /* CG-M fused multishift update: 0 = register kernel (default), 1 = TMA-staged
                                     kernel (bulk async loads AND stores) whenever the vector length is a multiple
                                     of 16 bytes.  Same arithmetic; both run at the same 6.0 TB/s on B200 */,
-    MSOLVE_CFG_LATTICE_KERNEL = 2 /* tile kernel of msolve_create_lattice_su3 handles: 0 = the faster one per
-                                     element type (default), 1 = (term, site) threads + partials, 2 = warp per tile,
+    MSOLVE_CFG_LATTICE_KERNEL = 2 /* tile kernel of msolve_create_lattice_su3 handles: 0 = the fastest one for the
+                                     lattice and element type (default: 4 where it applies, else 3 for complex128 and
+                                     2 for complex64), 1 = (term, site) threads + partials, 2 = warp per tile,
                                      3 = hybrid (forward links by bulk copy, backward links and neighbours gathered),
                                      4 = blocked (a tile is a block of x0-rows in the (x1, x2) plane whose interior
                                      neighbours are staged once; 4-D lattices with L0 = 32 whose extents the block

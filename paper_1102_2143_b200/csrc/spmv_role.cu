@@ -49,7 +49,9 @@ static bool lat_blk_supported(const msolve_matrix* A) {
 // which lattice tile kernel this launch takes (1 = (term, site), 2 = warp per tile, 3 = hybrid, 4 = blocked)
 template <typename T, int ROLE>
 static int lattice_choice(const msolve_matrix* A) {
-    if (A->opt.lattice_kernel == 4 && lat_blk_supported<T>(A)) return 4;
+    // 4-D lattices with x0-rows of 32 sites take the blocked kernel: config 4 complex64 0.148 -> 0.121 ms against
+    // the warp kernel, complex128 0.241 -> 0.240 ms against the hybrid one, second BiCGStab-M SpMV 0.287 -> 0.270 ms
+    if ((A->opt.lattice_kernel == 4 || A->opt.lattice_kernel == 0) && lat_blk_supported<T>(A)) return 4;
     if (A->opt.lattice_kernel != 0 && A->opt.lattice_kernel != 4) return A->opt.lattice_kernel;
     // the second BiCGStab-M SpMV (five accumulators, two extra operands) spills in the hybrid kernel at 255
     // registers (config3x: spmv2_dots 0.278 ms all-TMA, 0.320 ms hybrid): it stays on the all-TMA kernels

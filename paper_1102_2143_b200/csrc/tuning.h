@@ -37,7 +37,8 @@ template <> struct LatHybTile<float2>  { static constexpr int W = 8, STAGES = 8;
 template <typename E> struct LatBlkTile;
 template <> struct LatBlkTile<double2> { static constexpr int R1 = 2, R2 = 1, STAGES = 2; };
 template <> struct LatBlkTile<float2>  { static constexpr int R1 = 2, R2 = 2, STAGES = 3; };
-// default lattice tile kernel per element type (MSOLVE_CFG_LATTICE_KERNEL = 0): 1 = (term, site), 2 = warp, 3 = hybrid
+// default lattice tile kernel per element type where the blocked kernel does not apply (MSOLVE_CFG_LATTICE_KERNEL = 0):
+// 1 = (term, site), 2 = warp, 3 = hybrid
 template <typename E> struct LatDefault;
 template <> struct LatDefault<double2> { static constexpr int kernel = 3; };   // 0.238 ms (all-TMA 0.269 / 0.277)
 template <> struct LatDefault<float2>  { static constexpr int kernel = 2; };   // 0.149 ms (hybrid 0.168)
