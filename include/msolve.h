@@ -232,6 +232,26 @@ int msolve_solve_host_batch(const msolve_matrix *A, int algorithm, int nrhs, con
  * Exposed for parity tests of the SpMV kernels and for per-kernel timing. */
 int msolve_spmv(const msolve_matrix *A, const void *d_x, void *d_y, double *h_dot, void *stream);
 
+/* The same operation for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): y = A x for a CSR matrix and d_dot[0..1] = <x, A x> = sum_i conj(x_i) y_i
+ * (Alg. 1 l.18-19), without a handle.  The call allocates NOTHING (no cudaMalloc / cudaFree, no
+ * allocating library routine) and does not synchronise: two kernels are enqueued on `stream`.
+ *   n                 rows = columns, 0 <= n <= MSOLVE_NOALLOC_MAX_ROWS, else MSOLVE_EINVAL (nothing is launched);
+ *   d_rowptr [n+1], d_colidx [nnz], d_val [nnz]: device CSR arrays, borrowed, column indices in [0, n);
+ *   dtype             MSOLVE_C64 / C128 / F32 / F64: element type of d_val, d_x, d_y;
+ *   d_x [n] in, d_y [n] out, d_dot [2 doubles: re, im] out: device, caller-owned, aligned to their element size;
+ *                     for real types d_dot[1] = 0.  d_y must not alias d_x.
+ * Scratch: one (re, im) partial per 64 rows in a static device array of MSOLVE_NOALLOC_MAX_ROWS / 64 * 16 bytes =
+ * 256 KiB, which every GPU that loads the library holds until the process exits.  The first call on a device
+ * resolves the array's device address (cudaGetSymbolAddress, once per device): make that call outside graph
+ * capture.  All calls share the array: calls that overlap on the GPU (different streams, graph branches without a
+ * dependency between them) RACE on it and must be serialised by the caller; nothing in it needs clearing between
+ * calls (a call reads only the partials it has written itself).  Larger systems: msolve_create_csr + msolve_spmv.
+ * Returns MSOLVE_OK / MSOLVE_EINVAL / MSOLVE_ECUDA. */
+#define MSOLVE_NOALLOC_MAX_ROWS 1048576
+int msolve_spmv_csr_noalloc(int64_t n, const int32_t *d_rowptr, const int32_t *d_colidx, const void *d_val, int dtype,
+                            const void *d_x, void *d_y, double *d_dot, void *stream);
+
 /* Per-kernel timing of `iters` steady-state iterations (no convergence test, all shifts active),
  * each kernel bracketed by CUDA events on `stream`.  h_ms[j] receives the mean duration in ms of
  * kernel j, h_launches[j] its launches per iteration; names via msolve_kernel_name(algorithm, j).

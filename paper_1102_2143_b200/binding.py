@@ -35,7 +35,7 @@ MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT = 8
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",
-    "msolve_bicgstabm", "msolve_multirhs_workspace_bytes", "msolve_solve_multirhs", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_profile_iteration",
+    "msolve_bicgstabm", "msolve_multirhs_workspace_bytes", "msolve_solve_multirhs", "msolve_solve_host", "msolve_solve_host_batch", "msolve_spmv", "msolve_spmv_csr_noalloc", "msolve_profile_iteration",
     "msolve_kernel_name", "msolve_last_launch_count", "msolve_config", "msolve_set_history", "msolve_set_phase_clock", "msolve_destroy",
     "msolve_last_error",
     "msolve_slab_plan_create", "msolve_slab_plan_nlocal", "msolve_slab_plan_nhalo", "msolve_slab_plan_npeers",
@@ -86,6 +86,8 @@ def load_library() -> ctypes.CDLL:
     lib.msolve_config.argtypes = [vp, i32, i32]
     lib.msolve_set_history.argtypes = [vp, vp, i32]
     lib.msolve_set_phase_clock.argtypes = [vp, vp]
+    lib.msolve_spmv_csr_noalloc.argtypes = [ctypes.c_int64, vp, vp, vp, i32, vp, vp, vp, vp]
+    lib.msolve_spmv_csr_noalloc.restype = i32
     lib.msolve_destroy.argtypes = [vp]
     lib.msolve_destroy.restype = None
     lib.msolve_last_error.restype = ctypes.c_char_p
@@ -413,6 +415,31 @@ def msolve_spmv(A: Matrix, x: torch.Tensor, y: Optional[torch.Tensor] = None, st
     dot = np.zeros(2, dtype=np.float64)
     _check(lib.msolve_spmv(A.handle, x.data_ptr(), y.data_ptr(), dot.ctypes.data, _stream(stream)))
     return y, complex(dot[0], dot[1])
+
+
+MSOLVE_NOALLOC_MAX_ROWS = 1 << 20
+
+
+def msolve_spmv_csr_noalloc(rowptr: torch.Tensor, colidx: torch.Tensor, val: torch.Tensor, x: torch.Tensor,
+                            y: Optional[torch.Tensor] = None, dot: Optional[torch.Tensor] = None, stream=None):
+    """y = A x and <x, A x> for a CSR matrix without a handle and without any device allocation inside the library
+    (include/msolve.h: static scratch, n <= MSOLVE_NOALLOC_MAX_ROWS, calls that overlap on the GPU race).
+    Pass `y` [n] and `dot` [2] float64 CUDA tensors to keep torch from allocating either; does not synchronise.
+    Returns (y, dot) with dot = (re, im) on the device."""
+    lib = load_library()
+    rowptr, colidx, val = _dev(rowptr, torch.int32), _dev(colidx, torch.int32), _dev(val)
+    x = _dev(x, val.dtype)
+    n = rowptr.numel() - 1
+    if x.numel() != n:
+        raise ValueError("x must have n = rowptr.numel() - 1 entries")
+    if y is None:
+        y = torch.empty_like(x)
+    if dot is None:
+        dot = torch.empty(2, dtype=torch.float64, device=x.device)
+    y, dot = _dev(y, val.dtype), _dev(dot, torch.float64)
+    _check(lib.msolve_spmv_csr_noalloc(n, rowptr.data_ptr(), colidx.data_ptr(), val.data_ptr(), _dtype_code(val),
+                                       x.data_ptr(), y.data_ptr(), dot.data_ptr(), _stream(stream)))
+    return y, dot
 
 
 def msolve_profile_iteration(A: Matrix, algorithm: int, b: torch.Tensor, shifts, iters: int,

@@ -15,7 +15,8 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmsolve.so")
 # (source, object name, extra defines)
 UNITS = [("msolve.cu", "msolve.o", []), ("vec.cu", "vec.o", []), ("fused_small.cu", "fused_small.o", []),
-         ("slab.cu", "slab.o", []), ("multirhs.cu", "multirhs.o", []), ("resident.cu", "resident.o", [])] + \
+         ("slab.cu", "slab.o", []), ("multirhs.cu", "multirhs.o", []), ("resident.cu", "resident.o", []),
+         ("noalloc.cu", "noalloc.o", [])] + \
         [("spmv_role.cu", "spmv_role%d.o" % r, ["-DMSOLVE_ROLE=%d" % r]) for r in range(4)]
 
 NVCC_FLAGS = [
