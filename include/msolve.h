@@ -217,8 +217,9 @@ int msolve_solve_host(const msolve_matrix *A, int algorithm, const void *h_b, co
 
 /* The same for a batch of nrhs right-hand sides of one family (RHMC solves the same shifted family for
  * several pseudofermion fields): h_b[i] -> h_x[i] (nshifts*n each, shift-major), solved one
- * after the other on `stream`, software-pipelined: the device-to-host copy of solution set i runs on a
- * library-owned copy stream while solve i+1 is running (two device slots of b and x, kept in the handle).
+ * after the other on `stream`, software-pipelined: the device-to-host copy of solution set i and the host-to-device
+ * copy of the NEXT right-hand side run on two library-owned copy streams while a solve is running (two
+ * device slots of b and x, kept in the handle).
  * Host vectors should be pinned, or the copies do not overlap.  h_iterations: nrhs; h_conv_iter,
  * h_relres: nrhs*nshifts (or NULL).  Returns the largest status of the solves (MSOLVE_OK / MAXITER /
  * BREAKDOWN) or the first error (< 0); all copies have completed on return. */

@@ -71,7 +71,8 @@ struct msolve_matrix {
     char* d_batch_buf = nullptr;        // msolve_solve_host_batch: two (b, x) slots + workspace
     size_t batch_buf_bytes = 0;
     cudaStream_t copy_stream = nullptr; // D2H of solve i overlaps solve i+1
-    cudaEvent_t ev_solved[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr};
+    cudaStream_t h2d_stream = nullptr;  // H2D of b_{i+1} overlaps solve i (the other copy engine)
+    cudaEvent_t ev_solved[2] = {nullptr, nullptr}, ev_copied[2] = {nullptr, nullptr}, ev_loaded[2] = {nullptr, nullptr};
     cudaStream_t capture_stream = nullptr;
     msolve::LoopGraph graphs[2];
     int64_t last_launches = 0;

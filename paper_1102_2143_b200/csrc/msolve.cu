@@ -405,8 +405,10 @@ extern "C" void msolve_destroy(msolve_matrix* A) {
     for (int i = 0; i < 2; ++i) {
         if (A->ev_solved[i]) cudaEventDestroy(A->ev_solved[i]);
         if (A->ev_copied[i]) cudaEventDestroy(A->ev_copied[i]);
+        if (A->ev_loaded[i]) cudaEventDestroy(A->ev_loaded[i]);
     }
     if (A->copy_stream) cudaStreamDestroy(A->copy_stream);
+    if (A->h2d_stream) cudaStreamDestroy(A->h2d_stream);
     delete A;
 }
 
@@ -685,19 +687,31 @@ extern "C" int msolve_solve_host_batch(const msolve_matrix* A, int algorithm, in
             CU(cudaEventCreateWithFlags(&Am->ev_copied[j], cudaEventDisableTiming));
         }
     }
+    if (!Am->h2d_stream) {
+        CU(cudaStreamCreateWithFlags(&Am->h2d_stream, cudaStreamNonBlocking));
+        for (int j = 0; j < 2; ++j) CU(cudaEventCreateWithFlags(&Am->ev_loaded[j], cudaEventDisableTiming));
+    }
     char* d_ws = Am->d_batch_buf + 2 * slot;
     int worst = MSOLVE_OK;
+    // b_0 goes up front; b_{i+1} is sent on its own stream (the host-to-device copy engine) while solve i runs: the
+    // b of slot (i+1) & 1 was last read by solve i-1, which has completed (run_solver synchronises `stream`)
+    CU(cudaMemcpyAsync(Am->d_batch_buf, h_b[0], bbytes, cudaMemcpyHostToDevice, Am->h2d_stream));
+    CU(cudaEventRecord(Am->ev_loaded[0], Am->h2d_stream));
     for (int i = 0; i < nrhs; ++i) {
         const int j = i & 1;
         char* d_b = Am->d_batch_buf + (size_t)j * slot;
         char* d_x = d_b + align_up(bbytes, 256);
+        if (i + 1 < nrhs) {
+            CU(cudaMemcpyAsync(Am->d_batch_buf + (size_t)(j ^ 1) * slot, h_b[i + 1], bbytes, cudaMemcpyHostToDevice, Am->h2d_stream));
+            CU(cudaEventRecord(Am->ev_loaded[j ^ 1], Am->h2d_stream));
+        }
         if (i >= 2) CU(cudaStreamWaitEvent(stream, Am->ev_copied[j], 0));       // slot j has been read back
-        CU(cudaMemcpyAsync(d_b, h_b[i], bbytes, cudaMemcpyHostToDevice, stream));
+        CU(cudaStreamWaitEvent(stream, Am->ev_loaded[j], 0));                    // b_i has arrived
         const int rc = run_solver(algorithm, A, d_b, h_shifts, nshifts, tol, max_iter, d_x, d_ws, wsb + 256,
                                   h_iterations ? h_iterations + i : nullptr,
                                   h_conv_iter ? h_conv_iter + (size_t)i * nshifts : nullptr,
                                   h_relres ? h_relres + (size_t)i * nshifts : nullptr, stream_, 0);
-        if (rc < 0) { cudaStreamSynchronize(Am->copy_stream); return rc; }
+        if (rc < 0) { cudaStreamSynchronize(Am->copy_stream); cudaStreamSynchronize(Am->h2d_stream); return rc; }
         worst = std::max(worst, rc);
         CU(cudaEventRecord(Am->ev_solved[j], stream));
         CU(cudaStreamWaitEvent(Am->copy_stream, Am->ev_solved[j], 0));
