@@ -250,7 +250,7 @@ def config_dict(args, w, dtype, fmt, world, S, shifts_total):
     return {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
             "shifts": S, "tol": w.tol,
             "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world,
-            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "lattice_kernel": args.lattice_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "matrix_l2_keep_percent": args.matrix_l2_keep, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
+            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "defer_update": (16 if args.defer < 0 else args.defer) if args.update_kernel == "regs" else 0, "lattice_kernel": args.lattice_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "matrix_l2_keep_percent": args.matrix_l2_keep, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
 
 
 def run_reference(args, rank):
@@ -340,6 +340,9 @@ def main():
                     help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
     ap.add_argument("--lattice-kernel", type=int, default=0, choices=[0, 1, 2, 3, 4],
                     help="tile kernel of the lattice operator (MSOLVE_CFG_LATTICE_KERNEL; 0 = default per element type)")
+    ap.add_argument("--defer", type=int, default=-1,
+                    help="CG-M: chunk length of the deferred multishift update (MSOLVE_CFG_DEFER_UPDATE; 0 = update "
+                         "every x_k, p_k in every iteration; -1 = the library's default, 16)")
     ap.add_argument("--update-kernel", default="regs", choices=["regs", "tma"],
                     help="CG-M fused multishift update: register kernel (default) or the TMA-staged kernel")
     ap.add_argument("--x-window", action="store_true",
@@ -425,6 +428,8 @@ def main():
     ms.msolve_config(A, ms.MSOLVE_CFG_UPDATE_KERNEL, 1 if args.update_kernel == "tma" else 0)
     if args.lattice_kernel:
         ms.msolve_config(A, ms.MSOLVE_CFG_LATTICE_KERNEL, args.lattice_kernel)
+    if args.defer >= 0:
+        ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, args.defer)
     if args.x_window:
         ms.msolve_config(A, ms.MSOLVE_CFG_X_WINDOW, 1)
     ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, {"auto": 0, "graph": 1, "fused": 2, "resident": 3}[args.iter_path])

@@ -32,6 +32,7 @@ MSOLVE_CFG_MATRIX_L2 = 5
 MSOLVE_CFG_ITER_PATH = 6
 MSOLVE_CFG_FUSED_CTAS = 7
 MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT = 8
+MSOLVE_CFG_DEFER_UPDATE = 9
 
 EXPORTS = (
     "msolve_create_csr", "msolve_create_bsr3", "msolve_create_lattice_su3", "msolve_workspace_bytes", "msolve_cgm",

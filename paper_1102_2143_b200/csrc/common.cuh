@@ -217,6 +217,11 @@ struct SolveHeader {
     int hist_cap;
     unsigned long long* phase_ns;   // msolve_set_phase_clock (one-kernel path), NULL = off
     int per_shift_norm;  // eq. (6): the stop test of shift k is relative to rhs_norm[k] = ||b_k|| instead of ||b||
+    // deferred multishift update (CG-M, graph path; kernels.cuh "deferred update"): ring of defer + 1 residual vectors
+    // (r itself lives in it), defer = chunk length M (0 = the classic update of every x_k, p_k in every iteration)
+    void* ring;
+    long long ring_stride;   // BYTES between two slots of the ring
+    int defer;
     double sigma[kMaxShifts];
 };
 
@@ -248,6 +253,25 @@ struct Recur {
     double coef[kMaxShifts * 14];
 };
 
+// Deferred multishift update: bookkeeping of one chunk of at most kDeferMax iterations (kernels.cuh).  The shifts
+// that were active when the chunk began are `list`; for list position a and chunk-relative iteration j
+//   p_k(now)  = Ap[a] P_k + sum_j Cp[a][j] r_j,      x_k(now) = X_k + Ax[a] P_k + sum_j Cx[a][j] r_j
+// with P_k, X_k the vectors in memory (written by the previous flush) and r_j the residuals kept in the ring.
+constexpr int kDeferMax = 16;
+struct Defer {
+    int fill;            // residuals of the chunk whose coefficients are complete (= iterations done in the chunk)
+    int s0;              // ring slot of the chunk's first residual
+    int first;           // 1 until the first flush: P_k, X_k are not in memory yet (p_k(-1) = 0, x_k(0) = 0)
+    int need_begin;      // the next scal1 starts a new chunk
+    int nlist;
+    unsigned int ticket; // last-CTA detection of the flush kernel
+    void* r_next;        // where the r update of this iteration writes r_{n+1}
+    int list[kMaxShifts];    // shift index of list position a
+    int pos[kMaxShifts];     // list position of shift k
+    double Ap[kMaxShifts], Ax[kMaxShifts];
+    double Cp[kMaxShifts * kDeferMax], Cx[kMaxShifts * kDeferMax];
+};
+
 // one CTA's contribution to a grid-wide sum of the one-kernel path (fused_small.cu): values + generation tag
 constexpr int kFusedMaxCtas = 160;
 struct alignas(128) FusedSlot { unsigned long long w[2 * kAccMax]; unsigned long long tag; };
@@ -264,6 +288,7 @@ struct SolveState {
     // counter, which runs on from solve to solve (fused_gen)
     FusedSlot fslot[2][kFusedMaxCtas];
     unsigned long long fused_gen;
+    Defer df;
 };
 
 // Fixed-order reduction of `count` per-CTA partials (NACC rows of kMaxPartials) by ONE CTA: every thread of the

@@ -34,7 +34,8 @@ struct Options {
     int x_window = 0;        // MSOLVE_CFG_X_WINDOW
     int matrix_l2 = 0;       // MSOLVE_CFG_MATRIX_L2
     int fused_ctas = 0;      // MSOLVE_CFG_FUSED_CTAS
-    int graph_key() const { return loop_mode | (update_kernel << 1) | (lattice_kernel << 2) | (iter_path << 4) | (x_window << 6); }
+    int defer = kDeferMax;   // MSOLVE_CFG_DEFER_UPDATE: chunk length of the deferred multishift update (0 = off)
+    int graph_key() const { return loop_mode | (update_kernel << 1) | (lattice_kernel << 2) | (iter_path << 5) | (x_window << 7) | (defer << 8); }
 };
 
 struct LoopGraph {
@@ -94,6 +95,12 @@ int fail(int code, const char* fmt, ...);
         if (e_ != cudaSuccess)                                                                         \
             return ::msolve::fail(MSOLVE_ECUDA, "%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
     } while (0)
+
+// chunk length of the deferred multishift update this handle uses for `alg` (0: the update of every iteration):
+// CG-M with the register update kernel; BiCGStab-M and the TMA-staged update kernel keep the step-by-step form
+inline int defer_len(const msolve_matrix* A, int alg) {
+    return (alg == MSOLVE_ALG_CGM && A->opt.update_kernel == 0) ? A->opt.defer : 0;
+}
 
 inline size_t elem_bytes(int dtype) { return dtype == MSOLVE_C128 ? 16 : dtype == MSOLVE_F32 ? 4 : 8; }
 

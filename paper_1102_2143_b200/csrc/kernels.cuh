@@ -271,6 +271,210 @@ __global__ void __launch_bounds__(kThreads) k_cgm_update(SolveState* st) {
     }
 }
 
+// ----------------------------------------------------------------------------- CG-M, deferred multishift update
+// Alg. 1 l.28-29 touch every x_k and p_k in every iteration: 4 S + 3 vector passes, 2/3 of the
+// bytes of an iteration at S = 16.  But p_k(n) = zeta_k(n) r_n + alpha_k(n) p_k(n-1) and x_k(n+1) = x_k(n) -
+// beta_k(n) p_k(n) are LINEAR in the residuals with scalar coefficients the recurrences already produce, so over a
+// chunk of M iterations that starts with P_k = p_k(n0 - 1), X_k = x_k(n0) in memory
+//     p_k(n0 + m - 1) = Ap_k P_k + sum_j Cp_k[j] r_{n0+j},     x_k(n0 + m) = X_k + Ax_k P_k + sum_j Cx_k[j] r_{n0+j}
+// where appending iteration n (coefficients zeta, alpha_k, beta_k of cgm_scal1_fn) is
+//     Cp_k[j] <- alpha_k Cp_k[j] (j < f),  Cp_k[f] <- zeta,  Ap_k <- alpha_k Ap_k,  Cx_k[j] -= beta_k Cp_k[j],  Ax_k -= beta_k Ap_k.
+// The iteration keeps the residuals of the chunk (r lives in a ring of M + 1 vectors, so keeping them costs no
+// copy), the scalar kernel keeps the 2 M + 2 coefficients per shift in fp64, and ONE pass per chunk (k_cgm_flush)
+// forms p_k and x_k: (M + 4 S) / M vector passes per iteration instead of 4 S; a solve that ends inside its first
+// chunk writes every x_k exactly once and never touches p_k.  Scalars, residuals and stopping decisions are those
+// of the step-by-step form (they do not depend on x_k, p_k); x_k differs by the order of the additions.
+// A shift that stops inside a chunk keeps its coefficients until the flush (the flush walks the shifts that were
+// active when the chunk began).
+__device__ __forceinline__ void defer_init(Defer& df) {
+    if (threadIdx.x == 0) { df.fill = 0; df.s0 = 0; df.first = 1; df.need_begin = 1; df.nlist = 0; df.ticket = 0u; df.r_next = nullptr; }
+    __syncthreads();
+}
+
+// one CTA, right after cgm_scal1_fn of iteration n: start a chunk if the last one was flushed, append iteration n
+__device__ __forceinline__ void cgm_defer_coef_fn(const SolveHeader& h, const SolveResult& res, const Recur& rc, Defer& df) {
+    if (res.done) return;                                  // breakdown in this iteration: it is not applied
+    const int na = res.nactive;
+    if (df.need_begin) {
+        for (int a = threadIdx.x; a < na; a += blockDim.x) {
+            const int k = rc.active[a];
+            df.list[a] = k; df.pos[k] = a; df.Ap[a] = 1.0; df.Ax[a] = 0.0;
+            for (int j = 0; j < kDeferMax; ++j) { df.Cp[a * kDeferMax + j] = 0.0; df.Cx[a * kDeferMax + j] = 0.0; }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) { df.nlist = na; df.need_begin = 0; }
+        __syncthreads();
+    }
+    const int f = df.fill;
+    for (int idx = threadIdx.x; idx < na * (f + 1); idx += blockDim.x) {
+        const int a = idx / (f + 1), j = idx - a * (f + 1);
+        const int la = df.pos[rc.active[a]];
+        const double z = rc.coef[3 * a + 0], ak = rc.coef[3 * a + 1], bk = rc.coef[3 * a + 2];
+        const double cp = j < f ? ak * df.Cp[la * kDeferMax + j] : z;
+        df.Cp[la * kDeferMax + j] = cp;
+        df.Cx[la * kDeferMax + j] -= bk * cp;
+        if (j == 0) {
+            const double ap = ak * df.Ap[la];
+            df.Ap[la] = ap;
+            df.Ax[la] -= bk * ap;
+        }
+    }
+    if (threadIdx.x == 0) {
+        const int slots = h.defer + 1;
+        df.r_next = (char*)h.ring + (long long)((df.s0 + f + 1) % slots) * h.ring_stride;
+    }
+    __syncthreads();
+}
+
+// one CTA, right after cgm_scal2_fn: iteration n is complete, r_{n+1} is the residual from here on
+__device__ __forceinline__ void cgm_defer_advance(SolveHeader& h, Defer& df) {
+    if (threadIdx.x == 0) { df.fill += 1; h.r = df.r_next; }
+    __syncthreads();
+}
+
+// l.21, 24 alone: r_{n+1} = r_n + beta q into the next slot of the ring; returns the thread's |r_{n+1}|^2 share
+template <typename E, int VEC>
+__device__ __forceinline__ double cgm_rupdate_fn(const SolveHeader& h, const Recur& rc, const Defer& df, int cta, int ncta) {
+    typedef typename RealOf<E>::type T;
+    typedef Pack<E, VEC> P;
+    const long long nvec = h.n / VEC;
+    const P* r = (const P*)h.r;
+    const P* q = (const P*)h.q;
+    P* rn = (P*)df.r_next;
+    const T beta = (T)rc.beta.re;
+    const long long stride = (long long)ncta * blockDim.x;
+    constexpr int U = kPupdUnroll;
+    double acc = 0.0;
+    long long i = (long long)cta * blockDim.x + threadIdx.x;
+    for (; i + (U - 1) * stride < nvec; i += U * stride) {
+        P rv[U], qv[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { rv[u] = ld_pack<false>(r + i + u * stride); qv[u] = ld_pack<false>(q + i + u * stride); }
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+#pragma unroll
+            for (int e = 0; e < VEC; ++e) { rv[u].v[e] = caxpy_r(rv[u].v[e], beta, qv[u].v[e]); acc += cnorm2(rv[u].v[e]); }
+            st_pack<false>(rn + i + u * stride, rv[u]);
+        }
+    }
+    for (; i < nvec; i += stride) {
+        P rv = ld_pack<false>(r + i);
+        const P qv = ld_pack<false>(q + i);
+#pragma unroll
+        for (int e = 0; e < VEC; ++e) { rv.v[e] = caxpy_r(rv.v[e], beta, qv.v[e]); acc += cnorm2(rv.v[e]); }
+        st_pack<false>(rn + i, rv);
+    }
+    return acc;
+}
+
+template <typename E, int VEC>
+__global__ void __launch_bounds__(kThreads) k_cgm_rupdate(SolveState* st) {
+    if (st->res.done) return;
+    double acc[1] = {cgm_rupdate_fn<E, VEC>(st->h, st->rc, st->df, blockIdx.x, gridDim.x)};
+    __shared__ double red[32];
+    block_sum<1>(acc, red);
+    if (threadIdx.x == 0) {
+        st->partial[blockIdx.x] = acc[0];
+        if (blockIdx.x == 0) st->partial_count = gridDim.x;
+    }
+}
+
+// The pass that forms p_k and x_k of a chunk.  It sits at the end of the loop body and does something when the chunk
+// is full or the solve has just ended with residuals pending; the last CTA to finish retires the chunk.
+// Per element: the chunk's residuals into registers once, then per shift of the chunk's list two loads (unless this
+// is the first flush of the solve), 2 cnt multiply-adds per component, and the stores (p_k only while the shift is
+// still iterating).  Coefficients are rounded to the element's precision, sums run in it, as in cgm_update_fn.
+template <typename E, int VEC, int UNR>
+__global__ void __launch_bounds__(kThreads) k_cgm_flush(SolveState* st) {
+    typedef E C;
+    typedef typename RealOf<E>::type T;
+    typedef Pack<E, VEC> P;
+    const SolveHeader& h = st->h;
+    Defer& df = st->df;
+    const int cnt = df.fill;
+    const bool ended = st->res.done != 0;
+    if (!(cnt == h.defer || (ended && cnt > 0))) return;            // the same decision in every CTA
+    __shared__ T s_cp[kMaxShifts * kDeferMax], s_cx[kMaxShifts * kDeferMax], s_ap[kMaxShifts], s_ax[kMaxShifts];
+    __shared__ int s_k[kMaxShifts], s_wp[kMaxShifts];
+    __shared__ const P* s_r[kDeferMax];
+    __shared__ unsigned int s_last;
+    const int nl = df.nlist;
+    const bool first = df.first != 0;
+    for (int a = threadIdx.x; a < nl; a += blockDim.x) {
+        const int k = df.list[a];
+        s_k[a] = k;
+        s_wp[a] = !ended && st->res.conv_iter[k] < 0;              // p_k is needed again
+        s_ap[a] = (T)df.Ap[a]; s_ax[a] = (T)df.Ax[a];
+    }
+    for (int idx = threadIdx.x; idx < nl * cnt; idx += blockDim.x) {
+        const int a = idx / cnt, j = idx - a * cnt;
+        s_cp[a * kDeferMax + j] = (T)df.Cp[a * kDeferMax + j];
+        s_cx[a * kDeferMax + j] = (T)df.Cx[a * kDeferMax + j];
+    }
+    if (threadIdx.x < cnt) s_r[threadIdx.x] = (const P*)((const char*)h.ring + (long long)((df.s0 + threadIdx.x) % (h.defer + 1)) * h.ring_stride);
+    __syncthreads();
+    const long long nvec = h.n / VEC, pks = h.pk_stride, xs = h.x_stride;
+    C* x = (C*)h.x;
+    C* pk = (C*)h.pk;
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += stride) {
+        P rj[kDeferMax];
+#pragma unroll
+        for (int j = 0; j < kDeferMax; ++j)
+            if (j < cnt) rj[j] = ld_pack<true>(s_r[j] + i);
+        for (int a0 = 0; a0 < nl; a0 += UNR) {
+            P xv[UNR], pv[UNR];
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) {
+                if (a0 + u < nl && !first) {
+                    const int k = s_k[a0 + u];
+                    xv[u] = ld_pack<true>((const P*)(x + k * xs) + i);
+                    pv[u] = ld_pack<true>((const P*)(pk + k * pks) + i);
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < UNR; ++u) {
+                if (a0 + u < nl) {
+                    const int a = a0 + u, k = s_k[a];
+                    const T* cp = s_cp + a * kDeferMax;
+                    const T* cx = s_cx + a * kDeferMax;
+                    P xo, po;
+#pragma unroll
+                    for (int e = 0; e < VEC; ++e) {
+                        if (first) { po.v[e] = cmake<C>(0.0, 0.0); xo.v[e] = po.v[e]; }
+                        else {
+                            xo.v[e] = caxpy_r(xv[u].v[e], s_ax[a], pv[u].v[e]);
+                            po.v[e] = caxpy_r(cmake<C>(0.0, 0.0), s_ap[a], pv[u].v[e]);
+                        }
+                    }
+#pragma unroll
+                    for (int j = 0; j < kDeferMax; ++j) {
+                        if (j < cnt) {
+#pragma unroll
+                            for (int e = 0; e < VEC; ++e) {
+                                po.v[e] = caxpy_r(po.v[e], cp[j], rj[j].v[e]);
+                                xo.v[e] = caxpy_r(xo.v[e], cx[j], rj[j].v[e]);
+                            }
+                        }
+                    }
+                    st_pack<true>((P*)(x + k * xs) + i, xo);
+                    if (s_wp[a]) st_pack<true>((P*)(pk + k * pks) + i, po);
+                }
+            }
+        }
+    }
+    // the last CTA to get here retires the chunk: the next one starts at the current residual
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(&df.ticket, 1u) == gridDim.x - 1 ? 1u : 0u;
+    __syncthreads();
+    if (s_last && threadIdx.x == 0) {
+        df.s0 = (df.s0 + cnt) % (h.defer + 1);
+        df.fill = 0; df.first = 0; df.need_begin = 1; df.ticket = 0u;
+        __threadfence();
+    }
+}
+
 // Loop control shared by both algorithms: called by thread 0 after the per-shift stop test.
 __device__ __forceinline__ void finish_iteration(const SolveHeader& h, SolveResult& res, Recur& rc, bool bad) {
     // compact the active list in order (S <= 128: serial is fine)

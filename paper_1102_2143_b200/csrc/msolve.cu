@@ -82,13 +82,15 @@ static int merge_diag(int dtype) {
                          (MergeCfg<double, MergeTile<double>::CAP>::kDiag), (MergeCfg<float, MergeTile<float>::CAP>::kDiag));
 }
 
-static const char* kCgmNames[] = {"cgm_pupdate", "spmv_dot", "cgm_scal1", "cgm_update", "cgm_scal2"};
+static const char* kCgmNames[] = {"cgm_pupdate", "spmv_dot", "cgm_scal1", "cgm_update", "cgm_scal2", "cgm_flush"};
 static const char* kBiNames[] = {"spmv1_dot", "bi_scal1", "bi_supdate", "spmv2_dots", "bi_scal2", "bi_update", "bi_scal3"};
-static int kernels_per_iter(int alg) { return alg == MSOLVE_ALG_CGM ? 5 : 7; }
+// CG-M with the deferred update: cgm_update is the r update alone and the body ends with the flush kernel (a no-op
+// until the chunk is full or the solve has ended)
+static int kernels_per_iter(const msolve_matrix* A, int alg) { return alg == MSOLVE_ALG_CGM ? (defer_len(A, alg) > 0 ? 6 : 5) : 7; }
 // kernel launches per iteration body: the merge-path SpMV is two launches (tiles + carry fix-up)
 static int launches_per_iter(const msolve_matrix* A, int alg) {
     const int spmvs = alg == MSOLVE_ALG_CGM ? 1 : 2;
-    return kernels_per_iter(alg) + (spmv_launches(A) - 1) * spmvs;
+    return kernels_per_iter(A, alg) + (spmv_launches(A) - 1) * spmvs;
 }
 
 // One kernel of the iteration body.  Used for graph capture, and one-by-one for profiling.
@@ -109,7 +111,7 @@ static int build_graph(msolve_matrix* A, int alg) {
     if (g.exec && g.key == key && same_x) return MSOLVE_OK;
     if (g.exec) { cudaGraphExecDestroy(g.exec); g.exec = nullptr; }
     if (g.graph) { cudaGraphDestroy(g.graph); g.graph = nullptr; }
-    const int nk = kernels_per_iter(alg);
+    const int nk = kernels_per_iter(A, alg);
     int lrc = MSOLVE_OK;
     if (A->opt.loop_mode == 0) {
         CU(cudaGraphCreate(&g.graph, 0));
@@ -427,6 +429,7 @@ extern "C" int msolve_config(msolve_matrix* A, int key, int value) {
         A->dev.mat_keep = value == 2 ? 100 : 0;
         return MSOLVE_OK;
     }
+    if (key == MSOLVE_CFG_DEFER_UPDATE && value >= 0 && value <= kDeferMax) { A->opt.defer = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_MATRIX_L2_KEEP_PERCENT && value >= 0 && value <= 100) { A->dev.mat_keep = value; return MSOLVE_OK; }
     if (key == MSOLVE_CFG_X_WINDOW && (value == 0 || value == 1)) {
         if (value == 1) {
@@ -464,7 +467,7 @@ extern "C" int msolve_set_phase_clock(msolve_matrix* A, uint64_t* d_ns) {
 extern "C" int64_t msolve_last_launch_count(const msolve_matrix* A) { return A ? A->last_launches : 0; }
 
 extern "C" const char* msolve_kernel_name(int alg, int j) {
-    if (alg == MSOLVE_ALG_CGM && j >= 0 && j < 5) return kCgmNames[j];
+    if (alg == MSOLVE_ALG_CGM && j >= 0 && j < 6) return kCgmNames[j];
     if (alg == MSOLVE_ALG_BICGSTABM && j >= 0 && j < 7) return kBiNames[j];
     return "";
 }
@@ -476,7 +479,8 @@ static int base_vectors(int alg) { return alg == MSOLVE_ALG_CGM ? 3 : 5; }  // r
 extern "C" size_t msolve_workspace_bytes(const msolve_matrix* A, int nshifts, int algorithm) {
     if (!A || nshifts < 1 || nshifts > kMaxShifts || (algorithm != MSOLVE_ALG_CGM && algorithm != MSOLVE_ALG_BICGSTABM)) return 0;
     const size_t vb = align_up((size_t)pk_stride_elems(A) * elem_bytes(A->dtype), 256);
-    return vb * (size_t)(base_vectors(algorithm) + nshifts) + 256;
+    // the deferred update keeps r in a ring of defer + 1 vectors (defer more than the one r of the step-by-step form)
+    return vb * (size_t)(base_vectors(algorithm) + nshifts + defer_len(A, algorithm)) + 256;
 }
 
 static int fill_header(const msolve_matrix* A, int alg, const void* d_b, const double* h_shifts, int S, double tol,
@@ -492,14 +496,22 @@ static int fill_header(const msolve_matrix* A, int alg, const void* d_b, const d
     char* base = (char*)align_up((size_t)(uintptr_t)ws, 256);
     memset(h, 0, sizeof(*h));
     h->b = d_b; h->x = d_x;
+    const int defer = defer_len(A, alg);
     h->r = base; h->p = base + vb; h->q = base + 2 * vb;
     char* next = base + 3 * vb;
     if (alg == MSOLVE_ALG_BICGSTABM) { h->s = next; h->t = next + vb; next += 2 * vb; }
     h->pk = next;
+    if (defer > 0) {                              // the ring of defer + 1 residuals: r's own vector and the defer extra ones
+        h->p = base; h->q = base + vb; h->pk = base + 2 * vb;
+        h->ring = base + (size_t)(2 + S) * vb;
+        h->ring_stride = (long long)vb;
+        h->r = h->ring;                           // r_0 = slot 0
+    }
     h->n = A->dev.n;
     h->pk_stride = pk_stride_elems(A);
     h->x_stride = A->dev.n;
     h->tol = tol; h->S = S; h->max_iter = max_iter; h->force_all = force_all;
+    h->defer = defer;
     h->stop_rule = A->opt.stop_rule; h->hist = A->d_hist; h->hist_cap = A->hist_cap; h->phase_ns = A->d_phase_ns;
     for (int k = 0; k < S; ++k) h->sigma[k] = h_shifts[k];
     return MSOLVE_OK;
@@ -771,7 +783,7 @@ extern "C" int msolve_profile_iteration(const msolve_matrix* Ac, int alg, const 
     fill_result_init(&A->h_stage->res, S);
     CU(cudaMemcpyAsync(A->d_state, A->h_stage, sizeof(SolveHeader) + sizeof(SolveResult), cudaMemcpyHostToDevice, stream));
     if ((rc = launch_init(A, stream)) != MSOLVE_OK) return rc;
-    const int nk = kernels_per_iter(alg);
+    const int nk = kernels_per_iter(A, alg);
     cudaEvent_t ev[9];
     for (int j = 0; j <= nk; ++j) CU(cudaEventCreate(&ev[j]));
     double sum[8] = {0};

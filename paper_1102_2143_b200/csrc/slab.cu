@@ -241,6 +241,7 @@ static int slabs_create(msolve_slabs** out, int dof, int64_t nrows, int64_t nnz,
         else rc = msolve_create_csr(&d.A, nloc, lnnz, d.d_rowptr, d.d_colidx, d.d_val, dtype, flags, stream);
         if (rc != MSOLVE_OK) break;
         d.A->opt.iter_path = 1;                                         // the slab set owns the loop
+        d.A->opt.defer = 0;                                             // and runs the step-by-step update (slab_header has no ring)
         d.A->x_stride = S->n;                                           // x_k of a slab is a slice of the global [S][n] array
         d.next = (long long)((((size_t)(nloc + d.plan->nhalo) * dof * eb + 255) / 256 * 256) / eb);
     }

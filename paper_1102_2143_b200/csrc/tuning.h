@@ -56,6 +56,8 @@ template <typename E> struct CsrTile { static constexpr int STAGES = 3, CPS = 5;
 // Fused multishift updates: shifts in flight per thread (2 * UNR independent 16-byte loads on top of r and Ap);
 // 4 is the measured optimum for both k_cgm_update and k_bi_update.
 constexpr int kUnrollCgm = 4, kUnrollBi = 4;
+// shifts in flight per thread in the flush of the deferred update (on top of the chunk's residuals in registers)
+constexpr int kUnrollFlush = 2;
 // TMA-staged CG-M update: ring depth, and how many items later a stage is handed back
 constexpr int kUpdStages = 6, kUpdLag = 2;
 

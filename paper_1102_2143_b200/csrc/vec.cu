@@ -14,6 +14,7 @@ __global__ void __launch_bounds__(kThreads) k_init_state(SolveState* st) {
     double s[1];
     reduce_partials<1>(st, s, red);
     init_state_fn(st->h, st->res, st->rc, s[0]);
+    if (st->h.defer) defer_init(st->df);
 }
 
 __global__ void __launch_bounds__(kThreads) k_cgm_scal1(SolveState* st) {
@@ -22,6 +23,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal1(SolveState* st) {
     double s[1];
     reduce_partials<1>(st, s, red);
     cgm_scal1_fn(st->h, st->res, st->rc, s[0]);
+    if (st->h.defer) cgm_defer_coef_fn(st->h, st->res, st->rc, st->df);
 }
 
 __global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGraphConditionalHandle cond, int use_cond) {
@@ -30,6 +32,7 @@ __global__ void __launch_bounds__(kThreads) k_cgm_scal2(SolveState* st, cudaGrap
     double s[1];
     reduce_partials<1>(st, s, red);
     cgm_scal2_fn(st->h, st->res, st->rc, st->rhs_norm, s[0], st->h.hist);
+    if (st->h.defer) cgm_defer_advance(st->h, st->df);
     if (use_cond && threadIdx.x == 0) cudaGraphSetConditional(cond, st->res.done ? 0u : 1u);
 }
 
@@ -93,6 +96,8 @@ static int launch_cgm_update_tma(const msolve_matrix* A, cudaStream_t s) {
 #define L_CUPD(T, V, A, s) {                                                                            \
     if (V * sizeof(T) == 16 && (A)->opt.update_kernel == 1) rc = launch_cgm_update_tma<T>(A, s);           \
     else { auto k = k_cgm_update<T, V, kUnrollCgm>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); } }
+#define L_RUPD(T, V, A, s) { auto k = k_cgm_rupdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
+#define L_FLSH(T, V, A, s) { auto k = k_cgm_flush<T, V, kUnrollFlush>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
 #define L_SUPD(T, V, A, s) { auto k = k_bi_supdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
 #define L_BUPD(T, V, A, s) { auto k = k_bi_update<T, V, kUnrollBi>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
 
@@ -103,8 +108,9 @@ int launch_vec_kernel(const msolve_matrix* A, int alg, int j, cudaStream_t s, cu
         switch (j) {
             case 0: DISPATCH_VEC(A, L_PUPD, A, s); break;
             case 2: k_cgm_scal1<<<1, kThreads, 0, s>>>(st); break;
-            case 3: DISPATCH_VEC(A, L_CUPD, A, s); break;
+            case 3: if (defer_len(A, alg) > 0) { DISPATCH_VEC(A, L_RUPD, A, s); } else { DISPATCH_VEC(A, L_CUPD, A, s); } break;
             case 4: k_cgm_scal2<<<1, kThreads, 0, s>>>(st, cond, use_cond); break;
+            case 5: DISPATCH_VEC(A, L_FLSH, A, s); break;                    // deferred update only (kernels_per_iter)
             default: return fail(MSOLVE_EINVAL, "launch_vec_kernel: CG-M kernel %d is not a vector kernel", j);
         }
     } else {

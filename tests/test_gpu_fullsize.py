@@ -78,7 +78,7 @@ def c4():
     return w, refs
 
 
-C4_VARIANTS = ["bsr3", "csr", "csrmerge", "lat", "lat1", "lat2", "lat3", "lat4", "bsr3_updtma", "slabs8_bsr3", "slabs3_csr"]
+C4_VARIANTS = ["bsr3", "bsr3_stepwise", "bsr3_defer5", "csr", "csrmerge", "lat", "lat1", "lat2", "lat3", "lat4", "bsr3_updtma", "slabs8_bsr3", "slabs3_csr"]
 
 
 def _c4_matrix(ms, w, dtype, variant):
@@ -86,10 +86,14 @@ def _c4_matrix(ms, w, dtype, variant):
         return ms.msolve_slabs_create_bsr3(w.browptr, w.bcolidx, w.blocks.astype(dtype), 8)
     if variant == "slabs3_csr":         # three slabs that do not divide the lattice evenly, TMA-staged vector-CSR per slab
         return ms.msolve_slabs_create_csr(w.rowptr, w.colidx, w.val.astype(dtype), 3)
-    if variant in ("bsr3", "bsr3_updtma"):
+    if variant in ("bsr3", "bsr3_updtma", "bsr3_stepwise", "bsr3_defer5"):
         A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
         if variant == "bsr3_updtma":
             ms.msolve_config(A, ms.MSOLVE_CFG_UPDATE_KERNEL, 1)
+        if variant == "bsr3_stepwise":   # x_k, p_k updated in every iteration (the default defers them, chunk of 16)
+            ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, 0)
+        if variant == "bsr3_defer5":     # 24 (12) iterations = four full chunks and a partial one
+            ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, 5)
         return A
     if variant in ("csr", "csrmerge"):
         return ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val.astype(dtype)),

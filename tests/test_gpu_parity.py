@@ -186,7 +186,7 @@ def test_config1_cgm_c128(ms):
     g = gpu_solve(ms, w, np.complex128, "csr")
     o = oracle_solve(w, np.complex128)
     check_parity(w, np.complex128, g, o, w.tol)
-    assert g[5] == 2 + 5 * g[1]          # init + 5 kernels per iteration, no host round trips
+    assert g[5] == 2 + 6 * g[1]          # init + 6 kernels per iteration (the sixth is the deferred update's flush), no host round trips
 
 
 @pytest.mark.parametrize("fmt", ["csr", "bsr3", "bsr3rows"])
@@ -230,7 +230,7 @@ def test_config5_scaled_cgm(ms, fmt, dtype, tol):
     o = oracle_solve(w, dtype)
     check_parity(w, dtype, g, o, tol)
     assert np.all(np.diff(g[3]) <= 0)              # larger shifts never converge later
-    per_iter = 6 if fmt == "csrmerge" else 5       # merge-path SpMV = tile kernel + carry fix-up
+    per_iter = 7 if fmt == "csrmerge" else 6       # 6 kernels (the sixth: the deferred update's flush); merge-path SpMV = tile kernel + carry fix-up
     assert g[5] == 2 + per_iter * g[1]
 
 
@@ -564,6 +564,66 @@ def test_solve_host_batch_matches_single_solves(ms, alg):
     check_parity(w2, np.complex128, g, o, w2.tol)
     assert ms.msolve_solve_host_batch(A, code, [], w.shifts, w.tol, 500) == []
     ms.msolve_destroy(A)
+
+
+# ------------------------------------------------------------------------------- deferred multishift update
+DEFER_CASES = [("c1", "csr", np.complex128, 1e-10), ("c2", "bsr3", np.complex128, 1e-10), ("c2", "csr", np.complex64, 1e-5),
+               ("c2", "lat", np.complex128, 1e-10), ("c5", "csrvector", np.complex128, 1e-10), ("c5", "csrvector", np.complex64, 1e-5)]
+
+
+def _defer_workload(which):
+    return {"c1": W.config1, "c2": W.config2, "c5": lambda: W.config5(n=(1 << 14) + 13)}[which]()
+
+
+@pytest.mark.parametrize("defer", [1, 3, 7, 16])
+@pytest.mark.parametrize("which,fmt,dtype,tol", DEFER_CASES)
+def test_deferred_update_matches_oracle_and_stepwise(ms, which, fmt, dtype, tol, defer):
+    # MSOLVE_CFG_DEFER_UPDATE = M: p_k, x_k formed once per M iterations from the residuals of the chunk.  Scalars and
+    # residuals are those of the step-by-step form (up to the grouping of the |r|^2 partial sums: another grid), so
+    # iteration counts, conv_iter and relres agree; x_k against the oracle at the usual bar, and against the
+    # step-by-step GPU result
+    w = _defer_workload(which)
+    g = gpu_solve(ms, w, dtype, fmt, tol=tol, cfg={ms.MSOLVE_CFG_DEFER_UPDATE: defer})
+    o = oracle_solve(w, dtype, tol=tol)
+    check_parity(w, dtype, g, o, tol)
+    g0 = gpu_solve(ms, w, dtype, fmt, tol=tol, cfg={ms.MSOLVE_CFG_DEFER_UPDATE: 0})
+    assert abs(g[1] - g0[1]) <= 1 and np.all(np.abs(g[3] - g0[3]) <= 1)
+    if g[1] == g0[1] and np.array_equal(g[3], g0[3]):
+        assert np.allclose(g[4], g0[4], rtol=1e-9 if dtype == np.complex128 else 1e-3, atol=0)
+    assert g0[5] == 2 + 5 * g0[1] and g[5] == 2 + 6 * g[1]
+    for k in range(w.shifts.size):
+        d = np.linalg.norm(g[2][k].astype(np.complex128) - g0[2][k]) / np.linalg.norm(g0[2][k])
+        assert d <= REL[dtype], (k, d)      # two groupings of the |r|^2 sums, amplified by the iteration (as fused vs graph)
+
+
+@pytest.mark.parametrize("defer", [3, 16])
+@pytest.mark.parametrize("max_iter", [1, 2, 3, 4, 7])
+def test_deferred_update_when_the_solve_ends_inside_a_chunk(ms, defer, max_iter):
+    # MAXITER after max_iter iterations: the pending residuals are flushed, x_k = the iterate of that iteration
+    w = W.config2()
+    g = gpu_solve(ms, w, np.complex128, "bsr3", max_iter=max_iter, cfg={ms.MSOLVE_CFG_DEFER_UPDATE: defer})
+    g0 = gpu_solve(ms, w, np.complex128, "bsr3", max_iter=max_iter, cfg={ms.MSOLVE_CFG_DEFER_UPDATE: 0})
+    o = oracle_solve(w, np.complex128, max_iter=max_iter)
+    assert g[0] == g0[0] == o.status == oracle.MAXITER and g[1] == g0[1] == max_iter
+    for k in range(w.shifts.size):
+        assert np.linalg.norm(g[2][k] - o.x[k]) <= 1e-12 * np.linalg.norm(o.x[k]), k
+        assert np.linalg.norm(g[2][k] - g0[2][k]) <= 1e-12 * np.linalg.norm(g0[2][k]), k
+
+
+def test_deferred_update_shifts_that_stop_in_different_chunks(ms):
+    # shifts spread over six decades stop far apart (conv_iter from a few iterations to ~100): every x_k is frozen
+    # at its own iteration although it is only formed at the next flush; literal stop rule as well
+    w = W.config2()
+    w.shifts = np.array([0.0, 0.01, 0.1, 1.0, 10.0, 100.0, 1e3, 1e4])
+    for rule in (0, 1):
+        cfg = {ms.MSOLVE_CFG_DEFER_UPDATE: 5, ms.MSOLVE_CFG_STOP_RULE: rule}
+        g = gpu_solve(ms, w, np.complex128, "bsr3", cfg=cfg)
+        o = oracle.cgm(w.rowptr, w.colidx, w.val, w.b, w.shifts, w.tol, w.max_iter, stop_rule=rule)
+        assert g[0] == o.status == 0 and g[1] == o.iterations and np.array_equal(g[3], o.conv_iter)
+        if rule == 0:
+            assert len(set(g[3].tolist())) >= 4                          # they do stop at different iterations
+        for k in range(w.shifts.size):
+            assert np.linalg.norm(g[2][k] - o.x[k]) <= 1e-9 * np.linalg.norm(o.x[k]), (rule, k)
 
 
 # ------------------------------------------------------------------------------- determinism under repetition
