@@ -89,8 +89,12 @@ def make_workload(name: str, rank: int, want_csr: bool):
     return w, dt, fmt
 
 
-def algorithmic_bytes(w, dtype, fmt, s_active):
-    """bytes the method must move per kernel launch (x gathered once)."""
+def algorithmic_bytes(w, dtype, fmt, s_active, defer=0, profile_iters=20):
+    """bytes the method must move per kernel launch (x gathered once).
+    defer = M > 0 (CG-M, deferred multishift update): `cgm_update` is the r update alone (r, q in, r out) and
+    `cgm_flush` is launched in every iteration but moves bytes once per M: the mean over the launches that
+    msolve_profile_iteration times (bodies 2 .. profile_iters + 1 of a solve; the first flush of a solve reads M
+    residuals and writes S x_k and S p_k, a later one also reads them)."""
     e = np.dtype(dtype).itemsize
     n = w.n
     if fmt == "bsr3":
@@ -100,6 +104,11 @@ def algorithmic_bytes(w, dtype, fmt, s_active):
         spmv = w.links.size * e + 2 * n * e
     else:
         spmv = w.nnz * (e + 4) + (n + 1) * 4 + 2 * n * e
+    if w.algorithm == "cgm" and defer > 0:
+        flushes = [b for b in range(2, profile_iters + 2) if b % defer == 0]
+        fb = sum((defer + (2 if b == defer else 4) * s_active) * n * e for b in flushes) / max(1, profile_iters)
+        return {"cgm_pupdate": 3 * n * e, "spmv_dot": spmv, "cgm_update": 3 * n * e, "cgm_flush": fb,
+                "cgm_scal1": 0, "cgm_scal2": 0}
     if w.algorithm == "cgm":
         return {"cgm_pupdate": 3 * n * e, "spmv_dot": spmv, "cgm_update": (3 + 4 * s_active) * n * e,
                 "cgm_scal1": 0, "cgm_scal2": 0}
@@ -531,14 +540,17 @@ def main():
 
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
-        ab = algorithmic_bytes(w, dtype, fmt, S)
+        defer = 0 if (w.algorithm != "cgm" or args.update_kernel != "regs") else (16 if args.defer < 0 else args.defer)
+        ab = algorithmic_bytes(w, dtype, fmt, S, defer, args.profile_iters)
         kernels = {}
         for name, kms in prof.items():
             gbs = ab.get(name, 0) / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
             kernels[name] = {"ms": round(kms, 5), "alg_GB": round(ab.get(name, 0) / 1e9, 4),
                              "GBps": round(gbs, 1), "frac_measured_peak": round(gbs / peak, 4),
                              "frac_8TBps": round(gbs / 8000.0, 4)}
-        dom = "cgm_update" if w.algorithm == "cgm" else "bi_update"
+        # the dominant kernel: the one an iteration spends most of its time in (the fused multishift update while it
+        # runs in every iteration; the SpMV once the update is deferred)
+        dom = max((k for k in kernels if ab.get(k, 0) > 0), key=lambda k: kernels[k]["ms"])
         traffic, traffic_src = ncu_traffic_bytes(dom, args.workload)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["GBps"], "peak": peak,
                     "unit": "GB/s", "frac": round(kernels[dom]["GBps"] / peak, 4), "peak_source": peak_src,

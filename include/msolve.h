@@ -104,7 +104,8 @@ enum {
                                 shared memory of the SMs, a few MB: only the gathered vector and the dot products touch
                                 global memory per iteration),
                                 0 = by footprint (default): 3 when it fits, else 2 when matrix + (4 + 2 nshifts) vectors
-                                take at most 256 MB, else 1.
+                                take at most 256 MB (96 MB for CG-M with the deferred update, whose graph of
+                                kernels moves 2.2 times fewer bytes per iteration), else 1.
                                 Same arithmetic step for step; the paths group the dot products differently (per-CTA
                                 partials of different grids), so they agree to rounding, not bit for bit */,
     MSOLVE_CFG_FUSED_CTAS = 7 /* CTAs of the cooperative kernel of MSOLVE_CFG_ITER_PATH = 2: 0 = by problem size

@@ -150,6 +150,9 @@ static int build_graph(msolve_matrix* A, int alg) {
 // times, graph / one kernel (profiles/r02_sweeps.md): 11 MB 23.6 / 18.2 us, 150 MB 86 / 76 us, 200 MB 71 / 63 us,
 // 400 MB 119 / 115 us, 800 MB 218 / 223 us.
 constexpr size_t kFusedMaxBytes = (size_t)256 << 20;
+// CG-M with the deferred multishift update moves 2.2x fewer bytes per iteration as a graph of kernels: measured
+// crossover with the one-kernel path at 100 MB (config 4's operator, 16 shifts: n = 98 304; profiles/r02_sweeps.md section 6)
+constexpr size_t kFusedMaxBytesDeferred = (size_t)96 << 20;
 // ... and with everything resident in shared memory while it fits there (148 x ~200 KB; resident.cu checks the exact
 // per-CTA layout, this bound only saves the host copy of rowptr for matrices that cannot fit)
 constexpr size_t kResidentMaxBytes = (size_t)28 << 20;
@@ -565,7 +568,8 @@ int msolve::run_solver(int alg, const msolve_matrix* Ac, const void* d_b, const 
     if (A->opt.iter_path == 3 && !resident) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 3 needs a CSR / BSR3 handle whose matrix and vectors fit in shared memory");
     const bool fused = resident || A->opt.iter_path == 2 ||
                        (A->opt.iter_path == 0 && fused_supported(A) &&
-                        matrix_bytes(A) + (size_t)(4 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <= kFusedMaxBytes);
+                        matrix_bytes(A) + (size_t)(4 + 2 * S) * (size_t)A->dev.n * elem_bytes(A->dtype) <=
+                            (defer_len(A, alg) > 0 ? kFusedMaxBytesDeferred : kFusedMaxBytes));
     if (fused) {
         if (!resident && !fused_supported(A)) return fail(MSOLVE_EINVAL, "solve: MSOLVE_CFG_ITER_PATH = 2 needs a vector-CSR, BSR3 or lattice handle, the register update kernel and the WHILE loop mode");
         // the header travels as a kernel argument and the kernel initialises the result block itself: no H2D copy
