@@ -123,7 +123,7 @@ def test_auto_picks_by_footprint(ms):
     w = W.config4(extents=(8, 8, 8, 16), want_csr=True)
     A = ms.msolve_create_csr(dev(w.rowptr), dev(w.colidx), dev(w.val), ms.MSOLVE_SPMV_MERGE)
     r = ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
-    assert ms.msolve_last_launch_count(A) == 2 + 6 * r.iterations
+    assert ms.msolve_last_launch_count(A) == 2 + 7 * r.iterations      # merge-path SpMV = two launches
     ms.msolve_config(A, ms.MSOLVE_CFG_ITER_PATH, 2)
     with pytest.raises(ms.MsolveError):
         ms.msolve_cgm(A, dev(w.b), w.shifts, w.tol, w.max_iter)
