@@ -259,7 +259,7 @@ def config_dict(args, w, dtype, fmt, world, S, shifts_total):
     return {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
             "shifts": S, "tol": w.tol,
             "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world,
-            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "defer_update": (16 if args.defer < 0 else args.defer) if args.update_kernel == "regs" else 0, "lattice_kernel": args.lattice_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "matrix_l2_keep_percent": args.matrix_l2_keep, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
+            "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "defer_update": (32 if args.defer < 0 else args.defer) if args.update_kernel == "regs" else 0, "lattice_kernel": args.lattice_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "matrix_l2_keep_percent": args.matrix_l2_keep, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
 
 
 def run_reference(args, rank):
@@ -351,7 +351,7 @@ def main():
                     help="tile kernel of the lattice operator (MSOLVE_CFG_LATTICE_KERNEL; 0 = default per element type)")
     ap.add_argument("--defer", type=int, default=-1,
                     help="CG-M: chunk length of the deferred multishift update (MSOLVE_CFG_DEFER_UPDATE; 0 = update "
-                         "every x_k, p_k in every iteration; -1 = the library's default, 16)")
+                         "every x_k, p_k in every iteration; -1 = the library's default, 32)")
     ap.add_argument("--update-kernel", default="regs", choices=["regs", "tma"],
                     help="CG-M fused multishift update: register kernel (default) or the TMA-staged kernel")
     ap.add_argument("--x-window", action="store_true",
@@ -540,7 +540,7 @@ def main():
 
     if rank == 0:
         peak, peak_src = measured_peak_gbs()
-        defer = 0 if (w.algorithm != "cgm" or args.update_kernel != "regs") else (16 if args.defer < 0 else args.defer)
+        defer = 0 if (w.algorithm != "cgm" or args.update_kernel != "regs") else (32 if args.defer < 0 else args.defer)
         ab = algorithmic_bytes(w, dtype, fmt, S, defer, args.profile_iters)
         kernels = {}
         for name, kms in prof.items():

@@ -115,8 +115,8 @@ enum {
                                  evict-first -- for a matrix of which a part fits in L2 next to the vectors.  Applies to
                                  the TMA-staged kernels and to the BSR3 SpMV of the one-kernel path;
                                  MSOLVE_CFG_MATRIX_L2 = 1 / 2 set it to 0 / 100.  Default 0; profiles/r02_sweeps.md */,
-    MSOLVE_CFG_DEFER_UPDATE = 9 /* CG-M as a graph of kernels: chunk length M of the DEFERRED multishift update, 0 .. 16,
-                                 default 16.  Alg. 1 l.28-29 write every x_k and p_k in every
+    MSOLVE_CFG_DEFER_UPDATE = 9 /* CG-M as a graph of kernels: chunk length M of the DEFERRED multishift update, 0 .. 32,
+                                 default 32.  Alg. 1 l.28-29 write every x_k and p_k in every
                                  iteration; both are linear in the residuals r_n with coefficients the scalar
                                  recurrences already produce, so with M > 0 an iteration only updates r (kept in a ring
                                  of M + 1 vectors) while the scalar kernel accumulates 2 M + 2 fp64 coefficients per

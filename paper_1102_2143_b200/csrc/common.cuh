@@ -257,7 +257,7 @@ struct Recur {
 // that were active when the chunk began are `list`; for list position a and chunk-relative iteration j
 //   p_k(now)  = Ap[a] P_k + sum_j Cp[a][j] r_j,      x_k(now) = X_k + Ax[a] P_k + sum_j Cx[a][j] r_j
 // with P_k, X_k the vectors in memory (written by the previous flush) and r_j the residuals kept in the ring.
-constexpr int kDeferMax = 16;
+constexpr int kDeferMax = 32;
 struct Defer {
     int fill;            // residuals of the chunk whose coefficients are complete (= iterations done in the chunk)
     int s0;              // ring slot of the chunk's first residual

@@ -394,7 +394,10 @@ __global__ void __launch_bounds__(kThreads) k_cgm_flush(SolveState* st) {
     const int cnt = df.fill;
     const bool ended = st->res.done != 0;
     if (!(cnt == h.defer || (ended && cnt > 0))) return;            // the same decision in every CTA
-    __shared__ T s_cp[kMaxShifts * kDeferMax], s_cx[kMaxShifts * kDeferMax], s_ap[kMaxShifts], s_ax[kMaxShifts];
+    extern __shared__ __align__(16) unsigned char flush_dyn[];            // 2 x kMaxShifts x kDeferMax coefficients: beyond 48 KB in fp64
+    T* s_cp = (T*)flush_dyn;
+    T* s_cx = s_cp + kMaxShifts * kDeferMax;
+    __shared__ T s_ap[kMaxShifts], s_ax[kMaxShifts];
     __shared__ int s_k[kMaxShifts], s_wp[kMaxShifts];
     __shared__ const P* s_r[kDeferMax];
     __shared__ unsigned int s_last;

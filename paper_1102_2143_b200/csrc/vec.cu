@@ -78,6 +78,14 @@ static bool vec16(const msolve_matrix* A) {
         }                                                                                  \
     } while (0)
 
+// grid of the flush kernel: resident CTAs per SM with its dynamic shared memory, capped by the work
+static int flush_grid(const msolve_matrix* A, const void* k, int smem, long long work) {
+    int per_sm = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, kThreads, (size_t)smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    const long long need = (work + kThreads - 1) / kThreads;
+    return (int)std::max(1ll, std::min<long long>((long long)A->num_sms * per_sm, need));
+}
+
 template <typename T>
 static int launch_cgm_update_tma(const msolve_matrix* A, cudaStream_t s) {
     typedef UpdTmaCfg<T> U;
@@ -97,7 +105,11 @@ static int launch_cgm_update_tma(const msolve_matrix* A, cudaStream_t s) {
     if (V * sizeof(T) == 16 && (A)->opt.update_kernel == 1) rc = launch_cgm_update_tma<T>(A, s);           \
     else { auto k = k_cgm_update<T, V, kUnrollCgm>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); } }
 #define L_RUPD(T, V, A, s) { auto k = k_cgm_rupdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
-#define L_FLSH(T, V, A, s) { auto k = k_cgm_flush<T, V, kUnrollFlush>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
+#define L_FLSH(T, V, A, s) {                                                                            \
+    auto k = k_cgm_flush<T, V, kUnrollFlush>;                                                           \
+    const int smem = 2 * kMaxShifts * kDeferMax * (int)sizeof(typename RealOf<T>::type);                \
+    rc = ensure_smem(A, (const void*)k, smem);                                                          \
+    if (rc == MSOLVE_OK) k<<<flush_grid(A, (const void*)k, smem, (A)->dev.n / V), kThreads, smem, s>>>((A)->d_state); }
 #define L_SUPD(T, V, A, s) { auto k = k_bi_supdate<T, V>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads * 4), kThreads, 0, s>>>((A)->d_state); }
 #define L_BUPD(T, V, A, s) { auto k = k_bi_update<T, V, kUnrollBi>; k<<<grid_for(A, k, (A)->dev.n / V, kThreads), kThreads, 0, s>>>((A)->d_state); }
 

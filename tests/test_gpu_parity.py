@@ -575,7 +575,7 @@ def _defer_workload(which):
     return {"c1": W.config1, "c2": W.config2, "c5": lambda: W.config5(n=(1 << 14) + 13)}[which]()
 
 
-@pytest.mark.parametrize("defer", [1, 3, 7, 16])
+@pytest.mark.parametrize("defer", [1, 3, 7, 16, 32])
 @pytest.mark.parametrize("which,fmt,dtype,tol", DEFER_CASES)
 def test_deferred_update_matches_oracle_and_stepwise(ms, which, fmt, dtype, tol, defer):
     # MSOLVE_CFG_DEFER_UPDATE = M: p_k, x_k formed once per M iterations from the residuals of the chunk.  Scalars and
@@ -596,7 +596,7 @@ def test_deferred_update_matches_oracle_and_stepwise(ms, which, fmt, dtype, tol,
         assert d <= REL[dtype], (k, d)      # two groupings of the |r|^2 sums, amplified by the iteration (as fused vs graph)
 
 
-@pytest.mark.parametrize("defer", [3, 16])
+@pytest.mark.parametrize("defer", [3, 32])
 @pytest.mark.parametrize("max_iter", [1, 2, 3, 4, 7])
 def test_deferred_update_when_the_solve_ends_inside_a_chunk(ms, defer, max_iter):
     # MAXITER after max_iter iterations: the pending residuals are flushed, x_k = the iterate of that iteration
