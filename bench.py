@@ -36,9 +36,14 @@ UNIT = "iterations/s"
 
 
 # ----------------------------------------------------------------------------------- workloads
-def make_workload(name: str, rank: int, want_csr: bool):
-    """Returns (workload, dtype, format).  Right-hand side differs per rank (replicas)."""
-    if name == "config4_c128_bsr3":
+def make_workload(name: str, rank: int, want_csr: bool, extents=None):
+    """Returns (workload, dtype, format).  Right-hand side differs per rank (replicas).
+    extents: config 4's operator on another lattice (size sweeps; config4_c128_bsr3 / _lat only)."""
+    if extents is not None:
+        if name not in ("config4_c128_bsr3", "config4_c128_lat"):
+            raise SystemExit("--extents goes with --workload config4_c128_bsr3 or config4_c128_lat")
+        w, dt, fmt = W.config4(extents=tuple(extents), want_csr=want_csr), np.complex128, name.rsplit("_", 1)[1]
+    elif name == "config4_c128_bsr3":
         w, dt, fmt = W.config4(want_csr=want_csr), np.complex128, "bsr3"
     elif name == "config4_c64_bsr3":
         w, dt, fmt = W.config4(want_csr=want_csr, tol=1e-5), np.complex64, "bsr3"
@@ -256,7 +261,7 @@ def config_dict(args, w, dtype, fmt, world, S, shifts_total):
                if footprint_mb > 252 else
                "working set %.0f MB (matrix + %d vectors) is not larger than 2 x L2 (126 MB) and is NOT flushed between "
                "iterations: a solve re-reads its own vectors every iteration by construction" % (footprint_mb, 4 + 2 * S))
-    return {"workload": args.workload, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
+    return {"workload": args.workload, "extents": args.extents, "algorithm": w.algorithm, "n": w.n, "format": fmt, "nnz_or_blocks": units,
             "shifts": S, "tol": w.tol,
             "parallelism": ("shifts split over %d ranks (%d of %d per rank)" % (world, S, shifts_total)) if args.shard == "shifts" else "replicas x%d" % world,
             "loop_mode": args.loop_mode, "spmv": args.spmv, "update_kernel": args.update_kernel, "defer_update": (32 if args.defer < 0 else args.defer) if args.update_kernel == "regs" else 0, "lattice_kernel": args.lattice_kernel, "x_window": bool(args.x_window), "matrix_l2": args.matrix_l2, "matrix_l2_keep_percent": args.matrix_l2_keep, "iter_path": args.iter_path, "fused_ctas": args.fused_ctas, "l2": l2_note}
@@ -267,7 +272,7 @@ def run_reference(args, rank):
     step = the same bounded sample the cpu_baseline leg of the GPU arm times (--cpu-iters iterations, tol = 0)."""
     if rank != 0:
         return
-    w, dtype, fmt = make_workload(args.workload, 0, want_csr=True)
+    w, dtype, fmt = make_workload(args.workload, 0, want_csr=True, extents=args.extents)
     per_step = max(args.cpu_iters, 1)
     for _ in range(args.warmup):
         oracle_sample(w, dtype, per_step, True)
@@ -349,6 +354,8 @@ def main():
                     help="SpMV kernel for CSR workloads (BSR3: auto = TMA tile kernel, vector = row kernel)")
     ap.add_argument("--lattice-kernel", type=int, default=0, choices=[0, 1, 2, 3, 4],
                     help="tile kernel of the lattice operator (MSOLVE_CFG_LATTICE_KERNEL; 0 = default per element type)")
+    ap.add_argument("--extents", type=lambda t: [int(v) for v in t.split(",")], default=None,
+                    help="config4_c128_bsr3 / config4_c128_lat on another lattice, e.g. 16,16,16,16 (size sweeps)")
     ap.add_argument("--defer", type=int, default=-1,
                     help="CG-M: chunk length of the deferred multishift update (MSOLVE_CFG_DEFER_UPDATE; 0 = update "
                          "every x_k, p_k in every iteration; -1 = the library's default, 32)")
@@ -404,7 +411,7 @@ def main():
     ms.load_library()
 
     need_csr = args.workload.endswith("_csr") or (rank == 0 and world == 1 and args.cpu_iters > 0)
-    w, dtype, fmt = make_workload(args.workload, 0 if args.shard == "shifts" else rank, want_csr=need_csr)
+    w, dtype, fmt = make_workload(args.workload, 0 if args.shard == "shifts" else rank, want_csr=need_csr, extents=args.extents)
     shifts_total = int(w.shifts.size)
     if args.shard == "shifts":
         if world > shifts_total:

@@ -80,6 +80,7 @@ struct msolve_matrix {
     long long x_stride = 0;             // slab handles: elements between x_k and x_{k+1} in the caller's array (0 = n)
     size_t l2_persist_bytes = 0;        // MSOLVE_CFG_X_WINDOW: persisting L2 set-aside / largest window of the device
     size_t l2_window_max = 0;
+    mutable int flush_ctas_per_sm = 0;       // resident CTAs per SM of k_cgm_flush (0: not asked yet), vec.cu
     mutable std::vector<int32_t> h_rowptr;   // host copy of rowptr / browptr (resident.cu sizes its ranges from it), filled on demand
     mutable std::vector<const void*> smem_attr_done;   // kernels whose dynamic shared-memory limit is raised on `device`
     msolve_slab_set* slabs = nullptr;   // row-partitioned form (msolve_create_*_slabs)

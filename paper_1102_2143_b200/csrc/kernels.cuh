@@ -439,29 +439,34 @@ __global__ void __launch_bounds__(kThreads) k_cgm_flush(SolveState* st) {
             for (int u = 0; u < UNR; ++u) {
                 if (a0 + u < nl) {
                     const int a = a0 + u, k = s_k[a];
-                    const T* cp = s_cp + a * kDeferMax;
                     const T* cx = s_cx + a * kDeferMax;
-                    P xo, po;
+                    P xo;
 #pragma unroll
-                    for (int e = 0; e < VEC; ++e) {
-                        if (first) { po.v[e] = cmake<C>(0.0, 0.0); xo.v[e] = po.v[e]; }
-                        else {
-                            xo.v[e] = caxpy_r(xv[u].v[e], s_ax[a], pv[u].v[e]);
-                            po.v[e] = caxpy_r(cmake<C>(0.0, 0.0), s_ap[a], pv[u].v[e]);
-                        }
-                    }
+                    for (int e = 0; e < VEC; ++e)
+                        xo.v[e] = first ? cmake<C>(0.0, 0.0) : caxpy_r(xv[u].v[e], s_ax[a], pv[u].v[e]);
 #pragma unroll
                     for (int j = 0; j < kDeferMax; ++j) {
                         if (j < cnt) {
 #pragma unroll
-                            for (int e = 0; e < VEC; ++e) {
-                                po.v[e] = caxpy_r(po.v[e], cp[j], rj[j].v[e]);
-                                xo.v[e] = caxpy_r(xo.v[e], cx[j], rj[j].v[e]);
-                            }
+                            for (int e = 0; e < VEC; ++e) xo.v[e] = caxpy_r(xo.v[e], cx[j], rj[j].v[e]);
                         }
                     }
                     st_pack<true>((P*)(x + k * xs) + i, xo);
-                    if (s_wp[a]) st_pack<true>((P*)(pk + k * pks) + i, po);
+                    if (s_wp[a]) {                           // p_k only while it is needed again (half of the multiply-adds)
+                        const T* cp = s_cp + a * kDeferMax;
+                        P po;
+#pragma unroll
+                        for (int e = 0; e < VEC; ++e)
+                            po.v[e] = first ? cmake<C>(0.0, 0.0) : caxpy_r(cmake<C>(0.0, 0.0), s_ap[a], pv[u].v[e]);
+#pragma unroll
+                        for (int j = 0; j < kDeferMax; ++j) {
+                            if (j < cnt) {
+#pragma unroll
+                                for (int e = 0; e < VEC; ++e) po.v[e] = caxpy_r(po.v[e], cp[j], rj[j].v[e]);
+                            }
+                        }
+                        st_pack<true>((P*)(pk + k * pks) + i, po);
+                    }
                 }
             }
         }

@@ -80,10 +80,13 @@ static bool vec16(const msolve_matrix* A) {
 
 // grid of the flush kernel: resident CTAs per SM with its dynamic shared memory, capped by the work
 static int flush_grid(const msolve_matrix* A, const void* k, int smem, long long work) {
-    int per_sm = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, kThreads, (size_t)smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+    if (A->flush_ctas_per_sm < 1) {            // once per handle (one element type and pack width per handle)
+        int per_sm = 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, kThreads, (size_t)smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+        A->flush_ctas_per_sm = per_sm;
+    }
     const long long need = (work + kThreads - 1) / kThreads;
-    return (int)std::max(1ll, std::min<long long>((long long)A->num_sms * per_sm, need));
+    return (int)std::max(1ll, std::min<long long>((long long)A->num_sms * A->flush_ctas_per_sm, need));
 }
 
 template <typename T>
