@@ -188,11 +188,14 @@ def ncu_traffic_bytes(kernel: str, workload: str):
         if not os.path.exists(p):
             continue
         try:
+            hit = None
             for ln in open(p):
                 f = ln.strip().split(",")
                 if len(f) >= 6 and f[0] == kernel and f[5] == workload:
-                    commit = f[6] if len(f) > 6 else "round 1 (see profiles/r01_ncu_dram_traffic.md)"
-                    return float(f[1]), "profiles/%s: stored ncu --set full capture taken at commit %s; not re-measured in this run" % (name, commit)
+                    hit = f                      # the last row of a kernel is its newest capture
+            if hit:
+                commit = hit[6] if len(hit) > 6 else "round 1 (see profiles/r01_ncu_dram_traffic.md)"
+                return float(hit[1]), "profiles/%s: stored ncu --set full capture taken at commit %s; not re-measured in this run" % (name, commit)
         except Exception:
             continue
     return None, None

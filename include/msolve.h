@@ -166,7 +166,9 @@ int msolve_create_lattice_su3(msolve_matrix **A, int ndim, const int32_t *h_exte
                               double c_b, int dtype, int flags, void *stream);
 
 /* Bytes of caller-provided device workspace a solve with `nshifts` shifts needs
- * (r, p, Ap [, s, t] and one search direction p_k per shift, Alg. 1 l.10-11).  0 on bad input. */
+ * (r, p, Ap [, s, t] and one search direction p_k per shift, Alg. 1 l.10-11; for CG-M also the MSOLVE_CFG_DEFER_UPDATE
+ * residuals of the deferred update, as the handle is configured WHEN THIS IS CALLED: ask again after msolve_config).
+ * 0 on bad input. */
 size_t msolve_workspace_bytes(const msolve_matrix *A, int nshifts, int algorithm);
 
 /* CG-M, Algorithm 1 as read in DESIGN.md ("Readings of the paper").
