@@ -90,7 +90,7 @@ def _c4_matrix(ms, w, dtype, variant):
         A = ms.msolve_create_bsr3(dev(w.browptr), dev(w.bcolidx), dev(w.blocks.astype(dtype)))
         if variant == "bsr3_updtma":
             ms.msolve_config(A, ms.MSOLVE_CFG_UPDATE_KERNEL, 1)
-        if variant == "bsr3_stepwise":   # x_k, p_k updated in every iteration (the default defers them, chunk of 16)
+        if variant == "bsr3_stepwise":   # x_k, p_k updated in every iteration (the default defers them, chunk of 32)
             ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, 0)
         if variant == "bsr3_defer5":     # 24 (12) iterations = four full chunks and a partial one
             ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, 5)
