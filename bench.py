@@ -538,6 +538,28 @@ def main():
     prof = ms.msolve_profile_iteration(A, alg, b_dev, w.shifts, args.profile_iters, x=x_dev, workspace=ws)
     torch.cuda.synchronize()
 
+    # ---- CG-M with the deferred multishift update (the default): the same solves once more with the update of every
+    # x_k, p_k in every iteration (MSOLVE_CFG_DEFER_UPDATE = 0, Alg. 1 l.28-29 step by step), so that the line carries
+    # the fused multishift-update kernel and the iteration rate of that form as well (rank 0 reports its own numbers)
+    stepwise = None
+    defer_now = 0 if (w.algorithm != "cgm" or args.update_kernel != "regs") else (32 if args.defer < 0 else args.defer)
+    if defer_now > 0 and args.iter_path in ("auto", "graph") and ms.msolve_last_launch_count(A) > 1:
+        ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, 0)
+        for _ in range(2):
+            solve(A, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev, workspace=ws)
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        it0 = 0
+        t0.record()
+        for _ in range(args.steps):
+            it0 += solve(A, b_dev, w.shifts, w.tol, w.max_iter, x=x_dev, workspace=ws).iterations
+        t1.record()
+        torch.cuda.synchronize()
+        prof0 = ms.msolve_profile_iteration(A, alg, b_dev, w.shifts, args.profile_iters, x=x_dev, workspace=ws)
+        torch.cuda.synchronize()
+        ms.msolve_config(A, ms.MSOLVE_CFG_DEFER_UPDATE, defer_now)
+        stepwise = (it0, t0.elapsed_time(t1), prof0)
+
     # ---- reduce over ranks
     (ms_total, ms_e2e, ms_single), (iters_all, launches_all, it_e2e_all, it_single_all) = aggregate_over_ranks(
         [ms_total, e2e[1] if e2e else 0.0, e2e[5] if e2e else 0.0],
@@ -597,6 +619,21 @@ def main():
                                              "single_call_api": "msolve_solve_host per step, nothing overlapped"},
             "gpu_launches": int(launches_all), "clocks": clocks,
         }
+        if stepwise is not None:
+            it0, ms0, prof0 = stepwise
+            ab0 = algorithmic_bytes(w, dtype, fmt, S, 0, args.profile_iters)
+            k0 = {}
+            for name, kms in prof0.items():
+                gbs = ab0.get(name, 0) / (kms * 1e-3) / 1e9 if kms > 0 else 0.0
+                k0[name] = {"ms": round(kms, 5), "alg_GB": round(ab0.get(name, 0) / 1e9, 4), "GBps": round(gbs, 1),
+                            "frac_measured_peak": round(gbs / peak, 4), "frac_8TBps": round(gbs / 8000.0, 4)}
+            tr0, tr0_src = ncu_traffic_bytes("cgm_update", args.workload)
+            line["stepwise_update"] = {
+                "what": "the same solves with MSOLVE_CFG_DEFER_UPDATE = 0: every x_k, p_k updated in every iteration (Alg. 1 l.28-29 step by step)",
+                "value": throughput(it0, ms0), "unit": UNIT, "ms_per_step": ms0 / args.steps, "kernels": k0,
+                "roofline": {"bound": "hbm", "kernel": "cgm_update", "achieved": k0["cgm_update"]["GBps"], "peak": peak, "unit": "GB/s",
+                             "frac": round(k0["cgm_update"]["GBps"] / peak, 4), "traffic": tr0, "traffic_source": tr0_src,
+                             "algorithmic_bytes_per_launch": ab0["cgm_update"]}}
         if phases is not None:
             line["one_kernel_phases_us_per_iteration"] = phases
         print(json.dumps(line))
